@@ -1,0 +1,191 @@
+"""ctypes binding of the CPU oracle (oracle/mf_oracle.c).
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this package.  It
+imports nothing from paper_1006_4644_b200: the oracle and the CUDA path share no
+code.
+
+The oracle follows SURVEY.md §8(c) "Definition" (eq. 2.1,
+PAPER.md:96-103 steps 1-4); see the header of mf_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mf_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+OK, EINVAL, ESTATE, ENOMEM, WTRUNC = 0, -1, -2, -4, 1
+
+
+def build(force: bool = False) -> str:
+    """Compile mf_oracle.c with gcc -O2 (as it stands, never tuned)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class Peak(C.Structure):
+    _fields_ = [("snr_max", C.c_double), ("idx_peak", C.c_int64),
+                ("phase", C.c_double), ("sigma", C.c_double)]
+
+
+class Trigger(C.Structure):
+    _fields_ = [("template_idx", C.c_int64), ("sample_idx", C.c_int64),
+                ("snr", C.c_double), ("phase", C.c_double)]
+
+
+PEAK_DTYPE = np.dtype([("snr_max", "f8"), ("idx_peak", "i8"), ("phase", "f8"), ("sigma", "f8")])
+TRIG_DTYPE = np.dtype([("template_idx", "i8"), ("sample_idx", "i8"), ("snr", "f8"), ("phase", "f8")])
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        dp = C.POINTER(C.c_double)
+        L.orc_fft.argtypes = [dp, C.c_int64, C.c_int]
+        L.orc_f_isco.argtypes = [C.c_double, C.c_double]
+        L.orc_f_isco.restype = C.c_double
+        L.orc_psi.argtypes = [C.c_double] * 3
+        L.orc_psi.restype = C.c_double
+        L.orc_band.argtypes = [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double,
+                               C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.orc_create.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.c_double, C.c_double]
+        L.orc_destroy.argtypes = [C.c_void_p]
+        L.orc_set_psd.argtypes = [C.c_void_p, dp, C.c_int64]
+        L.orc_load_segment.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int64]
+        L.orc_template.argtypes = [C.c_void_p, C.c_double, C.c_double, dp]
+        L.orc_sigma2.argtypes = [C.c_void_p, C.c_double, C.c_double, dp]
+        L.orc_snr_series.argtypes = [C.c_void_p, C.c_double, C.c_double, dp, dp, dp]
+        L.orc_filter_bank.argtypes = [C.c_void_p, dp, C.c_int64, C.c_double, C.POINTER(Peak),
+                                      C.POINTER(Trigger), C.c_int64, C.POINTER(C.c_int64)]
+        L.orc_num_threads.restype = C.c_int
+        L.orc_set_num_threads.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+class OracleError(RuntimeError):
+    def __init__(self, rc, what):
+        super().__init__(f"oracle {what} failed: rc={rc}")
+        self.rc = rc
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def fft(x: np.ndarray, sign: int) -> np.ndarray:
+    """Radix-2 FFT of a complex128 vector; sign=-1 forward, +1 unnormalised inverse."""
+    a = np.ascontiguousarray(x, dtype=np.complex128).copy()
+    rc = lib().orc_fft(_dp(a.view(np.float64)), a.size, int(sign))
+    if rc:
+        raise OracleError(rc, "orc_fft")
+    return a
+
+
+def psi(m1: float, m2: float, f: float) -> float:
+    return lib().orc_psi(float(m1), float(m2), float(f))
+
+
+def f_isco(m1: float, m2: float) -> float:
+    return lib().orc_f_isco(float(m1), float(m2))
+
+
+def band(n: int, fs: float, f_low: float, m1: float, m2: float):
+    klo, khi = C.c_int64(), C.c_int64()
+    rc = lib().orc_band(n, fs, f_low, m1, m2, C.byref(klo), C.byref(khi))
+    if rc:
+        raise OracleError(rc, "orc_band")
+    return klo.value, khi.value
+
+
+def num_threads() -> int:
+    return lib().orc_num_threads()
+
+
+def set_num_threads(n: int) -> None:
+    lib().orc_set_num_threads(int(n))
+
+
+class Oracle:
+    """Context mirroring the product's C ABI (create / set_psd / load_segment / filter_bank)."""
+
+    def __init__(self, n: int, fs: float, f_low: float):
+        self.n, self.fs, self.f_low = int(n), float(fs), float(f_low)
+        self._h = C.c_void_p()
+        rc = lib().orc_create(C.byref(self._h), self.n, self.fs, self.f_low)
+        if rc:
+            raise OracleError(rc, "orc_create")
+
+    def close(self):
+        if self._h:
+            lib().orc_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_psd(self, psd: np.ndarray):
+        p = np.ascontiguousarray(psd, dtype=np.float64)
+        rc = lib().orc_set_psd(self._h, _dp(p), p.size)
+        if rc:
+            raise OracleError(rc, "orc_set_psd")
+
+    def load_segment(self, samples: np.ndarray):
+        s = np.ascontiguousarray(samples, dtype=np.float32)
+        rc = lib().orc_load_segment(self._h, s.ctypes.data_as(C.POINTER(C.c_float)), s.size)
+        if rc:
+            raise OracleError(rc, "orc_load_segment")
+
+    def template(self, m1: float, m2: float) -> np.ndarray:
+        h = np.empty(self.n // 2 + 1, dtype=np.complex128)
+        rc = lib().orc_template(self._h, m1, m2, _dp(h.view(np.float64)))
+        if rc:
+            raise OracleError(rc, "orc_template")
+        return h
+
+    def sigma2(self, m1: float, m2: float) -> float:
+        s = C.c_double()
+        rc = lib().orc_sigma2(self._h, m1, m2, C.byref(s))
+        if rc:
+            raise OracleError(rc, "orc_sigma2")
+        return s.value
+
+    def snr_series(self, m1: float, m2: float):
+        """-> (rho[n], z[n] complex128, sigma)"""
+        rho = np.empty(self.n, dtype=np.float64)
+        z = np.empty(self.n, dtype=np.complex128)
+        s = C.c_double()
+        rc = lib().orc_snr_series(self._h, m1, m2, _dp(rho), _dp(z.view(np.float64)), C.byref(s))
+        if rc:
+            raise OracleError(rc, "orc_snr_series")
+        return rho, z, s.value
+
+    def filter_bank(self, bank: np.ndarray, snr_threshold: float, trig_capacity: int = 1 << 20):
+        """-> (peaks[PEAK_DTYPE], triggers[TRIG_DTYPE], n_found, rc)"""
+        b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+        nt = b.shape[0]
+        peaks = np.zeros(max(nt, 1), dtype=PEAK_DTYPE)
+        trig = np.zeros(max(trig_capacity, 1), dtype=TRIG_DTYPE)
+        nf = C.c_int64()
+        rc = lib().orc_filter_bank(self._h, _dp(b), nt, float(snr_threshold),
+                                   peaks.ctypes.data_as(C.POINTER(Peak)),
+                                   trig.ctypes.data_as(C.POINTER(Trigger)), trig_capacity,
+                                   C.byref(nf))
+        if rc < 0:
+            raise OracleError(rc, "orc_filter_bank")
+        return peaks[:nt], trig[:min(nf.value, trig_capacity)], nf.value, rc

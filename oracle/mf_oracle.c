@@ -1,0 +1,421 @@
+/*
+ * mf_oracle.c -- CPU oracle for the cuInspiral matched-filter hot path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may load this library.  It
+ * shares no code, header, table or constant generator with the CUDA path under
+ * paper_1006_4644_b200/csrc/.
+ *
+ * Plain, slow, double precision; own radix-2 FFT with directly evaluated
+ * twiddles; no blocking, fusion or reordering beyond the definition.  The
+ * method is exact (an FFT evaluates the correlation of eq. 2.1 exactly), so the
+ * oracle is the definition written out (SURVEY.md §8(c) "Definition", items
+ * 1-9), which restates:
+ *   PAPER.md:82-88   eq. 2.1  c(t) = \int X(f) Theta*(f)/S_n(f) e^{2 pi i f t} df
+ *   PAPER.md:96-103  §2.1 steps 1-4 (generate+normalise, two correlators,
+ *                    quadrature sum, threshold/max)
+ *   PAPER.md:127-131 §3.1 device_template_proc / complex_mf / cufft_C2R /
+ *                    madd2 / maxfind
+ * The waveform formula (the paper prints none) is the 2PN SPA
+ * phase of BASELINE.json configs[0]; readings A1-A21 of SURVEY.md §8(c) are
+ * listed in DESIGN.md.
+ *
+ * Parity pins (tests/test_oracle_pins.py): every exported function is pinned;
+ * none is "parity unpinned".
+ *
+ * Threads: OpenMP across templates only (orc_filter_bank).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_OK       0
+#define ORC_EINVAL  -1
+#define ORC_ESTATE  -2
+#define ORC_ENOMEM  -4
+#define ORC_WTRUNC   1
+
+/* SURVEY.md §8(c) item 1 / reading A8: T_sun = G M_sun / c^3 with
+ * G M_sun = 1.3271244e20 m^3 s^-2, c = 299792458 m/s. */
+static const double ORC_TSUN = 4.925490947641267e-6;
+static const double ORC_PI = 3.14159265358979323846264338327950288;
+
+typedef struct { double snr_max; int64_t idx_peak; double phase; double sigma; } orc_peak;
+typedef struct { int64_t template_idx; int64_t sample_idx; double snr; double phase; } orc_trigger;
+
+typedef struct orc_ctx {
+    int64_t n;          /* samples per segment, power of two */
+    double fs, f_low;
+    double dt, df;
+    double *psd;        /* n/2+1 one-sided S_n, or NULL */
+    double *dtil;       /* 2*(n/2+1): d~[k] = dt * sum_j d[j] e^{-2 pi i jk/n}, or NULL */
+    double *tw_re, *tw_im;   /* cos/sin(2 pi k / n), k < n/2, each evaluated directly */
+} orc_ctx;
+
+/* ------------------------------------------------------------------ FFT */
+
+static int is_pow2(int64_t n) { return n > 0 && (n & (n - 1)) == 0; }
+
+/* In-place radix-2 decimation-in-time FFT on interleaved (re,im) doubles.
+ * sign = -1: X[k] = sum_j x[j] e^{-2 pi i jk/n}  (forward, PAPER.md:84 implies
+ *            the inverse carries e^{+2 pi i f t}, so the forward carries e^{-})
+ * sign = +1: unnormalised inverse.
+ * tw_re/tw_im: table of cos/sin(2 pi k/n), k < n/2 (may be NULL: evaluated here). */
+static int fft_radix2(double *x, int64_t n, int sign, const double *tw_re, const double *tw_im)
+{
+    if (!is_pow2(n)) return ORC_EINVAL;
+    if (n == 1) return ORC_OK;
+    double *lre = NULL, *lim = NULL;
+    if (!tw_re) {
+        lre = (double *)malloc(sizeof(double) * (size_t)(n / 2));
+        lim = (double *)malloc(sizeof(double) * (size_t)(n / 2));
+        if (!lre || !lim) { free(lre); free(lim); return ORC_ENOMEM; }
+        for (int64_t k = 0; k < n / 2; ++k) {
+            double a = 2.0 * ORC_PI * (double)k / (double)n;
+            lre[k] = cos(a); lim[k] = sin(a);
+        }
+        tw_re = lre; tw_im = lim;
+    }
+    /* bit reversal */
+    for (int64_t i = 1, j = 0; i < n; ++i) {
+        int64_t bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) {
+            double tr = x[2 * i], ti = x[2 * i + 1];
+            x[2 * i] = x[2 * j]; x[2 * i + 1] = x[2 * j + 1];
+            x[2 * j] = tr; x[2 * j + 1] = ti;
+        }
+    }
+    for (int64_t len = 2; len <= n; len <<= 1) {
+        int64_t half = len >> 1, step = n / len;
+        for (int64_t base = 0; base < n; base += len) {
+            for (int64_t j = 0; j < half; ++j) {
+                double wr = tw_re[j * step];
+                double wi = sign > 0 ? tw_im[j * step] : -tw_im[j * step];
+                int64_t a = base + j, b = a + half;
+                double br = x[2 * b] * wr - x[2 * b + 1] * wi;
+                double bi = x[2 * b] * wi + x[2 * b + 1] * wr;
+                x[2 * b] = x[2 * a] - br; x[2 * b + 1] = x[2 * a + 1] - bi;
+                x[2 * a] += br;           x[2 * a + 1] += bi;
+            }
+        }
+    }
+    free(lre); free(lim);
+    return ORC_OK;
+}
+
+/* Exported FFT (pins P1, P2). */
+int orc_fft(double *x_interleaved, int64_t n, int sign)
+{
+    if (!x_interleaved || (sign != 1 && sign != -1)) return ORC_EINVAL;
+    return fft_radix2(x_interleaved, n, sign, NULL, NULL);
+}
+
+/* ------------------------------------------------------------ waveform */
+
+/* f_ISCO = 1/(6^{3/2} pi M), M = (m1+m2) T_sun.  SURVEY.md §8(c) item 1. */
+double orc_f_isco(double m1, double m2)
+{
+    double M = (m1 + m2) * ORC_TSUN;
+    return 1.0 / (pow(6.0, 1.5) * ORC_PI * M);
+}
+
+/* 2PN stationary-phase-approximation phase, t_c = phi_c = 0
+ * (BASELINE.json configs[0], "v form"):
+ *   Psi_T(f) = -pi/4 + 3/(128 eta v^5) [ 1 + (3715/756 + 55 eta/9) v^2 - 16 pi v^3
+ *              + (15293365/508032 + 27145 eta/504 + 3085 eta^2/72) v^4 ],
+ *   v = (pi M f)^{1/3}. */
+double orc_psi(double m1, double m2, double f)
+{
+    double M = (m1 + m2) * ORC_TSUN;
+    double eta = m1 * m2 / ((m1 + m2) * (m1 + m2));
+    double v = cbrt(ORC_PI * M * f);
+    double v2 = v * v, v3 = v2 * v, v4 = v2 * v2, v5 = v4 * v;
+    double br = 1.0
+              + (3715.0 / 756.0 + 55.0 * eta / 9.0) * v2
+              - 16.0 * ORC_PI * v3
+              + (15293365.0 / 508032.0 + 27145.0 * eta / 504.0 + 3085.0 * eta * eta / 72.0) * v4;
+    return -ORC_PI / 4.0 + 3.0 / (128.0 * eta * v5) * br;
+}
+
+/* Band of a template on the DFT grid, SURVEY.md §8(c) item 2 / readings A6-A7:
+ * k_lo = ceil(f_low N/fs), k_hi = min(floor(f_ISCO N/fs), N/2-1); empty if k_hi<k_lo. */
+int orc_band(int64_t n, double fs, double f_low, double m1, double m2,
+             int64_t *k_lo, int64_t *k_hi)
+{
+    if (!is_pow2(n) || !(fs > 0) || !(f_low > 0) || !(m1 > 0) || !(m2 > 0)) return ORC_EINVAL;
+    double klo = ceil(f_low * ((double)n / fs));
+    double khi = floor(orc_f_isco(m1, m2) * ((double)n / fs));
+    if (khi > (double)(n / 2 - 1)) khi = (double)(n / 2 - 1);
+    *k_lo = (int64_t)klo; *k_hi = (int64_t)khi;
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------- context */
+
+int orc_destroy(orc_ctx *c)
+{
+    if (!c) return ORC_OK;
+    free(c->psd); free(c->dtil); free(c->tw_re); free(c->tw_im); free(c);
+    return ORC_OK;
+}
+
+int orc_create(orc_ctx **out, int64_t n, double fs_hz, double f_low_hz)
+{
+    if (!out) return ORC_EINVAL;
+    *out = NULL;
+    if (!is_pow2(n) || n < 4 || n > ((int64_t)1 << 24)) return ORC_EINVAL;
+    if (!(fs_hz > 0) || !isfinite(fs_hz)) return ORC_EINVAL;
+    if (!(f_low_hz > 0) || !(f_low_hz < fs_hz / 2)) return ORC_EINVAL;
+    orc_ctx *c = (orc_ctx *)calloc(1, sizeof(orc_ctx));
+    if (!c) return ORC_ENOMEM;
+    c->n = n; c->fs = fs_hz; c->f_low = f_low_hz;
+    c->dt = 1.0 / fs_hz; c->df = fs_hz / (double)n;
+    c->tw_re = (double *)malloc(sizeof(double) * (size_t)(n / 2));
+    c->tw_im = (double *)malloc(sizeof(double) * (size_t)(n / 2));
+    if (!c->tw_re || !c->tw_im) { orc_destroy(c); return ORC_ENOMEM; }
+    for (int64_t k = 0; k < n / 2; ++k) {
+        double a = 2.0 * ORC_PI * (double)k / (double)n;
+        c->tw_re[k] = cos(a); c->tw_im[k] = sin(a);
+    }
+    *out = c;
+    return ORC_OK;
+}
+
+/* One-sided PSD S_n[0..n/2].  +inf is legal (weight 0, reading A9); an entry
+ * <= 0 or NaN inside [f_low, Nyquist) is an error.  Changing the PSD
+ * invalidates the loaded segment. */
+int orc_set_psd(orc_ctx *c, const double *psd_onesided, int64_t n_bins)
+{
+    if (!c || !psd_onesided || n_bins != c->n / 2 + 1) return ORC_EINVAL;
+    int64_t klo = (int64_t)ceil(c->f_low * ((double)c->n / c->fs));
+    for (int64_t k = klo; k < c->n / 2; ++k) {
+        double s = psd_onesided[k];
+        if (isnan(s) || !(s > 0)) return ORC_EINVAL;
+    }
+    if (!c->psd) c->psd = (double *)malloc(sizeof(double) * (size_t)n_bins);
+    if (!c->psd) return ORC_ENOMEM;
+    memcpy(c->psd, psd_onesided, sizeof(double) * (size_t)n_bins);
+    free(c->dtil); c->dtil = NULL;
+    return ORC_OK;
+}
+
+/* d~[k] = dt * sum_j d[j] e^{-2 pi i jk/n} from the float32 samples widened to
+ * double (reading A21). */
+int orc_load_segment(orc_ctx *c, const float *samples, int64_t n_samples)
+{
+    if (!c || !samples || n_samples != c->n) return ORC_EINVAL;
+    if (!c->psd) return ORC_ESTATE;
+    int64_t n = c->n;
+    for (int64_t j = 0; j < n; ++j) if (!isfinite(samples[j])) return ORC_EINVAL;
+    double *x = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    if (!x) return ORC_ENOMEM;
+    for (int64_t j = 0; j < n; ++j) { x[2 * j] = (double)samples[j]; x[2 * j + 1] = 0.0; }
+    int rc = fft_radix2(x, n, -1, c->tw_re, c->tw_im);
+    if (rc) { free(x); return rc; }
+    if (!c->dtil) c->dtil = (double *)malloc(sizeof(double) * 2 * (size_t)(n / 2 + 1));
+    if (!c->dtil) { free(x); return ORC_ENOMEM; }
+    for (int64_t k = 0; k <= n / 2; ++k) {
+        c->dtil[2 * k] = c->dt * x[2 * k];
+        c->dtil[2 * k + 1] = c->dt * x[2 * k + 1];
+    }
+    free(x);
+    return ORC_OK;
+}
+
+/* Unit-amplitude template h~[k] = f_k^{-7/6} e^{-i Psi_T(f_k)} on [k_lo,k_hi],
+ * zero elsewhere; h_out holds 2*(n/2+1) doubles.  SURVEY.md §8(c) item 3. */
+int orc_template(const orc_ctx *c, double m1, double m2, double *h_out)
+{
+    if (!c || !h_out) return ORC_EINVAL;
+    int64_t klo, khi;
+    int rc = orc_band(c->n, c->fs, c->f_low, m1, m2, &klo, &khi);
+    if (rc) return rc;
+    memset(h_out, 0, sizeof(double) * 2 * (size_t)(c->n / 2 + 1));
+    for (int64_t k = klo; k <= khi; ++k) {
+        double f = (double)k * c->df;
+        double amp = pow(f, -7.0 / 6.0);
+        double psi = orc_psi(m1, m2, f);
+        h_out[2 * k] = amp * cos(psi);
+        h_out[2 * k + 1] = -amp * sin(psi);
+    }
+    return ORC_OK;
+}
+
+/* sigma^2 = 4 df sum_{k=k_lo}^{k_hi} |h~[k]|^2 / S_n[k] = 4 df sum f_k^{-7/3}/S_n[k]
+ * (SURVEY.md §8(c) item 5), the direct sum.  0 for an empty band. */
+int orc_sigma2(const orc_ctx *c, double m1, double m2, double *sigma2_out)
+{
+    if (!c || !sigma2_out) return ORC_EINVAL;
+    if (!c->psd) return ORC_ESTATE;
+    int64_t klo, khi;
+    int rc = orc_band(c->n, c->fs, c->f_low, m1, m2, &klo, &khi);
+    if (rc) return rc;
+    double s = 0.0;
+    for (int64_t k = klo; k <= khi; ++k) {
+        double f = (double)k * c->df;
+        s += pow(f, -7.0 / 3.0) / c->psd[k];
+    }
+    *sigma2_out = 4.0 * c->df * s;
+    return ORC_OK;
+}
+
+/* z[j] = 4 df sum_{k=k_lo}^{k_hi} d~[k] h~*[k] / S_n[k] e^{+2 pi i jk/n}, j=0..n-1
+ * (item 6; circular, no samples discarded, reading A11), into z (2n doubles). */
+static int filter_z(const orc_ctx *c, double m1, double m2, double *z,
+                    int64_t *klo_out, int64_t *khi_out)
+{
+    int64_t n = c->n, klo, khi;
+    int rc = orc_band(n, c->fs, c->f_low, m1, m2, &klo, &khi);
+    if (rc) return rc;
+    *klo_out = klo; *khi_out = khi;
+    memset(z, 0, sizeof(double) * 2 * (size_t)n);
+    for (int64_t k = klo; k <= khi; ++k) {
+        double f = (double)k * c->df;
+        double amp = pow(f, -7.0 / 6.0);
+        double psi = orc_psi(m1, m2, f);
+        /* conj(h~) = amp e^{+i psi} */
+        double hr = amp * cos(psi), hi = amp * sin(psi);
+        double dr = c->dtil[2 * k], di = c->dtil[2 * k + 1];
+        double wgt = 4.0 * c->df / c->psd[k];
+        z[2 * k]     = wgt * (dr * hr - di * hi);
+        z[2 * k + 1] = wgt * (dr * hi + di * hr);
+    }
+    return fft_radix2(z, n, +1, c->tw_re, c->tw_im);
+}
+
+/* Full series for one template: rho[j] = |z[j]|/sigma (item 7); z_out may be NULL.
+ * For an empty band rho = 0, z = 0, sigma = 0. */
+int orc_snr_series(const orc_ctx *c, double m1, double m2,
+                   double *rho_out /* n */, double *z_out_or_null /* 2n */, double *sigma_out)
+{
+    if (!c || !rho_out) return ORC_EINVAL;
+    if (!c->psd || !c->dtil) return ORC_ESTATE;
+    if (!(m1 > 0) || !(m2 > 0) || !isfinite(m1) || !isfinite(m2)) return ORC_EINVAL;
+    int64_t n = c->n, klo, khi;
+    double *z = z_out_or_null ? z_out_or_null : (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    if (!z) return ORC_ENOMEM;
+    int rc = filter_z(c, m1, m2, z, &klo, &khi);
+    double s2 = 0.0;
+    if (!rc) rc = orc_sigma2(c, m1, m2, &s2);
+    if (!rc) {
+        double sigma = (khi >= klo) ? sqrt(s2) : 0.0;
+        if (sigma_out) *sigma_out = sigma;
+        for (int64_t j = 0; j < n; ++j) {
+            double re = z[2 * j], im = z[2 * j + 1];
+            rho_out[j] = sigma > 0 ? sqrt(re * re + im * im) / sigma : 0.0;
+        }
+    }
+    if (!z_out_or_null) free(z);
+    return rc;
+}
+
+/* One template: peak (item 7) and raw triggers rho[j] > thr (strict, item 8).
+ * trig may be NULL (count only).  Returns the count via *n_found. */
+static int filter_one(const orc_ctx *c, double m1, double m2, double thr, int64_t tidx,
+                      double *z, double *rho, orc_peak *peak,
+                      orc_trigger **trig, int64_t *n_found)
+{
+    int64_t n = c->n;
+    double sigma = 0.0;
+    int rc = orc_snr_series(c, m1, m2, rho, z, &sigma);
+    if (rc) return rc;
+    *n_found = 0; *trig = NULL;
+    if (!(sigma > 0)) {            /* empty band: SURVEY.md §8(b) */
+        peak->snr_max = 0.0; peak->idx_peak = -1; peak->phase = 0.0; peak->sigma = 0.0;
+        return ORC_OK;
+    }
+    int64_t jbest = 0; double best = rho[0]; int64_t cnt = 0;
+    for (int64_t j = 0; j < n; ++j) {
+        if (rho[j] > best) { best = rho[j]; jbest = j; }   /* smallest j attaining the max */
+        if (rho[j] > thr) ++cnt;
+    }
+    peak->snr_max = best; peak->idx_peak = jbest; peak->sigma = sigma;
+    peak->phase = atan2(z[2 * jbest + 1], z[2 * jbest]);
+    if (cnt) {
+        orc_trigger *t = (orc_trigger *)malloc(sizeof(orc_trigger) * (size_t)cnt);
+        if (!t) return ORC_ENOMEM;
+        int64_t m = 0;
+        for (int64_t j = 0; j < n; ++j) if (rho[j] > thr) {
+            t[m].template_idx = tidx; t[m].sample_idx = j; t[m].snr = rho[j];
+            t[m].phase = atan2(z[2 * j + 1], z[2 * j]); ++m;
+        }
+        *trig = t; *n_found = cnt;
+    }
+    return ORC_OK;
+}
+
+/* The bank loop of PAPER.md:98-102.  bank = n_templates pairs (m1,m2) in solar
+ * masses.  Triggers sorted by (template, sample); list truncated at capacity
+ * (rc = ORC_WTRUNC) but *n_trig_found is always the full count. */
+int orc_filter_bank(const orc_ctx *c, const double *bank_m1m2, int64_t n_templates,
+                    double snr_threshold, orc_peak *peaks_out,
+                    orc_trigger *trig_out, int64_t trig_capacity, int64_t *n_trig_found)
+{
+    if (!c || (!bank_m1m2 && n_templates) || n_templates < 0 || (!peaks_out && n_templates))
+        return ORC_EINVAL;
+    if (!(snr_threshold >= 0)) return ORC_EINVAL;
+    if (!c->psd || !c->dtil) return ORC_ESTATE;
+    for (int64_t t = 0; t < n_templates; ++t) {
+        double m1 = bank_m1m2[2 * t], m2 = bank_m1m2[2 * t + 1];
+        if (!(m1 > 0) || !(m2 > 0) || !isfinite(m1) || !isfinite(m2)) return ORC_EINVAL;
+    }
+    int64_t n = c->n;
+    orc_trigger **lists = (orc_trigger **)calloc((size_t)(n_templates ? n_templates : 1), sizeof(*lists));
+    int64_t *counts = (int64_t *)calloc((size_t)(n_templates ? n_templates : 1), sizeof(*counts));
+    if (!lists || !counts) { free(lists); free(counts); return ORC_ENOMEM; }
+    int err = ORC_OK;
+#pragma omp parallel
+    {
+        double *z = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+        double *rho = (double *)malloc(sizeof(double) * (size_t)n);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t t = 0; t < n_templates; ++t) {
+            int rc = (z && rho) ? filter_one(c, bank_m1m2[2 * t], bank_m1m2[2 * t + 1],
+                                             snr_threshold, t, z, rho, &peaks_out[t],
+                                             &lists[t], &counts[t])
+                                : ORC_ENOMEM;
+            if (rc) {
+#pragma omp critical
+                err = rc;
+            }
+        }
+        free(z); free(rho);
+    }
+    int64_t total = 0, written = 0;
+    for (int64_t t = 0; t < n_templates; ++t) {
+        for (int64_t m = 0; m < counts[t]; ++m) {
+            if (trig_out && written < trig_capacity) trig_out[written++] = lists[t][m];
+        }
+        total += counts[t];
+        free(lists[t]);
+    }
+    free(lists); free(counts);
+    if (n_trig_found) *n_trig_found = total;
+    if (err) return err;
+    return (total > written && trig_out) ? ORC_WTRUNC : ORC_OK;
+}
+
+/* Threads orc_filter_bank will use (for bench.py's cpu_baseline "cores"). */
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}

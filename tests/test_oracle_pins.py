@@ -1,0 +1,491 @@
+"""Pins for the CPU oracle (oracle/mf_oracle.c): what the paper and the mathematics fix.
+
+No test here compares the oracle with itself or with the CUDA path.  The pins are P1-P13 of
+SURVEY.md §8(c): brute-force DFT, Parseval, quoted 40-digit phase values, the textbook
+chirp-time expansion, closed forms of the normalisation (noise-free injection recovers its
+optimal SNR at t_c with phase phi_c; self-match = 1), adaptive quadrature of sigma^2, noise
+statistics, covariances, Cauchy-Schwarz, the prefix-sum identity, and an O(N n_b) brute-force
+evaluation of the filter definition (eq. 2.1).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1006_4644_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _survey_values():
+    out = {}
+    for line in open(os.path.join(GOLD, "survey_values.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = float(line[1])
+    return out
+
+
+SV = _survey_values()
+
+
+def _direct_dft(x, sign):
+    n = x.size
+    jk = np.outer(np.arange(n), np.arange(n)) % n
+    return (np.exp(sign * 2j * np.pi * jk / n) * x[None, :]).sum(axis=1)
+
+
+# ------------------------------------------------------------------ P1, P2: the FFT
+
+@pytest.mark.parametrize("n", [2, 4, 8, 16, 32, 64, 128, 256])
+def test_p1_fft_equals_direct_dft(n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    for sign in (-1, +1):
+        got = oracle.fft(x, sign)
+        ref = _direct_dft(x, sign)
+        assert np.max(np.abs(got - ref)) < 1e-12 * np.linalg.norm(x) * np.sqrt(n)
+
+
+def test_p1_fft_roundtrip_delta_linearity():
+    n = 4096
+    rng = np.random.default_rng(0)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    y = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    assert np.allclose(oracle.fft(oracle.fft(x, -1), +1), n * x, rtol=0, atol=1e-9)
+    j0 = 37
+    d = np.zeros(n, complex)
+    d[j0] = 1.0
+    k = np.arange(n)
+    assert np.allclose(oracle.fft(d, -1), np.exp(-2j * np.pi * k * j0 / n), atol=1e-12)
+    assert np.allclose(oracle.fft(d, +1), np.exp(+2j * np.pi * k * j0 / n), atol=1e-12)
+    a, b = 0.3 - 1.1j, 2.0 + 0.5j
+    assert np.allclose(oracle.fft(a * x + b * y, -1), a * oracle.fft(x, -1) + b * oracle.fft(y, -1), atol=1e-9)
+
+
+def test_p1_fft_rejects_non_power_of_two():
+    with pytest.raises(oracle.OracleError):
+        oracle.fft(np.zeros(12, complex), -1)
+
+
+def test_p2_parseval():
+    n = 1 << 14
+    rng = np.random.default_rng(1)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    X = oracle.fft(x, -1)
+    assert abs(np.sum(np.abs(x) ** 2) - np.sum(np.abs(X) ** 2) / n) < 1e-12 * np.sum(np.abs(x) ** 2)
+
+
+# ------------------------------------------------------------------ P3, P4, P5: the phase
+
+def _psi_rows():
+    rows = []
+    for line in open(os.path.join(GOLD, "psi_values.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 4:
+            rows.append(tuple(float(v) for v in line))
+    return rows
+
+
+@pytest.mark.parametrize("m1,m2,f,want", _psi_rows())
+def test_p3_psi_quoted_values(m1, m2, f, want):
+    assert oracle.psi(m1, m2, f) == pytest.approx(want, rel=2e-13, abs=1e-11)
+
+
+def test_p3_brackets_at_eta_quarter():
+    # recover the 1PN and 2PN brackets from the oracle's Psi by solving for them at three v
+    # (eta = 1/4): Psi + pi/4 = 3/(32 v^5) [1 + B1 v^2 - 16 pi v^3 + B2 v^4]
+    m = 1.4
+    M = 2 * m * W.T_SUN_S
+    vs = np.array([0.10, 0.16, 0.22])
+    fs_ = vs ** 3 / (np.pi * M)
+    lhs = np.array([(oracle.psi(m, m, f) + np.pi / 4) * 32 * v ** 5 / 3 - 1 + 16 * np.pi * v ** 3
+                    for f, v in zip(fs_, vs)])
+    A = np.stack([vs ** 2, vs ** 4], axis=1)
+    b1, b2 = np.linalg.lstsq(A, lhs, rcond=None)[0]
+    assert b1 == pytest.approx(SV["bracket_1pn_eta_quarter"], rel=1e-8)
+    assert b2 == pytest.approx(SV["bracket_2pn_eta_quarter"], rel=1e-7)
+
+
+def test_p4_scaling_law_and_symmetry():
+    # Psi_T(f; lam m1, lam m2) = Psi_T(lam f; m1, m2); symmetric in m1 <-> m2
+    for (m1, m2, f, lam) in [(1.0, 1.0, 100.0, 10.0), (1.4, 2.3, 57.0, 3.5), (2.0, 9.0, 31.0, 0.37)]:
+        assert oracle.psi(lam * m1, lam * m2, f) == pytest.approx(oracle.psi(m1, m2, lam * f), rel=1e-13)
+        assert oracle.psi(m1, m2, f) == oracle.psi(m2, m1, f) or \
+            oracle.psi(m1, m2, f) == pytest.approx(oracle.psi(m2, m1, f), rel=1e-15)
+
+
+def _chirp_time_textbook(m1, m2, f):
+    """Chirp times tau0 + tau1 - tau1.5 + tau2 of the 2PN inspiral (the published
+    "chirp time" parametrisation of the restricted 2PN waveform), a different set of rational
+    coefficients from those of the phase: 743/336, 11/4, 3058673/1016064, 5429/1008, 617/144."""
+    M = (m1 + m2) * W.T_SUN_S
+    eta = m1 * m2 / (m1 + m2) ** 2
+    x = np.pi * M * f
+    t0 = 5.0 / (256.0 * np.pi * f * eta) * x ** (-5.0 / 3.0)
+    t1 = 5.0 / (192.0 * np.pi * f * eta) * (743.0 / 336.0 + 11.0 * eta / 4.0) / x
+    t15 = 1.0 / (8.0 * f * eta) * x ** (-2.0 / 3.0)
+    t2 = 5.0 / (128.0 * np.pi * f * eta) * (3058673.0 / 1016064.0 + 5429.0 * eta / 1008.0
+                                           + 617.0 * eta ** 2 / 144.0) * x ** (-1.0 / 3.0)
+    return t0, t0 + t1 - t15 + t2
+
+
+@pytest.mark.parametrize("m1,m2,f,key", [(1.4, 1.4, 40.0, "chirp_s_1p4_40hz"), (1.0, 1.0, 40.0, "chirp_s_1_1_40hz"),
+                                        (3.0, 3.0, 40.0, "chirp_s_3_3_40hz"), (10.0, 10.0, 40.0, "chirp_s_10_10_40hz"),
+                                        (1.4, 1.4, 10.0, "chirp_s_1p4_10hz")])
+def test_p5_stationary_phase_time_equals_chirp_time(m1, m2, f, key):
+    # stationary phase: the time before coalescence at which the chirp passes f is
+    # tau(f) = -(1/2pi) dPsi/df.  Central difference of the oracle's Psi vs the textbook series.
+    h = f * 1e-4
+    tau = -(oracle.psi(m1, m2, f + h) - oracle.psi(m1, m2, f - h)) / (2 * h) / (2 * np.pi)
+    t0, tsum = _chirp_time_textbook(m1, m2, f)
+    assert tau == pytest.approx(tsum, rel=1e-7)
+    assert tau == pytest.approx(SV[key], rel=2e-3)          # value printed in SURVEY.md P5
+    if key == "chirp_s_1p4_40hz":
+        assert t0 == pytest.approx(SV["chirp_newt_s_1p4_40hz"], rel=1e-3)
+
+
+def test_p5_sign_convention_chirp_sweeps_up_and_ends_at_tc():
+    # Reading A3: h~ ~ e^{-i Psi} with the forward transform e^{-2 pi i f t} gives a chirp whose
+    # frequency RISES with time and whose energy ends at t_c = 0 (mod T).
+    n, fs, f_low = 1 << 16, 2048.0, 40.0
+    o = oracle.Oracle(n, fs, f_low)
+    h = o.template(3.0, 3.0)                       # 7.1 s long from 40 Hz, fits the 32 s segment
+    full = np.zeros(n, complex)
+    full[: n // 2 + 1] = h
+    ht = oracle.fft(full, +1)                      # analytic signal h(t) + i H[h](t), t_c at j = 0 = n
+    p = np.abs(ht) ** 2
+    one_s = int(fs)
+    assert p[-one_s:].sum() > 50 * p[:one_s].sum()            # energy just before t_c, none after
+    assert p[-8 * one_s:].sum() > 0.97 * p.sum()
+    # instantaneous frequency from the phase increments, 6 s and 0.05 s before coalescence
+    def inst_f(j0):
+        seg = ht[j0: j0 + 64]
+        return np.angle(seg[1:] * np.conj(seg[:-1])).mean() * fs / (2 * np.pi)
+    f_early, f_late = inst_f(n - 6 * one_s), inst_f(n - int(0.05 * fs))
+    assert 40.0 < f_early < 50.0 and f_late > 150.0 and f_late > f_early
+    # and the early frequency is the one the chirp-time series predicts at tau = 6 s
+    lo, hi = 40.0, 60.0
+    for _ in range(60):
+        mid = 0.5 * (lo + hi)
+        lo, hi = (mid, hi) if _chirp_time_textbook(3.0, 3.0, mid)[1] > 6.0 - 32 / fs else (lo, mid)
+    assert f_early == pytest.approx(lo, rel=5e-3)
+
+
+# ------------------------------------------------------------------ band, f_ISCO, sigma
+
+def test_band_edges_and_fisco_quoted_values():
+    assert oracle.f_isco(1.0, 1.0) * 2.0 == pytest.approx(SV["f_isco_times_mtot_hz"], rel=1e-8)
+    assert oracle.f_isco(3.0, 7.0) * 10.0 == pytest.approx(SV["f_isco_times_mtot_hz"], rel=1e-8)
+    assert oracle.band(1 << 16, 2048.0, 40.0, 1.4, 1.4)[0] == SV["k_lo_cfg0"]
+    assert oracle.band(1 << 20, 4096.0, 40.0, 1.4, 1.4)[0] == SV["k_lo_cfg1"]
+    assert oracle.band(1 << 22, 4096.0, 10.0, 1.4, 1.4)[0] == SV["k_lo_cfg1"]
+    # Nyquist cap (A7): a light system at fs = 2048 is cut at N/2 - 1, never at N/2
+    assert oracle.band(1 << 16, 2048.0, 40.0, 1.0, 1.0)[1] == (1 << 15) - 1
+    # ISCO cut: floor(f_ISCO / df), inclusive
+    klo, khi = oracle.band(1 << 16, 2048.0, 40.0, 10.0, 10.0)
+    df = 2048.0 / (1 << 16)
+    assert khi * df <= oracle.f_isco(10, 10) < (khi + 1) * df
+    # empty band: f_ISCO <= f_low
+    klo, khi = oracle.band(1 << 12, 2048.0, 40.0, 60.0, 60.0)
+    assert khi < klo
+
+
+@pytest.mark.parametrize("log2n,fs,f_low,kind,key,tol", [
+    (16, 2048.0, 40.0, "A", "sigma_1p4_cfg0", 3e-6), (20, 4096.0, 40.0, "A", "sigma_1p4_cfg1", 3e-6),
+    (22, 4096.0, 10.0, "B", "sigma_1p4_cfg3", 3e-6)])
+def test_sigma_quoted_values(log2n, fs, f_low, kind, key, tol):
+    n = 1 << log2n
+    o = oracle.Oracle(n, fs, f_low)
+    o.set_psd(W.onesided_psd(kind, n, fs, f_low))
+    assert np.sqrt(o.sigma2(1.4, 1.4)) == pytest.approx(SV[key], rel=tol)
+
+
+@pytest.mark.parametrize("log2n,fs,f_low,kind,tol", [(16, 2048.0, 40.0, "A", 3e-5), (20, 4096.0, 40.0, "A", 4e-6)])
+def test_p7_sigma_vs_adaptive_quadrature(log2n, fs, f_low, kind, tol):
+    from scipy.integrate import quad
+    n = 1 << log2n
+    o = oracle.Oracle(n, fs, f_low)
+    o.set_psd(W.onesided_psd(kind, n, fs, f_low))
+    m1, m2 = 1.4, 1.4
+    klo, khi = oracle.band(n, fs, f_low, m1, m2)
+    df = fs / n
+    # the rectangle rule over bins [klo, khi] is the midpoint rule on [ (klo-1/2) df, (khi+1/2) df ]
+    a, b = (klo - 0.5) * df, (khi + 0.5) * df
+    val, _ = quad(lambda f: 4.0 * f ** (-7.0 / 3.0) / W.psd_A(f), a, b, epsabs=0, epsrel=1e-12, limit=400)
+    assert o.sigma2(m1, m2) == pytest.approx(val, rel=tol)
+
+
+def test_p11_prefix_table_equals_direct_sum():
+    n, fs, f_low = 1 << 16, 2048.0, 40.0
+    psd = W.onesided_psd("A", n, fs, f_low)
+    o = oracle.Oracle(n, fs, f_low)
+    o.set_psd(psd)
+    df = fs / n
+    k = np.arange(n // 2 + 1)
+    with np.errstate(divide="ignore"):
+        term = np.where(k >= 1280, (np.maximum(k, 1) * df) ** (-7.0 / 3.0) / psd, 0.0)
+    P = 4.0 * df * np.cumsum(term)
+    for m1, m2 in [(1.4, 1.4), (1.0, 1.0), (3.0, 9.0), (10.0, 10.0), (2.2, 1.1)]:
+        khi = oracle.band(n, fs, f_low, m1, m2)[1]
+        assert o.sigma2(m1, m2) == pytest.approx(P[khi], rel=1e-13)
+
+
+# ------------------------------------------------------------------ P6: closed forms
+
+def _oracle_for(w):
+    o = oracle.Oracle(w.n, w.fs, w.f_low)
+    o.set_psd(w.psd)
+    o.load_segment(w.samples)
+    return o
+
+
+def test_p6_noise_free_injection_recovers_snr_time_phase():
+    w = W.config0(noise=False)
+    o = _oracle_for(w)
+    pk, trig, nf, rc = o.filter_bank(w.bank, w.threshold)
+    inj = w.injections[0]
+    p = pk[inj.template_idx]
+    # samples are rounded to float32 (A21): 6e-8 per sample, ~1e-9 on the peak
+    assert p["snr_max"] == pytest.approx(inj.snr, rel=1e-8)
+    assert p["idx_peak"] == inj.sample(w.fs) == 40960
+    assert p["phase"] == pytest.approx(inj.phi_c, abs=1e-8)
+    assert p["sigma"] == pytest.approx(SV["sigma_1p4_cfg0"], rel=3e-6)
+    # P10 Cauchy-Schwarz: no other template reaches the exact one
+    others = np.delete(pk["snr_max"], inj.template_idx)
+    assert np.all(others < inj.snr * (1 - 1e-6))
+
+
+def test_p6_normalised_self_match_is_one():
+    n, fs, f_low = 1 << 14, 2048.0, 40.0
+    psd = W.onesided_psd("A", n, fs, f_low)
+    o = oracle.Oracle(n, fs, f_low)
+    o.set_psd(psd)
+    m1, m2 = 2.0, 1.3
+    h = o.template(m1, m2)
+    sigma = np.sqrt(o.sigma2(m1, m2))
+    shift = 5000
+    k = np.arange(n // 2 + 1)
+    d = W.to_time_domain(h / sigma * np.exp(-2j * np.pi * k * shift / n) * np.exp(1j * 1.1), n, fs)
+    o.load_segment(d)
+    pk, *_ = o.filter_bank(np.array([[m1, m2]]), 6.0)
+    assert pk[0]["snr_max"] == pytest.approx(1.0, rel=1e-7)
+    assert pk[0]["idx_peak"] == shift
+    assert pk[0]["phase"] == pytest.approx(1.1, abs=1e-7)
+
+
+def test_p13_bruteforce_definition():
+    # direct O(N n_b) evaluation of z[j] = 4 df sum_k d~[k] h~*[k]/S_n[k] e^{+2 pi i jk/N}
+    # with d~ from a direct DFT (no FFT anywhere), vs the oracle's FFT route
+    w = W.small_case(log2n=10, fs=1024.0, f_low=40.0, n_templates=3, seed=5)
+    n, df, dt = w.n, w.fs / w.n, 1.0 / w.fs
+    o = _oracle_for(w)
+    j = np.arange(n)
+    for (m1, m2) in w.bank:
+        klo, khi = oracle.band(n, w.fs, w.f_low, m1, m2)
+        k = np.arange(klo, khi + 1)
+        dtil = dt * (w.samples.astype(np.float64)[None, :] * np.exp(-2j * np.pi * np.outer(k, j) / n)).sum(axis=1)
+        f = k * df
+        hconj = f ** (-7.0 / 6.0) * np.exp(1j * np.array([oracle.psi(m1, m2, x) for x in f]))
+        q = 4.0 * df * dtil * hconj / w.psd[k]
+        z_ref = (q[None, :] * np.exp(2j * np.pi * np.outer(j, k) / n)).sum(axis=1)
+        sigma_ref = np.sqrt(4.0 * df * np.sum(f ** (-7.0 / 3.0) / w.psd[k]))
+        rho, z, sigma = o.snr_series(m1, m2)
+        assert sigma == pytest.approx(sigma_ref, rel=1e-13)
+        assert np.max(np.abs(z - z_ref)) < 1e-11 * np.max(np.abs(z_ref))
+        assert np.max(np.abs(rho - np.abs(z_ref) / sigma_ref)) < 1e-10
+
+
+# ------------------------------------------------------------------ P8: noise statistics
+
+def test_p8_pure_noise_statistics():
+    w = W.sweep_point(16, 4)            # noise only, N = 2^16
+    o = _oracle_for(w)
+    m2s, var_re, var_im, tail = [], [], [], []
+    for (m1, m2) in w.bank:
+        rho, z, sigma = o.snr_series(m1, m2)
+        m2s.append(np.mean(rho ** 2))
+        var_re.append(np.var(z.real / sigma))
+        var_im.append(np.var(z.imag / sigma))
+        tail.append(np.mean(rho > 2.5))
+    assert np.mean(m2s) == pytest.approx(2.0, rel=0.03)        # <rho^2> = 2 (A4)
+    assert np.mean(var_re) == pytest.approx(1.0, rel=0.04)
+    assert np.mean(var_im) == pytest.approx(1.0, rel=0.04)
+    assert np.mean(tail) == pytest.approx(np.exp(-2.5 ** 2 / 2), rel=0.15)   # Rayleigh tail
+
+
+# ------------------------------------------------------------------ P9: covariances
+
+def test_p9_linearity_shift_phase_scale():
+    w = W.small_case(log2n=13, n_templates=3, seed=21)
+    n = w.n
+    m1, m2 = w.bank[1]
+    o = _oracle_for(w)
+    rho, z, sigma = o.snr_series(m1, m2)
+    # circular shift of the data by s samples shifts the output by s
+    s = 1234
+    o.load_segment(np.roll(w.samples, s))
+    rho_s, z_s, _ = o.snr_series(m1, m2)
+    assert np.max(np.abs(np.roll(z, s) - z_s)) < 1e-12 * np.max(np.abs(z))
+    # d -> a d scales rho by |a|
+    o.load_segment((w.samples * np.float32(2.0)))
+    rho_a, *_ = o.snr_series(m1, m2)
+    assert np.allclose(rho_a, 2.0 * rho, rtol=1e-12)
+    # S_n -> c S_n (data fixed) scales rho by 1/sqrt(c); sigma by 1/sqrt(c)
+    o.set_psd(4.0 * w.psd)
+    o.load_segment(w.samples)
+    rho_c, _, sigma_c = o.snr_series(m1, m2)
+    assert np.allclose(rho_c, rho / 2.0, rtol=1e-12) and sigma_c == pytest.approx(sigma / 2.0, rel=1e-13)
+    # linearity in the data: z(a + b) = z(a) + z(b)
+    o.set_psd(w.psd)
+    a = w.samples.copy()
+    b = np.roll(w.samples, 77) * np.float32(0.5)
+    o.load_segment(a)
+    za = o.snr_series(m1, m2)[1]
+    o.load_segment(b)
+    zb = o.snr_series(m1, m2)[1]
+    ab = a.astype(np.float64) + b.astype(np.float64)
+    o.load_segment(ab.astype(np.float32))
+    zab = o.snr_series(m1, m2)[1]
+    assert np.max(np.abs(zab - (za + zb))) < 1e-6 * np.max(np.abs(za))   # float32 rounding of a+b
+
+
+def test_p9_coalescence_phase_rotates_z():
+    n, fs, f_low = 1 << 13, 2048.0, 40.0
+    psd = W.onesided_psd("A", n, fs, f_low)
+    m1, m2 = 1.7, 2.4
+    outs = []
+    for phi in (0.0, 0.9):
+        spec = W.source_spectrum(n, fs, f_low, psd, m1, m2, 2.0, phi, 10.0)
+        o = oracle.Oracle(n, fs, f_low)
+        o.set_psd(psd)
+        o.load_segment(W.to_time_domain(spec, n, fs))
+        outs.append(o.snr_series(m1, m2))
+    (rho0, z0, _), (rho1, z1, _) = outs
+    assert np.max(np.abs(rho0 - rho1)) < 1e-6 * rho0.max()
+    j = int(np.argmax(rho0))
+    assert np.angle(z1[j] / z0[j]) == pytest.approx(0.9, abs=1e-6)
+
+
+# ------------------------------------------------------------------ P12: injections in noise
+
+def test_p12_injection_in_noise_cfg0():
+    w = W.config0()
+    o = _oracle_for(w)
+    inj = w.injections[0]
+    pk, trig, nf, rc = o.filter_bank(w.bank, w.threshold)
+    p = pk[inj.template_idx]
+    assert abs(p["snr_max"] - inj.snr) < 3.0
+    assert abs(p["idx_peak"] - inj.sample(w.fs)) <= 2
+    # the exact template is the loudest of the bank
+    assert int(np.argmax(pk["snr_max"])) == inj.template_idx
+    # linearity: z(noise + signal) - z(noise) = z(signal)
+    z_ns = o.snr_series(inj.m1, inj.m2)[1]
+    w_s = W.config0(noise=False)
+    o.load_segment(w_s.samples)
+    z_s = o.snr_series(inj.m1, inj.m2)[1]
+    noise_only = (w.samples.astype(np.float64) - w_s.samples.astype(np.float64)).astype(np.float32)
+    o.load_segment(noise_only)
+    z_n = o.snr_series(inj.m1, inj.m2)[1]
+    assert np.max(np.abs(z_ns - z_n - z_s)) < 1e-5 * np.max(np.abs(z_s))   # float32 sample rounding
+
+
+# ------------------------------------------------------------------ peaks and triggers
+
+def test_triggers_are_exactly_the_samples_above_threshold():
+    w = W.config0()
+    o = _oracle_for(w)
+    thr = 5.0
+    pk, trig, nf, rc = o.filter_bank(w.bank, thr)
+    assert rc == oracle.OK and nf == len(trig) and nf > 20
+    keys = list(zip(trig["template_idx"], trig["sample_idx"]))
+    assert keys == sorted(keys)                                # sorted by (template, sample)
+    want = []
+    for t, (m1, m2) in enumerate(w.bank):
+        rho, z, _ = o.snr_series(m1, m2)
+        js = np.nonzero(rho > thr)[0]
+        want += [(t, int(j)) for j in js]
+        assert pk[t]["idx_peak"] == int(np.argmax(rho)) and pk[t]["snr_max"] == rho.max()
+        assert pk[t]["phase"] == pytest.approx(np.angle(z[int(np.argmax(rho))]), abs=1e-14)
+        sel = trig[trig["template_idx"] == t]
+        assert np.array_equal(sel["snr"], rho[js]) and np.allclose(sel["phase"], np.angle(z[js]), atol=1e-15)
+    assert keys == want
+    # strict '>' (A14): a threshold equal to a trigger's own SNR drops it
+    snr0 = float(trig["snr"].max())
+    _, trig2, nf2, _ = o.filter_bank(w.bank, snr0)
+    assert nf2 == 0
+    # capacity: list truncated, full count still returned, warning code
+    _, trig3, nf3, rc3 = o.filter_bank(w.bank, thr, trig_capacity=7)
+    assert rc3 == oracle.WTRUNC and nf3 == nf and len(trig3) == 7
+    assert list(zip(trig3["template_idx"], trig3["sample_idx"])) == keys[:7]
+
+
+def test_peak_tie_takes_lowest_index():
+    # a periodic input makes the output periodic: the maximum is attained (at least) twice, to
+    # within rounding; construct an exact tie instead with all-zero data
+    n, fs, f_low = 1 << 10, 1024.0, 40.0
+    o = oracle.Oracle(n, fs, f_low)
+    o.set_psd(W.onesided_psd("A", n, fs, f_low))
+    o.load_segment(np.zeros(n, np.float32))
+    pk, trig, nf, rc = o.filter_bank(np.array([[1.4, 1.4]]), 6.0)
+    assert pk[0]["snr_max"] == 0.0 and pk[0]["idx_peak"] == 0 and nf == 0
+
+
+def test_empty_band_template_and_errors():
+    w = W.small_case(log2n=12, n_templates=4, seed=3)
+    o = oracle.Oracle(w.n, w.fs, w.f_low)
+    with pytest.raises(oracle.OracleError) as e:      # segment before PSD
+        o.load_segment(w.samples)
+    assert e.value.rc == oracle.ESTATE
+    o.set_psd(w.psd)
+    with pytest.raises(oracle.OracleError) as e:      # filter before segment
+        o.filter_bank(w.bank, 6.0)
+    assert e.value.rc == oracle.ESTATE
+    o.load_segment(w.samples)
+    bank = np.vstack([w.bank, [[60.0, 60.0]]])          # f_ISCO = 36.6 Hz < f_low: empty band
+    pk, trig, nf, rc = o.filter_bank(bank, 6.0)
+    assert tuple(pk[-1]) == (0.0, -1, 0.0, 0.0)
+    for bad in ([[0.0, 1.0]], [[1.0, -2.0]], [[np.nan, 1.0]], [[np.inf, 1.0]]):
+        with pytest.raises(oracle.OracleError) as e:
+            o.filter_bank(np.array(bad), 6.0)
+        assert e.value.rc == oracle.EINVAL
+    with pytest.raises(oracle.OracleError):
+        o.filter_bank(w.bank, -1.0)
+    bad_psd = w.psd.copy()
+    bad_psd[w.n // 4] = 0.0
+    with pytest.raises(oracle.OracleError):
+        o.set_psd(bad_psd)
+    bad_psd[w.n // 4] = np.nan
+    with pytest.raises(oracle.OracleError):
+        o.set_psd(bad_psd)
+    s = w.samples.copy()
+    s[5] = np.inf
+    with pytest.raises(oracle.OracleError):
+        o.load_segment(s)
+    with pytest.raises(oracle.OracleError):
+        oracle.Oracle(1000, 2048.0, 40.0)
+    with pytest.raises(oracle.OracleError):
+        oracle.Oracle(1024, 2048.0, 2000.0)
+    # changing the PSD invalidates the segment
+    o.set_psd(w.psd)
+    with pytest.raises(oracle.OracleError) as e:
+        o.filter_bank(w.bank, 6.0)
+    assert e.value.rc == oracle.ESTATE
+
+
+def test_psd_infinite_weight_zero():
+    # A9: +inf PSD bins carry weight 0 -- making some in-band bins infinite must equal removing them
+    w = W.small_case(log2n=12, n_templates=2, seed=8)
+    psd = w.psd.copy()
+    psd[300:340] = np.inf
+    o = oracle.Oracle(w.n, w.fs, w.f_low)
+    o.set_psd(psd)
+    o.load_segment(w.samples)
+    m1, m2 = w.bank[0]
+    rho, z, sigma = o.snr_series(m1, m2)
+    klo, khi = oracle.band(w.n, w.fs, w.f_low, m1, m2)
+    k = np.array([kk for kk in range(klo, khi + 1) if not 300 <= kk < 340])
+    df = w.fs / w.n
+    assert sigma ** 2 == pytest.approx(4 * df * np.sum((k * df) ** (-7 / 3) / psd[k]), rel=1e-13)
+    assert np.all(np.isfinite(rho))
