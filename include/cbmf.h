@@ -1,0 +1,151 @@
+/*
+ * cbmf.h -- C ABI of the B200-native coalescing-binary matched filter
+ *           (hot path of "cuInspiral", arXiv 1006.4644).
+ *
+ * The library matched-filters ONE detector data segment against a bank of 2PN
+ * stationary-phase chirp templates (eq. 2.1; the per-chunk loop of
+ * PAPER.md:96-103).  For every template it generates h~(f) on the fly, forms
+ * d~ h~* / S_n, runs an N-point inverse FFT to the two-quadrature output z(t),
+ * normalises by sigma and reduces |z| to the peak SNR, its sample index, the
+ * coalescence phase and the list of samples above threshold.  Every step runs in
+ * hand-written sm_100a kernels; the host code below this ABI only validates
+ * arguments, allocates device memory and launches.  There is no CPU fallback.
+ *
+ * Conventions (readings A1-A21):
+ *   N samples, fs, dt = 1/fs, df = fs/N, f_k = k df.
+ *   forward transform  d~[k] = dt sum_j d[j] e^{-2 pi i jk/N}
+ *   template           h~[k] = f_k^{-7/6} e^{-i Psi_T(f_k)},  k_lo <= k <= k_hi, else 0
+ *                      k_lo = ceil(f_low/df), k_hi = min(floor(f_ISCO/df), N/2-1)
+ *   Psi_T              2PN SPA phase of BASELINE.json configs[0] with t_c = phi_c = 0
+ *   sigma^2            4 df sum_k |h~[k]|^2 / S_n[k]            (one-sided S_n)
+ *   z[j]               4 df sum_k d~[k] h~*[k] / S_n[k] e^{+2 pi i jk/N}, j = 0..N-1, circular
+ *   rho[j]             |z[j]| / sigma     (= sqrt(c_+^2 + c_x^2))
+ *   peak               smallest j attaining max rho; phase = atan2(Im z, Re z) in (-pi, pi]
+ *   trigger            every j with rho[j] > threshold (strict)
+ *
+ * Return codes: 0 success, < 0 error, > 0 warning.  All pointers are HOST pointers
+ * unless the function name ends in _dev, in which case every array pointer is a
+ * DEVICE pointer on the context's device (scalars stay host values).  The caller
+ * owns every array; the context owns all of its device memory.  Every call is
+ * synchronous with respect to the context's stream: results are complete on return.
+ * A context is not thread-safe; contexts are independent.
+ */
+#ifndef CBMF_H
+#define CBMF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CBMF_OK        0
+#define CBMF_EINVAL   -1   /* bad argument (see each call) */
+#define CBMF_ESTATE   -2   /* call order: PSD, then segment, then filter */
+#define CBMF_ECUDA    -3   /* a CUDA runtime call failed; cbmf_last_cuda_error() names it */
+#define CBMF_ENOMEM   -4   /* host or device allocation failed */
+#define CBMF_WTRUNC    1   /* more triggers found than trig_capacity: list truncated */
+
+typedef struct cbmf_ctx cbmf_ctx;                 /* opaque */
+
+/* One template = one point (m1, m2) of the bank, solar masses, both > 0 and finite
+ * ("(m1,m2)_i").  Layout: two consecutive doubles. */
+typedef struct { double m1, m2; } cbmf_template;
+
+/* Per-template result (candidate time and c(t_0) = SNR).
+ * idx_peak counts samples from segment start (t_peak = idx_peak / fs).  A template whose
+ * band is empty (f_ISCO < f_low) returns {0, -1, 0, 0}. */
+typedef struct { float snr_max; int32_t idx_peak; float phase; float sigma; } cbmf_peak;
+
+/* One above-threshold sample (PAPER.md:102, :131 device_maxfind). */
+typedef struct { int32_t template_idx; int32_t sample_idx; float snr; float phase; } cbmf_trigger;
+
+/* Create a context for segments of n samples (n a power of two, 2^12 <= n <= 2^24) at
+ * sample rate fs_hz, with lower cutoff f_low_hz (0 < f_low < fs/2), on CUDA device
+ * `device`.  cuda_stream is a cudaStream_t (e.g. torch's current stream) or NULL for the
+ * default stream.  Errors: EINVAL, ECUDA, ENOMEM. */
+int cbmf_create(cbmf_ctx **out, int device, int64_t n, double fs_hz, double f_low_hz,
+                void *cuda_stream);
+int cbmf_destroy(cbmf_ctx *ctx);
+
+/* S0: one-sided noise PSD S_n[k], k = 0..n/2 (n_bins == n/2+1).
+ * Builds, on the device in fp64, the weights 4 df dt f_k^{-7/6}/S_n[k] and the prefix table
+ * P[k] = 4 df sum_{k'=k_lo..k} f_k'^{-7/3}/S_n[k'] (sigma^2 of a template is P[k_hi]).
+ * +inf is legal (weight 0).  EINVAL if n_bins is wrong or an entry inside [k_lo, n/2) is
+ * <= 0 or NaN.  Invalidates the loaded segment. */
+int cbmf_set_psd(cbmf_ctx *ctx, const double *psd_onesided, int64_t n_bins);
+int cbmf_set_psd_dev(cbmf_ctx *ctx, const double *psd_onesided_dev, int64_t n_bins);
+
+/* S1: one data segment d[j], j = 0..n-1, float32 ("input data chunk").
+ * Computes w[k] = 4 df d~[k] f_k^{-7/6}/S_n[k] (k_lo <= k < n/2, else 0) with the
+ * library's own FFT and keeps it resident on the device for all following filter calls
+ * (PAPER.md:107, :157).  ESTATE if no PSD is set; EINVAL if n_samples != n or a sample
+ * is NaN/Inf. */
+int cbmf_load_segment(cbmf_ctx *ctx, const float *samples, int64_t n_samples);
+int cbmf_load_segment_dev(cbmf_ctx *ctx, const float *samples_dev, int64_t n_samples);
+
+/* S2-S8: the bank loop of PAPER.md:98-102.  For each template: SPA generation, correlate,
+ * inverse FFT, |z|/sigma, peak and triggers.
+ *   peaks_out[n_templates]   one cbmf_peak per template, bank order.
+ *   trig_out[trig_capacity]  triggers sorted by (template_idx, sample_idx); may be NULL
+ *                            with capacity 0 (triggers are still counted).
+ *   n_trig_found             total number of samples above threshold over the whole bank;
+ *                            if it exceeds trig_capacity the first trig_capacity entries
+ *                            written are an unspecified subset and the call returns
+ *                            CBMF_WTRUNC.
+ * snr_threshold >= 0.  n_templates may be 0.  ESTATE before PSD and segment are set;
+ * EINVAL on a non-positive or non-finite mass or a negative / NaN threshold. */
+int cbmf_filter_bank(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_templates,
+                     float snr_threshold, cbmf_peak *peaks_out,
+                     cbmf_trigger *trig_out, int64_t trig_capacity, int64_t *n_trig_found);
+/* Device-pointer variant: bank_dev, peaks_out_dev, trig_out_dev are device arrays;
+ * n_trig_found stays a HOST pointer. */
+int cbmf_filter_bank_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_t n_templates,
+                         float snr_threshold, cbmf_peak *peaks_out_dev,
+                         cbmf_trigger *trig_out_dev, int64_t trig_capacity,
+                         int64_t *n_trig_found);
+
+/* ---- diagnostics: used by the parity tests and the kernel sweep, never by filter_bank ---- */
+
+/* rho[j] (n floats) and optionally z[j] (2n floats, interleaved re,im) for one template,
+ * through the same generator / FFT kernels with a storing epilogue. */
+int cbmf_debug_snr_series(cbmf_ctx *ctx, cbmf_template t, float *snr_out, float *z_out_or_null);
+/* Unit-amplitude template h~[k] = f_k^{-7/6} e^{-i Psi_T}, k = 0..n/2 (2*(n/2+1) floats). */
+int cbmf_debug_template(cbmf_ctx *ctx, cbmf_template t, float *h_out);
+/* out[b][j] = sum_k in[b][k] e^{+2 pi i jk/n} (unnormalised inverse DFT), `batch` vectors of
+ * n complex floats (interleaved), n must equal the context's n. */
+int cbmf_debug_ifft(cbmf_ctx *ctx, const float *in, float *out, int64_t n, int64_t batch);
+int cbmf_debug_ifft_dev(cbmf_ctx *ctx, const float *in_dev, float *out_dev, int64_t n, int64_t batch);
+/* The generator alone: writes q~[b][k] = w[k] e^{+i Psi_b(f_k)} (n/2 complex floats per
+ * template, device array) -- SURVEY.md config 4 "template-generator-only throughput". */
+int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_t n_templates,
+                            float *q_out_dev);
+/* Copies of device state for tests: sigma^2 prefix table P[k] (n/2 doubles) and w[k]
+ * (n/2 complex floats, interleaved). */
+int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);
+int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
+
+/* ---- tuning ---- */
+/* Templates per launch pair (pass 1 + pass 2).  The default keeps the inter-pass buffer
+ * (8 n bytes per template in flight) inside the L2; results do not depend on it.
+ * 1 <= templates_per_launch <= 4096; ENOMEM if the larger buffer cannot be allocated. */
+int cbmf_set_sub_batch(cbmf_ctx *ctx, int templates_per_launch);
+int cbmf_get_sub_batch(const cbmf_ctx *ctx);
+
+/* ---- introspection ---- */
+/* Kernels launched by this context since creation (bench.py's gpu_launches). */
+int64_t cbmf_launch_count(const cbmf_ctx *ctx);
+/* Device time (ms, CUDA events on the context's stream) and launch count of the two FFT-pass
+ * kernels inside the last cbmf_filter_bank* call; used for the roofline line of bench.py.
+ * which = 0: pass 1 (generate + column FFT), 1: pass 2 (row FFT + epilogue). */
+int cbmf_last_pass_time(const cbmf_ctx *ctx, int which, double *ms_out, int64_t *launches_out);
+/* Enable (1) / disable (0) the per-pass event timing above (default off: no events recorded). */
+int cbmf_set_profiling(cbmf_ctx *ctx, int on);
+const char *cbmf_strerror(int rc);
+const char *cbmf_last_cuda_error(const cbmf_ctx *ctx);
+const char *cbmf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CBMF_H */

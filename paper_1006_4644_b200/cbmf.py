@@ -1,0 +1,250 @@
+"""Thin ctypes binding of the C-ABI library (include/cbmf.h): same names, argument
+marshalling only.  Every step of the path runs in the CUDA kernels behind the ABI.
+
+Loading fails loudly if libcbmf.so cannot be built or loaded: there is no CPU fallback,
+and this module never imports oracle/.
+
+Arrays may be numpy arrays / CPU torch tensors (host-pointer entry points) or CUDA torch
+tensors (the *_dev entry points); torch is used only for device memory and streams.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+OK, EINVAL, ESTATE, ECUDA, ENOMEM, WTRUNC = 0, -1, -2, -3, -4, 1
+
+PEAK_DTYPE = np.dtype([("snr_max", "<f4"), ("idx_peak", "<i4"), ("phase", "<f4"), ("sigma", "<f4")])
+TRIG_DTYPE = np.dtype([("template_idx", "<i4"), ("sample_idx", "<i4"), ("snr", "<f4"), ("phase", "<f4")])
+
+
+class Template(C.Structure):
+    _fields_ = [("m1", C.c_double), ("m2", C.c_double)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load (building if needed) libcbmf.so and declare every entry point of cbmf.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    vp, i64, dbl, flt = C.c_void_p, C.c_int64, C.c_double, C.c_float
+    sig = {
+        "cbmf_create": (C.c_int, [C.POINTER(vp), C.c_int, i64, dbl, dbl, vp]),
+        "cbmf_destroy": (C.c_int, [vp]),
+        "cbmf_set_psd": (C.c_int, [vp, vp, i64]),
+        "cbmf_set_psd_dev": (C.c_int, [vp, vp, i64]),
+        "cbmf_load_segment": (C.c_int, [vp, vp, i64]),
+        "cbmf_load_segment_dev": (C.c_int, [vp, vp, i64]),
+        "cbmf_filter_bank": (C.c_int, [vp, vp, i64, flt, vp, vp, i64, C.POINTER(i64)]),
+        "cbmf_filter_bank_dev": (C.c_int, [vp, vp, i64, flt, vp, vp, i64, C.POINTER(i64)]),
+        "cbmf_debug_snr_series": (C.c_int, [vp, Template, vp, vp]),
+        "cbmf_debug_template": (C.c_int, [vp, Template, vp]),
+        "cbmf_debug_ifft": (C.c_int, [vp, vp, vp, i64, i64]),
+        "cbmf_debug_ifft_dev": (C.c_int, [vp, vp, vp, i64, i64]),
+        "cbmf_debug_generate_dev": (C.c_int, [vp, vp, i64, vp]),
+        "cbmf_debug_get_prefix": (C.c_int, [vp, vp]),
+        "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
+        "cbmf_set_sub_batch": (C.c_int, [vp, C.c_int]),
+        "cbmf_get_sub_batch": (C.c_int, [vp]),
+        "cbmf_launch_count": (i64, [vp]),
+        "cbmf_last_pass_time": (C.c_int, [vp, C.c_int, C.POINTER(dbl), C.POINTER(i64)]),
+        "cbmf_set_profiling": (C.c_int, [vp, C.c_int]),
+        "cbmf_strerror": (C.c_char_p, [C.c_int]),
+        "cbmf_last_cuda_error": (C.c_char_p, [vp]),
+        "cbmf_version": (C.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)            # AttributeError if the library lacks a declared symbol
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
+           "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_debug_snr_series "
+           "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
+           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch "
+           "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_strerror "
+           "cbmf_last_cuda_error cbmf_version").split()
+
+
+class CbmfError(RuntimeError):
+    def __init__(self, rc: int, what: str, detail: str = ""):
+        msg = lib().cbmf_strerror(rc).decode()
+        super().__init__(f"{what}: {msg} (rc={rc})" + (f" [{detail}]" if detail else ""))
+        self.rc = rc
+
+
+def _is_tensor(a) -> bool:
+    return hasattr(a, "data_ptr") and hasattr(a, "is_cuda")
+
+
+def _ptr(a, dtype=None):
+    """-> (address, on_device).  numpy arrays and tensors must be contiguous (and of `dtype`)."""
+    if a is None:
+        return None, False
+    if _is_tensor(a):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return a.data_ptr(), bool(a.is_cuda)
+    if not isinstance(a, np.ndarray) or not a.flags["C_CONTIGUOUS"]:
+        raise ValueError("expected a C-contiguous numpy array or a torch tensor")
+    if dtype is not None and a.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {a.dtype}")
+    return a.ctypes.data, False
+
+
+class Context:
+    """cbmf_ctx: one segment length / sample rate / lower cutoff on one device and stream."""
+
+    def __init__(self, n: int, fs: float, f_low: float, device: int = 0, stream: int | None = None):
+        self.n, self.fs, self.f_low, self.device = int(n), float(fs), float(f_low), int(device)
+        self._h = C.c_void_p()
+        rc = lib().cbmf_create(C.byref(self._h), self.device, self.n, self.fs, self.f_low,
+                               C.c_void_p(stream or 0))
+        if rc:
+            self._h = C.c_void_p()
+            raise CbmfError(rc, "cbmf_create")
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().cbmf_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _check(self, rc: int, what: str) -> int:
+        if rc < 0:
+            raise CbmfError(rc, what, lib().cbmf_last_cuda_error(self._h).decode() if rc == ECUDA else "")
+        return rc
+
+    # -- the three calls of the path
+    def set_psd(self, psd):
+        if isinstance(psd, np.ndarray):
+            psd = np.ascontiguousarray(psd, dtype=np.float64)
+        p, dev = _ptr(psd)
+        n_bins = int(psd.numel() if _is_tensor(psd) else psd.size)
+        f = lib().cbmf_set_psd_dev if dev else lib().cbmf_set_psd
+        self._check(f(self._h, p, n_bins), "cbmf_set_psd")
+
+    def load_segment(self, samples):
+        if isinstance(samples, np.ndarray):
+            samples = np.ascontiguousarray(samples, dtype=np.float32)
+        p, dev = _ptr(samples)
+        n = int(samples.numel() if _is_tensor(samples) else samples.size)
+        f = lib().cbmf_load_segment_dev if dev else lib().cbmf_load_segment
+        self._check(f(self._h, p, n), "cbmf_load_segment")
+
+    def filter_bank(self, bank, snr_threshold: float, trig_capacity: int = 1 << 16):
+        """Host arrays in, host arrays out: -> (peaks[PEAK_DTYPE], triggers[TRIG_DTYPE], n_found, rc)."""
+        b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+        nt = b.shape[0]
+        peaks = np.zeros(nt, dtype=PEAK_DTYPE)
+        trig = np.zeros(max(int(trig_capacity), 1), dtype=TRIG_DTYPE)
+        nf = C.c_int64(0)
+        rc = lib().cbmf_filter_bank(self._h, b.ctypes.data if nt else None, nt, float(snr_threshold),
+                                    peaks.ctypes.data if nt else None,
+                                    trig.ctypes.data if trig_capacity else None, int(trig_capacity),
+                                    C.byref(nf))
+        self._check(rc, "cbmf_filter_bank")
+        return peaks, trig[:min(nf.value, int(trig_capacity))], nf.value, rc
+
+    def filter_bank_into(self, bank, snr_threshold: float, peaks_out, trig_out, trig_capacity: int):
+        """Caller-owned buffers (all host -- numpy / pinned tensors -- or all CUDA tensors):
+        bank float64 [B,2], peaks_out 16 B/template, trig_out 16 B/entry.  -> (n_found, rc)."""
+        pb, dev = _ptr(bank)
+        pp, devp = _ptr(peaks_out)
+        pt, devt = _ptr(trig_out)
+        if devp != dev or (trig_out is not None and devt != dev):
+            raise ValueError("bank, peaks_out and trig_out must all be host or all be device arrays")
+        nt = int((bank.numel() if _is_tensor(bank) else bank.size) // 2)
+        nf = C.c_int64(0)
+        f = lib().cbmf_filter_bank_dev if dev else lib().cbmf_filter_bank
+        rc = f(self._h, pb, nt, float(snr_threshold), pp, pt, int(trig_capacity), C.byref(nf))
+        self._check(rc, "cbmf_filter_bank")
+        return nf.value, rc
+
+    # -- diagnostics
+    def debug_snr_series(self, m1: float, m2: float, want_z: bool = True):
+        snr = np.empty(self.n, dtype=np.float32)
+        z = np.empty(self.n, dtype=np.complex64) if want_z else None
+        rc = lib().cbmf_debug_snr_series(self._h, Template(m1, m2), snr.ctypes.data,
+                                         z.ctypes.data if want_z else None)
+        self._check(rc, "cbmf_debug_snr_series")
+        return snr, z
+
+    def debug_template(self, m1: float, m2: float) -> np.ndarray:
+        h = np.empty(self.n // 2 + 1, dtype=np.complex64)
+        self._check(lib().cbmf_debug_template(self._h, Template(m1, m2), h.ctypes.data), "cbmf_debug_template")
+        return h
+
+    def debug_ifft(self, x):
+        """Unnormalised inverse DFT of `batch` vectors [batch, n] complex64 (numpy or CUDA tensor)."""
+        if _is_tensor(x) and x.is_cuda:
+            import torch
+            out = torch.empty_like(x)
+            batch = x.numel() // self.n
+            self._check(lib().cbmf_debug_ifft_dev(self._h, x.data_ptr(), out.data_ptr(), self.n, batch),
+                        "cbmf_debug_ifft_dev")
+            return out
+        a = np.ascontiguousarray(x, dtype=np.complex64)
+        out = np.empty_like(a)
+        self._check(lib().cbmf_debug_ifft(self._h, a.ctypes.data, out.ctypes.data, self.n, a.size // self.n),
+                    "cbmf_debug_ifft")
+        return out
+
+    def debug_generate_dev(self, bank_dev, q_out_dev):
+        nt = bank_dev.numel() // 2
+        self._check(lib().cbmf_debug_generate_dev(self._h, bank_dev.data_ptr(), nt, q_out_dev.data_ptr()),
+                    "cbmf_debug_generate_dev")
+
+    def debug_get_prefix(self) -> np.ndarray:
+        p = np.empty(self.n // 2, dtype=np.float64)
+        self._check(lib().cbmf_debug_get_prefix(self._h, p.ctypes.data), "cbmf_debug_get_prefix")
+        return p
+
+    def debug_get_weights(self) -> np.ndarray:
+        w = np.empty(self.n // 2, dtype=np.complex64)
+        self._check(lib().cbmf_debug_get_weights(self._h, w.ctypes.data), "cbmf_debug_get_weights")
+        return w
+
+    # -- tuning / introspection
+    def set_sub_batch(self, k: int):
+        self._check(lib().cbmf_set_sub_batch(self._h, int(k)), "cbmf_set_sub_batch")
+
+    def get_sub_batch(self) -> int:
+        return int(lib().cbmf_get_sub_batch(self._h))
+
+    def launch_count(self) -> int:
+        return int(lib().cbmf_launch_count(self._h))
+
+    def set_profiling(self, on: bool):
+        self._check(lib().cbmf_set_profiling(self._h, int(bool(on))), "cbmf_set_profiling")
+
+    def last_pass_time(self, which: int):
+        ms, nl = C.c_double(0), C.c_int64(0)
+        self._check(lib().cbmf_last_pass_time(self._h, int(which), C.byref(ms), C.byref(nl)), "cbmf_last_pass_time")
+        return ms.value, nl.value
+
+
+def version() -> str:
+    return lib().cbmf_version().decode()

@@ -1,0 +1,704 @@
+// cbmf.cu -- host side of the C ABI declared in include/cbmf.h.
+//
+// Argument checks, device allocations and kernel launches only: every arithmetic step of
+// the path (PSD tables, forward FFT of the segment, template constants, SPA generation,
+// correlation, inverse FFT, |z|/sigma, arg-max, threshold, trigger sort) runs in the kernels
+// of kernels.cuh.  There is no CPU fallback and nothing here touches oracle/.
+#include "../../include/cbmf.h"
+#include "kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace cbmf;
+
+struct cbmf_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int64_t n = 0;
+    int log2n = 0, lg1 = 0, lg2 = 0;      // N = N1 * N2, N1 = 2^lg1 (pass 1), N2 = 2^lg2 (pass 2)
+    double fs = 0, f_low = 0, df = 0, dt = 0;
+    int k_lo = 0;
+    bool have_psd = false, have_seg = false;
+    int sub_batch = 0;                     // templates per pass-1/pass-2 launch pair
+    int max_sub_batch = 0;
+
+    double* d_wfac = nullptr;              // [N/2]
+    double* d_term = nullptr;              // [N/2]
+    double* d_prefix = nullptr;            // [N/2]
+    float2* d_w = nullptr;                 // [N/2]
+    float2* d_Y = nullptr;                 // [max_sub_batch][N]
+    float4* d_cand = nullptr;              // [max_sub_batch][p2 grid.x]
+    unsigned int* d_done = nullptr;        // [max_sub_batch]
+    int* d_err = nullptr;                  // [1]
+    unsigned long long* d_cursor = nullptr;// [1]
+    TemplCoef* d_coef = nullptr;  int64_t coef_cap = 0;
+    double* d_bank = nullptr;     int64_t bank_cap = 0;
+    PeakOut* d_peaks = nullptr;   int64_t peaks_cap = 0;
+    TrigOut* d_trig = nullptr;    int64_t trig_cap = 0;       // entries (power of two)
+    void* d_scratch = nullptr;    size_t scratch_bytes = 0;   // debug paths / load_segment
+
+    int64_t launches = 0;
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev[2];        // per pass: start/stop pairs of the last filter call
+    size_t ev_used[2] = {0, 0};
+    double last_ms[2] = {0, 0};
+    int64_t last_launches[2] = {0, 0};
+    char cuda_err[256] = {0};
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; }
+        if (prev != dev) ok = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int cuda_fail(cbmf_ctx* c, cudaError_t e, const char* what)
+{
+    if (c) snprintf(c->cuda_err, sizeof(c->cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? CBMF_ENOMEM : CBMF_ECUDA;
+}
+#define CU(call)                                                         \
+    do {                                                                 \
+        cudaError_t e__ = (call);                                        \
+        if (e__ != cudaSuccess) return cuda_fail(c, e__, #call);         \
+    } while (0)
+
+template <typename T>
+int grow(cbmf_ctx* c, T*& p, int64_t& cap, int64_t need)
+{
+    if (need <= cap) return CBMF_OK;
+    if (p) { CU(cudaFree(p)); p = nullptr; cap = 0; }
+    CU(cudaMalloc(&p, sizeof(T) * (size_t)need));
+    cap = need;
+    return CBMF_OK;
+}
+
+int grow_scratch(cbmf_ctx* c, size_t bytes)
+{
+    if (bytes <= c->scratch_bytes) return CBMF_OK;
+    if (c->d_scratch) { CU(cudaFree(c->d_scratch)); c->d_scratch = nullptr; c->scratch_bytes = 0; }
+    CU(cudaMalloc(&c->d_scratch, bytes));
+    c->scratch_bytes = bytes;
+    return CBMF_OK;
+}
+
+int ilog2(int64_t n) { int l = 0; while ((int64_t(1) << l) < n) ++l; return l; }
+
+// ---------------------------------------------------------------- launch dispatch over L
+template <int L> size_t p1_smem() { return sizeof(float2) * (size_t)Cfg<L>::PADDED * Cfg<L>::C; }
+template <int L> size_t p2_smem() { return sizeof(float2) * (size_t)Cfg<L>::PADDED * Cfg<L>::ROWS; }
+
+template <int L, int MODE>
+cudaError_t launch_p1_L(cudaStream_t s, const P1Args& a, int batch)
+{
+    static bool attr_done = false;
+    const size_t smem = p1_smem<L>();
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(p1_kernel<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int n2 = 1 << a.log2_n2;
+    dim3 grid(n2 / Cfg<L>::C, batch);
+    p1_kernel<L, MODE><<<grid, Cfg<L>::NT1, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <int L, int MODE>
+cudaError_t launch_p2_L(cudaStream_t s, const P2Args& a, int batch)
+{
+    static bool attr_done = false;
+    const size_t smem = p2_smem<L>();
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(p2_kernel<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int n1 = 1 << a.log2_n1;
+    dim3 grid(n1 / Cfg<L>::ROWS, batch);
+    p2_kernel<L, MODE><<<grid, Cfg<L>::NT2, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+#define CBMF_DISPATCH_L(lg, FN, ...)                      \
+    switch (lg) {                                          \
+        case 6:  return FN<64, MODE>(__VA_ARGS__);         \
+        case 7:  return FN<128, MODE>(__VA_ARGS__);        \
+        case 8:  return FN<256, MODE>(__VA_ARGS__);        \
+        case 9:  return FN<512, MODE>(__VA_ARGS__);        \
+        case 10: return FN<1024, MODE>(__VA_ARGS__);       \
+        case 11: return FN<2048, MODE>(__VA_ARGS__);       \
+        case 12: return FN<4096, MODE>(__VA_ARGS__);       \
+        default: return cudaErrorInvalidValue;             \
+    }
+
+template <int MODE>
+cudaError_t launch_p1(int lg1, cudaStream_t s, const P1Args& a, int batch)
+{
+    CBMF_DISPATCH_L(lg1, launch_p1_L, s, a, batch)
+}
+template <int MODE>
+cudaError_t launch_p2(int lg2, cudaStream_t s, const P2Args& a, int batch)
+{
+    CBMF_DISPATCH_L(lg2, launch_p2_L, s, a, batch)
+}
+
+int p2_rows(int lg2)
+{
+    switch (lg2) {
+        case 6: return Cfg<64>::ROWS;   case 7: return Cfg<128>::ROWS;  case 8: return Cfg<256>::ROWS;
+        case 9: return Cfg<512>::ROWS;  case 10: return Cfg<1024>::ROWS; case 11: return Cfg<2048>::ROWS;
+        default: return Cfg<4096>::ROWS;
+    }
+}
+
+// pass-timing events (cbmf_set_profiling): one start/stop pair per launch
+int ev_begin(cbmf_ctx* c, int which)
+{
+    if (!c->profiling) return CBMF_OK;
+    auto& v = c->ev[which];
+    if (c->ev_used[which] + 2 > v.size()) {
+        for (int i = 0; i < 2; ++i) { cudaEvent_t e; CU(cudaEventCreate(&e)); v.push_back(e); }
+    }
+    CU(cudaEventRecord(v[c->ev_used[which]], c->stream));
+    return CBMF_OK;
+}
+int ev_end(cbmf_ctx* c, int which)
+{
+    if (!c->profiling) return CBMF_OK;
+    CU(cudaEventRecord(c->ev[which][c->ev_used[which] + 1], c->stream));
+    c->ev_used[which] += 2;
+    return CBMF_OK;
+}
+int ev_collect(cbmf_ctx* c)
+{
+    for (int w = 0; w < 2; ++w) {
+        c->last_ms[w] = 0; c->last_launches[w] = 0;
+        if (!c->profiling) continue;
+        for (size_t i = 0; i + 1 < c->ev_used[w]; i += 2) {
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, c->ev[w][i], c->ev[w][i + 1]));
+            c->last_ms[w] += ms; c->last_launches[w] += 1;
+        }
+        c->ev_used[w] = 0;
+    }
+    return CBMF_OK;
+}
+
+}  // namespace
+
+// ======================================================================= create / destroy
+extern "C" int cbmf_destroy(cbmf_ctx* c)
+{
+    if (!c) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_w);
+    cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_err);
+    cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
+    cudaFree(c->d_trig); cudaFree(c->d_scratch);
+    for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
+    cudaGetLastError();
+    delete c;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, double f_low_hz,
+                           void* cuda_stream)
+{
+    if (!out) return CBMF_EINVAL;
+    *out = nullptr;
+    if (n < (int64_t(1) << 12) || n > (int64_t(1) << 24) || (n & (n - 1)) != 0) return CBMF_EINVAL;
+    if (!(fs_hz > 0) || !std::isfinite(fs_hz)) return CBMF_EINVAL;
+    if (!(f_low_hz > 0) || !(f_low_hz < 0.5 * fs_hz)) return CBMF_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return CBMF_ECUDA; }
+    if (device < 0 || device >= ndev) return CBMF_EINVAL;
+
+    cbmf_ctx* c = new (std::nothrow) cbmf_ctx();
+    if (!c) return CBMF_ENOMEM;
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->n = n;
+    c->log2n = ilog2(n);
+    c->lg1 = c->log2n / 2;                 // the longer FFT goes to pass 2 (contiguous rows)
+    c->lg2 = c->log2n - c->lg1;
+    c->fs = fs_hz; c->f_low = f_low_hz;
+    c->df = fs_hz / (double)n; c->dt = 1.0 / fs_hz;
+    c->k_lo = (int)std::ceil(f_low_hz * ((double)n / fs_hz));       // reading A7: inclusive, in double
+    if (c->k_lo < 1) c->k_lo = 1;
+
+    // templates per launch pair: keep the inter-pass buffer Y inside the L2
+    int64_t sb = (int64_t(64) << 20) / (8 * n);
+    if (sb < 1) sb = 1;
+    if (sb > 256) sb = 256;
+    if (const char* e = getenv("CBMF_SUB_BATCH")) {
+        const long v = strtol(e, nullptr, 10);
+        if (v >= 1 && v <= 4096) sb = v;
+    }
+    c->sub_batch = (int)sb;
+    c->max_sub_batch = (int)sb;
+
+    DeviceGuard g(device);
+    auto fail = [&](int rc) { cbmf_destroy(c); return rc; };
+    if (!g.ok) return fail(CBMF_ECUDA);
+    const size_t nh = (size_t)n / 2;
+    const int p2grid = (1 << c->lg1) / p2_rows(c->lg2);
+#define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(cuda_fail(nullptr, e__, #call)); } while (0)
+    CUF(cudaMalloc(&c->d_wfac, sizeof(double) * nh));
+    CUF(cudaMalloc(&c->d_term, sizeof(double) * nh));
+    CUF(cudaMalloc(&c->d_prefix, sizeof(double) * nh));
+    CUF(cudaMalloc(&c->d_w, sizeof(float2) * nh));
+    CUF(cudaMalloc(&c->d_Y, sizeof(float2) * (size_t)n * c->max_sub_batch));
+    CUF(cudaMalloc(&c->d_cand, sizeof(float4) * (size_t)p2grid * c->max_sub_batch));
+    CUF(cudaMalloc(&c->d_done, sizeof(unsigned int) * c->max_sub_batch));
+    CUF(cudaMalloc(&c->d_err, sizeof(int)));
+    CUF(cudaMalloc(&c->d_cursor, sizeof(unsigned long long)));
+    CUF(cudaMemsetAsync(c->d_done, 0, sizeof(unsigned int) * c->max_sub_batch, c->stream));
+    CUF(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    CUF(cudaStreamSynchronize(c->stream));
+#undef CUF
+    *out = c;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_set_sub_batch(cbmf_ctx* c, int templates_per_launch)
+{
+    if (!c || templates_per_launch < 1 || templates_per_launch > 4096) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    if (templates_per_launch > c->max_sub_batch) {
+        CU(cudaStreamSynchronize(c->stream));
+        const int p2grid = (1 << c->lg1) / p2_rows(c->lg2);
+        float2* y = nullptr; float4* cand = nullptr; unsigned int* done = nullptr;
+        CU(cudaMalloc(&y, sizeof(float2) * (size_t)c->n * templates_per_launch));
+        cudaError_t e = cudaMalloc(&cand, sizeof(float4) * (size_t)p2grid * templates_per_launch);
+        if (e == cudaSuccess) e = cudaMalloc(&done, sizeof(unsigned int) * templates_per_launch);
+        if (e == cudaSuccess) e = cudaMemsetAsync(done, 0, sizeof(unsigned int) * templates_per_launch, c->stream);
+        if (e != cudaSuccess) { cudaFree(y); cudaFree(cand); cudaFree(done); return cuda_fail(c, e, "cbmf_set_sub_batch"); }
+        cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done);
+        c->d_Y = y; c->d_cand = cand; c->d_done = done;
+        c->max_sub_batch = templates_per_launch;
+    }
+    c->sub_batch = templates_per_launch;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_get_sub_batch(const cbmf_ctx* c) { return c ? c->sub_batch : CBMF_EINVAL; }
+
+// ======================================================================= S0: set_psd
+static int set_psd_impl(cbmf_ctx* c, const double* psd_dev)
+{
+    const int nh = (int)(c->n / 2);
+    c->have_psd = false; c->have_seg = false;
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    psd_terms_kernel<<<(nh + 255) / 256, 256, 0, c->stream>>>(psd_dev, c->d_wfac, c->d_term, nh, c->k_lo,
+                                                             c->df, c->dt, c->d_err);
+    CU(cudaGetLastError());
+    prefix_sum_kernel<<<1, 1024, 0, c->stream>>>(c->d_term, c->d_prefix, nh);
+    CU(cudaGetLastError());
+    c->launches += 2;
+    int err = 0;
+    CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (err) return CBMF_EINVAL;
+    c->have_psd = true;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_set_psd_dev(cbmf_ctx* c, const double* psd_dev, int64_t n_bins)
+{
+    if (!c || !psd_dev) return CBMF_EINVAL;
+    if (n_bins != c->n / 2 + 1) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    return set_psd_impl(c, psd_dev);
+}
+
+extern "C" int cbmf_set_psd(cbmf_ctx* c, const double* psd, int64_t n_bins)
+{
+    if (!c || !psd) return CBMF_EINVAL;
+    if (n_bins != c->n / 2 + 1) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    int rc = grow_scratch(c, sizeof(double) * (size_t)n_bins);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(c->d_scratch, psd, sizeof(double) * (size_t)n_bins, cudaMemcpyHostToDevice, c->stream));
+    return set_psd_impl(c, (const double*)c->d_scratch);
+}
+
+// ======================================================================= S1: load_segment
+// d~[k] = dt conj(IDFT(d)[k]) for real d, so the forward transform reuses the inverse kernels.
+static int load_segment_impl(cbmf_ctx* c, const float* samples_dev)
+{
+    c->have_seg = false;
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    // k_lo travels to the EPI_WSTORE epilogue in a one-entry TemplCoef
+    int rc = grow(c, c->d_coef, c->coef_cap, 1);
+    if (rc) return rc;
+    TemplCoef tc; memset(&tc, 0, sizeof(tc)); tc.k_lo = c->k_lo; tc.k_hi = (int)(c->n / 2 - 1);
+    CU(cudaMemcpyAsync(c->d_coef, &tc, sizeof(tc), cudaMemcpyHostToDevice, c->stream));
+    P1Args a1; memset(&a1, 0, sizeof(a1));
+    a1.in_r = samples_dev; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
+    CU(launch_p1<LOAD_REAL>(c->lg1, c->stream, a1, 1));
+    P2Args a2; memset(&a2, 0, sizeof(a2));
+    a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.coef = c->d_coef; a2.w_out = c->d_w; a2.wfac = c->d_wfac;
+    CU(launch_p2<EPI_WSTORE>(c->lg2, c->stream, a2, 1));
+    c->launches += 2;
+    int err = 0;
+    CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (err) return CBMF_EINVAL;
+    c->have_seg = true;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_load_segment_dev(cbmf_ctx* c, const float* samples_dev, int64_t n_samples)
+{
+    if (!c || !samples_dev) return CBMF_EINVAL;
+    if (n_samples != c->n) return CBMF_EINVAL;
+    if (!c->have_psd) return CBMF_ESTATE;
+    DeviceGuard g(c->device);
+    return load_segment_impl(c, samples_dev);
+}
+
+extern "C" int cbmf_load_segment(cbmf_ctx* c, const float* samples, int64_t n_samples)
+{
+    if (!c || !samples) return CBMF_EINVAL;
+    if (n_samples != c->n) return CBMF_EINVAL;
+    if (!c->have_psd) return CBMF_ESTATE;
+    DeviceGuard g(c->device);
+    int rc = grow_scratch(c, sizeof(float) * (size_t)c->n);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(c->d_scratch, samples, sizeof(float) * (size_t)c->n, cudaMemcpyHostToDevice, c->stream));
+    return load_segment_impl(c, (const float*)c->d_scratch);
+}
+
+// ======================================================================= S2-S8: filter_bank
+// Sort the first `count` entries of c->d_trig by (template, sample) on the device.
+static int sort_triggers(cbmf_ctx* c, int64_t count)
+{
+    if (count <= 1) return CBMF_OK;
+    long long np2 = 1;
+    while (np2 < count) np2 <<= 1;
+    if (np2 <= TRIG_SORT_SMEM_MAX) {
+        trig_sort_small_kernel<<<1, 1024, 0, c->stream>>>(c->d_trig, (int)count, (int)np2);
+        CU(cudaGetLastError());
+        c->launches += 1;
+        return CBMF_OK;
+    }
+    const unsigned blocks = (unsigned)((np2 + 255) / 256);
+    if (np2 > count) {
+        trig_pad_kernel<<<(unsigned)((np2 - count + 255) / 256), 256, 0, c->stream>>>(c->d_trig, count, np2);
+        CU(cudaGetLastError());
+        c->launches += 1;
+    }
+    for (long long kk = 2; kk <= np2; kk <<= 1)
+        for (long long jj = kk >> 1; jj > 0; jj >>= 1) {
+            trig_bitonic_kernel<<<blocks, 256, 0, c->stream>>>(c->d_trig, np2, kk, jj);
+            CU(cudaGetLastError());
+            c->launches += 1;
+        }
+    return CBMF_OK;
+}
+
+// bank_dev: [n][2] doubles on the device.  Outputs go to host or device pointers (out_kind).
+static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr,
+                            void* peaks_out, void* trig_out, int64_t trig_capacity,
+                            int64_t* n_trig_found, cudaMemcpyKind out_kind)
+{
+    if (n_trig_found) *n_trig_found = 0;
+    if (nt == 0) return CBMF_OK;
+    int rc;
+    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
+    // device trigger buffer: capacity rounded up to a power of two (bitonic padding), >= 1
+    int64_t tcap = 1;
+    while (tcap < trig_capacity) tcap <<= 1;
+    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
+
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
+    SetupArgs sa;
+    sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
+    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
+    sa.threshold = thr; sa.err_flag = c->d_err;
+    template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
+    CU(cudaGetLastError());
+    c->launches += 1;
+
+    c->ev_used[0] = c->ev_used[1] = 0;
+    const int sb = c->sub_batch;
+    for (int64_t t0 = 0; t0 < nt; t0 += sb) {
+        const int nb = (int)((nt - t0 < sb) ? (nt - t0) : sb);
+        P1Args a1; memset(&a1, 0, sizeof(a1));
+        a1.w = c->d_w; a1.coef = c->d_coef + t0; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
+        if ((rc = ev_begin(c, 0))) return rc;
+        CU(launch_p1<LOAD_GEN>(c->lg1, c->stream, a1, nb));
+        if ((rc = ev_end(c, 0))) return rc;
+        P2Args a2; memset(&a2, 0, sizeof(a2));
+        a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.coef = c->d_coef + t0; a2.cand = c->d_cand;
+        a2.done_ctr = c->d_done; a2.peaks = c->d_peaks + t0; a2.trig = c->d_trig;
+        a2.trig_cursor = c->d_cursor; a2.trig_cap = (unsigned long long)trig_capacity;
+        a2.tmpl_base = (int)t0;
+        if ((rc = ev_begin(c, 1))) return rc;
+        CU(launch_p2<EPI_MAX>(c->lg2, c->stream, a2, nb));
+        if ((rc = ev_end(c, 1))) return rc;
+        c->launches += 2;
+    }
+
+    // status word + trigger count back to the host, then sort what was kept
+    struct { int err; unsigned long long found; } st = {0, 0};
+    CU(cudaMemcpyAsync(&st.err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(&st.found, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if ((rc = ev_collect(c))) return rc;
+    if (st.err) return CBMF_EINVAL;                 // a non-positive / non-finite mass (device check)
+    const int64_t found = (int64_t)st.found;
+    const int64_t kept = found < trig_capacity ? found : trig_capacity;
+    if (n_trig_found) *n_trig_found = found;
+    if (kept > 0 && trig_out) {
+        if ((rc = sort_triggers(c, kept))) return rc;
+        CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, out_kind, c->stream));
+    }
+    CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, out_kind, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
+}
+
+static int filter_args_ok(cbmf_ctx* c, const void* bank, int64_t nt, float thr, void* peaks,
+                          void* trig, int64_t cap)
+{
+    if (!c || nt < 0 || cap < 0) return CBMF_EINVAL;
+    if (nt > 0 && (!bank || !peaks)) return CBMF_EINVAL;
+    if (cap > 0 && !trig) return CBMF_EINVAL;
+    if (!(thr >= 0.f)) return CBMF_EINVAL;                 // negative or NaN
+    if (nt > 0x7FFFFFFF) return CBMF_EINVAL;
+    if (!c->have_psd || !c->have_seg) return CBMF_ESTATE;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_filter_bank_dev(cbmf_ctx* c, const cbmf_template* bank_dev, int64_t nt, float thr,
+                                    cbmf_peak* peaks_out_dev, cbmf_trigger* trig_out_dev,
+                                    int64_t trig_capacity, int64_t* n_trig_found)
+{
+    int rc = filter_args_ok(c, bank_dev, nt, thr, peaks_out_dev, trig_out_dev, trig_capacity);
+    if (rc) return rc;
+    DeviceGuard g(c->device);
+    return filter_bank_impl(c, (const double*)bank_dev, nt, thr, peaks_out_dev, trig_out_dev,
+                            trig_capacity, n_trig_found, cudaMemcpyDeviceToDevice);
+}
+
+extern "C" int cbmf_filter_bank(cbmf_ctx* c, const cbmf_template* bank, int64_t nt, float thr,
+                                cbmf_peak* peaks_out, cbmf_trigger* trig_out, int64_t trig_capacity,
+                                int64_t* n_trig_found)
+{
+    int rc = filter_args_ok(c, bank, nt, thr, peaks_out, trig_out, trig_capacity);
+    if (rc) return rc;
+    if (n_trig_found) *n_trig_found = 0;
+    if (nt == 0) return CBMF_OK;
+    DeviceGuard g(c->device);
+    if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
+    CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
+    return filter_bank_impl(c, c->d_bank, nt, thr, peaks_out, trig_out, trig_capacity, n_trig_found,
+                            cudaMemcpyDeviceToHost);
+}
+
+// ======================================================================= diagnostics
+// One template's coefficients into d_coef[0] (threshold 0).
+static int setup_one(cbmf_ctx* c, cbmf_template t)
+{
+    int rc;
+    if ((rc = grow(c, c->d_coef, c->coef_cap, 1))) return rc;
+    if ((rc = grow(c, c->d_bank, c->bank_cap, 2))) return rc;
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    CU(cudaMemcpyAsync(c->d_bank, &t, sizeof(t), cudaMemcpyHostToDevice, c->stream));
+    SetupArgs sa;
+    sa.bank = c->d_bank; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = 1;
+    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
+    sa.threshold = 0.f; sa.err_flag = c->d_err;
+    template_setup_kernel<<<1, 32, 0, c->stream>>>(sa);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    int err = 0;
+    CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return err ? CBMF_EINVAL : CBMF_OK;
+}
+
+extern "C" int cbmf_debug_snr_series(cbmf_ctx* c, cbmf_template t, float* snr_out, float* z_out)
+{
+    if (!c || !snr_out) return CBMF_EINVAL;
+    if (!c->have_psd || !c->have_seg) return CBMF_ESTATE;
+    DeviceGuard g(c->device);
+    int rc;
+    if ((rc = setup_one(c, t))) return rc;
+    const size_t n = (size_t)c->n;
+    if ((rc = grow_scratch(c, sizeof(float2) * n + sizeof(float) * n))) return rc;
+    float2* z = (float2*)c->d_scratch;
+    float* snr = (float*)(z + n);
+    TemplCoef tc;
+    CU(cudaMemcpyAsync(&tc, c->d_coef, sizeof(tc), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    P1Args a1; memset(&a1, 0, sizeof(a1));
+    a1.w = c->d_w; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
+    CU(launch_p1<LOAD_GEN>(c->lg1, c->stream, a1, 1));
+    P2Args a2; memset(&a2, 0, sizeof(a2));
+    a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.z_out = z;
+    CU(launch_p2<EPI_STORE>(c->lg2, c->stream, a2, 1));
+    snr_from_z_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(z, snr, n, tc.inv_sigma);
+    CU(cudaGetLastError());
+    c->launches += 3;
+    CU(cudaMemcpyAsync(snr_out, snr, sizeof(float) * n, cudaMemcpyDeviceToHost, c->stream));
+    if (z_out) CU(cudaMemcpyAsync(z_out, z, sizeof(float2) * n, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_debug_template(cbmf_ctx* c, cbmf_template t, float* h_out)
+{
+    if (!c || !h_out) return CBMF_EINVAL;
+    if (!c->have_psd) return CBMF_ESTATE;                 // sigma comes from the PSD prefix table
+    DeviceGuard g(c->device);
+    int rc;
+    if ((rc = setup_one(c, t))) return rc;
+    const int nh = (int)(c->n / 2);
+    if ((rc = grow_scratch(c, sizeof(float2) * (size_t)(nh + 1)))) return rc;
+    debug_template_kernel<<<(nh + 1 + 255) / 256, 256, 0, c->stream>>>(c->d_coef, (float2*)c->d_scratch, nh, c->df);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    CU(cudaMemcpyAsync(h_out, c->d_scratch, sizeof(float2) * (size_t)(nh + 1), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_debug_ifft_dev(cbmf_ctx* c, const float* in_dev, float* out_dev, int64_t n, int64_t batch)
+{
+    if (!c || !in_dev || !out_dev || n != c->n || batch < 0) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    const int sb = c->sub_batch;
+    for (int64_t b0 = 0; b0 < batch; b0 += sb) {
+        const int nb = (int)((batch - b0 < sb) ? (batch - b0) : sb);
+        P1Args a1; memset(&a1, 0, sizeof(a1));
+        a1.in_c = (const float2*)in_dev + (size_t)b0 * n; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
+        CU(launch_p1<LOAD_CPLX>(c->lg1, c->stream, a1, nb));
+        P2Args a2; memset(&a2, 0, sizeof(a2));
+        a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.z_out = (float2*)out_dev + (size_t)b0 * n;
+        CU(launch_p2<EPI_STORE>(c->lg2, c->stream, a2, nb));
+        c->launches += 2;
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_debug_ifft(cbmf_ctx* c, const float* in, float* out, int64_t n, int64_t batch)
+{
+    if (!c || !in || !out || n != c->n || batch < 0) return CBMF_EINVAL;
+    if (batch == 0) return CBMF_OK;
+    DeviceGuard g(c->device);
+    const size_t bytes = sizeof(float2) * (size_t)n * (size_t)batch;
+    float2 *d_in = nullptr, *d_out = nullptr;
+    CU(cudaMalloc(&d_in, bytes));
+    cudaError_t e = cudaMalloc(&d_out, bytes);
+    if (e != cudaSuccess) { cudaFree(d_in); return cuda_fail(c, e, "cudaMalloc"); }
+    int rc = CBMF_OK;
+    e = cudaMemcpyAsync(d_in, in, bytes, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) {
+        rc = cbmf_debug_ifft_dev(c, (const float*)d_in, (float*)d_out, n, batch);
+        if (rc == CBMF_OK) e = cudaMemcpyAsync(out, d_out, bytes, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    }
+    cudaFree(d_in); cudaFree(d_out);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cbmf_debug_ifft");
+    return rc;
+}
+
+extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_dev, int64_t nt, float* q_out_dev)
+{
+    if (!c || nt < 0 || (nt && (!bank_dev || !q_out_dev)) || nt > 65535) return CBMF_EINVAL;
+    if (!c->have_psd || !c->have_seg) return CBMF_ESTATE;
+    if (nt == 0) return CBMF_OK;
+    DeviceGuard g(c->device);
+    int rc;
+    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    SetupArgs sa;
+    sa.bank = (const double*)bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
+    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
+    sa.threshold = 0.f; sa.err_flag = c->d_err;
+    template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
+    CU(cudaGetLastError());
+    const int nh = (int)(c->n / 2);
+    int gx = (nh + 255) / 256; if (gx > 592) gx = 592;
+    generate_only_kernel<<<dim3(gx, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_coef, (float2*)q_out_dev, nh);
+    CU(cudaGetLastError());
+    c->launches += 2;
+    int err = 0;
+    CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return err ? CBMF_EINVAL : CBMF_OK;
+}
+
+extern "C" int cbmf_debug_get_prefix(cbmf_ctx* c, double* p_out)
+{
+    if (!c || !p_out) return CBMF_EINVAL;
+    if (!c->have_psd) return CBMF_ESTATE;
+    DeviceGuard g(c->device);
+    CU(cudaMemcpyAsync(p_out, c->d_prefix, sizeof(double) * (size_t)(c->n / 2), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_debug_get_weights(cbmf_ctx* c, float* w_out)
+{
+    if (!c || !w_out) return CBMF_EINVAL;
+    if (!c->have_seg) return CBMF_ESTATE;
+    DeviceGuard g(c->device);
+    CU(cudaMemcpyAsync(w_out, c->d_w, sizeof(float2) * (size_t)(c->n / 2), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return CBMF_OK;
+}
+
+// ======================================================================= introspection
+extern "C" int64_t cbmf_launch_count(const cbmf_ctx* c) { return c ? c->launches : -1; }
+
+extern "C" int cbmf_last_pass_time(const cbmf_ctx* c, int which, double* ms_out, int64_t* launches_out)
+{
+    if (!c || which < 0 || which > 1) return CBMF_EINVAL;
+    if (ms_out) *ms_out = c->last_ms[which];
+    if (launches_out) *launches_out = c->last_launches[which];
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_set_profiling(cbmf_ctx* c, int on)
+{
+    if (!c) return CBMF_EINVAL;
+    c->profiling = (on != 0);
+    return CBMF_OK;
+}
+
+extern "C" const char* cbmf_strerror(int rc)
+{
+    switch (rc) {
+        case CBMF_OK: return "success";
+        case CBMF_EINVAL: return "invalid argument";
+        case CBMF_ESTATE: return "call order: set_psd, then load_segment, then filter_bank";
+        case CBMF_ECUDA: return "CUDA runtime error";
+        case CBMF_ENOMEM: return "out of memory";
+        case CBMF_WTRUNC: return "trigger list truncated at trig_capacity";
+        default: return "unknown code";
+    }
+}
+
+extern "C" const char* cbmf_last_cuda_error(const cbmf_ctx* c) { return c ? c->cuda_err : ""; }
+
+extern "C" const char* cbmf_version(void) { return "cbmf 0.1 (sm_100a)"; }

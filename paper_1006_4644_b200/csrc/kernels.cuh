@@ -1,0 +1,619 @@
+// kernels.cuh -- sm_100a kernels of the matched-filter hot path.
+//
+//   N = N1 * N2.  Frequency bin k = N2*k1 + k2, output sample j = j1 + N1*j2.
+//   pass 1 (p1_kernel): for a tile of C adjacent columns k2, generate q~[k] = w[k] e^{+i Psi(f_k)}
+//       in registers (S3, S4), N1-point inverse FFT over k1 -> Y[j1][k2]            (S5, first half)
+//   pass 2 (p2_kernel): for ROWS adjacent rows j1, multiply by W_N^{j1 k2}, N2-point inverse FFT
+//       over k2 -> z[j1 + N1 j2] in registers, |z|^2, arg-max, threshold              (S5-S7)
+//   Y (N complex floats per template in flight) is the only materialised intermediate.
+//
+// Each per-pass FFT is a Stockham autosort FFT whose butterflies (radix 8/16/32) live in
+// registers and whose digit exchanges go through shared memory.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "fft_regs.cuh"
+
+namespace cbmf {
+
+// ------------------------------------------------------------------ per-template constants (S2)
+struct __align__(16) TemplCoef {
+    // phase in cycles: Psi/(2 pi) = -1/8 + u (A1 + u (A2 + u (A3 + u^2 A5))),  u = k^{-1/3}
+    double A1, A2, A3, A5;
+    int k_lo, k_hi;              // inclusive band on the DFT grid; empty if k_hi < k_lo
+    float sigma, inv_sigma;      // sqrt(P[k_hi]), 1/sigma (0 for an empty band)
+    float thr2;                  // (threshold * sigma)^2 : |z|^2 > thr2  <=>  rho > threshold
+    int nz_class;                // reserved
+    int pad_[2];
+};
+static_assert(sizeof(TemplCoef) == 64, "TemplCoef layout");
+
+struct PeakOut { float snr_max; int32_t idx_peak; float phase; float sigma; };
+struct TrigOut { int32_t template_idx; int32_t sample_idx; float snr; float phase; };
+
+// ------------------------------------------------------------------ FFT configurations
+template <int L> struct Cfg;
+#define CBMF_CFG(L_, E_, R1_, R2_, R3_, NT1_)                                            \
+    template <> struct Cfg<L_> {                                                         \
+        static constexpr int E = E_, R1 = R1_, R2 = R2_, R3 = R3_, T = L_ / E_;          \
+        static constexpr int NT1 = NT1_, NT2 = 256;                                      \
+        static constexpr int C = NT1 / T, ROWS = NT2 / T;                                \
+        static constexpr int PADDED = L_ + L_ / R1_;                                     \
+        static_assert(R1_ * R2_ * R3_ == L_, "radices");                                 \
+    };
+CBMF_CFG(64, 8, 8, 8, 1, 256)
+CBMF_CFG(128, 16, 16, 8, 1, 256)
+CBMF_CFG(256, 16, 16, 16, 1, 256)
+CBMF_CFG(512, 32, 32, 16, 1, 256)
+CBMF_CFG(1024, 32, 32, 32, 1, 256)
+CBMF_CFG(2048, 16, 16, 16, 8, 512)
+CBMF_CFG(4096, 16, 16, 16, 16, 1024)
+#undef CBMF_CFG
+
+__host__ __device__ constexpr int ilog2c(int x) { return x <= 1 ? 0 : 1 + ilog2c(x >> 1); }
+
+// Stockham steps 1..3 of one L-point inverse FFT distributed over T threads (thread index t),
+// E values per thread.  On entry v[u*R1 + r] = x[t + T*u + (L/R1)*r]; on exit
+// v[u*RL + q] = X[t + T*u + (L/RL)*q] (RL = last radix).  sm points at this FFT's shared
+// memory (element stride SS), padded by one element every R1.  NZ1: only r < NZ1 is non-zero.
+template <int L, int NZ1, int SS, bool WARP_SYNC>
+__device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, float2* __restrict__ sm)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, T = C::T, R1 = C::R1, R2 = C::R2, R3 = C::R3;
+    constexpr int LG_R1 = ilog2c(R1);
+    auto pad = [](int pos) { return pos + (pos >> LG_R1); };
+    auto sync = []() { if constexpr (WARP_SYNC) __syncwarp(); else __syncthreads(); };
+
+    // ---- step 1: radix R1, no twiddles (Ns = 1); out position i*R1 + q
+    {
+        constexpr int NB = E / R1;
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            float2 x[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) x[r] = v[u * R1 + r];
+            DftP<R1, NZ1>::run(x);
+            const int i = t + T * u;
+#pragma unroll
+            for (int q = 0; q < R1; ++q) sm[pad(i * R1 + q) * SS] = x[q];
+        }
+    }
+    sync();
+    // ---- step 2: radix R2, Ns = R1
+    {
+        constexpr int NB = E / R2, NS = R1;
+        float2 y[E];
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            float2 x[R2];
+            const int i = t + T * u;
+#pragma unroll
+            for (int r = 0; r < R2; ++r) x[r] = sm[pad(i + (L / R2) * r) * SS];
+            const int k = i & (NS - 1);
+            mul_powers<R2, false>(x, expi_frac(k, 2.0f / (float)(NS * R2)), make_float2(1.f, 0.f));
+            dft<R2>(x);
+#pragma unroll
+            for (int q = 0; q < R2; ++q) y[u * R2 + q] = x[q];
+        }
+        if constexpr (R3 == 1) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) v[e] = y[e];
+            return;
+        } else {
+            sync();   // all step-2 reads done before the buffer is overwritten
+#pragma unroll
+            for (int u = 0; u < NB; ++u) {
+                const int i = t + T * u;
+                const int k = i & (NS - 1);
+                const int base = (i >> LG_R1) * (NS * R2) + k;
+#pragma unroll
+                for (int q = 0; q < R2; ++q) sm[pad(base + q * NS) * SS] = y[u * R2 + q];
+            }
+        }
+    }
+    if constexpr (R3 > 1) {
+        sync();
+        // ---- step 3: radix R3, Ns = R1*R2
+        constexpr int NB = E / R3, NS = R1 * R2;
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            float2 x[R3];
+            const int i = t + T * u;
+#pragma unroll
+            for (int r = 0; r < R3; ++r) x[r] = sm[pad(i + (L / R3) * r) * SS];
+            const int k = i & (NS - 1);
+            mul_powers<R3, false>(x, expi_frac(k, 2.0f / (float)L), make_float2(1.f, 0.f));
+            dft<R3>(x);
+#pragma unroll
+            for (int q = 0; q < R3; ++q) v[u * R3 + q] = x[q];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ S3: SPA phasor
+// e^{+i Psi_T(f_k)} for bin k >= 1 ("x form" in cycles).  The phase
+// reaches 1e4 cycles, so the polynomial and the reduction to [-1/2, 1/2] cycles run in fp64;
+// the fraction is then exact to 3e-8 cycles in fp32.  u = k^{-1/3}: fp32 seed + one Newton
+// step in fp64 (relative error ~ 2 (1.2e-7)^2).
+__device__ __forceinline__ float2 spa_phasor(const int k, const double A1, const double A2,
+                                             const double A3, const double A5)
+{
+    const double kd = (double)k;
+    double u = (double)rcbrtf((float)k);
+    const double e = fma(-kd * u, u * u, 1.0);
+    u = fma(u * e, 1.0 / 3.0, u);
+    double ph = fma(u * u, A5, A3);
+    ph = fma(ph, u, A2);
+    ph = fma(ph, u, A1);
+    ph = fma(ph, u, -0.125);
+    const float fr = (float)(ph - rint(ph));
+    float s, c;
+    sincospif(2.0f * fr, &s, &c);
+    return make_float2(c, s);
+}
+
+// ------------------------------------------------------------------ pass 1
+enum { LOAD_GEN = 0, LOAD_CPLX = 1, LOAD_REAL = 2 };
+
+struct P1Args {
+    const float2* __restrict__ w;          // [N/2] weighted data spectrum (LOAD_GEN)
+    const TemplCoef* __restrict__ coef;    // [batch] (LOAD_GEN)
+    const float2* __restrict__ in_c;       // [batch][N] (LOAD_CPLX)
+    const float* __restrict__ in_r;        // [batch][N] (LOAD_REAL)
+    float2* __restrict__ Y;                // [batch][N], Y[j1*N2 + k2]
+    int* err_flag;                         // set to 1 on a non-finite real input sample
+    int log2_n2;
+};
+
+template <int L, int MODE>
+__global__ void __launch_bounds__(Cfg<L>::NT1, (Cfg<L>::NT1 <= 256 ? 2 : 1)) p1_kernel(const P1Args a)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, T = C::T, R1 = C::R1, NC = C::C;
+    constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
+    constexpr int NZ1 = (MODE == LOAD_GEN) ? R1 / 2 : R1;    // bins k >= N/2 are zero
+    extern __shared__ float2 smem[];
+
+    const int c = threadIdx.x % NC, t = threadIdx.x / NC;
+    const int k2 = blockIdx.x * NC + c;
+    const int b = blockIdx.y;
+    const int lg2 = a.log2_n2;
+    const size_t n_total = (size_t)L << lg2;
+
+    float2 v[E];
+    if constexpr (MODE == LOAD_GEN) {
+        const TemplCoef* tc = a.coef + b;
+        const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+        const int k_lo = tc->k_lo, k_hi = tc->k_hi;
+#pragma unroll
+        for (int u = 0; u < E / R1; ++u) {
+#pragma unroll
+            for (int r = 0; r < R1; ++r) {
+                float2 val = make_float2(0.f, 0.f);
+                if (r < NZ1) {
+                    const int k1 = t + T * u + (L / R1) * r;
+                    const int k = (k1 << lg2) + k2;
+                    if (k >= k_lo && k <= k_hi) val = cmul(__ldg(a.w + k), spa_phasor(k, A1, A2, A3, A5));
+                }
+                v[u * R1 + r] = val;
+            }
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < E / R1; ++u) {
+#pragma unroll
+            for (int r = 0; r < R1; ++r) {
+                const int k1 = t + T * u + (L / R1) * r;
+                const size_t k = ((size_t)k1 << lg2) + k2;
+                if constexpr (MODE == LOAD_CPLX) {
+                    v[u * R1 + r] = __ldg(a.in_c + (size_t)b * n_total + k);
+                } else {
+                    const float x = __ldg(a.in_r + (size_t)b * n_total + k);
+                    if (!isfinite(x)) *a.err_flag = 1;
+                    v[u * R1 + r] = make_float2(x, 0.f);
+                }
+            }
+        }
+    }
+
+    fft_core<L, NZ1, NC, false>(v, t, smem + c);
+
+    float2* __restrict__ yb = a.Y + (size_t)b * n_total;
+#pragma unroll
+    for (int u = 0; u < E / RL; ++u) {
+#pragma unroll
+        for (int q = 0; q < RL; ++q) {
+            const int j1 = t + T * u + (L / RL) * q;
+            yb[((size_t)j1 << lg2) + k2] = v[u * RL + q];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ pass 2
+enum { EPI_MAX = 0, EPI_STORE = 1, EPI_WSTORE = 2 };
+
+struct P2Args {
+    const float2* __restrict__ Y;          // [batch][N]
+    int log2_n1;                           // N1 = number of rows
+    // EPI_MAX
+    const TemplCoef* __restrict__ coef;    // [batch]
+    float4* cand;                          // [batch][gridDim.x]  (|z|^2, j as int bits, re, im)
+    unsigned int* done_ctr;                // [batch], zero on entry, zero again on exit
+    PeakOut* peaks;                        // [batch] (already offset to this sub-batch)
+    TrigOut* trig;                         // bounded trigger list
+    unsigned long long* trig_cursor;       // total found so far
+    unsigned long long trig_cap;
+    int tmpl_base;                         // bank index of template 0 of this sub-batch
+    // EPI_STORE
+    float2* __restrict__ z_out;            // [batch][N], natural order
+    // EPI_WSTORE (load_segment): w[k] = conj(Z[k]) * wfac[k] for k < N/2
+    float2* __restrict__ w_out;            // [N/2]
+    const double* __restrict__ wfac;       // [N/2]
+};
+
+__device__ __forceinline__ unsigned long long pack_key(float p, int j)
+{
+    return ((unsigned long long)__float_as_uint(p) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)j);
+}
+
+template <int L, int MODE>
+__global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, T = C::T, R1 = C::R1, ROWS = C::ROWS;
+    constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
+    constexpr bool WSYNC = (T <= 32);
+    extern __shared__ float2 smem[];
+
+    const int t = threadIdx.x % T, row = threadIdx.x / T;
+    const int j1 = blockIdx.x * ROWS + row;
+    const int b = blockIdx.y;
+    const int lg1 = a.log2_n1;
+    const int n1 = 1 << lg1;
+    const size_t n_total = (size_t)L << lg1;
+    const float two_over_n = 2.0f / (float)n_total;
+
+    // load row j1 and apply the inter-pass twiddle W_N^{j1 k2}, k2 = t + T u + (L/R1) r
+    float2 v[E];
+    const float2* __restrict__ yrow = a.Y + (size_t)b * n_total + (size_t)j1 * L;
+    const float2 g = expi_frac(j1, 2.0f / (float)(n1 * R1));      // W_N^{j1 L/R1}
+#pragma unroll
+    for (int u = 0; u < E / R1; ++u) {
+        float2 x[R1];
+        const int p0 = t + T * u;
+#pragma unroll
+        for (int r = 0; r < R1; ++r) x[r] = __ldcg(yrow + p0 + (L / R1) * r);
+        mul_powers<R1, true>(x, g, expi_frac((j1 * p0) & (int)(n_total - 1), two_over_n));
+#pragma unroll
+        for (int r = 0; r < R1; ++r) v[u * R1 + r] = x[r];
+    }
+
+    fft_core<L, R1, 1, WSYNC>(v, t, smem + row * C::PADDED);
+
+    // v[u*RL + q] = z[j1 + N1 * j2],  j2 = t + T u + (L/RL) q
+    if constexpr (MODE == EPI_STORE) {
+        float2* __restrict__ zb = a.z_out + (size_t)b * n_total;
+#pragma unroll
+        for (int u = 0; u < E / RL; ++u)
+#pragma unroll
+            for (int q = 0; q < RL; ++q) {
+                const int j2 = t + T * u + (L / RL) * q;
+                zb[((size_t)j2 << lg1) + j1] = v[u * RL + q];
+            }
+    } else if constexpr (MODE == EPI_WSTORE) {
+        const int k_lo = a.coef->k_lo;
+#pragma unroll
+        for (int u = 0; u < E / RL; ++u)
+#pragma unroll
+            for (int q = 0; q < RL; ++q) {
+                const int j2 = t + T * u + (L / RL) * q;
+                const size_t k = ((size_t)j2 << lg1) + j1;
+                if (k < n_total / 2) {
+                    float2 o = make_float2(0.f, 0.f);
+                    if ((long long)k >= k_lo) {
+                        const double f = a.wfac[k];
+                        o = make_float2((float)(f * (double)v[u * RL + q].x), (float)(-f * (double)v[u * RL + q].y));
+                    }
+                    a.w_out[k] = o;
+                }
+            }
+    } else {
+        // ---- S6/S7: |z|^2, arg-max (lowest index on ties), threshold
+        const TemplCoef* tc = a.coef + b;
+        const float thr2 = tc->thr2, inv_sigma = tc->inv_sigma;
+        float best = -1.0f;
+        int best_e = 0;
+#pragma unroll
+        for (int q = 0; q < RL; ++q)            // j2 increases with (q, u): first maximum kept
+#pragma unroll
+            for (int u = 0; u < E / RL; ++u) {
+                const int e = u * RL + q;
+                const float p = fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
+                if (p > best) { best = p; best_e = e; }
+            }
+        if (best > thr2 && inv_sigma > 0.f) {
+#pragma unroll
+            for (int q = 0; q < RL; ++q)
+#pragma unroll
+                for (int u = 0; u < E / RL; ++u) {
+                    const int e = u * RL + q;
+                    const float p = fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
+                    if (p > thr2) {
+                        const unsigned long long slot = atomicAdd(a.trig_cursor, 1ULL);
+                        if (slot < a.trig_cap) {
+                            const int j2 = t + T * u + (L / RL) * q;
+                            TrigOut o;
+                            o.template_idx = a.tmpl_base + b;
+                            o.sample_idx = (j2 << lg1) + j1;
+                            o.snr = sqrtf(p) * inv_sigma;
+                            o.phase = atan2f(v[e].y, v[e].x);
+                            a.trig[slot] = o;
+                        }
+                    }
+                }
+        }
+        const int best_j2 = t + T * (best_e / RL) + (L / RL) * (best_e % RL);
+        const int best_j = (best_j2 << lg1) + j1;
+        const unsigned long long mykey = pack_key(best, best_j);
+        unsigned long long key = mykey;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const unsigned long long o = __shfl_xor_sync(0xFFFFFFFFu, key, off);
+            key = o > key ? o : key;
+        }
+        __shared__ unsigned long long s_keys[8];
+        __shared__ unsigned long long s_win;
+        __shared__ int s_last;
+        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        if (lane == 0) s_keys[warp] = key;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long k8 = s_keys[0];
+#pragma unroll
+            for (int i = 1; i < 8; ++i) k8 = s_keys[i] > k8 ? s_keys[i] : k8;
+            s_win = k8;
+        }
+        __syncthreads();
+        if (mykey == s_win) {            // exactly one thread: sample indices are unique
+            float re = 0.f, im = 0.f;
+#pragma unroll
+            for (int e = 0; e < E; ++e)
+                if (e == best_e) { re = v[e].x; im = v[e].y; }
+            float4 rec = make_float4(best, __int_as_float(best_j), re, im);
+            __stcg(a.cand + (size_t)b * gridDim.x + blockIdx.x, rec);
+            __threadfence();
+            const unsigned int prev = atomicAdd(a.done_ctr + b, 1u);
+            s_last = (prev == gridDim.x - 1);
+        }
+        __syncthreads();
+        if (s_last && warp == 0) {
+            __threadfence();
+            unsigned long long bk = 0ULL;
+            float bre = 0.f, bim = 0.f;
+            for (int i = lane; i < (int)gridDim.x; i += 32) {
+                const float4 r = __ldcg(a.cand + (size_t)b * gridDim.x + i);
+                const unsigned long long kk = pack_key(r.x, __float_as_int(r.y));
+                if (kk > bk) { bk = kk; bre = r.z; bim = r.w; }
+            }
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                const unsigned long long ok = __shfl_xor_sync(0xFFFFFFFFu, bk, off);
+                const float ore = __shfl_xor_sync(0xFFFFFFFFu, bre, off);
+                const float oim = __shfl_xor_sync(0xFFFFFFFFu, bim, off);
+                if (ok > bk) { bk = ok; bre = ore; bim = oim; }
+            }
+            if (lane == 0) {
+                PeakOut o;
+                if (tc->k_hi < tc->k_lo) {          // empty band
+                    o.snr_max = 0.f; o.idx_peak = -1; o.phase = 0.f; o.sigma = 0.f;
+                } else {
+                    const float p = __uint_as_float((unsigned)(bk >> 32));
+                    o.snr_max = sqrtf(p) * tc->inv_sigma;
+                    o.idx_peak = (int)(0xFFFFFFFFu - (unsigned)(bk & 0xFFFFFFFFu));
+                    o.phase = atan2f(bim, bre);
+                    o.sigma = tc->sigma;
+                }
+                a.peaks[b] = o;
+                a.done_ctr[b] = 0u;                 // self-cleaning for the next launch
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------ S0: PSD tables (fp64)
+// wfac[k] = 4 df dt f_k^{-7/6} / S_n[k]; term[k] = 4 df f_k^{-7/3} / S_n[k]  (0 outside
+// [k_lo, N/2) or where S_n = +inf).  err_flag = 1 if S_n <= 0 or NaN inside the band.
+__global__ void psd_terms_kernel(const double* __restrict__ psd, double* __restrict__ wfac,
+                                 double* __restrict__ term, int n_half, int k_lo, double df,
+                                 double dt, int* err_flag)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_half) return;
+    double wf = 0.0, tm = 0.0;
+    if (k >= k_lo) {
+        const double s = psd[k];
+        if (!(s > 0.0)) {
+            *err_flag = 1;                       // <= 0 or NaN
+        } else if (!isinf(s)) {
+            const double f = (double)k * df;
+            const double a = pow(f, -7.0 / 6.0);
+            wf = 4.0 * df * dt * a / s;
+            tm = 4.0 * df * a * a / s;
+        }
+    }
+    wfac[k] = wf;
+    term[k] = tm;
+}
+
+// Inclusive prefix sum of term[0..n) in fp64 by ONE block of 1024 threads (once per PSD).
+__global__ void __launch_bounds__(1024) prefix_sum_kernel(const double* __restrict__ term,
+                                                          double* __restrict__ prefix, int n)
+{
+    __shared__ double s_tot[1024];
+    const int tid = threadIdx.x;
+    const int chunk = (n + 1023) / 1024;
+    const int lo = tid * chunk, hi = min(n, lo + chunk);
+    double s = 0.0;
+    for (int i = lo; i < hi; ++i) s += term[i];
+    s_tot[tid] = s;
+    __syncthreads();
+    // Hillis-Steele scan over the 1024 per-thread totals
+    for (int off = 1; off < 1024; off <<= 1) {
+        const double add = (tid >= off) ? s_tot[tid - off] : 0.0;
+        __syncthreads();
+        s_tot[tid] += add;
+        __syncthreads();
+    }
+    double run = (tid > 0) ? s_tot[tid - 1] : 0.0;
+    for (int i = lo; i < hi; ++i) { run += term[i]; prefix[i] = run; }
+}
+
+// ------------------------------------------------------------------ S2: template constants (fp64)
+struct SetupArgs {
+    const double* __restrict__ bank;     // [n][2] (m1, m2)
+    const double* __restrict__ prefix;   // [N/2]
+    TemplCoef* __restrict__ coef;        // [n]
+    int n_templates;
+    int n_half;                          // N/2
+    int k_lo;
+    double n_over_fs;                    // N / fs  (= 1/df)
+    double df;
+    float threshold;
+    int* err_flag;
+};
+
+__global__ void template_setup_kernel(const SetupArgs a)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.n_templates) return;
+    const double m1 = a.bank[2 * i], m2 = a.bank[2 * i + 1];
+    TemplCoef c;
+    c.A1 = c.A2 = c.A3 = c.A5 = 0.0;
+    c.k_lo = a.k_lo; c.k_hi = -1;
+    c.sigma = c.inv_sigma = 0.f; c.thr2 = 0.f; c.nz_class = 0; c.pad_[0] = c.pad_[1] = 0;
+    if (!(m1 > 0.0) || !(m2 > 0.0) || isinf(m1) || isinf(m2)) {
+        *a.err_flag = 1;
+        a.coef[i] = c;
+        return;
+    }
+    const double PI = 3.14159265358979323846;
+    const double TSUN = 4.925490947641267e-6;           // G Msun / c^3 [s]
+    const double mt = m1 + m2;
+    const double M = mt * TSUN;
+    const double eta = m1 * m2 / (mt * mt);
+    const double f_isco = 1.0 / (pow(6.0, 1.5) * PI * M);
+    double khi = floor(f_isco * a.n_over_fs);
+    if (khi > (double)(a.n_half - 1)) khi = (double)(a.n_half - 1);
+    c.k_hi = (int)khi;
+    // Psi_T = -pi/4 + x (b4 + x (b3 + x (b2 + x^2 b0))),  x = f^{-1/3} = df^{-1/3} k^{-1/3}
+    const double c0 = 3.0 / (128.0 * eta), p = PI * M;
+    const double p13 = cbrt(p);
+    const double b0 = c0 / (p * p13 * p13);
+    const double b2 = c0 * (3715.0 / 756.0 + 55.0 * eta / 9.0) / p;
+    const double b3 = -16.0 * PI * c0 / (p13 * p13);
+    const double b4 = c0 * (15293365.0 / 508032.0 + 27145.0 * eta / 504.0 + 3085.0 * eta * eta / 72.0) / p13;
+    const double s = 1.0 / cbrt(a.df);
+    const double i2pi = 1.0 / (2.0 * PI);
+    c.A1 = b4 * s * i2pi;
+    c.A2 = b3 * s * s * i2pi;
+    c.A3 = b2 * s * s * s * i2pi;
+    c.A5 = b0 * s * s * s * s * s * i2pi;
+    if (c.k_hi >= c.k_lo) {
+        const double sig = sqrt(a.prefix[c.k_hi]);
+        c.sigma = (float)sig;
+        c.inv_sigma = (float)(1.0 / sig);
+        const double th = (double)a.threshold * sig;
+        c.thr2 = (float)(th * th);
+    }
+    a.coef[i] = c;
+}
+
+// ------------------------------------------------------------------ triggers: bitonic sort
+__device__ __forceinline__ unsigned long long trig_key(const TrigOut& t)
+{
+    return ((unsigned long long)(unsigned)t.template_idx << 32) | (unsigned)t.sample_idx;
+}
+__global__ void trig_pad_kernel(TrigOut* trig, long long n, long long n_pow2)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x + n;
+    if (i < n_pow2) { TrigOut o; o.template_idx = 0x7FFFFFFF; o.sample_idx = 0x7FFFFFFF; o.snr = 0.f; o.phase = 0.f; trig[i] = o; }
+}
+__global__ void trig_bitonic_kernel(TrigOut* trig, long long n_pow2, long long kk, long long jj)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_pow2) return;
+    const long long ixj = i ^ jj;
+    if (ixj > i) {
+        const TrigOut a = trig[i], b = trig[ixj];
+        const bool up = ((i & kk) == 0);
+        const bool gt = trig_key(a) > trig_key(b);
+        if (gt == up) { trig[i] = b; trig[ixj] = a; }
+    }
+}
+
+// Up to TRIG_SORT_SMEM_MAX triggers: one block, bitonic network in shared memory.
+constexpr int TRIG_SORT_SMEM_MAX = 2048;
+__global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, int n, int n_pow2)
+{
+    __shared__ TrigOut s[TRIG_SORT_SMEM_MAX];
+    for (int i = threadIdx.x; i < n_pow2; i += blockDim.x) {
+        TrigOut o;
+        if (i < n) o = trig[i];
+        else { o.template_idx = 0x7FFFFFFF; o.sample_idx = 0x7FFFFFFF; o.snr = 0.f; o.phase = 0.f; }
+        s[i] = o;
+    }
+    __syncthreads();
+    for (int kk = 2; kk <= n_pow2; kk <<= 1)
+        for (int jj = kk >> 1; jj > 0; jj >>= 1) {
+            for (int i = threadIdx.x; i < n_pow2; i += blockDim.x) {
+                const int ixj = i ^ jj;
+                if (ixj > i) {
+                    const TrigOut a = s[i], b = s[ixj];
+                    const bool up = ((i & kk) == 0);
+                    if ((trig_key(a) > trig_key(b)) == up) { s[i] = b; s[ixj] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = s[i];
+}
+
+// ------------------------------------------------------------------ diagnostics
+__global__ void snr_from_z_kernel(const float2* __restrict__ z, float* __restrict__ snr, size_t n, float inv_sigma)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) snr[i] = sqrtf(fmaf(z[i].x, z[i].x, z[i].y * z[i].y)) * inv_sigma;
+}
+
+// h~[k] = f_k^{-7/6} e^{-i Psi_T(f_k)} on the band, zero elsewhere, k = 0..N/2
+__global__ void debug_template_kernel(const TemplCoef* __restrict__ tc, float2* __restrict__ h, int n_half, double df)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > n_half) return;
+    float2 o = make_float2(0.f, 0.f);
+    if (k >= tc->k_lo && k <= tc->k_hi) {
+        const float2 ph = spa_phasor(k, tc->A1, tc->A2, tc->A3, tc->A5);
+        const float amp = (float)pow((double)k * df, -7.0 / 6.0);
+        o = make_float2(amp * ph.x, -amp * ph.y);
+    }
+    h[k] = o;
+}
+
+// generator alone: q~[b][k] = w[k] e^{+i Psi_b(f_k)}, k < N/2  (config-4 generator throughput)
+__global__ void __launch_bounds__(256) generate_only_kernel(const float2* __restrict__ w,
+                                                            const TemplCoef* __restrict__ coef,
+                                                            float2* __restrict__ q, int n_half)
+{
+    const int b = blockIdx.y;
+    const TemplCoef* tc = coef + b;
+    const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+    const int k_lo = tc->k_lo, k_hi = tc->k_hi;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_half; k += gridDim.x * blockDim.x) {
+        float2 o = make_float2(0.f, 0.f);
+        if (k >= k_lo && k <= k_hi) o = cmul(__ldg(w + k), spa_phasor(k, A1, A2, A3, A5));
+        q[(size_t)b * n_half + k] = o;
+    }
+}
+
+}  // namespace cbmf

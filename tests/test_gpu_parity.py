@@ -1,0 +1,325 @@
+"""-m gpu: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances: tests/parity.py (north_star).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1006_4644_b200 import workloads as W
+
+from parity import (PHASE_TOL, SERIES_TOL_OF_PEAK, check_peaks, check_triggers, mismatch, wrap_pi)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def cbmf():
+    from paper_1006_4644_b200 import cbmf as m
+    m.lib()
+    return m
+
+
+def _pair(cbmf, wl):
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd)
+    g.load_segment(wl.samples)
+    o = oracle.Oracle(wl.n, wl.fs, wl.f_low)
+    o.set_psd(wl.psd)
+    o.load_segment(wl.samples)
+    return g, o
+
+
+# ------------------------------------------------------------------ S5: the FFT alone
+
+@pytest.mark.parametrize("log2n", list(range(12, 25)))
+def test_ifft_matches_oracle_fft(cbmf, log2n):
+    """cbmf_debug_ifft vs the oracle's radix-2 FFT on random complex input, every N of the
+    sweep (configs[4]); batch 3 with sub-batch 2 -> a ragged last launch."""
+    n = 1 << log2n
+    batch = 3 if log2n <= 20 else 1
+    rng = np.random.default_rng(100 + log2n)
+    x = (rng.standard_normal((batch, n)) + 1j * rng.standard_normal((batch, n))).astype(np.complex64)
+    with cbmf.Context(n, 4096.0, 40.0) as g:
+        if batch > 1:
+            g.set_sub_batch(2)
+        got = g.debug_ifft(x)
+    for b in range(batch):
+        ref = oracle.fft(x[b].astype(np.complex128), +1)
+        err = np.max(np.abs(got[b] - ref)) / np.sqrt(np.mean(np.abs(ref) ** 2))
+        assert err < 3e-5, (log2n, b, err)          # fp32: ~ eps * log2 N * few, relative to rms
+
+
+def test_ifft_delta_and_constant(cbmf):
+    """Closed forms: delta at k0 -> e^{+2 pi i j k0/n}; constant -> n at j = 0."""
+    n = 1 << 14
+    x = np.zeros((2, n), np.complex64)
+    k0 = 1234
+    x[0, k0] = 1.0
+    x[1, :] = 1.0
+    with cbmf.Context(n, 4096.0, 40.0) as g:
+        got = g.debug_ifft(x)
+    j = np.arange(n)
+    assert np.max(np.abs(got[0] - np.exp(2j * np.pi * ((j * k0) % n) / n))) < 2e-6
+    assert abs(got[1, 0] - n) < 1e-3 * n and np.max(np.abs(got[1, 1:])) < 1e-3 * np.sqrt(n) * 4
+
+
+# ------------------------------------------------------------------ S0-S3: tables, template
+
+def test_prefix_table_and_weights_cfg0(cbmf):
+    wl = W.config0()
+    g, o = _pair(cbmf, wl)
+    P = g.debug_get_prefix()
+    for m1, m2 in wl.bank:
+        klo, khi = oracle.band(wl.n, wl.fs, wl.f_low, m1, m2)
+        assert abs(P[khi] - o.sigma2(m1, m2)) <= 1e-12 * P[khi]
+    # w[k] = 4 df d~[k] f^-7/6 / S_n[k]: rebuild from the oracle's unit template (f^-7/6 = |h~|)
+    # and its SNR series is checked elsewhere; here only structure: zero below k_lo, finite above
+    w = g.debug_get_weights()
+    klo = int(np.ceil(wl.f_low * wl.n / wl.fs))
+    assert np.all(w[:klo] == 0) and np.all(np.isfinite(w.view(np.float32)))
+    assert np.all(np.abs(w[klo:]) > 0)
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("m1,m2", [(1.4, 1.4), (1.0, 1.0), (1.0, 3.0), (10.0, 10.0), (3.0, 2.5)])
+def test_template_mismatch_vs_oracle(cbmf, m1, m2):
+    """Paper's accuracy metric (< 3e-4 / 1e-3 fp32 vs fp64); bar here 1e-6,
+    and pointwise |h_gpu - h_orc| <= 2e-5 |h| (phase error <= 2e-5 rad)."""
+    wl = W.config1(n_templates=1)
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd)
+    o = oracle.Oracle(wl.n, wl.fs, wl.f_low)
+    o.set_psd(wl.psd)
+    hg = g.debug_template(m1, m2)
+    ho = o.template(m1, m2)
+    assert np.array_equal(hg == 0, ho == 0)                       # same band
+    wgt = np.where(np.isfinite(wl.psd), 1.0 / wl.psd, 0.0)
+    assert abs(mismatch(hg, ho, wgt)) <= 1e-6
+    nz = ho != 0
+    assert np.max(np.abs(hg[nz] - ho[nz]) / np.abs(ho[nz])) <= 2e-5
+    g.close(); o.close()
+
+
+def test_template_phase_long_chirp_cfg3(cbmf):
+    """configs[3]: f_low = 10 Hz, 1+1 Msun -> Psi up to 6.7e4 rad; the fp64 phase keeps it exact."""
+    n, fs, f_low = 1 << 22, 4096.0, 10.0
+    psd = W.onesided_psd("B", n, fs, f_low)
+    g = cbmf.Context(n, fs, f_low)
+    g.set_psd(psd)
+    o = oracle.Oracle(n, fs, f_low)
+    o.set_psd(psd)
+    hg, ho = g.debug_template(1.0, 1.0), o.template(1.0, 1.0)
+    nz = ho != 0
+    assert np.array_equal(hg == 0, ho == 0)
+    assert np.max(np.abs(hg[nz] - ho[nz]) / np.abs(ho[nz])) <= 2e-5
+    g.close(); o.close()
+
+
+# ------------------------------------------------------------------ S3-S6: the SNR series
+
+def _series_case(cbmf, wl, templates):
+    g, o = _pair(cbmf, wl)
+    for (m1, m2) in templates:
+        rho_g, z_g = g.debug_snr_series(m1, m2)
+        rho_o, z_o, sig = o.snr_series(m1, m2)
+        if not sig > 0:
+            assert np.all(rho_g == 0)
+            continue
+        peak = rho_o.max()
+        assert np.max(np.abs(rho_g - rho_o)) <= SERIES_TOL_OF_PEAK * peak, (m1, m2)
+        assert np.max(np.abs(z_g - z_o)) <= SERIES_TOL_OF_PEAK * peak * sig, (m1, m2)
+    g.close(); o.close()
+
+
+def test_snr_series_cfg0_all_templates(cbmf):
+    wl = W.config0()
+    _series_case(cbmf, wl, [tuple(t) for t in wl.bank])
+
+
+@pytest.mark.parametrize("log2n", [12, 13, 15, 17, 19])
+def test_snr_series_small_sizes(cbmf, log2n):
+    """Every N1 x N2 split shape (square and 1:2), light and heavy (ISCO-cut, empty-band) banks."""
+    for heavy in (False, True):
+        wl = W.small_case(log2n=log2n, n_templates=4, heavy=heavy, seed=20 + log2n)
+        _series_case(cbmf, wl, [tuple(t) for t in wl.bank])
+
+
+# ------------------------------------------------------------------ S2-S8: filter_bank
+
+def _bank_case(cbmf, wl, sub_batch=None, idx=None):
+    """Full comparison of filter_bank on templates `idx` (default: all)."""
+    g, o = _pair(cbmf, wl)
+    if sub_batch:
+        g.set_sub_batch(sub_batch)
+    pk_g, tr_g, nf_g, rc_g = g.filter_bank(wl.bank, wl.threshold, trig_capacity=1 << 16)
+    assert rc_g == 0
+    sel = np.arange(wl.n_templates) if idx is None else np.asarray(idx)
+    pk_o, tr_o, nf_o, _ = o.filter_bank(wl.bank[sel], wl.threshold)
+    rho_cache = {}
+
+    def rho_at(t, j):
+        if t not in rho_cache:
+            rho_cache[t] = o.snr_series(*wl.bank[sel[t]])[0]
+        return rho_cache[t][j]
+
+    near = check_peaks(pk_g[sel], pk_o, rho_at)
+    # triggers of the selected templates only, oracle indices mapped back to bank indices
+    tr_o = tr_o.copy()
+    tr_o["template_idx"] = sel[tr_o["template_idx"]]
+    keep = np.isin(tr_g["template_idx"], sel)
+    ng, no = check_triggers(tr_g[keep], tr_o, wl.threshold)
+    g.close(); o.close()
+    return pk_g, tr_g, near, (ng, no)
+
+
+def test_filter_bank_cfg0(cbmf):
+    """configs[0]: 17 templates, N = 2^16, injection (1.4, 1.4) at t_c = 20 s, SNR 12."""
+    wl = W.config0()
+    pk, tr, near, (ng, no) = _bank_case(cbmf, wl)
+    inj = wl.injections[0]
+    assert pk[16]["idx_peak"] == inj.sample(wl.fs)
+    assert abs(pk[16]["snr_max"] - inj.snr) < 3.0
+    assert abs(wrap_pi(pk[16]["phase"] - inj.phi_c)) < 0.5
+    assert ng > 0 and no > 0
+    assert 16 not in near
+
+
+@pytest.mark.parametrize("sub_batch", [1, 3, 5, 64])
+def test_filter_bank_independent_of_sub_batch(cbmf, sub_batch):
+    """Ragged last launch; results bit-identical whatever the launch grouping."""
+    wl = W.config0()
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd); g.load_segment(wl.samples)
+    ref = g.filter_bank(wl.bank, wl.threshold)
+    g.set_sub_batch(sub_batch)
+    got = g.filter_bank(wl.bank, wl.threshold)
+    assert np.array_equal(ref[0], got[0]) and np.array_equal(ref[1], got[1]) and ref[2] == got[2]
+    g.close()
+
+
+@pytest.mark.parametrize("log2n", [12, 14, 17])
+def test_filter_bank_small_heavy(cbmf, log2n):
+    """Heavy masses: bands cut by f_ISCO, some empty (idx_peak = -1)."""
+    wl = W.small_case(log2n=log2n, n_templates=9, heavy=True, seed=40 + log2n)
+    wl.bank[0] = (80.0, 90.0)                         # f_ISCO ~ 25.9 Hz < f_low: empty band
+    pk, tr, near, _ = _bank_case(cbmf, wl, sub_batch=4)
+    assert pk[0]["idx_peak"] == -1
+
+
+def test_filter_bank_cfg1_sampled(cbmf):
+    """configs[1] at full size (N = 2^20, 1024 templates, the launch configuration bench.py
+    times): the 4 injection templates plus every 64th template against the oracle."""
+    wl = W.config1()
+    idx = sorted(set(range(0, 1024, 64)) | {i.template_idx for i in wl.injections})
+    pk, tr, near, (ng, no) = _bank_case(cbmf, wl, idx=idx)
+    for inj in wl.injections:
+        p = pk[inj.template_idx]
+        assert abs(int(p["idx_peak"]) - inj.sample(wl.fs)) <= 2
+        assert abs(p["snr_max"] - inj.snr) < 3.5
+        assert inj.template_idx not in near
+    assert len(near) <= 2
+    # properties that hold for every template at any size (A4: pure noise <rho^2> = 2)
+    assert np.all(pk["snr_max"] > 3.5) and np.all(pk["snr_max"] < 20)
+    assert np.all((pk["idx_peak"] >= 0) & (pk["idx_peak"] < wl.n))
+    assert np.all(tr["snr"] > wl.threshold * (1 - 1e-6))
+
+
+# ------------------------------------------------------------------ edge cases, errors
+
+def test_edge_cases_and_errors(cbmf):
+    wl = W.small_case(log2n=12, n_templates=3)
+    with pytest.raises(cbmf.CbmfError) as e:
+        cbmf.Context(3000, 2048.0, 40.0)
+    assert e.value.rc == cbmf.EINVAL
+    with pytest.raises(cbmf.CbmfError):
+        cbmf.Context(1 << 11, 2048.0, 40.0)
+    with pytest.raises(cbmf.CbmfError):
+        cbmf.Context(1 << 12, 2048.0, 2000.0)          # f_low >= fs/2
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.load_segment(wl.samples)                     # before the PSD
+    assert e.value.rc == cbmf.ESTATE
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.set_psd(wl.psd[:-1])
+    assert e.value.rc == cbmf.EINVAL
+    bad = wl.psd.copy(); bad[wl.n // 4] = -1.0
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.set_psd(bad)
+    assert e.value.rc == cbmf.EINVAL
+    bad = wl.psd.copy(); bad[wl.n // 4] = np.nan
+    with pytest.raises(cbmf.CbmfError):
+        g.set_psd(bad)
+    g.set_psd(wl.psd)
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.filter_bank(wl.bank, 6.0)                    # no segment yet
+    assert e.value.rc == cbmf.ESTATE
+    s = wl.samples.copy(); s[17] = np.inf
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.load_segment(s)
+    assert e.value.rc == cbmf.EINVAL
+    with pytest.raises(cbmf.CbmfError):
+        g.load_segment(wl.samples[:-1])
+    g.load_segment(wl.samples)
+    # empty bank
+    pk, tr, nf, rc = g.filter_bank(np.zeros((0, 2)), 6.0)
+    assert len(pk) == 0 and len(tr) == 0 and nf == 0 and rc == 0
+    # bad masses / threshold
+    for b in ([[1.4, -1.0]], [[0.0, 1.0]], [[np.nan, 1.0]], [[np.inf, 1.0]]):
+        with pytest.raises(cbmf.CbmfError) as e:
+            g.filter_bank(np.array(b), 6.0)
+        assert e.value.rc == cbmf.EINVAL
+    with pytest.raises(cbmf.CbmfError):
+        g.filter_bank(wl.bank, -1.0)
+    with pytest.raises(cbmf.CbmfError):
+        g.filter_bank(wl.bank, float("nan"))
+    # a new PSD invalidates the segment
+    g.set_psd(wl.psd)
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.filter_bank(wl.bank, 6.0)
+    assert e.value.rc == cbmf.ESTATE
+    g.close()
+
+
+def test_trigger_truncation_and_threshold_zero(cbmf):
+    """threshold 0: every sample of every non-empty template is a trigger; capacity smaller
+    than that -> WTRUNC with the full count reported; capacity 0 / NULL list allowed."""
+    wl = W.small_case(log2n=12, n_templates=3)
+    g, o = _pair(cbmf, wl)
+    pk, tr, nf, rc = g.filter_bank(wl.bank, 0.0, trig_capacity=100)
+    assert rc == cbmf.WTRUNC and nf == 3 * wl.n and len(tr) == 100
+    pk, tr, nf, rc = g.filter_bank(wl.bank, 0.0, trig_capacity=0)
+    assert nf == 3 * wl.n and len(tr) == 0
+    # everything kept: 12288 triggers through the multi-launch bitonic sort
+    pk, tr, nf, rc = g.filter_bank(wl.bank, 0.0, trig_capacity=3 * wl.n)
+    assert rc == 0 and nf == 3 * wl.n
+    assert np.array_equal(tr["template_idx"], np.repeat(np.arange(3), wl.n))
+    assert np.array_equal(tr["sample_idx"], np.tile(np.arange(wl.n), 3))
+    for t in range(3):
+        rho_o = o.snr_series(*wl.bank[t])[0]
+        assert np.max(np.abs(tr["snr"][t * wl.n:(t + 1) * wl.n] - rho_o)) <= 1e-3 * rho_o.max()
+    g.close(); o.close()
+
+
+def test_device_pointer_entry_points(cbmf):
+    """The *_dev calls (torch CUDA tensors, torch's current stream) give the same bytes."""
+    import torch
+    wl = W.config0()
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd); g.load_segment(wl.samples)
+    ref_pk, ref_tr, ref_nf, _ = g.filter_bank(wl.bank, wl.threshold, trig_capacity=4096)
+    g.close()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        g = cbmf.Context(wl.n, wl.fs, wl.f_low, stream=s.cuda_stream)
+        g.set_psd(torch.from_numpy(wl.psd).cuda())
+        g.load_segment(torch.from_numpy(wl.samples).cuda())
+        bank = torch.from_numpy(wl.bank).cuda()
+        peaks = torch.zeros(wl.n_templates * 16, dtype=torch.uint8, device="cuda")
+        trig = torch.zeros(4096 * 16, dtype=torch.uint8, device="cuda")
+        nf, rc = g.filter_bank_into(bank, wl.threshold, peaks, trig, 4096)
+        s.synchronize()
+    assert rc == 0 and nf == ref_nf
+    pk = peaks.cpu().numpy().view(cbmf.PEAK_DTYPE)
+    tr = trig.cpu().numpy().view(cbmf.TRIG_DTYPE)[:nf]
+    assert np.array_equal(pk, ref_pk) and np.array_equal(tr, ref_tr)
+    g.close()
