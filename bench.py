@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py -- templates/s matched-filtered at N = 2^20 on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg3] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (set_psd,
+load_segment, template setup, SPA generation, correlate, inverse FFT, |z|/sigma, peak +
+threshold, results) of ONE data segment against ONE bank, through the C ABI of
+include/cbmf.h.  Default workload: BASELINE.json configs[1] (N = 2^20, fs = 4096 Hz,
+1024 templates U[1,3]^2 Msun, 4 injections, threshold 6).
+
+  value     templates/s, inputs and outputs resident in HBM (cbmf_*_dev entry points),
+            CUDA events on the context's stream, L2 flushed between timed steps.
+  e2e       the same step through the host-pointer entry points: pinned host PSD /
+            samples / bank in, peaks and triggers out, every copy inside the timed region.
+  roofline  dominant kernel (the slower of the two FFT passes): algorithmic flops per
+            launch / mean launch duration (CUDA events around every launch of the pass,
+            taken in a second set of K steps so the events do not perturb `value`).
+  cpu_baseline  the CPU oracle (oracle/, fp64, as it stands) on a bounded sample of the
+            same workload, host cores of this box.
+
+Multi-GPU (torchrun, one rank per GPU): the bank is sharded by contiguous slices, the
+segment is replicated, no data-path collective; weak scaling: every rank
+filters a full-size bank slice.  --impl reference times the oracle (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "templates/sec matched-filtered at N=2^20 (1 B200) and % of FFT roofline"
+UNIT = "templates/s"
+# FP32 ALU peak of one B200 from unit counts and clocks (B200_PROFILING.md table: 148 SMs,
+# clocks.max.sm 1965 MHz; 128 FP32 lanes per SM, FMA = 2 flop): DESIGN.md §6.
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def make_workload(name: str, world: int, rank: int):
+    """Seeded synthetic workload; for world > 1 the bank is world x the config's size and
+    this rank takes slice `rank` (weak scaling)."""
+    from paper_1006_4644_b200 import workloads as W
+    from paper_1006_4644_b200.sharding import shard_range
+    wl = W.by_name(name)
+    per_rank = wl.n_templates
+    if world > 1:
+        seed, lo, hi = {"cfg1": (3, 1.0, 3.0), "cfg2": (4, 1.0, 10.0), "cfg3": (5, 1.0, 5.0)}[name]
+        full = W.draw_bank(seed, per_rank * world, lo, hi)      # first per_rank rows == the config's bank
+        a, b = shard_range(per_rank * world, rank, world)
+        wl.bank = np.ascontiguousarray(full[a:b])
+    return wl
+
+
+class ClockSampler:
+    """SM clock and throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index: int, period_s: float = 0.05):
+        self.index, self.period = index, period_s
+        self.sm, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self._nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = index
+            if vis:
+                ids = [v for v in vis.split(",") if v.strip() != ""]
+                if index < len(ids) and ids[index].strip().isdigit():
+                    phys = int(ids[index])
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nvml = None
+
+    def _run(self):
+        n = self._nvml
+        names = {
+            "hw_slowdown": getattr(n, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(n, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(n, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(n, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(n, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.sm.append(float(n.nvmlDeviceGetClockInfo(self._h, n.NVML_CLOCK_SM)))
+                r = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self._nvml is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                    "note": "nvml unavailable or region shorter than one sample"}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+def pass_flops(n: int, lg1: int, lg2: int, n_b_mean: float):
+    """Algorithmic flops per template of the two FFT passes:
+    pass 1 = N1-point column FFTs (5 N log2 N1) + generator/correlate (48 per in-band bin);
+    pass 2 = N2-point row FFTs (5 N log2 N2) + |z|^2 / peak / threshold (6 N)."""
+    return 5.0 * n * lg1 + 48.0 * n_b_mean, 5.0 * n * lg2 + 6.0 * n
+
+
+def mean_band_bins(wl) -> float:
+    """Mean number of in-band bins k_lo..k_hi over the bank (host arithmetic on inputs only)."""
+    from paper_1006_4644_b200.workloads import T_SUN_S
+    mt = wl.bank[:, 0] + wl.bank[:, 1]
+    f_isco = 1.0 / (6.0 ** 1.5 * np.pi * mt * T_SUN_S)
+    k_lo = math.ceil(wl.f_low * wl.n / wl.fs)
+    k_hi = np.minimum(np.floor(f_isco * wl.n / wl.fs), wl.n // 2 - 1)
+    return float(np.mean(np.maximum(k_hi - k_lo + 1, 0)))
+
+
+def oracle_rate(wl, n_sample: int, repeats: int = 1):
+    """Time the CPU oracle, as it stands, on the first n_sample templates of the workload."""
+    import oracle
+    o = oracle.Oracle(wl.n, wl.fs, wl.f_low)
+    o.set_psd(wl.psd)
+    o.load_segment(wl.samples)
+    bank = np.ascontiguousarray(wl.bank[:n_sample])
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        o.filter_bank(bank, wl.threshold)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    o.close()
+    return n_sample / best, best, oracle.num_threads()
+
+
+# --------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    rank = _env_int("RANK", 0)
+    if rank != 0:
+        return 0
+    import oracle
+    wl = make_workload(args.workload, 1, 0)
+    cores = oracle.num_threads()
+    n_sample = max(1, min(wl.n_templates, cores))          # one template per thread per step
+    o = oracle.Oracle(wl.n, wl.fs, wl.f_low)
+    bank = np.ascontiguousarray(wl.bank[:n_sample])
+    def step():
+        o.set_psd(wl.psd)
+        o.load_segment(wl.samples)
+        o.filter_bank(bank, wl.threshold)
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    value = n_sample * args.steps / dt
+    sample = f"first {n_sample} templates of {wl.name} per step (1 per thread), set_psd + load_segment + filter_bank"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": wl.name, "n": wl.n, "fs_hz": wl.fs, "f_low_hz": wl.f_low,
+                   "templates_per_step": n_sample, "threshold": wl.threshold},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1006_4644_b200 import cbmf
+
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = make_workload(args.workload, world, rank)
+    B, n = wl.n_templates, wl.n
+    cap = args.trig_capacity
+    stream = torch.cuda.Stream(device=dev)
+    K, Wm = args.steps, args.warmup
+
+    with torch.cuda.stream(stream):
+        ctx = cbmf.Context(n, wl.fs, wl.f_low, device=local, stream=stream.cuda_stream)
+        if args.sub_batch:
+            ctx.set_sub_batch(args.sub_batch)
+        psd_d = torch.from_numpy(wl.psd).to(dev)
+        smp_d = torch.from_numpy(wl.samples).to(dev)
+        bank_d = torch.from_numpy(np.ascontiguousarray(wl.bank)).to(dev)
+        peaks_d = torch.empty(B * 16, dtype=torch.uint8, device=dev)
+        trig_d = torch.empty(cap * 16, dtype=torch.uint8, device=dev)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+        def step_dev():
+            ctx.set_psd(psd_d)
+            ctx.load_segment(smp_d)
+            return ctx.filter_bank_into(bank_d, wl.threshold, peaks_d, trig_d, cap)
+
+        def timed(fn, k, with_flush=True):
+            """k steps, each bracketed by CUDA events on the context's stream; L2 flushed
+            (untimed) before every step.  -> (sum of step times in ms, last result)"""
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+            res = None
+            for i in range(k):
+                if with_flush:
+                    flush.fill_(i & 0xFF)
+                evs[i][0].record(stream)
+                res = fn()
+                evs[i][1].record(stream)
+            stream.synchronize()
+            return sum(a.elapsed_time(b) for a, b in evs), res
+
+        def barrier():
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+
+        # ---- device-resident leg: `value`
+        for _ in range(Wm):
+            flush.fill_(1)
+            step_dev()
+        barrier()
+        l0 = ctx.launch_count()
+        with ClockSampler(local) as clk:
+            ms_total, (nf, rc) = timed(step_dev, K)
+        barrier()
+        launches = ctx.launch_count() - l0
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_max = float(t.item())
+        value = B * world * K / (ms_max * 1e-3)
+
+        # ---- roofline leg: per-launch events inside K more steps
+        ctx.set_profiling(True)
+        p_ms, p_n = [0.0, 0.0], [0, 0]
+        for i in range(K):
+            flush.fill_(i & 0xFF)
+            step_dev()
+            for w in (0, 1):
+                ms, nl = ctx.last_pass_time(w)
+                p_ms[w] += ms
+                p_n[w] += nl
+        ctx.set_profiling(False)
+        sub = ctx.get_sub_batch()
+
+        # ---- e2e leg: host-pointer entry points, pinned host buffers
+        psd_h = torch.from_numpy(wl.psd).pin_memory()
+        smp_h = torch.from_numpy(wl.samples).pin_memory()
+        bank_h = torch.from_numpy(np.ascontiguousarray(wl.bank)).pin_memory()
+        peaks_h = torch.empty(B * 16, dtype=torch.uint8).pin_memory()
+        trig_h = torch.empty(cap * 16, dtype=torch.uint8).pin_memory()
+
+        def step_host():
+            ctx.set_psd(psd_h)
+            ctx.load_segment(smp_h)
+            return ctx.filter_bank_into(bank_h, wl.threshold, peaks_h, trig_h, cap)
+
+        for _ in range(Wm):
+            step_host()
+        barrier()
+        e_ms, (nf_h, rc_h) = timed(step_host, K)
+        barrier()
+        te = torch.tensor([e_ms], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e_value = B * world * K / (float(te.item()) * 1e-3)
+        h2d = psd_h.numel() * 8 + smp_h.numel() * 4 + bank_h.numel() * 8
+        d2h = B * 16 + min(nf_h, cap) * 16 + 4 + 4 + 4 + 8      # peaks, triggers, 3 status words, trigger count
+
+        peaks = np.frombuffer(peaks_h.numpy().tobytes(), dtype=cbmf.PEAK_DTYPE)
+        ctx.close()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline numbers for the dominant pass
+    lg = int(math.log2(n))
+    lg1 = lg // 2
+    lg2 = lg - lg1
+    n_b = mean_band_bins(wl)
+    f1, f2 = pass_flops(n, lg1, lg2, n_b)
+    which = 0 if p_ms[0] >= p_ms[1] else 1
+    avg_launch_ms = p_ms[which] / max(p_n[which], 1)
+    tmpl_per_launch = B * K / max(p_n[which], 1)
+    flops_launch = (f1, f2)[which] * tmpl_per_launch
+    achieved = flops_launch / (avg_launch_ms * 1e-3) / 1e12
+    peaks_file = {}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            peaks_file = json.load(fh)
+    except Exception:
+        pass
+    roofline = {
+        "bound": "alu", "kernel": ("p1_kernel (SPA generate + correlate + column FFT)",
+                                   "p2_kernel (twiddle + row FFT + |z|^2 + arg-max/threshold)")[which],
+        "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
+        "peak_source": "148 SM x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md §6)",
+        "traffic": None,
+        "flops_per_launch": flops_launch, "avg_launch_ms": avg_launch_ms, "templates_per_launch": tmpl_per_launch,
+        "pass_ms_per_step": [p_ms[0] / K, p_ms[1] / K],
+        "whole_path": {
+            "flops_per_template": f1 + f2, "us_per_template": 1e3 * ms_max / (B * K),
+            "achieved_tflops": (f1 + f2) * B * world * K / (ms_max * 1e-3) / 1e12 / world,
+            "frac_of_fp32_peak": (f1 + f2) * B * K / (ms_max * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+            "inter_pass_bytes_per_template": 16 * n,
+            "hbm_gbs_measured_peak": peaks_file.get("hbm_gbs"),
+        },
+    }
+
+    # ---- CPU oracle on a bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        import oracle
+        cores = oracle.num_threads()
+        n_sample = min(B, max(32, 2 * cores))
+        v, secs, cores = oracle_rate(wl, n_sample)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {n_sample} templates of {wl.name}, filter_bank only, {secs:.2f} s wall"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": wl.name, "n": n, "fs_hz": wl.fs, "f_low_hz": wl.f_low,
+                   "templates_per_step_per_gpu": B, "threshold": wl.threshold, "sub_batch": sub,
+                   "l2": "flushed (256 MiB fill) before every timed step",
+                   "step": "set_psd + load_segment + filter_bank (S0-S8)",
+                   "parallelism": f"bank sharded over {world} GPU(s), segment replicated"},
+        "segment_seconds_per_wall_second": (n / wl.fs) / (ms_max / K * 1e-3),
+        "triggers_found": int(nf), "peak_snr_max": float(peaks["snr_max"].max()),
+        "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": int(launches),
+        "clocks": clk.summary(),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3"], default="cfg1")
+    ap.add_argument("--sub-batch", type=int, default=0, help="templates per launch pair (0 = library default)")
+    ap.add_argument("--trig-capacity", type=int, default=1 << 16)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
