@@ -30,6 +30,7 @@ struct cbmf_ctx {
     double* d_wfac = nullptr;              // [N/2]
     double* d_term = nullptr;              // [N/2]
     double* d_prefix = nullptr;            // [N/2]
+    double* d_bsum = nullptr;              // [ceil(N/2 / SCAN_TILE)] scan block totals / offsets
     float2* d_w = nullptr;                 // [N/2]
     float2* d_Y = nullptr;                 // [max_sub_batch][N]
     float4* d_cand = nullptr;              // [max_sub_batch][p2 grid.x]
@@ -205,7 +206,7 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     if (!c) return CBMF_EINVAL;
     DeviceGuard g(c->device);
     cudaStreamSynchronize(c->stream);
-    cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_w);
+    cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_bsum); cudaFree(c->d_w);
     cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_err);
     cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
     cudaFree(c->d_trig); cudaFree(c->d_scratch);
@@ -260,6 +261,7 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     CUF(cudaMalloc(&c->d_wfac, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_term, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_prefix, sizeof(double) * nh));
+    CUF(cudaMalloc(&c->d_bsum, sizeof(double) * ((nh + SCAN_TILE - 1) / SCAN_TILE)));
     CUF(cudaMalloc(&c->d_w, sizeof(float2) * nh));
     CUF(cudaMalloc(&c->d_Y, sizeof(float2) * (size_t)n * c->max_sub_batch));
     CUF(cudaMalloc(&c->d_cand, sizeof(float4) * (size_t)p2grid * c->max_sub_batch));
@@ -303,12 +305,15 @@ static int set_psd_impl(cbmf_ctx* c, const double* psd_dev)
     const int nh = (int)(c->n / 2);
     c->have_psd = false; c->have_seg = false;
     CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
-    psd_terms_kernel<<<(nh + 255) / 256, 256, 0, c->stream>>>(psd_dev, c->d_wfac, c->d_term, nh, c->k_lo,
-                                                             c->df, c->dt, c->d_err);
+    const int nblk = (nh + SCAN_TILE - 1) / SCAN_TILE;
+    psd_terms_kernel<<<nblk, SCAN_THREADS, 0, c->stream>>>(psd_dev, c->d_wfac, c->d_term, c->d_bsum, nh, c->k_lo,
+                                                           c->df, c->dt, c->d_err);
     CU(cudaGetLastError());
-    prefix_sum_kernel<<<1, 1024, 0, c->stream>>>(c->d_term, c->d_prefix, nh);
+    scan_block_sums_kernel<<<1, SCAN_THREADS, 0, c->stream>>>(c->d_bsum, nblk);
     CU(cudaGetLastError());
-    c->launches += 2;
+    prefix_tile_kernel<<<nblk, SCAN_THREADS, 0, c->stream>>>(c->d_term, c->d_bsum, c->d_prefix, nh);
+    CU(cudaGetLastError());
+    c->launches += 3;
     int err = 0;
     CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
@@ -390,24 +395,29 @@ static int sort_triggers(cbmf_ctx* c, int64_t count)
     if (count <= 1) return CBMF_OK;
     long long np2 = 1;
     while (np2 < count) np2 <<= 1;
-    if (np2 <= TRIG_SORT_SMEM_MAX) {
-        trig_sort_small_kernel<<<1, 1024, 0, c->stream>>>(c->d_trig, (int)count, (int)np2);
-        CU(cudaGetLastError());
-        c->launches += 1;
-        return CBMF_OK;
+    const int tile = (int)(np2 < TRIG_TILE ? np2 : TRIG_TILE);
+    const size_t smem = sizeof(TrigOut) * (size_t)tile;
+    static bool attr_done = false;
+    if (!attr_done) {
+        CU(cudaFuncSetAttribute(trig_sort_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(sizeof(TrigOut) * TRIG_TILE)));
+        attr_done = true;
     }
+    const unsigned tiles = (unsigned)(np2 / tile);
+    trig_sort_tile_kernel<<<tiles, 1024, smem, c->stream>>>(c->d_trig, count, tile, 0);
+    CU(cudaGetLastError());
+    c->launches += 1;
     const unsigned blocks = (unsigned)((np2 + 255) / 256);
-    if (np2 > count) {
-        trig_pad_kernel<<<(unsigned)((np2 - count + 255) / 256), 256, 0, c->stream>>>(c->d_trig, count, np2);
-        CU(cudaGetLastError());
-        c->launches += 1;
-    }
-    for (long long kk = 2; kk <= np2; kk <<= 1)
-        for (long long jj = kk >> 1; jj > 0; jj >>= 1) {
+    for (long long kk = 2LL * tile; kk <= np2; kk <<= 1) {
+        for (long long jj = kk >> 1; jj >= tile; jj >>= 1) {
             trig_bitonic_kernel<<<blocks, 256, 0, c->stream>>>(c->d_trig, np2, kk, jj);
             CU(cudaGetLastError());
             c->launches += 1;
         }
+        trig_sort_tile_kernel<<<tiles, 1024, smem, c->stream>>>(c->d_trig, count, tile, kk);
+        CU(cudaGetLastError());
+        c->launches += 1;
+    }
     return CBMF_OK;
 }
 

@@ -424,49 +424,97 @@ __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
 // ------------------------------------------------------------------ S0: PSD tables (fp64)
 // wfac[k] = 4 df dt f_k^{-7/6} / S_n[k]; term[k] = 4 df f_k^{-7/3} / S_n[k]  (0 outside
 // [k_lo, N/2) or where S_n = +inf).  err_flag = 1 if S_n <= 0 or NaN inside the band.
-__global__ void psd_terms_kernel(const double* __restrict__ psd, double* __restrict__ wfac,
-                                 double* __restrict__ term, int n_half, int k_lo, double df,
-                                 double dt, int* err_flag)
+// prefix[k] = sum_{k' <= k} term[k'] is built by a three-launch scan: every block of
+// SCAN_TILE bins writes its total (psd_terms_kernel), one block scans the totals
+// (scan_block_sums_kernel), every block rescans its tile from its offset (prefix_tile_kernel).
+constexpr int SCAN_THREADS = 256, SCAN_PER_THREAD = 4, SCAN_TILE = SCAN_THREADS * SCAN_PER_THREAD;
+
+// Exclusive scan of one value per thread over a block of SCAN_THREADS threads; *total = block sum.
+__device__ __forceinline__ double block_exclusive_scan(double x, double* total)
 {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_half) return;
-    double wf = 0.0, tm = 0.0;
-    if (k >= k_lo) {
-        const double s = psd[k];
-        if (!(s > 0.0)) {
-            *err_flag = 1;                       // <= 0 or NaN
-        } else if (!isinf(s)) {
-            const double f = (double)k * df;
-            const double a = pow(f, -7.0 / 6.0);
-            wf = 4.0 * df * dt * a / s;
-            tm = 4.0 * df * a * a / s;
-        }
+    __shared__ double s_warp[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double inc = x;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const double o = __shfl_up_sync(0xFFFFFFFFu, inc, off);
+        if (lane >= off) inc += o;
     }
-    wfac[k] = wf;
-    term[k] = tm;
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    double base = 0.0, tot = 0.0;
+#pragma unroll
+    for (int i = 0; i < SCAN_THREADS / 32; ++i) {
+        const double v = s_warp[i];
+        if (i < warp) base += v;
+        tot += v;
+    }
+    __syncthreads();
+    *total = tot;
+    return base + inc - x;
 }
 
-// Inclusive prefix sum of term[0..n) in fp64 by ONE block of 1024 threads (once per PSD).
-__global__ void __launch_bounds__(1024) prefix_sum_kernel(const double* __restrict__ term,
-                                                          double* __restrict__ prefix, int n)
+__global__ void __launch_bounds__(SCAN_THREADS) psd_terms_kernel(
+    const double* __restrict__ psd, double* __restrict__ wfac, double* __restrict__ term,
+    double* __restrict__ block_sum, int n_half, int k_lo, double df, double dt, int* err_flag)
 {
-    __shared__ double s_tot[1024];
-    const int tid = threadIdx.x;
-    const int chunk = (n + 1023) / 1024;
-    const int lo = tid * chunk, hi = min(n, lo + chunk);
-    double s = 0.0;
-    for (int i = lo; i < hi; ++i) s += term[i];
-    s_tot[tid] = s;
-    __syncthreads();
-    // Hillis-Steele scan over the 1024 per-thread totals
-    for (int off = 1; off < 1024; off <<= 1) {
-        const double add = (tid >= off) ? s_tot[tid - off] : 0.0;
-        __syncthreads();
-        s_tot[tid] += add;
-        __syncthreads();
+    const int k0 = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_PER_THREAD;
+    double local = 0.0;
+#pragma unroll
+    for (int i = 0; i < SCAN_PER_THREAD; ++i) {
+        const int k = k0 + i;
+        if (k >= n_half) break;
+        double wf = 0.0, tm = 0.0;
+        if (k >= k_lo) {
+            const double s = psd[k];
+            if (!(s > 0.0)) {
+                *err_flag = 1;                       // <= 0 or NaN
+            } else if (!isinf(s)) {
+                const double f = (double)k * df;
+                const double a = pow(f, -7.0 / 6.0);
+                wf = 4.0 * df * dt * a / s;
+                tm = 4.0 * df * a * a / s;
+            }
+        }
+        wfac[k] = wf;
+        term[k] = tm;
+        local += tm;
     }
-    double run = (tid > 0) ? s_tot[tid - 1] : 0.0;
-    for (int i = lo; i < hi; ++i) { run += term[i]; prefix[i] = run; }
+    double total;
+    block_exclusive_scan(local, &total);
+    if (threadIdx.x == 0) block_sum[blockIdx.x] = total;
+}
+
+// In-place exclusive scan of the block totals (at most 2^23 / SCAN_TILE = 8192) by one block.
+__global__ void __launch_bounds__(SCAN_THREADS) scan_block_sums_kernel(double* __restrict__ block_sum, int n_blocks)
+{
+    const int chunk = (n_blocks + SCAN_THREADS - 1) / SCAN_THREADS;
+    const int lo = threadIdx.x * chunk, hi = min(n_blocks, lo + chunk);
+    double s = 0.0;
+    for (int i = lo; i < hi; ++i) s += block_sum[i];
+    double total;
+    double run = block_exclusive_scan(s, &total);
+    for (int i = lo; i < hi; ++i) { const double v = block_sum[i]; block_sum[i] = run; run += v; }
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) prefix_tile_kernel(
+    const double* __restrict__ term, const double* __restrict__ block_off, double* __restrict__ prefix, int n_half)
+{
+    const int k0 = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_PER_THREAD;
+    double v[SCAN_PER_THREAD];
+    double local = 0.0;
+#pragma unroll
+    for (int i = 0; i < SCAN_PER_THREAD; ++i) {
+        v[i] = (k0 + i < n_half) ? term[k0 + i] : 0.0;
+        local += v[i];
+    }
+    double total;
+    double run = block_off[blockIdx.x] + block_exclusive_scan(local, &total);
+#pragma unroll
+    for (int i = 0; i < SCAN_PER_THREAD; ++i) {
+        run += v[i];
+        if (k0 + i < n_half) prefix[k0 + i] = run;
+    }
 }
 
 // ------------------------------------------------------------------ S2: template constants (fp64)
@@ -530,14 +578,13 @@ __global__ void template_setup_kernel(const SetupArgs a)
 }
 
 // ------------------------------------------------------------------ triggers: bitonic sort
+// Sort by (template, sample).  Tiles of up to TRIG_TILE records are sorted / merged in shared
+// memory (trig_sort_tile_kernel); only compare distances >= TRIG_TILE go through global memory
+// (trig_bitonic_kernel).  Entries at index >= n are padding (maximal key).
+constexpr int TRIG_TILE = 8192;                 // 128 KB of shared memory
 __device__ __forceinline__ unsigned long long trig_key(const TrigOut& t)
 {
     return ((unsigned long long)(unsigned)t.template_idx << 32) | (unsigned)t.sample_idx;
-}
-__global__ void trig_pad_kernel(TrigOut* trig, long long n, long long n_pow2)
-{
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x + n;
-    if (i < n_pow2) { TrigOut o; o.template_idx = 0x7FFFFFFF; o.sample_idx = 0x7FFFFFFF; o.snr = 0.f; o.phase = 0.f; trig[i] = o; }
 }
 __global__ void trig_bitonic_kernel(TrigOut* trig, long long n_pow2, long long kk, long long jj)
 {
@@ -552,31 +599,34 @@ __global__ void trig_bitonic_kernel(TrigOut* trig, long long n_pow2, long long k
     }
 }
 
-// Up to TRIG_SORT_SMEM_MAX triggers: one block, bitonic network in shared memory.
-constexpr int TRIG_SORT_SMEM_MAX = 2048;
-__global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, int n, int n_pow2)
+// tile = min(n_pow2, TRIG_TILE) records per block.  kk_merge == 0: load with padding and run the
+// whole network kk = 2..tile; otherwise finish stage kk_merge (jj = tile/2 .. 1).
+__global__ void __launch_bounds__(1024) trig_sort_tile_kernel(TrigOut* trig, long long n, int tile, long long kk_merge)
 {
-    __shared__ TrigOut s[TRIG_SORT_SMEM_MAX];
-    for (int i = threadIdx.x; i < n_pow2; i += blockDim.x) {
+    extern __shared__ __align__(16) unsigned char trig_smem_raw[];
+    TrigOut* s = reinterpret_cast<TrigOut*>(trig_smem_raw);
+    const long long base = (long long)blockIdx.x * tile;
+    for (int i = threadIdx.x; i < tile; i += blockDim.x) {
         TrigOut o;
-        if (i < n) o = trig[i];
+        if (kk_merge != 0 || base + i < n) o = trig[base + i];
         else { o.template_idx = 0x7FFFFFFF; o.sample_idx = 0x7FFFFFFF; o.snr = 0.f; o.phase = 0.f; }
         s[i] = o;
     }
     __syncthreads();
-    for (int kk = 2; kk <= n_pow2; kk <<= 1)
-        for (int jj = kk >> 1; jj > 0; jj >>= 1) {
-            for (int i = threadIdx.x; i < n_pow2; i += blockDim.x) {
+    const long long kk_first = kk_merge ? kk_merge : 2, kk_last = kk_merge ? kk_merge : tile;
+    for (long long kk = kk_first; kk <= kk_last; kk <<= 1)
+        for (int jj = (int)((kk >> 1) < tile ? (kk >> 1) : (tile >> 1)); jj > 0; jj >>= 1) {
+            for (int i = threadIdx.x; i < tile; i += blockDim.x) {
                 const int ixj = i ^ jj;
                 if (ixj > i) {
                     const TrigOut a = s[i], b = s[ixj];
-                    const bool up = ((i & kk) == 0);
+                    const bool up = (((base + i) & kk) == 0);
                     if ((trig_key(a) > trig_key(b)) == up) { s[i] = b; s[ixj] = a; }
                 }
             }
             __syncthreads();
         }
-    for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = s[i];
+    for (int i = threadIdx.x; i < tile; i += blockDim.x) trig[base + i] = s[i];
 }
 
 // ------------------------------------------------------------------ diagnostics
