@@ -97,72 +97,76 @@ int grow_scratch(cbmf_ctx* c, size_t bytes)
 
 int ilog2(int64_t n) { int l = 0; while ((int64_t(1) << l) < n) ++l; return l; }
 
-// ---------------------------------------------------------------- launch dispatch over L
-template <int L> size_t p1_smem() { return sizeof(float2) * (size_t)Cfg<L>::PADDED * Cfg<L>::C; }
-template <int L> size_t p2_smem() { return sizeof(float2) * (size_t)Cfg<L>::PADDED * Cfg<L>::ROWS; }
-
-template <int L, int MODE>
+// ---------------------------------------------------------------- launch dispatch over (N1, N2)
+template <int L1, int L2, int MODE>
 cudaError_t launch_p1_L(cudaStream_t s, const P1Args& a, int batch)
 {
     static bool attr_done = false;
-    const size_t smem = p1_smem<L>();
+    const size_t smem = sizeof(float2) * (size_t)Cfg<L1>::PADDED * Cfg<L1>::C;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(p1_kernel<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(p1_kernel<L1, L2, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int n2 = 1 << a.log2_n2;
-    dim3 grid(n2 / Cfg<L>::C, batch);
-    p1_kernel<L, MODE><<<grid, Cfg<L>::NT1, smem, s>>>(a);
+    dim3 grid(L2 / Cfg<L1>::C, batch);
+    p1_kernel<L1, L2, MODE><<<grid, Cfg<L1>::NT1, smem, s>>>(a);
     return cudaGetLastError();
 }
 
-template <int L, int MODE>
+template <int L1, int L2, int MODE>
+constexpr int p2_items() { return L1 / (Cfg<L2>::ROWS * (MODE == EPI_MAX ? p2_rpw<L1, L2>() : 1)); }
+
+template <int L1, int L2, int MODE>
 cudaError_t launch_p2_L(cudaStream_t s, const P2Args& a, int batch)
 {
     static bool attr_done = false;
-    const size_t smem = p2_smem<L>();
+    const size_t smem = sizeof(float2) * (size_t)p2_row_stride<L2>() * Cfg<L2>::ROWS;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(p2_kernel<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(p2_kernel<L1, L2, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int n1 = 1 << a.log2_n1;
-    dim3 grid(n1 / Cfg<L>::ROWS, batch);
-    p2_kernel<L, MODE><<<grid, Cfg<L>::NT2, smem, s>>>(a);
+    dim3 grid(p2_items<L1, L2, MODE>(), batch);
+    p2_kernel<L1, L2, MODE><<<grid, Cfg<L2>::NT2, smem, s>>>(a);
     return cudaGetLastError();
 }
 
-#define CBMF_DISPATCH_L(lg, FN, ...)                      \
-    switch (lg) {                                          \
-        case 6:  return FN<64, MODE>(__VA_ARGS__);         \
-        case 7:  return FN<128, MODE>(__VA_ARGS__);        \
-        case 8:  return FN<256, MODE>(__VA_ARGS__);        \
-        case 9:  return FN<512, MODE>(__VA_ARGS__);        \
-        case 10: return FN<1024, MODE>(__VA_ARGS__);       \
-        case 11: return FN<2048, MODE>(__VA_ARGS__);       \
-        case 12: return FN<4096, MODE>(__VA_ARGS__);       \
-        default: return cudaErrorInvalidValue;             \
+// N = 2^(lg1 + lg2) with lg2 = lg1 or lg1 + 1 (cbmf_create), 6 <= lg1 <= 12
+#define CBMF_DISPATCH(lg1, lg2, EXPR)                                               \
+    switch ((lg1) * 2 + ((lg2) - (lg1))) {                                         \
+        case 12: { constexpr int L1 = 64,   L2 = 64;   return EXPR; }              \
+        case 13: { constexpr int L1 = 64,   L2 = 128;  return EXPR; }              \
+        case 14: { constexpr int L1 = 128,  L2 = 128;  return EXPR; }              \
+        case 15: { constexpr int L1 = 128,  L2 = 256;  return EXPR; }              \
+        case 16: { constexpr int L1 = 256,  L2 = 256;  return EXPR; }              \
+        case 17: { constexpr int L1 = 256,  L2 = 512;  return EXPR; }              \
+        case 18: { constexpr int L1 = 512,  L2 = 512;  return EXPR; }              \
+        case 19: { constexpr int L1 = 512,  L2 = 1024; return EXPR; }              \
+        case 20: { constexpr int L1 = 1024, L2 = 1024; return EXPR; }              \
+        case 21: { constexpr int L1 = 1024, L2 = 2048; return EXPR; }              \
+        case 22: { constexpr int L1 = 2048, L2 = 2048; return EXPR; }              \
+        case 23: { constexpr int L1 = 2048, L2 = 4096; return EXPR; }              \
+        case 24: { constexpr int L1 = 4096, L2 = 4096; return EXPR; }              \
+        default: return cudaErrorInvalidValue;                                      \
     }
 
 template <int MODE>
-cudaError_t launch_p1(int lg1, cudaStream_t s, const P1Args& a, int batch)
+cudaError_t launch_p1(int lg1, int lg2, cudaStream_t s, const P1Args& a, int batch)
 {
-    CBMF_DISPATCH_L(lg1, launch_p1_L, s, a, batch)
+    CBMF_DISPATCH(lg1, lg2, (launch_p1_L<L1, L2, MODE>(s, a, batch)))
 }
 template <int MODE>
-cudaError_t launch_p2(int lg2, cudaStream_t s, const P2Args& a, int batch)
+cudaError_t launch_p2(int lg1, int lg2, cudaStream_t s, const P2Args& a, int batch)
 {
-    CBMF_DISPATCH_L(lg2, launch_p2_L, s, a, batch)
+    CBMF_DISPATCH(lg1, lg2, (launch_p2_L<L1, L2, MODE>(s, a, batch)))
 }
 
-int p2_rows(int lg2)
+// blocks per template of the arg-max pass (size of one row of the candidate buffer)
+int p2_peak_items(int lg1, int lg2)
 {
-    switch (lg2) {
-        case 6: return Cfg<64>::ROWS;   case 7: return Cfg<128>::ROWS;  case 8: return Cfg<256>::ROWS;
-        case 9: return Cfg<512>::ROWS;  case 10: return Cfg<1024>::ROWS; case 11: return Cfg<2048>::ROWS;
-        default: return Cfg<4096>::ROWS;
-    }
+    auto f = [&]() -> int { CBMF_DISPATCH(lg1, lg2, (p2_items<L1, L2, EPI_MAX>())) };
+    const int v = f();
+    return v > 0 ? v : 1;
 }
 
 // pass-timing events (cbmf_set_profiling): one start/stop pair per launch
@@ -256,7 +260,7 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     auto fail = [&](int rc) { cbmf_destroy(c); return rc; };
     if (!g.ok) return fail(CBMF_ECUDA);
     const size_t nh = (size_t)n / 2;
-    const int p2grid = (1 << c->lg1) / p2_rows(c->lg2);
+    const int p2grid = p2_peak_items(c->lg1, c->lg2);
 #define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(cuda_fail(nullptr, e__, #call)); } while (0)
     CUF(cudaMalloc(&c->d_wfac, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_term, sizeof(double) * nh));
@@ -282,7 +286,7 @@ extern "C" int cbmf_set_sub_batch(cbmf_ctx* c, int templates_per_launch)
     DeviceGuard g(c->device);
     if (templates_per_launch > c->max_sub_batch) {
         CU(cudaStreamSynchronize(c->stream));
-        const int p2grid = (1 << c->lg1) / p2_rows(c->lg2);
+        const int p2grid = p2_peak_items(c->lg1, c->lg2);
         float2* y = nullptr; float4* cand = nullptr; unsigned int* done = nullptr;
         CU(cudaMalloc(&y, sizeof(float2) * (size_t)c->n * templates_per_launch));
         cudaError_t e = cudaMalloc(&cand, sizeof(float4) * (size_t)p2grid * templates_per_launch);
@@ -353,11 +357,11 @@ static int load_segment_impl(cbmf_ctx* c, const float* samples_dev)
     TemplCoef tc; memset(&tc, 0, sizeof(tc)); tc.k_lo = c->k_lo; tc.k_hi = (int)(c->n / 2 - 1);
     CU(cudaMemcpyAsync(c->d_coef, &tc, sizeof(tc), cudaMemcpyHostToDevice, c->stream));
     P1Args a1; memset(&a1, 0, sizeof(a1));
-    a1.in_r = samples_dev; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
-    CU(launch_p1<LOAD_REAL>(c->lg1, c->stream, a1, 1));
+    a1.in_r = samples_dev; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+    CU(launch_p1<LOAD_REAL>(c->lg1, c->lg2, c->stream, a1, 1));
     P2Args a2; memset(&a2, 0, sizeof(a2));
-    a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.coef = c->d_coef; a2.w_out = c->d_w; a2.wfac = c->d_wfac;
-    CU(launch_p2<EPI_WSTORE>(c->lg2, c->stream, a2, 1));
+    a2.Y = c->d_Y; a2.coef = c->d_coef; a2.w_out = c->d_w; a2.wfac = c->d_wfac;
+    CU(launch_p2<EPI_WSTORE>(c->lg1, c->lg2, c->stream, a2, 1));
     c->launches += 2;
     int err = 0;
     CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -451,17 +455,17 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     for (int64_t t0 = 0; t0 < nt; t0 += sb) {
         const int nb = (int)((nt - t0 < sb) ? (nt - t0) : sb);
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = c->d_w; a1.coef = c->d_coef + t0; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
+        a1.w = c->d_w; a1.coef = c->d_coef + t0; a1.Y = c->d_Y; a1.err_flag = c->d_err;
         if ((rc = ev_begin(c, 0))) return rc;
-        CU(launch_p1<LOAD_GEN>(c->lg1, c->stream, a1, nb));
+        CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, c->stream, a1, nb));
         if ((rc = ev_end(c, 0))) return rc;
         P2Args a2; memset(&a2, 0, sizeof(a2));
-        a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.coef = c->d_coef + t0; a2.cand = c->d_cand;
+        a2.Y = c->d_Y; a2.coef = c->d_coef + t0; a2.cand = c->d_cand;
         a2.done_ctr = c->d_done; a2.peaks = c->d_peaks + t0; a2.trig = c->d_trig;
         a2.trig_cursor = c->d_cursor; a2.trig_cap = (unsigned long long)trig_capacity;
         a2.tmpl_base = (int)t0;
         if ((rc = ev_begin(c, 1))) return rc;
-        CU(launch_p2<EPI_MAX>(c->lg2, c->stream, a2, nb));
+        CU(launch_p2<EPI_MAX>(c->lg1, c->lg2, c->stream, a2, nb));
         if ((rc = ev_end(c, 1))) return rc;
         c->launches += 2;
     }
@@ -560,11 +564,11 @@ extern "C" int cbmf_debug_snr_series(cbmf_ctx* c, cbmf_template t, float* snr_ou
     CU(cudaMemcpyAsync(&tc, c->d_coef, sizeof(tc), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     P1Args a1; memset(&a1, 0, sizeof(a1));
-    a1.w = c->d_w; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
-    CU(launch_p1<LOAD_GEN>(c->lg1, c->stream, a1, 1));
+    a1.w = c->d_w; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+    CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, c->stream, a1, 1));
     P2Args a2; memset(&a2, 0, sizeof(a2));
-    a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.z_out = z;
-    CU(launch_p2<EPI_STORE>(c->lg2, c->stream, a2, 1));
+    a2.Y = c->d_Y; a2.z_out = z;
+    CU(launch_p2<EPI_STORE>(c->lg1, c->lg2, c->stream, a2, 1));
     snr_from_z_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(z, snr, n, tc.inv_sigma);
     CU(cudaGetLastError());
     c->launches += 3;
@@ -599,11 +603,11 @@ extern "C" int cbmf_debug_ifft_dev(cbmf_ctx* c, const float* in_dev, float* out_
     for (int64_t b0 = 0; b0 < batch; b0 += sb) {
         const int nb = (int)((batch - b0 < sb) ? (batch - b0) : sb);
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.in_c = (const float2*)in_dev + (size_t)b0 * n; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.log2_n2 = c->lg2;
-        CU(launch_p1<LOAD_CPLX>(c->lg1, c->stream, a1, nb));
+        a1.in_c = (const float2*)in_dev + (size_t)b0 * n; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+        CU(launch_p1<LOAD_CPLX>(c->lg1, c->lg2, c->stream, a1, nb));
         P2Args a2; memset(&a2, 0, sizeof(a2));
-        a2.Y = c->d_Y; a2.log2_n1 = c->lg1; a2.z_out = (float2*)out_dev + (size_t)b0 * n;
-        CU(launch_p2<EPI_STORE>(c->lg2, c->stream, a2, nb));
+        a2.Y = c->d_Y; a2.z_out = (float2*)out_dev + (size_t)b0 * n;
+        CU(launch_p2<EPI_STORE>(c->lg1, c->lg2, c->stream, a2, nb));
         c->launches += 2;
     }
     CU(cudaStreamSynchronize(c->stream));

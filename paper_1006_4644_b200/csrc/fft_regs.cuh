@@ -46,6 +46,36 @@ __device__ __forceinline__ float2 twmul(float2 x, int q)
     return make_float2(fmaf(x.x, c, -x.y * s), fmaf(x.x, s, x.y * c));
 }
 
+// Butterfly lo = e + o w, hi = e - o w with w = e^{+2 pi i q / R}, 0 <= q < R/2 (compile-time
+// after unrolling).  Non-trivial twiddles are folded into FMAs: lo = e + o w costs four FFMA
+// and hi = 2e - lo two more (6 instead of 8 instructions); w = (+-1 +- i)/sqrt 2 costs 2 FADD +
+// 4 FFMA with no doubling.
+template <int R>
+__device__ __forceinline__ void bfly(const float2 e, const float2 o, const int q, float2& lo, float2& hi)
+{
+    const int a = q * (32 / R);                 // angle index, 0..15
+    if (a == 0) {
+        lo = cadd(e, o); hi = csub(e, o);
+    } else if (a == 8) {                        // w = i
+        lo = make_float2(e.x - o.y, e.y + o.x); hi = make_float2(e.x + o.y, e.y - o.x);
+    } else if (a == 4) {                        // w = (1 + i) c
+        const float c = cos32_table(4);
+        const float dx = o.x - o.y, dy = o.x + o.y;
+        lo = make_float2(fmaf(c, dx, e.x), fmaf(c, dy, e.y));
+        hi = make_float2(fmaf(-c, dx, e.x), fmaf(-c, dy, e.y));
+    } else if (a == 12) {                       // w = (-1 + i) c
+        const float c = cos32_table(4);
+        const float dx = o.x + o.y, dy = o.x - o.y;
+        lo = make_float2(fmaf(-c, dx, e.x), fmaf(c, dy, e.y));
+        hi = make_float2(fmaf(c, dx, e.x), fmaf(-c, dy, e.y));
+    } else {
+        const float c = (a <= 8) ? cos32_table(a) : -cos32_table(16 - a);
+        const float s = (a <= 8) ? cos32_table(8 - a) : cos32_table(a - 8);
+        lo = make_float2(fmaf(-o.y, s, fmaf(o.x, c, e.x)), fmaf(o.y, c, fmaf(o.x, s, e.y)));
+        hi = make_float2(fmaf(2.0f, e.x, -lo.x), fmaf(2.0f, e.y, -lo.y));
+    }
+}
+
 // Radix-R inverse DFT in registers, natural order in and out, decimation in time.
 // NZ: only inputs v[0..NZ) are non-zero (the rest are never read), which prunes the leaves.
 template <int R, int NZ>
@@ -65,11 +95,7 @@ struct DftP {
             DftP<H, NZE>::run(e);
             DftP<H, NZO>::run(o);
 #pragma unroll
-            for (int q = 0; q < H; ++q) {
-                const float2 t = twmul<R>(o[q], q);
-                v[q] = cadd(e[q], t);
-                v[q + H] = csub(e[q], t);
-            }
+            for (int q = 0; q < H; ++q) bfly<R>(e[q], o[q], q, v[q], v[q + H]);
         }
     }
 };

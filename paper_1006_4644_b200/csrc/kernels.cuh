@@ -56,8 +56,16 @@ __host__ __device__ constexpr int ilog2c(int x) { return x <= 1 ? 0 : 1 + ilog2c
 // E values per thread.  On entry v[u*R1 + r] = x[t + T*u + (L/R1)*r]; on exit
 // v[u*RL + q] = X[t + T*u + (L/RL)*q] (RL = last radix).  sm points at this FFT's shared
 // memory (element stride SS), padded by one element every R1.  NZ1: only r < NZ1 is non-zero.
-template <int L, int NZ1, int SS, bool WARP_SYNC>
-__device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, float2* __restrict__ sm)
+//
+// ROWTW (pass 2): the FFT is row j1 of the four-step decomposition and its input should have
+// been multiplied by the inter-pass twiddle W_N^{j1 k2}, k2 = p0 + (L/R1) r, p0 = t + T u.
+// The caller multiplies only by (W_N^{j1 L/R1})^r; the factor W_N^{j1 p0} is constant over
+// the step-1 DFT, so it commutes with it and is folded here into the step-2 twiddles: the
+// step-2 reader at position i + (L/R2) r' sees writer p0 = (i >> lg R1) + R3 r', i.e. an extra
+// W_N^{j1 (i >> lg R1)} (W_N^{j1 R3})^{r'}.  n1 = N / L.
+template <int L, int NZ1, int SS, bool WARP_SYNC, bool ROWTW>
+__device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, float2* __restrict__ sm,
+                                         const int j1 = 0, const int n1 = 1)
 {
     using C = Cfg<L>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, R2 = C::R2, R3 = C::R3;
@@ -91,7 +99,18 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
 #pragma unroll
             for (int r = 0; r < R2; ++r) x[r] = sm[pad(i + (L / R2) * r) * SS];
             const int k = i & (NS - 1);
-            mul_powers<R2, false>(x, expi_frac(k, 2.0f / (float)(NS * R2)), make_float2(1.f, 0.f));
+            if constexpr (ROWTW) {
+                // e^{2 pi i (k / (R1 R2) + j1 R3 / N)}: numerator over N = n1 L is an exact integer < N
+                const float two_over_n = 2.0f / ((float)n1 * (float)L);
+                const float2 g = expi_frac(k * (n1 * R3) + j1 * R3, two_over_n);
+                if constexpr (R3 > 1) {
+                    mul_powers<R2, true>(x, g, expi_frac(j1 * (i >> LG_R1), two_over_n));
+                } else {
+                    mul_powers<R2, false>(x, g, make_float2(1.f, 0.f));
+                }
+            } else {
+                mul_powers<R2, false>(x, expi_frac(k, 2.0f / (float)(NS * R2)), make_float2(1.f, 0.f));
+            }
             dft<R2>(x);
 #pragma unroll
             for (int q = 0; q < R2; ++q) y[u * R2 + q] = x[q];
@@ -135,7 +154,9 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
 // e^{+i Psi_T(f_k)} for bin k >= 1 ("x form" in cycles).  The phase
 // reaches 1e4 cycles, so the polynomial and the reduction to [-1/2, 1/2] cycles run in fp64;
 // the fraction is then exact to 3e-8 cycles in fp32.  u = k^{-1/3}: fp32 seed + one Newton
-// step in fp64 (relative error ~ 2 (1.2e-7)^2).
+// step in fp64 (relative error ~ 2 (1.2e-7)^2).  The reduced angle lies in [-pi, pi], where
+// the SFU sine/cosine (MUFU.SIN/COS) have absolute error <= 2^-21.4 (CUDA math API, __sinf):
+// a template mismatch of order 1e-13, against the 1e-6 bound of tests/parity.py.
 __device__ __forceinline__ float2 spa_phasor(const int k, const double A1, const double A2,
                                              const double A3, const double A5)
 {
@@ -147,10 +168,8 @@ __device__ __forceinline__ float2 spa_phasor(const int k, const double A1, const
     ph = fma(ph, u, A2);
     ph = fma(ph, u, A1);
     ph = fma(ph, u, -0.125);
-    const float fr = (float)(ph - rint(ph));
-    float s, c;
-    sincospif(2.0f * fr, &s, &c);
-    return make_float2(c, s);
+    const float ang = 6.28318530717958647692f * (float)(ph - rint(ph));
+    return make_float2(__cosf(ang), __sinf(ang));
 }
 
 // ------------------------------------------------------------------ pass 1
@@ -163,49 +182,48 @@ struct P1Args {
     const float* __restrict__ in_r;        // [batch][N] (LOAD_REAL)
     float2* __restrict__ Y;                // [batch][N], Y[j1*N2 + k2]
     int* err_flag;                         // set to 1 on a non-finite real input sample
-    int log2_n2;
 };
 
-template <int L, int MODE>
-__global__ void __launch_bounds__(Cfg<L>::NT1, (Cfg<L>::NT1 <= 256 ? 2 : 1)) p1_kernel(const P1Args a)
+// One tile of NC adjacent columns k2 of template slot b: N1 = L1-point inverse FFT over k1 of
+// x[k1*L2 + k2] -> Y[b][j1*L2 + k2].  All Cfg<L1>::NT1 threads of the block take part.
+template <int L1, int L2, int MODE>
+__device__ __forceinline__ void p1_tile(const P1Args& a, const int tile, const int b, float2* __restrict__ smem)
 {
-    using C = Cfg<L>;
+    using C = Cfg<L1>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, NC = C::C;
     constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
     constexpr int NZ1 = (MODE == LOAD_GEN) ? R1 / 2 : R1;    // bins k >= N/2 are zero
-    extern __shared__ float2 smem[];
+    constexpr size_t n_total = (size_t)L1 * L2;
 
     const int c = threadIdx.x % NC, t = threadIdx.x / NC;
-    const int k2 = blockIdx.x * NC + c;
-    const int b = blockIdx.y;
-    const int lg2 = a.log2_n2;
-    const size_t n_total = (size_t)L << lg2;
+    const int k2 = tile * NC + c;
 
     float2 v[E];
     if constexpr (MODE == LOAD_GEN) {
         const TemplCoef* tc = a.coef + b;
-        const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
         const int k_lo = tc->k_lo, k_hi = tc->k_hi;
+        // all loads of w first (w is zero below k_lo), then the phasors of the in-band bins
 #pragma unroll
-        for (int u = 0; u < E / R1; ++u) {
+        for (int u = 0; u < E / R1; ++u)
 #pragma unroll
-            for (int r = 0; r < R1; ++r) {
+            for (int r = 0; r < R1; ++r)
+                v[u * R1 + r] = (r < NZ1) ? __ldg(a.w + ((t + T * u + (L1 / R1) * r) * L2 + k2)) : make_float2(0.f, 0.f);
+        const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+#pragma unroll
+        for (int u = 0; u < E / R1; ++u)
+#pragma unroll
+            for (int r = 0; r < NZ1; ++r) {
+                const int k = (t + T * u + (L1 / R1) * r) * L2 + k2;
                 float2 val = make_float2(0.f, 0.f);
-                if (r < NZ1) {
-                    const int k1 = t + T * u + (L / R1) * r;
-                    const int k = (k1 << lg2) + k2;
-                    if (k >= k_lo && k <= k_hi) val = cmul(__ldg(a.w + k), spa_phasor(k, A1, A2, A3, A5));
-                }
+                if (k >= k_lo && k <= k_hi) val = cmul(v[u * R1 + r], spa_phasor(k, A1, A2, A3, A5));
                 v[u * R1 + r] = val;
             }
-        }
     } else {
 #pragma unroll
         for (int u = 0; u < E / R1; ++u) {
 #pragma unroll
             for (int r = 0; r < R1; ++r) {
-                const int k1 = t + T * u + (L / R1) * r;
-                const size_t k = ((size_t)k1 << lg2) + k2;
+                const size_t k = (size_t)(t + T * u + (L1 / R1) * r) * L2 + k2;
                 if constexpr (MODE == LOAD_CPLX) {
                     v[u * R1 + r] = __ldg(a.in_c + (size_t)b * n_total + k);
                 } else {
@@ -217,17 +235,22 @@ __global__ void __launch_bounds__(Cfg<L>::NT1, (Cfg<L>::NT1 <= 256 ? 2 : 1)) p1_
         }
     }
 
-    fft_core<L, NZ1, NC, false>(v, t, smem + c);
+    fft_core<L1, NZ1, NC, false, false>(v, t, smem + c);
 
-    float2* __restrict__ yb = a.Y + (size_t)b * n_total;
+    float2* __restrict__ yb = a.Y + (size_t)b * n_total + (size_t)t * L2 + k2;
 #pragma unroll
     for (int u = 0; u < E / RL; ++u) {
 #pragma unroll
-        for (int q = 0; q < RL; ++q) {
-            const int j1 = t + T * u + (L / RL) * q;
-            yb[((size_t)j1 << lg2) + k2] = v[u * RL + q];
-        }
+        for (int q = 0; q < RL; ++q)
+            yb[(size_t)(T * u + (L1 / RL) * q) * L2] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
     }
+}
+
+template <int L1, int L2, int MODE>
+__global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p1_kernel(const P1Args a)
+{
+    extern __shared__ float2 smem[];
+    p1_tile<L1, L2, MODE>(a, blockIdx.x, blockIdx.y, smem);
 }
 
 // ------------------------------------------------------------------ pass 2
@@ -235,7 +258,6 @@ enum { EPI_MAX = 0, EPI_STORE = 1, EPI_WSTORE = 2 };
 
 struct P2Args {
     const float2* __restrict__ Y;          // [batch][N]
-    int log2_n1;                           // N1 = number of rows
     // EPI_MAX
     const TemplCoef* __restrict__ coef;    // [batch]
     float4* cand;                          // [batch][gridDim.x]  (|z|^2, j as int bits, re, im)
@@ -257,58 +279,95 @@ __device__ __forceinline__ unsigned long long pack_key(float p, int j)
     return ((unsigned long long)__float_as_uint(p) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)j);
 }
 
-template <int L, int MODE>
-__global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
+// Rows per thread group and block in the arg-max pass: each group of T threads walks RPW rows
+// and keeps its running maximum in registers, so the block-level reduction is paid once.
+template <int L1, int L2>
+__host__ __device__ constexpr int p2_rpw()
 {
-    using C = Cfg<L>;
-    constexpr int E = C::E, T = C::T, R1 = C::R1, ROWS = C::ROWS;
+    constexpr int per8 = L1 / Cfg<L2>::ROWS / 8;
+    return per8 >= 4 ? 4 : (per8 >= 1 ? per8 : 1);
+}
+template <int L2> __host__ __device__ constexpr int p2_row_stride()
+{
+    return Cfg<L2>::PADDED + (Cfg<L2>::T <= 32 ? Cfg<L2>::R1 : 0);      // exchange buffer + G table
+}
+
+// Shared per-thread state of the arg-max epilogue (S6/S7).
+struct PeakAcc {
+    float best; int j; float re, im;
+};
+
+// Row j1 of template slot b: twiddle, N2 = L2-point inverse FFT over k2 -> z[j1 + L1 j2] in
+// registers, then the epilogue of MODE.  Called by the T threads of one row group.
+template <int L1, int L2, int MODE>
+__device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int b, const int t,
+                                       float2* __restrict__ sm, PeakAcc& acc)
+{
+    using C = Cfg<L2>;
+    constexpr int E = C::E, T = C::T, R1 = C::R1;
     constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
     constexpr bool WSYNC = (T <= 32);
-    extern __shared__ float2 smem[];
+    constexpr int LG1 = ilog2c(L1);
+    constexpr size_t n_total = (size_t)L1 * L2;
 
-    const int t = threadIdx.x % T, row = threadIdx.x / T;
-    const int j1 = blockIdx.x * ROWS + row;
-    const int b = blockIdx.y;
-    const int lg1 = a.log2_n1;
-    const int n1 = 1 << lg1;
-    const size_t n_total = (size_t)L << lg1;
-    const float two_over_n = 2.0f / (float)n_total;
-
-    // load row j1 and apply the inter-pass twiddle W_N^{j1 k2}, k2 = t + T u + (L/R1) r
+    // load row j1; multiply by (W_N^{j1 L2/R1})^r (the rest of the inter-pass twiddle is folded
+    // into the step-2 twiddles of fft_core)
     float2 v[E];
-    const float2* __restrict__ yrow = a.Y + (size_t)b * n_total + (size_t)j1 * L;
-    const float2 g = expi_frac(j1, 2.0f / (float)(n1 * R1));      // W_N^{j1 L/R1}
+    const float2* __restrict__ yrow = a.Y + (size_t)b * n_total + (size_t)j1 * L2;
 #pragma unroll
-    for (int u = 0; u < E / R1; ++u) {
-        float2 x[R1];
-        const int p0 = t + T * u;
+    for (int u = 0; u < E / R1; ++u)
 #pragma unroll
-        for (int r = 0; r < R1; ++r) x[r] = __ldcg(yrow + p0 + (L / R1) * r);
-        mul_powers<R1, true>(x, g, expi_frac((j1 * p0) & (int)(n_total - 1), two_over_n));
+        for (int r = 0; r < R1; ++r) v[u * R1 + r] = __ldcg(yrow + t + T * u + (L2 / R1) * r);
+    if constexpr (WSYNC) {
+        // G[r] = e^{2 pi i j1 r / (L1 R1)}, r < R1: one sincospi per lane, broadcast through shared memory
+        float2* __restrict__ G = sm + C::PADDED;
+        for (int r = t; r < R1; r += T) G[r] = expi_frac((j1 * r) & (L1 * R1 - 1), 2.0f / (float)(L1 * R1));
+        __syncwarp();
 #pragma unroll
-        for (int r = 0; r < R1; ++r) v[u * R1 + r] = x[r];
+        for (int r = 2; r < R1; r += 2) {
+            const float4 g = *reinterpret_cast<const float4*>(G + r);
+#pragma unroll
+            for (int u = 0; u < E / R1; ++u) {
+                v[u * R1 + r] = cmul(v[u * R1 + r], make_float2(g.x, g.y));
+                v[u * R1 + r + 1] = cmul(v[u * R1 + r + 1], make_float2(g.z, g.w));
+            }
+        }
+        {
+            const float2 g1 = G[1];
+#pragma unroll
+            for (int u = 0; u < E / R1; ++u) v[u * R1 + 1] = cmul(v[u * R1 + 1], g1);
+        }
+    } else {
+        const float2 g = expi_frac(j1, 2.0f / (float)(L1 * R1));      // W_N^{j1 L2/R1}
+#pragma unroll
+        for (int u = 0; u < E / R1; ++u) {
+            float2 x[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) x[r] = v[u * R1 + r];
+            mul_powers<R1, false>(x, g, make_float2(1.f, 0.f));
+#pragma unroll
+            for (int r = 0; r < R1; ++r) v[u * R1 + r] = x[r];
+        }
     }
 
-    fft_core<L, R1, 1, WSYNC>(v, t, smem + row * C::PADDED);
+    fft_core<L2, R1, 1, WSYNC, true>(v, t, sm, j1, L1);
 
-    // v[u*RL + q] = z[j1 + N1 * j2],  j2 = t + T u + (L/RL) q
+    // v[u*RL + q] = z[j1 + L1 * j2],  j2 = t + T u + (L2/RL) q
     if constexpr (MODE == EPI_STORE) {
-        float2* __restrict__ zb = a.z_out + (size_t)b * n_total;
+        float2* __restrict__ zb = a.z_out + (size_t)b * n_total + j1;
 #pragma unroll
         for (int u = 0; u < E / RL; ++u)
 #pragma unroll
-            for (int q = 0; q < RL; ++q) {
-                const int j2 = t + T * u + (L / RL) * q;
-                zb[((size_t)j2 << lg1) + j1] = v[u * RL + q];
-            }
+            for (int q = 0; q < RL; ++q)
+                zb[(size_t)(t + T * u + (L2 / RL) * q) << LG1] = v[u * RL + q];
     } else if constexpr (MODE == EPI_WSTORE) {
         const int k_lo = a.coef->k_lo;
 #pragma unroll
         for (int u = 0; u < E / RL; ++u)
 #pragma unroll
             for (int q = 0; q < RL; ++q) {
-                const int j2 = t + T * u + (L / RL) * q;
-                const size_t k = ((size_t)j2 << lg1) + j1;
+                const int j2 = t + T * u + (L2 / RL) * q;
+                const size_t k = ((size_t)j2 << LG1) + j1;
                 if (k < n_total / 2) {
                     float2 o = make_float2(0.f, 0.f);
                     if ((long long)k >= k_lo) {
@@ -322,17 +381,30 @@ __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
         // ---- S6/S7: |z|^2, arg-max (lowest index on ties), threshold
         const TemplCoef* tc = a.coef + b;
         const float thr2 = tc->thr2, inv_sigma = tc->inv_sigma;
-        float best = -1.0f;
-        int best_e = 0;
+        float m = -1.0f;
 #pragma unroll
-        for (int q = 0; q < RL; ++q)            // j2 increases with (q, u): first maximum kept
+        for (int e = 0; e < E; ++e) m = fmaxf(m, fmaf(v[e].x, v[e].x, v[e].y * v[e].y));
+        if (m >= acc.best) {                    // rare after the first rows: locate the sample
+            int best_e = 0;
+            bool found = false;
 #pragma unroll
-            for (int u = 0; u < E / RL; ++u) {
-                const int e = u * RL + q;
-                const float p = fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
-                if (p > best) { best = p; best_e = e; }
+            for (int q = 0; q < RL; ++q)        // j2 increases with (q, u): first maximum kept
+#pragma unroll
+                for (int u = 0; u < E / RL; ++u) {
+                    const int e = u * RL + q;
+                    const float p = fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
+                    if (!found && p == m) { found = true; best_e = e; }
+                }
+            const int j2 = t + T * (best_e / RL) + (L2 / RL) * (best_e % RL);
+            const int j = (j2 << LG1) + j1;
+            if (m > acc.best || j < acc.j) {
+                acc.best = m; acc.j = j;
+#pragma unroll
+                for (int e = 0; e < E; ++e)
+                    if (e == best_e) { acc.re = v[e].x; acc.im = v[e].y; }
             }
-        if (best > thr2 && inv_sigma > 0.f) {
+        }
+        if (m > thr2 && inv_sigma > 0.f) {
 #pragma unroll
             for (int q = 0; q < RL; ++q)
 #pragma unroll
@@ -342,10 +414,10 @@ __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
                     if (p > thr2) {
                         const unsigned long long slot = atomicAdd(a.trig_cursor, 1ULL);
                         if (slot < a.trig_cap) {
-                            const int j2 = t + T * u + (L / RL) * q;
+                            const int j2 = t + T * u + (L2 / RL) * q;
                             TrigOut o;
                             o.template_idx = a.tmpl_base + b;
-                            o.sample_idx = (j2 << lg1) + j1;
+                            o.sample_idx = (j2 << LG1) + j1;
                             o.snr = sqrtf(p) * inv_sigma;
                             o.phase = atan2f(v[e].y, v[e].x);
                             a.trig[slot] = o;
@@ -353,72 +425,100 @@ __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
                     }
                 }
         }
-        const int best_j2 = t + T * (best_e / RL) + (L / RL) * (best_e % RL);
-        const int best_j = (best_j2 << lg1) + j1;
-        const unsigned long long mykey = pack_key(best, best_j);
-        unsigned long long key = mykey;
+    }
+}
+
+// Block-level end of the arg-max pass: the block's best sample goes to cand[b][item]; the last
+// of the n_items blocks of template slot b reduces the candidates to the PeakOut record.
+__device__ __forceinline__ void p2_finish(const P2Args& a, const PeakAcc& acc, const int b,
+                                          const int item, const int n_items)
+{
+    __shared__ unsigned long long s_keys[32];
+    __shared__ unsigned long long s_win;
+    __shared__ int s_last;
+    const unsigned long long mykey = pack_key(acc.best, acc.j);
+    unsigned long long key = mykey;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const unsigned long long o = __shfl_xor_sync(0xFFFFFFFFu, key, off);
+        key = o > key ? o : key;
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+    if (lane == 0) s_keys[warp] = key;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long k8 = s_keys[0];
+        for (int i = 1; i < nwarp; ++i) k8 = s_keys[i] > k8 ? s_keys[i] : k8;
+        s_win = k8;
+        s_last = 0;
+    }
+    __syncthreads();
+    if (mykey == s_win) {            // exactly one thread: sample indices are unique
+        float4 rec = make_float4(acc.best, __int_as_float(acc.j), acc.re, acc.im);
+        __stcg(a.cand + (size_t)b * n_items + item, rec);
+        __threadfence();
+        const unsigned int prev = atomicAdd(a.done_ctr + b, 1u);
+        s_last = (prev == (unsigned)n_items - 1u);
+    }
+    __syncthreads();
+    if (s_last && warp == 0) {
+        __threadfence();
+        const TemplCoef* tc = a.coef + b;
+        unsigned long long bk = 0ULL;
+        float bre = 0.f, bim = 0.f;
+        for (int i = lane; i < n_items; i += 32) {
+            const float4 r = __ldcg(a.cand + (size_t)b * n_items + i);
+            const unsigned long long kk = pack_key(r.x, __float_as_int(r.y));
+            if (kk > bk) { bk = kk; bre = r.z; bim = r.w; }
+        }
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
-            const unsigned long long o = __shfl_xor_sync(0xFFFFFFFFu, key, off);
-            key = o > key ? o : key;
+            const unsigned long long ok = __shfl_xor_sync(0xFFFFFFFFu, bk, off);
+            const float ore = __shfl_xor_sync(0xFFFFFFFFu, bre, off);
+            const float oim = __shfl_xor_sync(0xFFFFFFFFu, bim, off);
+            if (ok > bk) { bk = ok; bre = ore; bim = oim; }
         }
-        __shared__ unsigned long long s_keys[8];
-        __shared__ unsigned long long s_win;
-        __shared__ int s_last;
-        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-        if (lane == 0) s_keys[warp] = key;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            unsigned long long k8 = s_keys[0];
-#pragma unroll
-            for (int i = 1; i < 8; ++i) k8 = s_keys[i] > k8 ? s_keys[i] : k8;
-            s_win = k8;
-        }
-        __syncthreads();
-        if (mykey == s_win) {            // exactly one thread: sample indices are unique
-            float re = 0.f, im = 0.f;
-#pragma unroll
-            for (int e = 0; e < E; ++e)
-                if (e == best_e) { re = v[e].x; im = v[e].y; }
-            float4 rec = make_float4(best, __int_as_float(best_j), re, im);
-            __stcg(a.cand + (size_t)b * gridDim.x + blockIdx.x, rec);
-            __threadfence();
-            const unsigned int prev = atomicAdd(a.done_ctr + b, 1u);
-            s_last = (prev == gridDim.x - 1);
-        }
-        __syncthreads();
-        if (s_last && warp == 0) {
-            __threadfence();
-            unsigned long long bk = 0ULL;
-            float bre = 0.f, bim = 0.f;
-            for (int i = lane; i < (int)gridDim.x; i += 32) {
-                const float4 r = __ldcg(a.cand + (size_t)b * gridDim.x + i);
-                const unsigned long long kk = pack_key(r.x, __float_as_int(r.y));
-                if (kk > bk) { bk = kk; bre = r.z; bim = r.w; }
+        if (lane == 0) {
+            PeakOut o;
+            if (tc->k_hi < tc->k_lo) {          // empty band
+                o.snr_max = 0.f; o.idx_peak = -1; o.phase = 0.f; o.sigma = 0.f;
+            } else {
+                const float p = __uint_as_float((unsigned)(bk >> 32));
+                o.snr_max = sqrtf(p) * tc->inv_sigma;
+                o.idx_peak = (int)(0xFFFFFFFFu - (unsigned)(bk & 0xFFFFFFFFu));
+                o.phase = atan2f(bim, bre);
+                o.sigma = tc->sigma;
             }
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) {
-                const unsigned long long ok = __shfl_xor_sync(0xFFFFFFFFu, bk, off);
-                const float ore = __shfl_xor_sync(0xFFFFFFFFu, bre, off);
-                const float oim = __shfl_xor_sync(0xFFFFFFFFu, bim, off);
-                if (ok > bk) { bk = ok; bre = ore; bim = oim; }
-            }
-            if (lane == 0) {
-                PeakOut o;
-                if (tc->k_hi < tc->k_lo) {          // empty band
-                    o.snr_max = 0.f; o.idx_peak = -1; o.phase = 0.f; o.sigma = 0.f;
-                } else {
-                    const float p = __uint_as_float((unsigned)(bk >> 32));
-                    o.snr_max = sqrtf(p) * tc->inv_sigma;
-                    o.idx_peak = (int)(0xFFFFFFFFu - (unsigned)(bk & 0xFFFFFFFFu));
-                    o.phase = atan2f(bim, bre);
-                    o.sigma = tc->sigma;
-                }
-                a.peaks[b] = o;
-                a.done_ctr[b] = 0u;                 // self-cleaning for the next launch
-            }
+            a.peaks[b] = o;
+            a.done_ctr[b] = 0u;                 // self-cleaning for the next launch
         }
     }
+    __syncthreads();                            // s_keys / s_win reusable by the caller's next item
+}
+
+// One item of pass 2: ROWS * RPW rows of template slot b.
+template <int L1, int L2, int MODE>
+__device__ __forceinline__ void p2_item(const P2Args& a, const int item, const int b, float2* __restrict__ smem)
+{
+    using C = Cfg<L2>;
+    constexpr int T = C::T, ROWS = C::ROWS;
+    constexpr int RPW = (MODE == EPI_MAX) ? p2_rpw<L1, L2>() : 1;
+    const int t = threadIdx.x % T, row = threadIdx.x / T;
+    float2* sm = smem + row * p2_row_stride<L2>();
+    PeakAcc acc; acc.best = -1.0f; acc.j = 0x7FFFFFFF; acc.re = 0.f; acc.im = 0.f;
+#pragma unroll 1
+    for (int it = 0; it < RPW; ++it) {
+        if (it > 0) { if constexpr (T <= 32) __syncwarp(); else __syncthreads(); }
+        p2_row<L1, L2, MODE>(a, (item * RPW + it) * ROWS + row, b, t, sm, acc);
+    }
+    if constexpr (MODE == EPI_MAX) p2_finish(a, acc, b, item, L1 / (ROWS * RPW));
+}
+
+template <int L1, int L2, int MODE>
+__global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
+{
+    extern __shared__ float2 smem[];
+    p2_item<L1, L2, MODE>(a, blockIdx.x, blockIdx.y, smem);
 }
 
 // ------------------------------------------------------------------ S0: PSD tables (fp64)
