@@ -227,6 +227,8 @@ def run_ours(args):
         ctx = cbmf.Context(n, wl.fs, wl.f_low, device=local, stream=stream.cuda_stream)
         if args.sub_batch:
             ctx.set_sub_batch(args.sub_batch)
+        if args.streams:
+            ctx.set_streams(args.streams)
         psd_d = torch.from_numpy(wl.psd).to(dev)
         smp_d = torch.from_numpy(wl.samples).to(dev)
         bank_d = torch.from_numpy(np.ascontiguousarray(wl.bank)).to(dev)
@@ -286,6 +288,7 @@ def run_ours(args):
                 p_n[w] += nl
         ctx.set_profiling(False)
         sub = ctx.get_sub_batch()
+        ctx_streams = ctx.get_streams()
 
         # ---- e2e leg: host-pointer entry points, pinned host buffers
         psd_h = torch.from_numpy(wl.psd).pin_memory()
@@ -368,7 +371,7 @@ def run_ours(args):
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name, "n": n, "fs_hz": wl.fs, "f_low_hz": wl.f_low,
-                   "templates_per_step_per_gpu": B, "threshold": wl.threshold, "sub_batch": sub,
+                   "templates_per_step_per_gpu": B, "threshold": wl.threshold, "sub_batch": sub, "streams": ctx_streams,
                    "l2": "flushed (256 MiB fill) before every timed step",
                    "step": "set_psd + load_segment + filter_bank (S0-S8)",
                    "parallelism": f"bank sharded over {world} GPU(s), segment replicated"},
@@ -394,6 +397,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3"], default="cfg1")
     ap.add_argument("--sub-batch", type=int, default=0, help="templates per launch pair (0 = library default)")
+    ap.add_argument("--streams", type=int, default=0, help="launch pairs in flight (0 = library default)")
     ap.add_argument("--trig-capacity", type=int, default=1 << 16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()

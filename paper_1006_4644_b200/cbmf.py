@@ -54,6 +54,8 @@ def lib() -> C.CDLL:
         "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
         "cbmf_set_sub_batch": (C.c_int, [vp, C.c_int]),
         "cbmf_get_sub_batch": (C.c_int, [vp]),
+        "cbmf_set_streams": (C.c_int, [vp, C.c_int]),
+        "cbmf_get_streams": (C.c_int, [vp]),
         "cbmf_launch_count": (i64, [vp]),
         "cbmf_last_pass_time": (C.c_int, [vp, C.c_int, C.POINTER(dbl), C.POINTER(i64)]),
         "cbmf_set_profiling": (C.c_int, [vp, C.c_int]),
@@ -71,7 +73,7 @@ def lib() -> C.CDLL:
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
-           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch "
+           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch cbmf_set_streams cbmf_get_streams "
            "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_strerror "
            "cbmf_last_cuda_error cbmf_version").split()
 
@@ -233,6 +235,12 @@ class Context:
 
     def get_sub_batch(self) -> int:
         return int(lib().cbmf_get_sub_batch(self._h))
+
+    def set_streams(self, k: int):
+        self._check(lib().cbmf_set_streams(self._h, int(k)), "cbmf_set_streams")
+
+    def get_streams(self) -> int:
+        return int(lib().cbmf_get_streams(self._h))
 
     def launch_count(self) -> int:
         return int(lib().cbmf_launch_count(self._h))

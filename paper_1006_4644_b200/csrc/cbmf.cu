@@ -16,6 +16,8 @@
 
 using namespace cbmf;
 
+#define CBMF_MAX_STREAMS 8
+
 struct cbmf_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -26,6 +28,10 @@ struct cbmf_ctx {
     bool have_psd = false, have_seg = false;
     int sub_batch = 0;                     // templates per pass-1/pass-2 launch pair
     int max_sub_batch = 0;
+    int n_streams = 1;                     // launch pairs in flight (each on its own stream and Y slice)
+    int max_streams = 0;                   // slices allocated in d_Y / d_cand / d_done
+    cudaStream_t aux[CBMF_MAX_STREAMS] = {};
+    cudaEvent_t ev_fork = nullptr, ev_join[CBMF_MAX_STREAMS] = {};
 
     double* d_wfac = nullptr;              // [N/2]
     double* d_term = nullptr;              // [N/2]
@@ -202,6 +208,34 @@ int ev_collect(cbmf_ctx* c)
     return CBMF_OK;
 }
 
+// (Re)allocate the per-slot buffers for `sb` templates per launch pair and `ns` pairs in flight.
+int alloc_pipeline(cbmf_ctx* c, int sb, int ns)
+{
+    if (sb <= c->max_sub_batch && ns <= c->max_streams) return CBMF_OK;
+    if (sb < c->max_sub_batch) sb = c->max_sub_batch;
+    if (ns < c->max_streams) ns = c->max_streams;
+    CU(cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < c->max_streams; ++i) if (c->aux[i]) CU(cudaStreamSynchronize(c->aux[i]));
+    const size_t slots = (size_t)sb * ns;
+    const int p2grid = p2_peak_items(c->lg1, c->lg2);
+    float2* y = nullptr; float4* cand = nullptr; unsigned int* done = nullptr;
+    cudaError_t e = cudaMalloc(&y, sizeof(float2) * (size_t)c->n * slots);
+    if (e == cudaSuccess) e = cudaMalloc(&cand, sizeof(float4) * (size_t)p2grid * slots);
+    if (e == cudaSuccess) e = cudaMalloc(&done, sizeof(unsigned int) * slots);
+    if (e == cudaSuccess) e = cudaMemsetAsync(done, 0, sizeof(unsigned int) * slots, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    for (int i = c->max_streams; i < ns && e == cudaSuccess; ++i) {
+        e = cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess && !c->ev_fork) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+    if (e != cudaSuccess) { cudaFree(y); cudaFree(cand); cudaFree(done); return cuda_fail(c, e, "alloc_pipeline"); }
+    cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done);
+    c->d_Y = y; c->d_cand = cand; c->d_done = done;
+    c->max_sub_batch = sb; c->max_streams = ns;
+    return CBMF_OK;
+}
+
 }  // namespace
 
 // ======================================================================= create / destroy
@@ -215,6 +249,11 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
     cudaFree(c->d_trig); cudaFree(c->d_scratch);
     for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
+    for (int i = 0; i < CBMF_MAX_STREAMS; ++i) {
+        if (c->aux[i]) { cudaStreamSynchronize(c->aux[i]); cudaStreamDestroy(c->aux[i]); }
+        if (c->ev_join[i]) cudaEventDestroy(c->ev_join[i]);
+    }
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     cudaGetLastError();
     delete c;
     return CBMF_OK;
@@ -253,29 +292,30 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
         const long v = strtol(e, nullptr, 10);
         if (v >= 1 && v <= 4096) sb = v;
     }
+    int ns = 2;
+    if (const char* e = getenv("CBMF_STREAMS")) {
+        const long v = strtol(e, nullptr, 10);
+        if (v >= 1 && v <= CBMF_MAX_STREAMS) ns = (int)v;
+    }
     c->sub_batch = (int)sb;
-    c->max_sub_batch = (int)sb;
+    c->n_streams = ns;
 
     DeviceGuard g(device);
     auto fail = [&](int rc) { cbmf_destroy(c); return rc; };
     if (!g.ok) return fail(CBMF_ECUDA);
     const size_t nh = (size_t)n / 2;
-    const int p2grid = p2_peak_items(c->lg1, c->lg2);
 #define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(cuda_fail(nullptr, e__, #call)); } while (0)
     CUF(cudaMalloc(&c->d_wfac, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_term, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_prefix, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_bsum, sizeof(double) * ((nh + SCAN_TILE - 1) / SCAN_TILE)));
     CUF(cudaMalloc(&c->d_w, sizeof(float2) * nh));
-    CUF(cudaMalloc(&c->d_Y, sizeof(float2) * (size_t)n * c->max_sub_batch));
-    CUF(cudaMalloc(&c->d_cand, sizeof(float4) * (size_t)p2grid * c->max_sub_batch));
-    CUF(cudaMalloc(&c->d_done, sizeof(unsigned int) * c->max_sub_batch));
     CUF(cudaMalloc(&c->d_err, sizeof(int)));
     CUF(cudaMalloc(&c->d_cursor, sizeof(unsigned long long)));
-    CUF(cudaMemsetAsync(c->d_done, 0, sizeof(unsigned int) * c->max_sub_batch, c->stream));
     CUF(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
     CUF(cudaStreamSynchronize(c->stream));
 #undef CUF
+    { const int rc = alloc_pipeline(c, c->sub_batch, c->n_streams); if (rc) return fail(rc); }
     *out = c;
     return CBMF_OK;
 }
@@ -284,22 +324,23 @@ extern "C" int cbmf_set_sub_batch(cbmf_ctx* c, int templates_per_launch)
 {
     if (!c || templates_per_launch < 1 || templates_per_launch > 4096) return CBMF_EINVAL;
     DeviceGuard g(c->device);
-    if (templates_per_launch > c->max_sub_batch) {
-        CU(cudaStreamSynchronize(c->stream));
-        const int p2grid = p2_peak_items(c->lg1, c->lg2);
-        float2* y = nullptr; float4* cand = nullptr; unsigned int* done = nullptr;
-        CU(cudaMalloc(&y, sizeof(float2) * (size_t)c->n * templates_per_launch));
-        cudaError_t e = cudaMalloc(&cand, sizeof(float4) * (size_t)p2grid * templates_per_launch);
-        if (e == cudaSuccess) e = cudaMalloc(&done, sizeof(unsigned int) * templates_per_launch);
-        if (e == cudaSuccess) e = cudaMemsetAsync(done, 0, sizeof(unsigned int) * templates_per_launch, c->stream);
-        if (e != cudaSuccess) { cudaFree(y); cudaFree(cand); cudaFree(done); return cuda_fail(c, e, "cbmf_set_sub_batch"); }
-        cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done);
-        c->d_Y = y; c->d_cand = cand; c->d_done = done;
-        c->max_sub_batch = templates_per_launch;
-    }
+    const int rc = alloc_pipeline(c, templates_per_launch, c->n_streams);
+    if (rc) return rc;
     c->sub_batch = templates_per_launch;
     return CBMF_OK;
 }
+
+extern "C" int cbmf_set_streams(cbmf_ctx* c, int launch_pairs_in_flight)
+{
+    if (!c || launch_pairs_in_flight < 1 || launch_pairs_in_flight > CBMF_MAX_STREAMS) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    const int rc = alloc_pipeline(c, c->sub_batch, launch_pairs_in_flight);
+    if (rc) return rc;
+    c->n_streams = launch_pairs_in_flight;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_get_streams(const cbmf_ctx* c) { return c ? c->n_streams : CBMF_EINVAL; }
 
 extern "C" int cbmf_get_sub_batch(const cbmf_ctx* c) { return c ? c->sub_batch : CBMF_EINVAL; }
 
@@ -452,22 +493,42 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
 
     c->ev_used[0] = c->ev_used[1] = 0;
     const int sb = c->sub_batch;
-    for (int64_t t0 = 0; t0 < nt; t0 += sb) {
+    // Launch pairs go round-robin over ns streams, each with its own slice of Y / cand / done, so
+    // that the tail of one kernel overlaps the head of the next pair.  With per-pass event timing on
+    // (cbmf_set_profiling) everything stays on the context's stream: each launch is timed alone.
+    const int ns = (c->profiling || nt <= sb) ? 1 : c->n_streams;
+    const int p2grid = p2_peak_items(c->lg1, c->lg2);
+    if (ns > 1) {
+        CU(cudaEventRecord(c->ev_fork, c->stream));
+        for (int s = 0; s < ns; ++s) CU(cudaStreamWaitEvent(c->aux[s], c->ev_fork, 0));
+    }
+    int64_t pair = 0;
+    for (int64_t t0 = 0; t0 < nt; t0 += sb, ++pair) {
         const int nb = (int)((nt - t0 < sb) ? (nt - t0) : sb);
+        const int slot = (int)(pair % ns);
+        cudaStream_t st = (ns > 1) ? c->aux[slot] : c->stream;
+        float2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = c->d_w; a1.coef = c->d_coef + t0; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+        a1.w = c->d_w; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err;
         if ((rc = ev_begin(c, 0))) return rc;
-        CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, c->stream, a1, nb));
+        CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, st, a1, nb));
         if ((rc = ev_end(c, 0))) return rc;
         P2Args a2; memset(&a2, 0, sizeof(a2));
-        a2.Y = c->d_Y; a2.coef = c->d_coef + t0; a2.cand = c->d_cand;
-        a2.done_ctr = c->d_done; a2.peaks = c->d_peaks + t0; a2.trig = c->d_trig;
+        a2.Y = Y; a2.coef = c->d_coef + t0;
+        a2.cand = c->d_cand + (size_t)slot * c->max_sub_batch * (size_t)p2grid;
+        a2.done_ctr = c->d_done + (size_t)slot * c->max_sub_batch; a2.peaks = c->d_peaks + t0; a2.trig = c->d_trig;
         a2.trig_cursor = c->d_cursor; a2.trig_cap = (unsigned long long)trig_capacity;
         a2.tmpl_base = (int)t0;
         if ((rc = ev_begin(c, 1))) return rc;
-        CU(launch_p2<EPI_MAX>(c->lg1, c->lg2, c->stream, a2, nb));
+        CU(launch_p2<EPI_MAX>(c->lg1, c->lg2, st, a2, nb));
         if ((rc = ev_end(c, 1))) return rc;
         c->launches += 2;
+    }
+    if (ns > 1) {
+        for (int s = 0; s < ns; ++s) {
+            CU(cudaEventRecord(c->ev_join[s], c->aux[s]));
+            CU(cudaStreamWaitEvent(c->stream, c->ev_join[s], 0));
+        }
     }
 
     // status word + trigger count back to the host, then sort what was kept

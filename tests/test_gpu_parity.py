@@ -184,14 +184,18 @@ def test_filter_bank_cfg0(cbmf):
     assert 16 not in near
 
 
-@pytest.mark.parametrize("sub_batch", [1, 3, 5, 64])
-def test_filter_bank_independent_of_sub_batch(cbmf, sub_batch):
-    """Ragged last launch; results bit-identical whatever the launch grouping."""
+@pytest.mark.parametrize("sub_batch,streams", [(1, 1), (3, 2), (5, 3), (64, 2), (2, 8), (4, 1)])
+def test_filter_bank_independent_of_sub_batch(cbmf, sub_batch, streams):
+    """Ragged last launch; results bit-identical whatever the launch grouping and however many
+    launch pairs are in flight."""
     wl = W.config0()
     g = cbmf.Context(wl.n, wl.fs, wl.f_low)
     g.set_psd(wl.psd); g.load_segment(wl.samples)
+    g.set_streams(1)
     ref = g.filter_bank(wl.bank, wl.threshold)
     g.set_sub_batch(sub_batch)
+    g.set_streams(streams)
+    assert g.get_streams() == streams and g.get_sub_batch() == sub_batch
     got = g.filter_bank(wl.bank, wl.threshold)
     assert np.array_equal(ref[0], got[0]) and np.array_equal(ref[1], got[1]) and ref[2] == got[2]
     g.close()
