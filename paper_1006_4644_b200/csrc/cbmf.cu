@@ -104,17 +104,23 @@ int grow_scratch(cbmf_ctx* c, size_t bytes)
 int ilog2(int64_t n) { int l = 0; while ((int64_t(1) << l) < n) ++l; return l; }
 
 // ---------------------------------------------------------------- launch dispatch over (N1, N2)
+// Templates one pass-1 block works through with its staged w tile (LOAD_GEN): the launch uses
+// ceil(batch / P1_TEMPLATES_PER_BLOCK) blocks per column tile.
+constexpr int P1_TEMPLATES_PER_BLOCK = 4;
+
 template <int L1, int L2, int MODE>
-cudaError_t launch_p1_L(cudaStream_t s, const P1Args& a, int batch)
+cudaError_t launch_p1_L(cudaStream_t s, P1Args a, int batch)
 {
     static bool attr_done = false;
-    const size_t smem = sizeof(float2) * (size_t)Cfg<L1>::PADDED * Cfg<L1>::C;
+    const size_t smem = p1_smem_bytes<L1, MODE>();
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(p1_kernel<L1, L2, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    dim3 grid(L2 / Cfg<L1>::C, batch);
+    a.batch = batch;
+    const int groups = (MODE == LOAD_GEN) ? (batch + P1_TEMPLATES_PER_BLOCK - 1) / P1_TEMPLATES_PER_BLOCK : batch;
+    dim3 grid(L2 / Cfg<L1>::C, groups);
     p1_kernel<L1, L2, MODE><<<grid, Cfg<L1>::NT1, smem, s>>>(a);
     return cudaGetLastError();
 }

@@ -52,6 +52,17 @@ CBMF_CFG(4096, 16, 16, 16, 16, 1024)
 
 __host__ __device__ constexpr int ilog2c(int x) { return x <= 1 ? 0 : 1 + ilog2c(x >> 1); }
 
+// cp.async (LDGSTS) helpers: 16-byte global -> shared copies that bypass registers and L1.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+struct NoHook { __device__ __forceinline__ void operator()() const {} };
+
 // Stockham steps 1..3 of one L-point inverse FFT distributed over T threads (thread index t),
 // E values per thread.  On entry v[u*R1 + r] = x[t + T*u + (L/R1)*r]; on exit
 // v[u*RL + q] = X[t + T*u + (L/RL)*q] (RL = last radix).  sm points at this FFT's shared
@@ -63,9 +74,13 @@ __host__ __device__ constexpr int ilog2c(int x) { return x <= 1 ? 0 : 1 + ilog2c
 // the step-1 DFT, so it commutes with it and is folded here into the step-2 twiddles: the
 // step-2 reader at position i + (L/R2) r' sees writer p0 = (i >> lg R1) + R3 r', i.e. an extra
 // W_N^{j1 (i >> lg R1)} (W_N^{j1 R3})^{r'}.  n1 = N / L.
-template <int L, int NZ1, int SS, bool WARP_SYNC, bool ROWTW>
+//
+// after_last_read() is called once, after this thread's last read of the exchange buffer and
+// before the arithmetic of the last step; pass 2 uses it to start the asynchronous copy of the
+// next row into the same buffer (the hook must synchronise the group before it overwrites).
+template <int L, int NZ1, int SS, bool WARP_SYNC, bool ROWTW, typename Hook = NoHook>
 __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, float2* __restrict__ sm,
-                                         const int j1 = 0, const int n1 = 1)
+                                         const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook())
 {
     using C = Cfg<L>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, R2 = C::R2, R3 = C::R3;
@@ -91,13 +106,19 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
     // ---- step 2: radix R2, Ns = R1
     {
         constexpr int NB = E / R2, NS = R1;
-        float2 y[E];
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int i = t + T * u;
+#pragma unroll
+            for (int r = 0; r < R2; ++r) v[u * R2 + r] = sm[pad(i + (L / R2) * r) * SS];
+        }
+        if constexpr (R3 == 1) after_last_read();
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
             float2 x[R2];
             const int i = t + T * u;
 #pragma unroll
-            for (int r = 0; r < R2; ++r) x[r] = sm[pad(i + (L / R2) * r) * SS];
+            for (int r = 0; r < R2; ++r) x[r] = v[u * R2 + r];
             const int k = i & (NS - 1);
             if constexpr (ROWTW) {
                 // e^{2 pi i (k / (R1 R2) + j1 R3 / N)}: numerator over N = n1 L is an exact integer < N
@@ -113,11 +134,9 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
             }
             dft<R2>(x);
 #pragma unroll
-            for (int q = 0; q < R2; ++q) y[u * R2 + q] = x[q];
+            for (int q = 0; q < R2; ++q) v[u * R2 + q] = x[q];
         }
         if constexpr (R3 == 1) {
-#pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = y[e];
             return;
         } else {
             sync();   // all step-2 reads done before the buffer is overwritten
@@ -127,7 +146,7 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
                 const int k = i & (NS - 1);
                 const int base = (i >> LG_R1) * (NS * R2) + k;
 #pragma unroll
-                for (int q = 0; q < R2; ++q) sm[pad(base + q * NS) * SS] = y[u * R2 + q];
+                for (int q = 0; q < R2; ++q) sm[pad(base + q * NS) * SS] = v[u * R2 + q];
             }
         }
     }
@@ -137,10 +156,17 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
         constexpr int NB = E / R3, NS = R1 * R2;
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
+            const int i = t + T * u;
+#pragma unroll
+            for (int r = 0; r < R3; ++r) v[u * R3 + r] = sm[pad(i + (L / R3) * r) * SS];
+        }
+        after_last_read();
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
             float2 x[R3];
             const int i = t + T * u;
 #pragma unroll
-            for (int r = 0; r < R3; ++r) x[r] = sm[pad(i + (L / R3) * r) * SS];
+            for (int r = 0; r < R3; ++r) x[r] = v[u * R3 + r];
             const int k = i & (NS - 1);
             mul_powers<R3, false>(x, expi_frac(k, 2.0f / (float)L), make_float2(1.f, 0.f));
             dft<R3>(x);
@@ -182,75 +208,102 @@ struct P1Args {
     const float* __restrict__ in_r;        // [batch][N] (LOAD_REAL)
     float2* __restrict__ Y;                // [batch][N], Y[j1*N2 + k2]
     int* err_flag;                         // set to 1 on a non-finite real input sample
+    int batch;                             // templates (or vectors) in this launch
 };
 
-// One tile of NC adjacent columns k2 of template slot b: N1 = L1-point inverse FFT over k1 of
-// x[k1*L2 + k2] -> Y[b][j1*L2 + k2].  All Cfg<L1>::NT1 threads of the block take part.
-template <int L1, int L2, int MODE>
-__device__ __forceinline__ void p1_tile(const P1Args& a, const int tile, const int b, float2* __restrict__ smem)
+// Shared memory of one pass-1 block: the exchange buffer of NC column FFTs and, for LOAD_GEN,
+// the tile w[k1][k2 in tile], k1 < N1/2 (the upper half of the spectrum is zero), staged once
+// per block and reused by every template the block works through.
+template <int L1, int MODE>
+__host__ __device__ constexpr size_t p1_smem_bytes()
 {
     using C = Cfg<L1>;
-    constexpr int E = C::E, T = C::T, R1 = C::R1, NC = C::C;
+    return sizeof(float2) * ((size_t)C::PADDED * C::C + (MODE == LOAD_GEN ? (size_t)(L1 / 2) * C::C : 0));
+}
+
+// One pass-1 block = one tile of NC adjacent columns k2.  For every template slot b of the
+// launch with b = blockIdx.y (mod gridDim.y): N1 = L1-point inverse FFT over k1 of
+// x[k1*L2 + k2] -> Y[b][j1*L2 + k2].
+template <int L1, int L2, int MODE>
+__global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p1_kernel(const P1Args a)
+{
+    extern __shared__ __align__(16) float2 smem[];
+    using C = Cfg<L1>;
+    constexpr int E = C::E, T = C::T, R1 = C::R1, NC = C::C, NT = C::NT1;
     constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
     constexpr int NZ1 = (MODE == LOAD_GEN) ? R1 / 2 : R1;    // bins k >= N/2 are zero
     constexpr size_t n_total = (size_t)L1 * L2;
 
+    const int tile = blockIdx.x;
     const int c = threadIdx.x % NC, t = threadIdx.x / NC;
     const int k2 = tile * NC + c;
+    float2* __restrict__ wt = smem + (size_t)C::PADDED * NC;      // [L1/2][NC]
 
-    float2 v[E];
     if constexpr (MODE == LOAD_GEN) {
-        const TemplCoef* tc = a.coef + b;
-        const int k_lo = tc->k_lo, k_hi = tc->k_hi;
-        // all loads of w first (w is zero below k_lo), then the phasors of the in-band bins
+        // stage the w tile: rows of NC float2 = NC/2 chunks of 16 bytes
+        constexpr int CPR = NC / 2, NCHUNK = (L1 / 2) * CPR;
+        for (int ci = threadIdx.x; ci < NCHUNK; ci += NT) {
+            const int row = ci / CPR, part = ci % CPR;
+            cp_async16(wt + row * NC + 2 * part, a.w + ((size_t)row * L2 + tile * NC + 2 * part));
+        }
+        cp_async_commit();
+    }
+
+    bool first = true;
+    for (int b = blockIdx.y; b < a.batch; b += gridDim.y) {
+        float2 v[E];
+        if constexpr (MODE == LOAD_GEN) {
+            const TemplCoef* tc = a.coef + b;
+            const int k_lo = tc->k_lo, k_hi = tc->k_hi;
+            const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+            // the phasors of the in-band bins first (they do not need w) ...
 #pragma unroll
-        for (int u = 0; u < E / R1; ++u)
+            for (int u = 0; u < E / R1; ++u)
 #pragma unroll
-            for (int r = 0; r < R1; ++r)
-                v[u * R1 + r] = (r < NZ1) ? __ldg(a.w + ((t + T * u + (L1 / R1) * r) * L2 + k2)) : make_float2(0.f, 0.f);
-        const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+                for (int r = 0; r < NZ1; ++r) {
+                    const int k = (t + T * u + (L1 / R1) * r) * L2 + k2;
+                    float2 val = make_float2(0.f, 0.f);
+                    if (k >= k_lo && k <= k_hi) val = spa_phasor(k, A1, A2, A3, A5);
+                    v[u * R1 + r] = val;
+                }
+            if (first) { cp_async_wait_all(); __syncthreads(); first = false; }
+            // ... then q~ = w e^{+i Psi}; outside the band the phasor is 0
 #pragma unroll
-        for (int u = 0; u < E / R1; ++u)
+            for (int u = 0; u < E / R1; ++u) {
 #pragma unroll
-            for (int r = 0; r < NZ1; ++r) {
-                const int k = (t + T * u + (L1 / R1) * r) * L2 + k2;
-                float2 val = make_float2(0.f, 0.f);
-                if (k >= k_lo && k <= k_hi) val = cmul(v[u * R1 + r], spa_phasor(k, A1, A2, A3, A5));
-                v[u * R1 + r] = val;
+                for (int r = 0; r < NZ1; ++r)
+                    v[u * R1 + r] = cmul(wt[(t + T * u + (L1 / R1) * r) * NC + c], v[u * R1 + r]);
+#pragma unroll
+                for (int r = NZ1; r < R1; ++r) v[u * R1 + r] = make_float2(0.f, 0.f);
             }
-    } else {
+        } else {
 #pragma unroll
-        for (int u = 0; u < E / R1; ++u) {
+            for (int u = 0; u < E / R1; ++u) {
 #pragma unroll
-            for (int r = 0; r < R1; ++r) {
-                const size_t k = (size_t)(t + T * u + (L1 / R1) * r) * L2 + k2;
-                if constexpr (MODE == LOAD_CPLX) {
-                    v[u * R1 + r] = __ldg(a.in_c + (size_t)b * n_total + k);
-                } else {
-                    const float x = __ldg(a.in_r + (size_t)b * n_total + k);
-                    if (!isfinite(x)) *a.err_flag = 1;
-                    v[u * R1 + r] = make_float2(x, 0.f);
+                for (int r = 0; r < R1; ++r) {
+                    const size_t k = (size_t)(t + T * u + (L1 / R1) * r) * L2 + k2;
+                    if constexpr (MODE == LOAD_CPLX) {
+                        v[u * R1 + r] = __ldg(a.in_c + (size_t)b * n_total + k);
+                    } else {
+                        const float x = __ldg(a.in_r + (size_t)b * n_total + k);
+                        if (!isfinite(x)) *a.err_flag = 1;
+                        v[u * R1 + r] = make_float2(x, 0.f);
+                    }
                 }
             }
         }
-    }
 
-    fft_core<L1, NZ1, NC, false, false>(v, t, smem + c);
+        fft_core<L1, NZ1, NC, false, false>(v, t, smem + c);
 
-    float2* __restrict__ yb = a.Y + (size_t)b * n_total + (size_t)t * L2 + k2;
+        float2* __restrict__ yb = a.Y + (size_t)b * n_total + (size_t)t * L2 + k2;
 #pragma unroll
-    for (int u = 0; u < E / RL; ++u) {
+        for (int u = 0; u < E / RL; ++u) {
 #pragma unroll
-        for (int q = 0; q < RL; ++q)
-            yb[(size_t)(T * u + (L1 / RL) * q) * L2] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
+            for (int q = 0; q < RL; ++q)
+                yb[(size_t)(T * u + (L1 / RL) * q) * L2] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
+        }
+        __syncthreads();      // last exchange reads done before the next template's step-1 writes
     }
-}
-
-template <int L1, int L2, int MODE>
-__global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p1_kernel(const P1Args a)
-{
-    extern __shared__ float2 smem[];
-    p1_tile<L1, L2, MODE>(a, blockIdx.x, blockIdx.y, smem);
 }
 
 // ------------------------------------------------------------------ pass 2
@@ -297,11 +350,24 @@ struct PeakAcc {
     float best; int j; float re, im;
 };
 
+// Start the asynchronous copy of one row of Y (L2 complex floats, contiguous) into the row
+// group's shared-memory buffer (unpadded, element k2 at sm[k2]); T threads take part.
+template <int L2>
+__device__ __forceinline__ void p2_prefetch_row(float2* __restrict__ sm, const float2* __restrict__ yrow, const int t)
+{
+    constexpr int T = Cfg<L2>::T, E = Cfg<L2>::E;
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) cp_async16(sm + 2 * (t + T * i), yrow + 2 * (t + T * i));
+    cp_async_commit();
+}
+
 // Row j1 of template slot b: twiddle, N2 = L2-point inverse FFT over k2 -> z[j1 + L1 j2] in
-// registers, then the epilogue of MODE.  Called by the T threads of one row group.
+// registers, then the epilogue of MODE.  Called by the T threads of one row group.  On entry the
+// copy of the row into sm has been started by p2_prefetch_row; next_row (or nullptr) is the row
+// whose copy is started as soon as the exchange buffer is free again.
 template <int L1, int L2, int MODE>
 __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int b, const int t,
-                                       float2* __restrict__ sm, PeakAcc& acc)
+                                       float2* __restrict__ sm, PeakAcc& acc, const float2* __restrict__ next_row)
 {
     using C = Cfg<L2>;
     constexpr int E = C::E, T = C::T, R1 = C::R1;
@@ -309,15 +375,17 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
     constexpr bool WSYNC = (T <= 32);
     constexpr int LG1 = ilog2c(L1);
     constexpr size_t n_total = (size_t)L1 * L2;
+    auto gsync = []() { if constexpr (WSYNC) __syncwarp(); else __syncthreads(); };
 
-    // load row j1; multiply by (W_N^{j1 L2/R1})^r (the rest of the inter-pass twiddle is folded
-    // into the step-2 twiddles of fft_core)
+    // row j1 from the staging buffer; multiply by (W_N^{j1 L2/R1})^r (the rest of the inter-pass
+    // twiddle is folded into the step-2 twiddles of fft_core)
     float2 v[E];
-    const float2* __restrict__ yrow = a.Y + (size_t)b * n_total + (size_t)j1 * L2;
+    cp_async_wait_all();
+    gsync();
 #pragma unroll
     for (int u = 0; u < E / R1; ++u)
 #pragma unroll
-        for (int r = 0; r < R1; ++r) v[u * R1 + r] = __ldcg(yrow + t + T * u + (L2 / R1) * r);
+        for (int r = 0; r < R1; ++r) v[u * R1 + r] = sm[t + T * u + (L2 / R1) * r];
     if constexpr (WSYNC) {
         // G[r] = e^{2 pi i j1 r / (L1 R1)}, r < R1: one sincospi per lane, broadcast through shared memory
         float2* __restrict__ G = sm + C::PADDED;
@@ -338,6 +406,7 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
             for (int u = 0; u < E / R1; ++u) v[u * R1 + 1] = cmul(v[u * R1 + 1], g1);
         }
     } else {
+        __syncthreads();                                              // staging reads done before the exchange writes
         const float2 g = expi_frac(j1, 2.0f / (float)(L1 * R1));      // W_N^{j1 L2/R1}
 #pragma unroll
         for (int u = 0; u < E / R1; ++u) {
@@ -350,7 +419,13 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
         }
     }
 
-    fft_core<L2, R1, 1, WSYNC, true>(v, t, sm, j1, L1);
+    auto start_next = [&]() {
+        if (next_row != nullptr) {          // uniform over the row group
+            gsync();                        // every thread of the group has read the exchange buffer
+            p2_prefetch_row<L2>(sm, next_row, t);
+        }
+    };
+    fft_core<L2, R1, 1, WSYNC, true>(v, t, sm, j1, L1, start_next);
 
     // v[u*RL + q] = z[j1 + L1 * j2],  j2 = t + T u + (L2/RL) q
     if constexpr (MODE == EPI_STORE) {
@@ -503,13 +578,17 @@ __device__ __forceinline__ void p2_item(const P2Args& a, const int item, const i
     using C = Cfg<L2>;
     constexpr int T = C::T, ROWS = C::ROWS;
     constexpr int RPW = (MODE == EPI_MAX) ? p2_rpw<L1, L2>() : 1;
+    constexpr size_t n_total = (size_t)L1 * L2;
     const int t = threadIdx.x % T, row = threadIdx.x / T;
     float2* sm = smem + row * p2_row_stride<L2>();
+    const float2* __restrict__ yb = a.Y + (size_t)b * n_total;
     PeakAcc acc; acc.best = -1.0f; acc.j = 0x7FFFFFFF; acc.re = 0.f; acc.im = 0.f;
+    p2_prefetch_row<L2>(sm, yb + (size_t)((item * RPW) * ROWS + row) * L2, t);
 #pragma unroll 1
     for (int it = 0; it < RPW; ++it) {
-        if (it > 0) { if constexpr (T <= 32) __syncwarp(); else __syncthreads(); }
-        p2_row<L1, L2, MODE>(a, (item * RPW + it) * ROWS + row, b, t, sm, acc);
+        const int j1 = (item * RPW + it) * ROWS + row;
+        const float2* next_row = (it + 1 < RPW) ? yb + (size_t)(j1 + ROWS) * L2 : nullptr;
+        p2_row<L1, L2, MODE>(a, j1, b, t, sm, acc, next_row);
     }
     if constexpr (MODE == EPI_MAX) p2_finish(a, acc, b, item, L1 / (ROWS * RPW));
 }
@@ -517,7 +596,7 @@ __device__ __forceinline__ void p2_item(const P2Args& a, const int item, const i
 template <int L1, int L2, int MODE>
 __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
 {
-    extern __shared__ float2 smem[];
+    extern __shared__ __align__(16) float2 smem[];
     p2_item<L1, L2, MODE>(a, blockIdx.x, blockIdx.y, smem);
 }
 
