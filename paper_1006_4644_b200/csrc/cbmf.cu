@@ -37,9 +37,11 @@ struct cbmf_ctx {
     double* d_term = nullptr;              // [N/2]
     double* d_prefix = nullptr;            // [N/2]
     double* d_bsum = nullptr;              // [ceil(N/2 / SCAN_TILE)] scan block totals / offsets
-    float2* d_w = nullptr;                 // [N/2]
-    float2* d_Y = nullptr;                 // [max_sub_batch][N]
-    float4* d_cand = nullptr;              // [max_sub_batch][p2 grid.x]
+    double* d_u = nullptr;                 // [N/2] k^{-1/3}
+    c2* d_w = nullptr;                     // [N/2]
+    c2* d_Y = nullptr;                     // [slots][N]
+    c2* d_cand = nullptr;                  // [slots][N / E2] arg-max candidates, one per (row, thread)
+    unsigned long long* d_key = nullptr;   // [slots] running arg-max keys
     unsigned int* d_done = nullptr;        // [max_sub_batch]
     int* d_err = nullptr;                  // [1]
     unsigned long long* d_cursor = nullptr;// [1]
@@ -132,7 +134,7 @@ template <int L1, int L2, int MODE>
 cudaError_t launch_p2_L(cudaStream_t s, const P2Args& a, int batch)
 {
     static bool attr_done = false;
-    const size_t smem = sizeof(float2) * (size_t)p2_row_stride<L2>() * Cfg<L2>::ROWS;
+    const size_t smem = sizeof(c2) * (size_t)p2_row_stride<L2>() * Cfg<L2>::ROWS;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(p2_kernel<L1, L2, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -173,12 +175,13 @@ cudaError_t launch_p2(int lg1, int lg2, cudaStream_t s, const P2Args& a, int bat
     CBMF_DISPATCH(lg1, lg2, (launch_p2_L<L1, L2, MODE>(s, a, batch)))
 }
 
-// blocks per template of the arg-max pass (size of one row of the candidate buffer)
-int p2_peak_items(int lg1, int lg2)
+// candidate slots per template of the arg-max pass: one per (row j1, thread of the row group) = N / E2
+template <int L1, int L2> constexpr int cand_count() { return L1 * Cfg<L2>::T; }
+size_t cand_per_template(const cbmf_ctx* c)
 {
-    auto f = [&]() -> int { CBMF_DISPATCH(lg1, lg2, (p2_items<L1, L2, EPI_MAX>())) };
+    auto f = [&]() -> int { CBMF_DISPATCH(c->lg1, c->lg2, (cand_count<L1, L2>())) };
     const int v = f();
-    return v > 0 ? v : 1;
+    return v > 0 ? (size_t)v : 1;
 }
 
 // pass-timing events (cbmf_set_profiling): one start/stop pair per launch
@@ -223,21 +226,23 @@ int alloc_pipeline(cbmf_ctx* c, int sb, int ns)
     CU(cudaStreamSynchronize(c->stream));
     for (int i = 0; i < c->max_streams; ++i) if (c->aux[i]) CU(cudaStreamSynchronize(c->aux[i]));
     const size_t slots = (size_t)sb * ns;
-    const int p2grid = p2_peak_items(c->lg1, c->lg2);
-    float2* y = nullptr; float4* cand = nullptr; unsigned int* done = nullptr;
-    cudaError_t e = cudaMalloc(&y, sizeof(float2) * (size_t)c->n * slots);
-    if (e == cudaSuccess) e = cudaMalloc(&cand, sizeof(float4) * (size_t)p2grid * slots);
+    const size_t ncand = cand_per_template(c);
+    c2* y = nullptr; c2* cand = nullptr; unsigned int* done = nullptr; unsigned long long* key = nullptr;
+    cudaError_t e = cudaMalloc(&y, sizeof(c2) * (size_t)c->n * slots);
+    if (e == cudaSuccess) e = cudaMalloc(&cand, sizeof(c2) * ncand * slots);
     if (e == cudaSuccess) e = cudaMalloc(&done, sizeof(unsigned int) * slots);
+    if (e == cudaSuccess) e = cudaMalloc(&key, sizeof(unsigned long long) * slots);
     if (e == cudaSuccess) e = cudaMemsetAsync(done, 0, sizeof(unsigned int) * slots, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(key, 0, sizeof(unsigned long long) * slots, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     for (int i = c->max_streams; i < ns && e == cudaSuccess; ++i) {
         e = cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming);
     }
     if (e == cudaSuccess && !c->ev_fork) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
-    if (e != cudaSuccess) { cudaFree(y); cudaFree(cand); cudaFree(done); return cuda_fail(c, e, "alloc_pipeline"); }
-    cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done);
-    c->d_Y = y; c->d_cand = cand; c->d_done = done;
+    if (e != cudaSuccess) { cudaFree(y); cudaFree(cand); cudaFree(done); cudaFree(key); return cuda_fail(c, e, "alloc_pipeline"); }
+    cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key);
+    c->d_Y = y; c->d_cand = cand; c->d_done = done; c->d_key = key;
     c->max_sub_batch = sb; c->max_streams = ns;
     return CBMF_OK;
 }
@@ -251,7 +256,7 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     DeviceGuard g(c->device);
     cudaStreamSynchronize(c->stream);
     cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_bsum); cudaFree(c->d_w);
-    cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_err);
+    cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key); cudaFree(c->d_err); cudaFree(c->d_u);
     cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
     cudaFree(c->d_trig); cudaFree(c->d_scratch);
     for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
@@ -315,10 +320,14 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     CUF(cudaMalloc(&c->d_term, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_prefix, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_bsum, sizeof(double) * ((nh + SCAN_TILE - 1) / SCAN_TILE)));
-    CUF(cudaMalloc(&c->d_w, sizeof(float2) * nh));
+    CUF(cudaMalloc(&c->d_w, sizeof(c2) * nh));
+    CUF(cudaMalloc(&c->d_u, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_err, sizeof(int)));
     CUF(cudaMalloc(&c->d_cursor, sizeof(unsigned long long)));
     CUF(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    rcbrt_table_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(c->d_u, (int)nh);
+    CUF(cudaGetLastError());
+    c->launches += 1;
     CUF(cudaStreamSynchronize(c->stream));
 #undef CUF
     { const int rc = alloc_pipeline(c, c->sub_batch, c->n_streams); if (rc) return fail(rc); }
@@ -503,7 +512,7 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     // that the tail of one kernel overlaps the head of the next pair.  With per-pass event timing on
     // (cbmf_set_profiling) everything stays on the context's stream: each launch is timed alone.
     const int ns = (c->profiling || nt <= sb) ? 1 : c->n_streams;
-    const int p2grid = p2_peak_items(c->lg1, c->lg2);
+    const size_t ncand = cand_per_template(c);
     if (ns > 1) {
         CU(cudaEventRecord(c->ev_fork, c->stream));
         for (int s = 0; s < ns; ++s) CU(cudaStreamWaitEvent(c->aux[s], c->ev_fork, 0));
@@ -513,15 +522,16 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
         const int nb = (int)((nt - t0 < sb) ? (nt - t0) : sb);
         const int slot = (int)(pair % ns);
         cudaStream_t st = (ns > 1) ? c->aux[slot] : c->stream;
-        float2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
+        c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = c->d_w; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err;
+        a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err;
         if ((rc = ev_begin(c, 0))) return rc;
         CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, st, a1, nb));
         if ((rc = ev_end(c, 0))) return rc;
         P2Args a2; memset(&a2, 0, sizeof(a2));
         a2.Y = Y; a2.coef = c->d_coef + t0;
-        a2.cand = c->d_cand + (size_t)slot * c->max_sub_batch * (size_t)p2grid;
+        a2.cand = c->d_cand + (size_t)slot * c->max_sub_batch * ncand;
+        a2.best_key = c->d_key + (size_t)slot * c->max_sub_batch;
         a2.done_ctr = c->d_done + (size_t)slot * c->max_sub_batch; a2.peaks = c->d_peaks + t0; a2.trig = c->d_trig;
         a2.trig_cursor = c->d_cursor; a2.trig_cap = (unsigned long long)trig_capacity;
         a2.tmpl_base = (int)t0;
@@ -625,18 +635,18 @@ extern "C" int cbmf_debug_snr_series(cbmf_ctx* c, cbmf_template t, float* snr_ou
     if ((rc = setup_one(c, t))) return rc;
     const size_t n = (size_t)c->n;
     if ((rc = grow_scratch(c, sizeof(float2) * n + sizeof(float) * n))) return rc;
-    float2* z = (float2*)c->d_scratch;
+    c2* z = (c2*)c->d_scratch;
     float* snr = (float*)(z + n);
     TemplCoef tc;
     CU(cudaMemcpyAsync(&tc, c->d_coef, sizeof(tc), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     P1Args a1; memset(&a1, 0, sizeof(a1));
-    a1.w = c->d_w; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+    a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err;
     CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, c->stream, a1, 1));
     P2Args a2; memset(&a2, 0, sizeof(a2));
     a2.Y = c->d_Y; a2.z_out = z;
     CU(launch_p2<EPI_STORE>(c->lg1, c->lg2, c->stream, a2, 1));
-    snr_from_z_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(z, snr, n, tc.inv_sigma);
+    snr_from_z_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>((const float2*)z, snr, n, tc.inv_sigma);
     CU(cudaGetLastError());
     c->launches += 3;
     CU(cudaMemcpyAsync(snr_out, snr, sizeof(float) * n, cudaMemcpyDeviceToHost, c->stream));
@@ -654,7 +664,7 @@ extern "C" int cbmf_debug_template(cbmf_ctx* c, cbmf_template t, float* h_out)
     if ((rc = setup_one(c, t))) return rc;
     const int nh = (int)(c->n / 2);
     if ((rc = grow_scratch(c, sizeof(float2) * (size_t)(nh + 1)))) return rc;
-    debug_template_kernel<<<(nh + 1 + 255) / 256, 256, 0, c->stream>>>(c->d_coef, (float2*)c->d_scratch, nh, c->df);
+    debug_template_kernel<<<(nh + 1 + 255) / 256, 256, 0, c->stream>>>(c->d_coef, c->d_u, (float2*)c->d_scratch, nh, c->df);
     CU(cudaGetLastError());
     c->launches += 1;
     CU(cudaMemcpyAsync(h_out, c->d_scratch, sizeof(float2) * (size_t)(nh + 1), cudaMemcpyDeviceToHost, c->stream));
@@ -670,10 +680,10 @@ extern "C" int cbmf_debug_ifft_dev(cbmf_ctx* c, const float* in_dev, float* out_
     for (int64_t b0 = 0; b0 < batch; b0 += sb) {
         const int nb = (int)((batch - b0 < sb) ? (batch - b0) : sb);
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.in_c = (const float2*)in_dev + (size_t)b0 * n; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+        a1.in_c = (const c2*)in_dev + (size_t)b0 * n; a1.Y = c->d_Y; a1.err_flag = c->d_err;
         CU(launch_p1<LOAD_CPLX>(c->lg1, c->lg2, c->stream, a1, nb));
         P2Args a2; memset(&a2, 0, sizeof(a2));
-        a2.Y = c->d_Y; a2.z_out = (float2*)out_dev + (size_t)b0 * n;
+        a2.Y = c->d_Y; a2.z_out = (c2*)out_dev + (size_t)b0 * n;
         CU(launch_p2<EPI_STORE>(c->lg1, c->lg2, c->stream, a2, nb));
         c->launches += 2;
     }
@@ -686,8 +696,8 @@ extern "C" int cbmf_debug_ifft(cbmf_ctx* c, const float* in, float* out, int64_t
     if (!c || !in || !out || n != c->n || batch < 0) return CBMF_EINVAL;
     if (batch == 0) return CBMF_OK;
     DeviceGuard g(c->device);
-    const size_t bytes = sizeof(float2) * (size_t)n * (size_t)batch;
-    float2 *d_in = nullptr, *d_out = nullptr;
+    const size_t bytes = sizeof(c2) * (size_t)n * (size_t)batch;
+    c2 *d_in = nullptr, *d_out = nullptr;
     CU(cudaMalloc(&d_in, bytes));
     cudaError_t e = cudaMalloc(&d_out, bytes);
     if (e != cudaSuccess) { cudaFree(d_in); return cuda_fail(c, e, "cudaMalloc"); }
@@ -720,7 +730,7 @@ extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_de
     CU(cudaGetLastError());
     const int nh = (int)(c->n / 2);
     int gx = (nh + 255) / 256; if (gx > 592) gx = 592;
-    generate_only_kernel<<<dim3(gx, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_coef, (float2*)q_out_dev, nh);
+    generate_only_kernel<<<dim3(gx, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_u, c->d_coef, (c2*)q_out_dev, nh);
     CU(cudaGetLastError());
     c->launches += 2;
     int err = 0;

@@ -3,21 +3,74 @@
 // Everything here is the unnormalised INVERSE transform y_q = sum_r x_r e^{+2 pi i rq/R}
 // (the e^{+2 pi i f t} of eq. 2.1).  The forward transform of load_segment is
 // obtained from it by conjugation.  No code is shared with oracle/.
+//
+// Complex numbers are PACKED: one 64-bit register pair (re in the low word, im in the high
+// word), and the arithmetic is the sm_100 two-wide FP32 instructions (PTX add/mul/fma.f32x2,
+// SASS FADD2 / FMUL2 / FFMA2).  A complex add is one instruction, a complex multiply two, a
+// radix-2 butterfly with a general twiddle three; the swaps, broadcasts and per-half sign
+// flips written below as pk(...) are operand modifiers of those instructions (.LO_HI, .F32,
+// .NP), not extra moves.  The FP32 pipe time is that of the scalar code, the number of issue
+// slots is half.
 #pragma once
 #include <cuda_runtime.h>
 
 namespace cbmf {
 
-__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+typedef unsigned long long c2;            // packed complex float: (re, im)
+
+__device__ __forceinline__ c2 pk(float x, float y)
 {
-    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+    c2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
+    return r;
 }
-__device__ __forceinline__ float2 csqr(float2 a)
+__device__ __forceinline__ void unpk(c2 v, float& x, float& y)
 {
-    return make_float2(fmaf(a.x, a.x, -a.y * a.y), 2.0f * a.x * a.y);
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v));
 }
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float re(c2 v) { float x, y; unpk(v, x, y); return x; }
+__device__ __forceinline__ float im(c2 v) { float x, y; unpk(v, x, y); return y; }
+__device__ __forceinline__ c2 bc(float s) { return pk(s, s); }
+__device__ __forceinline__ c2 czero() { return 0ULL; }
+
+__device__ __forceinline__ c2 add2(c2 a, c2 b)
+{
+    c2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ c2 sub2(c2 a, c2 b)
+{
+    c2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ c2 mul2(c2 a, c2 b)
+{
+    c2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ c2 fma2(c2 a, c2 b, c2 c)
+{
+    c2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+
+// a * w = a.x (w.x, w.y) + a.y (-w.y, w.x): FMUL2 + FFMA2 (the (-w.y, w.x) operand is the
+// .LO_HI.NP form of w and must be the FIRST source of the multiply for ptxas to fold it).
+__device__ __forceinline__ c2 cmul(c2 a, c2 w)
+{
+    float ax, ay, wx, wy;
+    unpk(a, ax, ay);
+    unpk(w, wx, wy);
+    return fma2(bc(ax), w, mul2(pk(-wy, wx), bc(ay)));
+}
+__device__ __forceinline__ c2 csqr(c2 a) { return cmul(a, a); }
+// i * a
+__device__ __forceinline__ c2 mul_i(c2 a) { float x, y; unpk(a, x, y); return pk(-y, x); }
+__device__ __forceinline__ c2 neg2(c2 a) { float x, y; unpk(a, x, y); return pk(-x, -y); }
 
 // cos(2 pi a / 32), a = 0..8, correctly rounded to float.
 __device__ __forceinline__ constexpr float cos32_table(int a)
@@ -33,46 +86,32 @@ __device__ __forceinline__ constexpr float cos32_table(int a)
          : 0.0f;
 }
 
-// x * e^{+2 pi i q / R}, 0 <= q < R/2, R a power of two <= 32; q and R are compile-time
-// constants after unrolling, so the branches fold away.
-template <int R>
-__device__ __forceinline__ float2 twmul(float2 x, int q)
-{
-    const int a = q * (32 / R);                 // angle index, 0..15
-    if (a == 0) return x;
-    if (a == 8) return make_float2(-x.y, x.x);  // * i
-    const float c = (a <= 8) ? cos32_table(a) : -cos32_table(16 - a);
-    const float s = (a <= 8) ? cos32_table(8 - a) : cos32_table(a - 8);
-    return make_float2(fmaf(x.x, c, -x.y * s), fmaf(x.x, s, x.y * c));
-}
-
 // Butterfly lo = e + o w, hi = e - o w with w = e^{+2 pi i q / R}, 0 <= q < R/2 (compile-time
-// after unrolling).  Non-trivial twiddles are folded into FMAs: lo = e + o w costs four FFMA
-// and hi = 2e - lo two more (6 instead of 8 instructions); w = (+-1 +- i)/sqrt 2 costs 2 FADD +
-// 4 FFMA with no doubling.
+// after unrolling).  w = 1 or i: two FADD2; w = (+-1 + i)/sqrt 2: FADD2 + two FFMA2; general:
+// lo = e + o.x (c, s) + o.y (-s, c) is two FFMA2 and hi = 2 e - lo a third.
 template <int R>
-__device__ __forceinline__ void bfly(const float2 e, const float2 o, const int q, float2& lo, float2& hi)
+__device__ __forceinline__ void bfly(const c2 e, const c2 o, const int q, c2& lo, c2& hi)
 {
     const int a = q * (32 / R);                 // angle index, 0..15
+    float ox, oy;
+    unpk(o, ox, oy);
     if (a == 0) {
-        lo = cadd(e, o); hi = csub(e, o);
+        lo = add2(e, o); hi = sub2(e, o);
     } else if (a == 8) {                        // w = i
-        lo = make_float2(e.x - o.y, e.y + o.x); hi = make_float2(e.x + o.y, e.y - o.x);
-    } else if (a == 4) {                        // w = (1 + i) c
+        lo = add2(e, pk(-oy, ox)); hi = add2(e, pk(oy, -ox));
+    } else if (a == 4) {                        // w = (1 + i) c :  o w = c (ox - oy, ox + oy)
         const float c = cos32_table(4);
-        const float dx = o.x - o.y, dy = o.x + o.y;
-        lo = make_float2(fmaf(c, dx, e.x), fmaf(c, dy, e.y));
-        hi = make_float2(fmaf(-c, dx, e.x), fmaf(-c, dy, e.y));
-    } else if (a == 12) {                       // w = (-1 + i) c
+        const c2 d = add2(o, pk(-oy, ox));
+        lo = fma2(d, bc(c), e); hi = fma2(d, bc(-c), e);
+    } else if (a == 12) {                       // w = (-1 + i) c : o w = -c (ox + oy, oy - ox)
         const float c = cos32_table(4);
-        const float dx = o.x + o.y, dy = o.x - o.y;
-        lo = make_float2(fmaf(-c, dx, e.x), fmaf(c, dy, e.y));
-        hi = make_float2(fmaf(c, dx, e.x), fmaf(-c, dy, e.y));
+        const c2 d = add2(o, pk(oy, -ox));
+        lo = fma2(d, bc(-c), e); hi = fma2(d, bc(c), e);
     } else {
         const float c = (a <= 8) ? cos32_table(a) : -cos32_table(16 - a);
         const float s = (a <= 8) ? cos32_table(8 - a) : cos32_table(a - 8);
-        lo = make_float2(fmaf(-o.y, s, fmaf(o.x, c, e.x)), fmaf(o.y, c, fmaf(o.x, s, e.y)));
-        hi = make_float2(fmaf(2.0f, e.x, -lo.x), fmaf(2.0f, e.y, -lo.y));
+        lo = fma2(bc(oy), pk(-s, c), fma2(bc(ox), pk(c, s), e));
+        hi = fma2(e, bc(2.0f), neg2(lo));
     }
 }
 
@@ -80,7 +119,7 @@ __device__ __forceinline__ void bfly(const float2 e, const float2 o, const int q
 // NZ: only inputs v[0..NZ) are non-zero (the rest are never read), which prunes the leaves.
 template <int R, int NZ>
 struct DftP {
-    static __device__ __forceinline__ void run(float2 (&v)[R])
+    static __device__ __forceinline__ void run(c2 (&v)[R])
     {
         if constexpr (NZ <= 1) {
 #pragma unroll
@@ -89,7 +128,7 @@ struct DftP {
             constexpr int H = R / 2;
             constexpr int NZE = ((NZ + 1) / 2 < H) ? (NZ + 1) / 2 : H;
             constexpr int NZO = (NZ / 2 < H) ? NZ / 2 : H;
-            float2 e[H], o[H];
+            c2 e[H], o[H];
 #pragma unroll
             for (int i = 0; i < H; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
             DftP<H, NZE>::run(e);
@@ -101,38 +140,38 @@ struct DftP {
 };
 template <int NZ>
 struct DftP<1, NZ> {
-    static __device__ __forceinline__ void run(float2 (&)[1]) {}
+    static __device__ __forceinline__ void run(c2 (&)[1]) {}
 };
 
 template <int R>
-__device__ __forceinline__ void dft(float2 (&v)[R]) { DftP<R, R>::run(v); }
+__device__ __forceinline__ void dft(c2 (&v)[R]) { DftP<R, R>::run(v); }
 
 // e^{+2 pi i num/den} with den a power of two <= 2^24 and 0 <= num < den: the argument of
 // sincospif is formed exactly (integers below 2^24 and a power-of-two scale).
-__device__ __forceinline__ float2 expi_frac(int num, float two_over_den)
+__device__ __forceinline__ c2 expi_frac(int num, float two_over_den)
 {
     float s, c;
     sincospif((float)num * two_over_den, &s, &c);
-    return make_float2(c, s);
+    return pk(c, s);
 }
 
 // x[r] *= base * g^r for r = 0..R-1 (r = 0 multiplies by base only when HAS_BASE).
 // Powers are built as g^(8 hi) * (base g^lo): every factor is at most 6 roundings deep.
 template <int R, bool HAS_BASE>
-__device__ __forceinline__ void mul_powers(float2 (&x)[R], float2 g, float2 base)
+__device__ __forceinline__ void mul_powers(c2 (&x)[R], c2 g, c2 base)
 {
     constexpr int LO = (R < 8) ? R : 8;
-    float2 pl[LO];
-    const float2 g2 = csqr(g);
+    c2 pl[LO];
+    const c2 g2 = csqr(g);
     if constexpr (HAS_BASE) {
         pl[0] = base;
         pl[1] = cmul(base, g);
     } else {
-        pl[0] = make_float2(1.0f, 0.0f);
+        pl[0] = pk(1.0f, 0.0f);
         pl[1] = g;
     }
     if constexpr (LO > 2) {
-        const float2 g4 = csqr(g2);
+        const c2 g4 = csqr(g2);
         pl[2] = HAS_BASE ? cmul(pl[0], g2) : g2;
         pl[3] = cmul(pl[1], g2);
         if constexpr (LO > 4) {
@@ -142,8 +181,8 @@ __device__ __forceinline__ void mul_powers(float2 (&x)[R], float2 g, float2 base
             pl[7] = cmul(pl[3], g4);
         }
         if constexpr (R > 8) {
-            const float2 g8 = csqr(g4);
-            float2 ph = g8;
+            const c2 g8 = csqr(g4);
+            c2 ph = g8;
 #pragma unroll
             for (int hi = 1; hi < R / 8; ++hi) {
 #pragma unroll

@@ -63,6 +63,23 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 struct NoHook { __device__ __forceinline__ void operator()() const {} };
 
+// Row stride (in c2) of the step-2 twiddle table TW[k][r] = e^{2 pi i k r / (R1 R2)}, k < R1,
+// r < R2: even (rows are read with 16-byte loads) and = 2 mod 32 words so that the few rows a
+// warp touches fall on different banks.
+template <int L> __host__ __device__ constexpr int twtab_stride() { return Cfg<L>::R2 + 2; }
+template <int L> __host__ __device__ constexpr int twtab_elems() { return Cfg<L>::R1 * twtab_stride<L>(); }
+
+// Fill the step-2 twiddle table of an L-point FFT (all threads of the block take part).
+template <int L>
+__device__ __forceinline__ void twtab_fill(c2* __restrict__ tw, const int tid, const int nthreads)
+{
+    using C = Cfg<L>;
+    for (int e = tid; e < C::R1 * C::R2; e += nthreads) {
+        const int k = e / C::R2, r = e % C::R2;
+        tw[k * twtab_stride<L>() + r] = expi_frac((k * r) & (C::R1 * C::R2 - 1), 2.0f / (float)(C::R1 * C::R2));
+    }
+}
+
 // Stockham steps 1..3 of one L-point inverse FFT distributed over T threads (thread index t),
 // E values per thread.  On entry v[u*R1 + r] = x[t + T*u + (L/R1)*r]; on exit
 // v[u*RL + q] = X[t + T*u + (L/RL)*q] (RL = last radix).  sm points at this FFT's shared
@@ -75,12 +92,16 @@ struct NoHook { __device__ __forceinline__ void operator()() const {} };
 // step-2 reader at position i + (L/R2) r' sees writer p0 = (i >> lg R1) + R3 r', i.e. an extra
 // W_N^{j1 (i >> lg R1)} (W_N^{j1 R3})^{r'}.  n1 = N / L.
 //
+// tw (pass 1, may be null): the table of twtab_fill; the step-2 twiddles are then read from it
+// instead of being built as powers (one multiply per element instead of two).
+//
 // after_last_read() is called once, after this thread's last read of the exchange buffer and
 // before the arithmetic of the last step; pass 2 uses it to start the asynchronous copy of the
 // next row into the same buffer (the hook must synchronise the group before it overwrites).
 template <int L, int NZ1, int SS, bool WARP_SYNC, bool ROWTW, typename Hook = NoHook>
-__device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, float2* __restrict__ sm,
-                                         const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook())
+__device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm,
+                                         const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook(),
+                                         const c2* __restrict__ tw = nullptr)
 {
     using C = Cfg<L>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, R2 = C::R2, R3 = C::R3;
@@ -93,7 +114,7 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
         constexpr int NB = E / R1;
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
-            float2 x[R1];
+            c2 x[R1];
 #pragma unroll
             for (int r = 0; r < R1; ++r) x[r] = v[u * R1 + r];
             DftP<R1, NZ1>::run(x);
@@ -115,7 +136,7 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
         if constexpr (R3 == 1) after_last_read();
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
-            float2 x[R2];
+            c2 x[R2];
             const int i = t + T * u;
 #pragma unroll
             for (int r = 0; r < R2; ++r) x[r] = v[u * R2 + r];
@@ -123,14 +144,24 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
             if constexpr (ROWTW) {
                 // e^{2 pi i (k / (R1 R2) + j1 R3 / N)}: numerator over N = n1 L is an exact integer < N
                 const float two_over_n = 2.0f / ((float)n1 * (float)L);
-                const float2 g = expi_frac(k * (n1 * R3) + j1 * R3, two_over_n);
+                const c2 g = expi_frac(k * (n1 * R3) + j1 * R3, two_over_n);
                 if constexpr (R3 > 1) {
                     mul_powers<R2, true>(x, g, expi_frac(j1 * (i >> LG_R1), two_over_n));
                 } else {
-                    mul_powers<R2, false>(x, g, make_float2(1.f, 0.f));
+                    mul_powers<R2, false>(x, g, pk(1.f, 0.f));
                 }
             } else {
-                mul_powers<R2, false>(x, expi_frac(k, 2.0f / (float)(NS * R2)), make_float2(1.f, 0.f));
+                if (tw != nullptr) {                 // uniform over the launch
+                    const ulonglong2* __restrict__ row = reinterpret_cast<const ulonglong2*>(tw + k * twtab_stride<L>());
+#pragma unroll
+                    for (int r = 0; r < R2; r += 2) {
+                        const ulonglong2 w2 = row[r / 2];
+                        if (r > 0) x[r] = cmul(x[r], w2.x);
+                        x[r + 1] = cmul(x[r + 1], w2.y);
+                    }
+                } else {
+                    mul_powers<R2, false>(x, expi_frac(k, 2.0f / (float)(NS * R2)), pk(1.f, 0.f));
+                }
             }
             dft<R2>(x);
 #pragma unroll
@@ -163,12 +194,12 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
         after_last_read();
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
-            float2 x[R3];
+            c2 x[R3];
             const int i = t + T * u;
 #pragma unroll
             for (int r = 0; r < R3; ++r) x[r] = v[u * R3 + r];
             const int k = i & (NS - 1);
-            mul_powers<R3, false>(x, expi_frac(k, 2.0f / (float)L), make_float2(1.f, 0.f));
+            mul_powers<R3, false>(x, expi_frac(k, 2.0f / (float)L), pk(1.f, 0.f));
             dft<R3>(x);
 #pragma unroll
             for (int q = 0; q < R3; ++q) v[u * R3 + q] = x[q];
@@ -178,47 +209,66 @@ __device__ __forceinline__ void fft_core(float2 (&v)[Cfg<L>::E], const int t, fl
 
 // ------------------------------------------------------------------ S3: SPA phasor
 // e^{+i Psi_T(f_k)} for bin k >= 1 ("x form" in cycles).  The phase
-// reaches 1e4 cycles, so the polynomial and the reduction to [-1/2, 1/2] cycles run in fp64;
-// the fraction is then exact to 3e-8 cycles in fp32.  u = k^{-1/3}: fp32 seed + one Newton
-// step in fp64 (relative error ~ 2 (1.2e-7)^2).  The reduced angle lies in [-pi, pi], where
-// the SFU sine/cosine (MUFU.SIN/COS) have absolute error <= 2^-21.4 (CUDA math API, __sinf):
-// a template mismatch of order 1e-13, against the 1e-6 bound of tests/parity.py.
-__device__ __forceinline__ float2 spa_phasor(const int k, const double A1, const double A2,
-                                             const double A3, const double A5)
+// reaches 1e4 cycles, so the polynomial and the reduction to [-1/2, 1/2] cycles run in fp64
+// (the FP64 pipe is otherwise idle); the fraction is then exact to 3e-8 cycles in fp32.
+// u = k^{-1/3} in double comes from the template-independent table built by cbmf_create
+// (rcbrt_table_kernel, 8 bytes per bin, L2-resident).  ph - rint(ph) is taken with the
+// 1.5 * 2^52 trick (two DADD) instead of a conversion.  The reduced angle lies in [-pi, pi],
+// where the SFU sine/cosine (MUFU.SIN/COS) have absolute error <= 2^-21.4 (CUDA math API,
+// __sinf): a template mismatch of order 1e-13, against the 1e-6 bound of tests/parity.py.
+__device__ __forceinline__ c2 spa_phasor_u(const double u, const double A1, const double A2,
+                                           const double A3, const double A5)
 {
-    const double kd = (double)k;
-    double u = (double)rcbrtf((float)k);
-    const double e = fma(-kd * u, u * u, 1.0);
-    u = fma(u * e, 1.0 / 3.0, u);
     double ph = fma(u * u, A5, A3);
     ph = fma(ph, u, A2);
     ph = fma(ph, u, A1);
     ph = fma(ph, u, -0.125);
-    const float ang = 6.28318530717958647692f * (float)(ph - rint(ph));
-    return make_float2(__cosf(ang), __sinf(ang));
+    const double big = 6755399441055744.0;                 // 1.5 * 2^52: (ph + big) - big = rint(ph)
+    const double rn = __dadd_rn(__dadd_rn(ph, big), -big);
+    const float ang = 6.28318530717958647692f * (float)(ph - rn);
+    return pk(__cosf(ang), __sinf(ang));
+}
+
+// u[k] = k^{-1/3} in double (k >= 1; u[0] = 0), one Newton step on the library cube root.
+__global__ void rcbrt_table_kernel(double* __restrict__ u, int n_half)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_half) return;
+    double r = 0.0;
+    if (k > 0) {
+        const double kd = (double)k;
+        r = 1.0 / cbrt(kd);
+        r = fma(r * fma(-kd * r, r * r, 1.0), 1.0 / 3.0, r);
+    }
+    u[k] = r;
 }
 
 // ------------------------------------------------------------------ pass 1
 enum { LOAD_GEN = 0, LOAD_CPLX = 1, LOAD_REAL = 2 };
 
 struct P1Args {
-    const float2* __restrict__ w;          // [N/2] weighted data spectrum (LOAD_GEN)
+    const c2* __restrict__ w;              // [N/2] weighted data spectrum (LOAD_GEN)
+    const double* __restrict__ u;          // [N/2] k^{-1/3} (LOAD_GEN)
     const TemplCoef* __restrict__ coef;    // [batch] (LOAD_GEN)
-    const float2* __restrict__ in_c;       // [batch][N] (LOAD_CPLX)
+    const c2* __restrict__ in_c;           // [batch][N] (LOAD_CPLX)
     const float* __restrict__ in_r;        // [batch][N] (LOAD_REAL)
-    float2* __restrict__ Y;                // [batch][N], Y[j1*N2 + k2]
+    c2* __restrict__ Y;                    // [batch][N], Y[j1*N2 + k2]
     int* err_flag;                         // set to 1 on a non-finite real input sample
     int batch;                             // templates (or vectors) in this launch
 };
 
-// Shared memory of one pass-1 block: the exchange buffer of NC column FFTs and, for LOAD_GEN,
-// the tile w[k1][k2 in tile], k1 < N1/2 (the upper half of the spectrum is zero), staged once
-// per block and reused by every template the block works through.
+// The step-2 twiddle table is used where the FFT has two steps (L <= 1024).
+template <int L> __host__ __device__ constexpr bool p1_use_twtab() { return Cfg<L>::R3 == 1; }
+
+// Shared memory of one pass-1 block: the exchange buffer of NC column FFTs, the step-2 twiddle
+// table and, for LOAD_GEN, the tile w[k1][k2 in tile], k1 < N1/2 (the upper half of the
+// spectrum is zero), staged once per block and reused by every template the block works through.
 template <int L1, int MODE>
 __host__ __device__ constexpr size_t p1_smem_bytes()
 {
     using C = Cfg<L1>;
-    return sizeof(float2) * ((size_t)C::PADDED * C::C + (MODE == LOAD_GEN ? (size_t)(L1 / 2) * C::C : 0));
+    return sizeof(c2) * ((size_t)C::PADDED * C::C + (p1_use_twtab<L1>() ? (size_t)twtab_elems<L1>() : 0) +
+                         (MODE == LOAD_GEN ? (size_t)(L1 / 2) * C::C : 0));
 }
 
 // One pass-1 block = one tile of NC adjacent columns k2.  For every template slot b of the
@@ -227,20 +277,22 @@ __host__ __device__ constexpr size_t p1_smem_bytes()
 template <int L1, int L2, int MODE>
 __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p1_kernel(const P1Args a)
 {
-    extern __shared__ __align__(16) float2 smem[];
+    extern __shared__ __align__(16) c2 smem[];
     using C = Cfg<L1>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, NC = C::C, NT = C::NT1;
     constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
     constexpr int NZ1 = (MODE == LOAD_GEN) ? R1 / 2 : R1;    // bins k >= N/2 are zero
     constexpr size_t n_total = (size_t)L1 * L2;
+    constexpr bool TWTAB = p1_use_twtab<L1>();
 
     const int tile = blockIdx.x;
     const int c = threadIdx.x % NC, t = threadIdx.x / NC;
     const int k2 = tile * NC + c;
-    float2* __restrict__ wt = smem + (size_t)C::PADDED * NC;      // [L1/2][NC]
+    c2* __restrict__ tw = smem + (size_t)C::PADDED * NC;                               // [R1][R2 + 2]
+    c2* __restrict__ wt = tw + (TWTAB ? twtab_elems<L1>() : 0);                          // [L1/2][NC]
 
     if constexpr (MODE == LOAD_GEN) {
-        // stage the w tile: rows of NC float2 = NC/2 chunks of 16 bytes
+        // stage the w tile: rows of NC complex = NC/2 chunks of 16 bytes
         constexpr int CPR = NC / 2, NCHUNK = (L1 / 2) * CPR;
         for (int ci = threadIdx.x; ci < NCHUNK; ci += NT) {
             const int row = ci / CPR, part = ci % CPR;
@@ -248,10 +300,12 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
         }
         cp_async_commit();
     }
+    if constexpr (TWTAB) twtab_fill<L1>(tw, threadIdx.x, NT);
+    if constexpr (MODE != LOAD_GEN) __syncthreads();
 
     bool first = true;
     for (int b = blockIdx.y; b < a.batch; b += gridDim.y) {
-        float2 v[E];
+        c2 v[E];
         if constexpr (MODE == LOAD_GEN) {
             const TemplCoef* tc = a.coef + b;
             const int k_lo = tc->k_lo, k_hi = tc->k_hi;
@@ -262,8 +316,8 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
 #pragma unroll
                 for (int r = 0; r < NZ1; ++r) {
                     const int k = (t + T * u + (L1 / R1) * r) * L2 + k2;
-                    float2 val = make_float2(0.f, 0.f);
-                    if (k >= k_lo && k <= k_hi) val = spa_phasor(k, A1, A2, A3, A5);
+                    c2 val = czero();
+                    if (k >= k_lo && k <= k_hi) val = spa_phasor_u(__ldg(a.u + k), A1, A2, A3, A5);
                     v[u * R1 + r] = val;
                 }
             if (first) { cp_async_wait_all(); __syncthreads(); first = false; }
@@ -274,7 +328,7 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
                 for (int r = 0; r < NZ1; ++r)
                     v[u * R1 + r] = cmul(wt[(t + T * u + (L1 / R1) * r) * NC + c], v[u * R1 + r]);
 #pragma unroll
-                for (int r = NZ1; r < R1; ++r) v[u * R1 + r] = make_float2(0.f, 0.f);
+                for (int r = NZ1; r < R1; ++r) v[u * R1 + r] = czero();
             }
         } else {
 #pragma unroll
@@ -287,15 +341,15 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
                     } else {
                         const float x = __ldg(a.in_r + (size_t)b * n_total + k);
                         if (!isfinite(x)) *a.err_flag = 1;
-                        v[u * R1 + r] = make_float2(x, 0.f);
+                        v[u * R1 + r] = pk(x, 0.f);
                     }
                 }
             }
         }
 
-        fft_core<L1, NZ1, NC, false, false>(v, t, smem + c);
+        fft_core<L1, NZ1, NC, false, false>(v, t, smem + c, 0, 1, NoHook(), TWTAB ? tw : nullptr);
 
-        float2* __restrict__ yb = a.Y + (size_t)b * n_total + (size_t)t * L2 + k2;
+        c2* __restrict__ yb = a.Y + (size_t)b * n_total + (size_t)t * L2 + k2;
 #pragma unroll
         for (int u = 0; u < E / RL; ++u) {
 #pragma unroll
@@ -310,10 +364,11 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
 enum { EPI_MAX = 0, EPI_STORE = 1, EPI_WSTORE = 2 };
 
 struct P2Args {
-    const float2* __restrict__ Y;          // [batch][N]
+    const c2* __restrict__ Y;              // [batch][N]
     // EPI_MAX
     const TemplCoef* __restrict__ coef;    // [batch]
-    float4* cand;                          // [batch][gridDim.x]  (|z|^2, j as int bits, re, im)
+    unsigned long long* best_key;          // [batch] running arg-max key, zero on entry, zero again on exit
+    c2* cand;                              // [batch][N / E]  z at the candidate of (row j1, thread t)
     unsigned int* done_ctr;                // [batch], zero on entry, zero again on exit
     PeakOut* peaks;                        // [batch] (already offset to this sub-batch)
     TrigOut* trig;                         // bounded trigger list
@@ -321,19 +376,20 @@ struct P2Args {
     unsigned long long trig_cap;
     int tmpl_base;                         // bank index of template 0 of this sub-batch
     // EPI_STORE
-    float2* __restrict__ z_out;            // [batch][N], natural order
+    c2* __restrict__ z_out;                // [batch][N], natural order
     // EPI_WSTORE (load_segment): w[k] = conj(Z[k]) * wfac[k] for k < N/2
-    float2* __restrict__ w_out;            // [N/2]
+    c2* __restrict__ w_out;                // [N/2]
     const double* __restrict__ wfac;       // [N/2]
 };
 
+// (|z|^2 bits, ~j): the larger value wins and, among equal values, the smaller sample index,
+// whatever the order of arrival (|z|^2 >= 0, so its bit pattern orders like the value).
 __device__ __forceinline__ unsigned long long pack_key(float p, int j)
 {
     return ((unsigned long long)__float_as_uint(p) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)j);
 }
 
-// Rows per thread group and block in the arg-max pass: each group of T threads walks RPW rows
-// and keeps its running maximum in registers, so the block-level reduction is paid once.
+// Rows each thread group walks in the arg-max pass.
 template <int L1, int L2>
 __host__ __device__ constexpr int p2_rpw()
 {
@@ -345,15 +401,10 @@ template <int L2> __host__ __device__ constexpr int p2_row_stride()
     return Cfg<L2>::PADDED + (Cfg<L2>::T <= 32 ? Cfg<L2>::R1 : 0);      // exchange buffer + G table
 }
 
-// Shared per-thread state of the arg-max epilogue (S6/S7).
-struct PeakAcc {
-    float best; int j; float re, im;
-};
-
 // Start the asynchronous copy of one row of Y (L2 complex floats, contiguous) into the row
 // group's shared-memory buffer (unpadded, element k2 at sm[k2]); T threads take part.
 template <int L2>
-__device__ __forceinline__ void p2_prefetch_row(float2* __restrict__ sm, const float2* __restrict__ yrow, const int t)
+__device__ __forceinline__ void p2_prefetch_row(c2* __restrict__ sm, const c2* __restrict__ yrow, const int t)
 {
     constexpr int T = Cfg<L2>::T, E = Cfg<L2>::E;
 #pragma unroll
@@ -367,7 +418,7 @@ __device__ __forceinline__ void p2_prefetch_row(float2* __restrict__ sm, const f
 // whose copy is started as soon as the exchange buffer is free again.
 template <int L1, int L2, int MODE>
 __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int b, const int t,
-                                       float2* __restrict__ sm, PeakAcc& acc, const float2* __restrict__ next_row)
+                                       c2* __restrict__ sm, const c2* __restrict__ next_row)
 {
     using C = Cfg<L2>;
     constexpr int E = C::E, T = C::T, R1 = C::R1;
@@ -377,9 +428,13 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
     constexpr size_t n_total = (size_t)L1 * L2;
     auto gsync = []() { if constexpr (WSYNC) __syncwarp(); else __syncthreads(); };
 
+    // the running maximum of this template, read early (S7): rows that cannot beat it skip the search
+    unsigned best_bits = 0u;
+    if constexpr (MODE == EPI_MAX) best_bits = (unsigned)(__ldcg(a.best_key + b) >> 32);
+
     // row j1 from the staging buffer; multiply by (W_N^{j1 L2/R1})^r (the rest of the inter-pass
     // twiddle is folded into the step-2 twiddles of fft_core)
-    float2 v[E];
+    c2 v[E];
     cp_async_wait_all();
     gsync();
 #pragma unroll
@@ -388,32 +443,32 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
         for (int r = 0; r < R1; ++r) v[u * R1 + r] = sm[t + T * u + (L2 / R1) * r];
     if constexpr (WSYNC) {
         // G[r] = e^{2 pi i j1 r / (L1 R1)}, r < R1: one sincospi per lane, broadcast through shared memory
-        float2* __restrict__ G = sm + C::PADDED;
+        c2* __restrict__ G = sm + C::PADDED;
         for (int r = t; r < R1; r += T) G[r] = expi_frac((j1 * r) & (L1 * R1 - 1), 2.0f / (float)(L1 * R1));
         __syncwarp();
 #pragma unroll
         for (int r = 2; r < R1; r += 2) {
-            const float4 g = *reinterpret_cast<const float4*>(G + r);
+            const ulonglong2 g = *reinterpret_cast<const ulonglong2*>(G + r);
 #pragma unroll
             for (int u = 0; u < E / R1; ++u) {
-                v[u * R1 + r] = cmul(v[u * R1 + r], make_float2(g.x, g.y));
-                v[u * R1 + r + 1] = cmul(v[u * R1 + r + 1], make_float2(g.z, g.w));
+                v[u * R1 + r] = cmul(v[u * R1 + r], g.x);
+                v[u * R1 + r + 1] = cmul(v[u * R1 + r + 1], g.y);
             }
         }
         {
-            const float2 g1 = G[1];
+            const c2 g1 = G[1];
 #pragma unroll
             for (int u = 0; u < E / R1; ++u) v[u * R1 + 1] = cmul(v[u * R1 + 1], g1);
         }
     } else {
         __syncthreads();                                              // staging reads done before the exchange writes
-        const float2 g = expi_frac(j1, 2.0f / (float)(L1 * R1));      // W_N^{j1 L2/R1}
+        const c2 g = expi_frac(j1, 2.0f / (float)(L1 * R1));          // W_N^{j1 L2/R1}
 #pragma unroll
         for (int u = 0; u < E / R1; ++u) {
-            float2 x[R1];
+            c2 x[R1];
 #pragma unroll
             for (int r = 0; r < R1; ++r) x[r] = v[u * R1 + r];
-            mul_powers<R1, false>(x, g, make_float2(1.f, 0.f));
+            mul_powers<R1, false>(x, g, pk(1.f, 0.f));
 #pragma unroll
             for (int r = 0; r < R1; ++r) v[u * R1 + r] = x[r];
         }
@@ -429,7 +484,7 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
 
     // v[u*RL + q] = z[j1 + L1 * j2],  j2 = t + T u + (L2/RL) q
     if constexpr (MODE == EPI_STORE) {
-        float2* __restrict__ zb = a.z_out + (size_t)b * n_total + j1;
+        c2* __restrict__ zb = a.z_out + (size_t)b * n_total + j1;
 #pragma unroll
         for (int u = 0; u < E / RL; ++u)
 #pragma unroll
@@ -444,39 +499,52 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
                 const int j2 = t + T * u + (L2 / RL) * q;
                 const size_t k = ((size_t)j2 << LG1) + j1;
                 if (k < n_total / 2) {
-                    float2 o = make_float2(0.f, 0.f);
+                    c2 o = czero();
                     if ((long long)k >= k_lo) {
                         const double f = a.wfac[k];
-                        o = make_float2((float)(f * (double)v[u * RL + q].x), (float)(-f * (double)v[u * RL + q].y));
+                        o = pk((float)(f * (double)re(v[u * RL + q])), (float)(-f * (double)im(v[u * RL + q])));
                     }
                     a.w_out[k] = o;
                 }
             }
     } else {
-        // ---- S6/S7: |z|^2, arg-max (lowest index on ties), threshold
+        // ---- S6/S7: |z|^2, arg-max (lowest index on ties), threshold.
+        // Fast path: the thread's maximum of |z|^2 against the template's running maximum (read at
+        // the start of the row) and against the threshold.  A thread that may hold a new maximum
+        // locates its sample, publishes (|z|^2, ~j) with one 64-bit atomicMax and, if it won,
+        // leaves z in its own candidate slot (j1, t) for the block that finishes the template.
         const TemplCoef* tc = a.coef + b;
         const float thr2 = tc->thr2, inv_sigma = tc->inv_sigma;
-        float m = -1.0f;
+        auto pw = [&](int e) { float x, y; unpk(v[e], x, y); return fmaf(x, x, y * y); };
+        float m = pw(0);
 #pragma unroll
-        for (int e = 0; e < E; ++e) m = fmaxf(m, fmaf(v[e].x, v[e].x, v[e].y * v[e].y));
-        if (m >= acc.best) {                    // rare after the first rows: locate the sample
-            int best_e = 0;
-            bool found = false;
+        for (int e = 1; e < E; ++e) m = fmaxf(m, pw(e));
+        const unsigned mbits = __float_as_uint(m);
+        if (mbits >= best_bits) {
+            // only the lanes holding the group's largest value go on (usually one per warp)
+            unsigned gm = mbits;
+            if constexpr (WSYNC) gm = __reduce_max_sync(__activemask(), mbits);
+            if (mbits == gm) {
+                int best_e = 0;
+                bool found = false;
 #pragma unroll
-            for (int q = 0; q < RL; ++q)        // j2 increases with (q, u): first maximum kept
+                for (int q = 0; q < RL; ++q)        // j2 increases with (q, u): first maximum kept
 #pragma unroll
-                for (int u = 0; u < E / RL; ++u) {
-                    const int e = u * RL + q;
-                    const float p = fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
-                    if (!found && p == m) { found = true; best_e = e; }
+                    for (int u = 0; u < E / RL; ++u) {
+                        const int e = u * RL + q;
+                        if (!found && pw(e) == m) { found = true; best_e = e; }
+                    }
+                const int j2 = t + T * (best_e / RL) + (L2 / RL) * (best_e % RL);
+                const int j = (j2 << LG1) + j1;
+                const unsigned long long key = pack_key(m, j);
+                const unsigned long long old = atomicMax(a.best_key + b, key);
+                if (old < key) {
+                    c2 zb = v[0];
+#pragma unroll
+                    for (int e = 1; e < E; ++e)
+                        if (e == best_e) zb = v[e];
+                    __stcg(a.cand + (size_t)b * (n_total / E) + (size_t)j1 * T + t, zb);
                 }
-            const int j2 = t + T * (best_e / RL) + (L2 / RL) * (best_e % RL);
-            const int j = (j2 << LG1) + j1;
-            if (m > acc.best || j < acc.j) {
-                acc.best = m; acc.j = j;
-#pragma unroll
-                for (int e = 0; e < E; ++e)
-                    if (e == best_e) { acc.re = v[e].x; acc.im = v[e].y; }
             }
         }
         if (m > thr2 && inv_sigma > 0.f) {
@@ -485,16 +553,16 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
 #pragma unroll
                 for (int u = 0; u < E / RL; ++u) {
                     const int e = u * RL + q;
-                    const float p = fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
-                    if (p > thr2) {
+                    const float pe = pw(e);
+                    if (pe > thr2) {
                         const unsigned long long slot = atomicAdd(a.trig_cursor, 1ULL);
                         if (slot < a.trig_cap) {
                             const int j2 = t + T * u + (L2 / RL) * q;
                             TrigOut o;
                             o.template_idx = a.tmpl_base + b;
                             o.sample_idx = (j2 << LG1) + j1;
-                            o.snr = sqrtf(p) * inv_sigma;
-                            o.phase = atan2f(v[e].y, v[e].x);
+                            o.snr = sqrtf(pe) * inv_sigma;
+                            o.phase = atan2f(im(v[e]), re(v[e]));
                             a.trig[slot] = o;
                         }
                     }
@@ -503,100 +571,67 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
     }
 }
 
-// Block-level end of the arg-max pass: the block's best sample goes to cand[b][item]; the last
-// of the n_items blocks of template slot b reduces the candidates to the PeakOut record.
-__device__ __forceinline__ void p2_finish(const P2Args& a, const PeakAcc& acc, const int b,
-                                          const int item, const int n_items)
+// Block-level end of the arg-max pass: the last of the n_items blocks of template slot b turns
+// the template's key and the winner's candidate slot into the PeakOut record.
+template <int L1, int L2>
+__device__ __forceinline__ void p2_finish(const P2Args& a, const int b, const int n_items)
 {
-    __shared__ unsigned long long s_keys[32];
-    __shared__ unsigned long long s_win;
-    __shared__ int s_last;
-    const unsigned long long mykey = pack_key(acc.best, acc.j);
-    unsigned long long key = mykey;
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        const unsigned long long o = __shfl_xor_sync(0xFFFFFFFFu, key, off);
-        key = o > key ? o : key;
-    }
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
-    if (lane == 0) s_keys[warp] = key;
-    __syncthreads();
+    using C = Cfg<L2>;
+    constexpr int LG1 = ilog2c(L1);
+    constexpr size_t n_total = (size_t)L1 * L2;
+    __syncthreads();                                // every row of this block has published
     if (threadIdx.x == 0) {
-        unsigned long long k8 = s_keys[0];
-        for (int i = 1; i < nwarp; ++i) k8 = s_keys[i] > k8 ? s_keys[i] : k8;
-        s_win = k8;
-        s_last = 0;
-    }
-    __syncthreads();
-    if (mykey == s_win) {            // exactly one thread: sample indices are unique
-        float4 rec = make_float4(acc.best, __int_as_float(acc.j), acc.re, acc.im);
-        __stcg(a.cand + (size_t)b * n_items + item, rec);
         __threadfence();
         const unsigned int prev = atomicAdd(a.done_ctr + b, 1u);
-        s_last = (prev == (unsigned)n_items - 1u);
-    }
-    __syncthreads();
-    if (s_last && warp == 0) {
-        __threadfence();
-        const TemplCoef* tc = a.coef + b;
-        unsigned long long bk = 0ULL;
-        float bre = 0.f, bim = 0.f;
-        for (int i = lane; i < n_items; i += 32) {
-            const float4 r = __ldcg(a.cand + (size_t)b * n_items + i);
-            const unsigned long long kk = pack_key(r.x, __float_as_int(r.y));
-            if (kk > bk) { bk = kk; bre = r.z; bim = r.w; }
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            const unsigned long long ok = __shfl_xor_sync(0xFFFFFFFFu, bk, off);
-            const float ore = __shfl_xor_sync(0xFFFFFFFFu, bre, off);
-            const float oim = __shfl_xor_sync(0xFFFFFFFFu, bim, off);
-            if (ok > bk) { bk = ok; bre = ore; bim = oim; }
-        }
-        if (lane == 0) {
+        if (prev == (unsigned)n_items - 1u) {
+            __threadfence();
+            const TemplCoef* tc = a.coef + b;
+            const unsigned long long bk = __ldcg(a.best_key + b);
             PeakOut o;
-            if (tc->k_hi < tc->k_lo) {          // empty band
+            if (tc->k_hi < tc->k_lo) {              // empty band
                 o.snr_max = 0.f; o.idx_peak = -1; o.phase = 0.f; o.sigma = 0.f;
             } else {
                 const float p = __uint_as_float((unsigned)(bk >> 32));
+                const int j = (int)(0xFFFFFFFFu - (unsigned)(bk & 0xFFFFFFFFu));
+                const int j1 = j & (L1 - 1), tt = (j >> LG1) & (C::T - 1);
+                const c2 z = __ldcg(a.cand + (size_t)b * (n_total / C::E) + (size_t)j1 * C::T + tt);
                 o.snr_max = sqrtf(p) * tc->inv_sigma;
-                o.idx_peak = (int)(0xFFFFFFFFu - (unsigned)(bk & 0xFFFFFFFFu));
-                o.phase = atan2f(bim, bre);
+                o.idx_peak = j;
+                o.phase = atan2f(im(z), re(z));
                 o.sigma = tc->sigma;
             }
             a.peaks[b] = o;
-            a.done_ctr[b] = 0u;                 // self-cleaning for the next launch
+            a.best_key[b] = 0ULL;                   // self-cleaning for the next launch
+            a.done_ctr[b] = 0u;
         }
     }
-    __syncthreads();                            // s_keys / s_win reusable by the caller's next item
 }
 
 // One item of pass 2: ROWS * RPW rows of template slot b.
 template <int L1, int L2, int MODE>
-__device__ __forceinline__ void p2_item(const P2Args& a, const int item, const int b, float2* __restrict__ smem)
+__device__ __forceinline__ void p2_item(const P2Args& a, const int item, const int b, c2* __restrict__ smem)
 {
     using C = Cfg<L2>;
     constexpr int T = C::T, ROWS = C::ROWS;
     constexpr int RPW = (MODE == EPI_MAX) ? p2_rpw<L1, L2>() : 1;
     constexpr size_t n_total = (size_t)L1 * L2;
     const int t = threadIdx.x % T, row = threadIdx.x / T;
-    float2* sm = smem + row * p2_row_stride<L2>();
-    const float2* __restrict__ yb = a.Y + (size_t)b * n_total;
-    PeakAcc acc; acc.best = -1.0f; acc.j = 0x7FFFFFFF; acc.re = 0.f; acc.im = 0.f;
+    c2* sm = smem + row * p2_row_stride<L2>();
+    const c2* __restrict__ yb = a.Y + (size_t)b * n_total;
     p2_prefetch_row<L2>(sm, yb + (size_t)((item * RPW) * ROWS + row) * L2, t);
 #pragma unroll 1
     for (int it = 0; it < RPW; ++it) {
         const int j1 = (item * RPW + it) * ROWS + row;
-        const float2* next_row = (it + 1 < RPW) ? yb + (size_t)(j1 + ROWS) * L2 : nullptr;
-        p2_row<L1, L2, MODE>(a, j1, b, t, sm, acc, next_row);
+        const c2* next_row = (it + 1 < RPW) ? yb + (size_t)(j1 + ROWS) * L2 : nullptr;
+        p2_row<L1, L2, MODE>(a, j1, b, t, sm, next_row);
     }
-    if constexpr (MODE == EPI_MAX) p2_finish(a, acc, b, item, L1 / (ROWS * RPW));
+    if constexpr (MODE == EPI_MAX) p2_finish<L1, L2>(a, b, L1 / (ROWS * RPW));
 }
 
 template <int L1, int L2, int MODE>
 __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
 {
-    extern __shared__ __align__(16) float2 smem[];
+    extern __shared__ __align__(16) c2 smem[];
     p2_item<L1, L2, MODE>(a, blockIdx.x, blockIdx.y, smem);
 }
 
@@ -816,31 +851,32 @@ __global__ void snr_from_z_kernel(const float2* __restrict__ z, float* __restric
 }
 
 // h~[k] = f_k^{-7/6} e^{-i Psi_T(f_k)} on the band, zero elsewhere, k = 0..N/2
-__global__ void debug_template_kernel(const TemplCoef* __restrict__ tc, float2* __restrict__ h, int n_half, double df)
+__global__ void debug_template_kernel(const TemplCoef* __restrict__ tc, const double* __restrict__ u,
+                                      float2* __restrict__ h, int n_half, double df)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k > n_half) return;
     float2 o = make_float2(0.f, 0.f);
     if (k >= tc->k_lo && k <= tc->k_hi) {
-        const float2 ph = spa_phasor(k, tc->A1, tc->A2, tc->A3, tc->A5);
+        const c2 ph = spa_phasor_u(u[k], tc->A1, tc->A2, tc->A3, tc->A5);
         const float amp = (float)pow((double)k * df, -7.0 / 6.0);
-        o = make_float2(amp * ph.x, -amp * ph.y);
+        o = make_float2(amp * re(ph), -amp * im(ph));
     }
     h[k] = o;
 }
 
 // generator alone: q~[b][k] = w[k] e^{+i Psi_b(f_k)}, k < N/2  (config-4 generator throughput)
-__global__ void __launch_bounds__(256) generate_only_kernel(const float2* __restrict__ w,
+__global__ void __launch_bounds__(256) generate_only_kernel(const c2* __restrict__ w, const double* __restrict__ u,
                                                             const TemplCoef* __restrict__ coef,
-                                                            float2* __restrict__ q, int n_half)
+                                                            c2* __restrict__ q, int n_half)
 {
     const int b = blockIdx.y;
     const TemplCoef* tc = coef + b;
     const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
     const int k_lo = tc->k_lo, k_hi = tc->k_hi;
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_half; k += gridDim.x * blockDim.x) {
-        float2 o = make_float2(0.f, 0.f);
-        if (k >= k_lo && k <= k_hi) o = cmul(__ldg(w + k), spa_phasor(k, A1, A2, A3, A5));
+        c2 o = czero();
+        if (k >= k_lo && k <= k_hi) o = cmul(__ldg(w + k), spa_phasor_u(__ldg(u + k), A1, A2, A3, A5));
         q[(size_t)b * n_half + k] = o;
     }
 }
