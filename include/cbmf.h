@@ -124,6 +124,11 @@ int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_
  * (n/2 complex floats, interleaved). */
 int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);
 int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
+/* Scheduler statistics of the last fused launch (cbmf_set_fused): per block six 64-bit values,
+ * SM cycles spent choosing work, in pass-1 steps, in pass-2 items, the numbers of pass-1 steps
+ * and pass-2 items, and the block's total cycles.  out: host, 6 * max_blocks values;
+ * *n_blocks = blocks written.  ESTATE before the first fused launch. */
+int cbmf_debug_fused_stats(cbmf_ctx *ctx, uint64_t *out, int64_t max_blocks, int64_t *n_blocks);
 
 /* ---- tuning ---- */
 /* Templates per launch pair (pass 1 + pass 2).  The default keeps the inter-pass buffer
@@ -138,13 +143,23 @@ int cbmf_get_sub_batch(const cbmf_ctx *ctx);
  * 1 <= launch_pairs_in_flight <= 8. */
 int cbmf_set_streams(cbmf_ctx *ctx, int launch_pairs_in_flight);
 int cbmf_get_streams(const cbmf_ctx *ctx);
+/* Fused persistent path (csrc/fused.cuh): the whole bank in ONE cooperative launch with one
+ * block per SM; pass-1 and pass-2 work is scheduled inside the kernel and the inter-pass buffer
+ * is a ring of ring_templates * 8 n bytes that stays in the L2.  Available for n = 2^20 on a
+ * device with at least n2/8 = 128 SMs and cooperative launch.  Off by default (the launch
+ * pairs above are faster at present); results do not depend on the choice.  ring_templates: even, 2..64, or 0 to keep the current value
+ * (default 6).  EINVAL if on = 1 where the fused path is not available.
+ * cbmf_get_fused returns 1 / 0 (in use or not) and stores the ring size. */
+int cbmf_set_fused(cbmf_ctx *ctx, int on, int ring_templates);
+int cbmf_get_fused(const cbmf_ctx *ctx, int *ring_templates);
 
 /* ---- introspection ---- */
 /* Kernels launched by this context since creation (bench.py's gpu_launches). */
 int64_t cbmf_launch_count(const cbmf_ctx *ctx);
 /* Device time (ms, CUDA events on the context's stream) and launch count of the two FFT-pass
  * kernels inside the last cbmf_filter_bank* call; used for the roofline line of bench.py.
- * which = 0: pass 1 (generate + column FFT), 1: pass 2 (row FFT + epilogue). */
+ * which = 0: pass 1 (generate + column FFT), 1: pass 2 (row FFT + epilogue).  On the fused
+ * path which = 0 is the one bank_kernel launch (both passes) and which = 1 reports nothing. */
 int cbmf_last_pass_time(const cbmf_ctx *ctx, int which, double *ms_out, int64_t *launches_out);
 /* Enable (1) / disable (0) the per-pass event timing above (default off: no events recorded). */
 int cbmf_set_profiling(cbmf_ctx *ctx, int on);

@@ -13,6 +13,8 @@ import ctypes as C
 
 import numpy as np
 
+i64_t = C.c_int64
+
 from . import build as _build
 
 OK, EINVAL, ESTATE, ECUDA, ENOMEM, WTRUNC = 0, -1, -2, -3, -4, 1
@@ -52,10 +54,13 @@ def lib() -> C.CDLL:
         "cbmf_debug_generate_dev": (C.c_int, [vp, vp, i64, vp]),
         "cbmf_debug_get_prefix": (C.c_int, [vp, vp]),
         "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
+        "cbmf_debug_fused_stats": (C.c_int, [vp, vp, i64, C.POINTER(i64)]),
         "cbmf_set_sub_batch": (C.c_int, [vp, C.c_int]),
         "cbmf_get_sub_batch": (C.c_int, [vp]),
         "cbmf_set_streams": (C.c_int, [vp, C.c_int]),
         "cbmf_get_streams": (C.c_int, [vp]),
+        "cbmf_set_fused": (C.c_int, [vp, C.c_int, C.c_int]),
+        "cbmf_get_fused": (C.c_int, [vp, C.POINTER(C.c_int)]),
         "cbmf_launch_count": (i64, [vp]),
         "cbmf_last_pass_time": (C.c_int, [vp, C.c_int, C.POINTER(dbl), C.POINTER(i64)]),
         "cbmf_set_profiling": (C.c_int, [vp, C.c_int]),
@@ -73,7 +78,7 @@ def lib() -> C.CDLL:
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
-           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch cbmf_set_streams cbmf_get_streams "
+           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_debug_fused_stats cbmf_set_sub_batch cbmf_get_sub_batch cbmf_set_streams cbmf_get_streams cbmf_set_fused cbmf_get_fused "
            "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_strerror "
            "cbmf_last_cuda_error cbmf_version").split()
 
@@ -229,6 +234,13 @@ class Context:
         self._check(lib().cbmf_debug_get_weights(self._h, w.ctypes.data), "cbmf_debug_get_weights")
         return w
 
+    def debug_fused_stats(self) -> np.ndarray:
+        """[blocks][6] uint64: cycles choosing / in P1 / in P2, P1 steps, P2 items, total cycles."""
+        out = np.zeros((1024, 6), dtype=np.uint64)
+        nb = i64_t(0)
+        self._check(lib().cbmf_debug_fused_stats(self._h, out.ctypes.data, 1024, C.byref(nb)), "cbmf_debug_fused_stats")
+        return out[: int(nb.value)]
+
     # -- tuning / introspection
     def set_sub_batch(self, k: int):
         self._check(lib().cbmf_set_sub_batch(self._h, int(k)), "cbmf_set_sub_batch")
@@ -241,6 +253,15 @@ class Context:
 
     def get_streams(self) -> int:
         return int(lib().cbmf_get_streams(self._h))
+
+    def set_fused(self, on: bool, ring: int = 0):
+        self._check(lib().cbmf_set_fused(self._h, int(bool(on)), int(ring)), "cbmf_set_fused")
+
+    def get_fused(self):
+        """-> (in use, ring size in templates)"""
+        ring = C.c_int(0)
+        r = int(lib().cbmf_get_fused(self._h, C.byref(ring)))
+        return bool(r > 0), int(ring.value)
 
     def launch_count(self) -> int:
         return int(lib().cbmf_launch_count(self._h))

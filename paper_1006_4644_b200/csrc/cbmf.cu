@@ -6,6 +6,7 @@
 // of kernels.cuh.  There is no CPU fallback and nothing here touches oracle/.
 #include "../../include/cbmf.h"
 #include "kernels.cuh"
+#include "fused.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -50,6 +51,16 @@ struct cbmf_ctx {
     PeakOut* d_peaks = nullptr;   int64_t peaks_cap = 0;
     TrigOut* d_trig = nullptr;    int64_t trig_cap = 0;       // entries (power of two)
     void* d_scratch = nullptr;    size_t scratch_bytes = 0;   // debug paths / load_segment
+
+    // fused persistent launch (fused.cuh): one cooperative launch per filter_bank call
+    bool fused_ok = false;                 // this N and this device can run it
+    bool fused = false;                    // use it
+    int ring = 6;                          // templates of Y in flight (even)
+    int p2_first = 1;                      // scheduling preference (fused.cuh)
+    int n_sm = 0;
+    unsigned int* d_sync = nullptr;  int64_t sync_cap = 0;        // [3 * cap + 2] counters, see launch_fused
+    unsigned long long* d_fkey = nullptr;  int64_t fkey_cap = 0;  // [n_templates] arg-max keys
+    unsigned long long* d_fstats = nullptr;                       // [n_sm][6] scheduler statistics of the last fused launch
 
     int64_t launches = 0;
     bool profiling = false;
@@ -247,6 +258,43 @@ int alloc_pipeline(cbmf_ctx* c, int sb, int ns)
     return CBMF_OK;
 }
 
+// ---------------------------------------------------------------- fused persistent launch
+template <int L1, int L2>
+cudaError_t fused_query(int* blocks_per_sm)
+{
+    using F = FusedCfg<L1, L2>;
+    cudaError_t e = cudaFuncSetAttribute(bank_kernel<L1, L2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, bank_kernel<L1, L2>, F::NT, F::SMEM_BYTES);
+}
+template <int L1, int L2>
+cudaError_t fused_launch(cudaStream_t s, int grid, FusedArgs a)
+{
+    using F = FusedCfg<L1, L2>;
+    void* params[] = {(void*)&a};
+    return cudaLaunchCooperativeKernel((const void*)bank_kernel<L1, L2>, dim3((unsigned)grid), dim3(F::NT), params,
+                                       F::SMEM_BYTES, s);
+}
+// Sizes for which bank_kernel is instantiated: (lg1, lg2) -> tiles, or 0.
+int fused_tiles(int lg1, int lg2)
+{
+    if (lg1 == 10 && lg2 == 10) return FusedCfg<1024, 1024>::NTILES;
+    return 0;
+}
+bool fused_probe(cbmf_ctx* c)
+{
+    int coop = 0;
+    if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device) != cudaSuccess || !coop) { cudaGetLastError(); return false; }
+    if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { cudaGetLastError(); return false; }
+    const int tiles = fused_tiles(c->lg1, c->lg2);
+    if (tiles == 0 || c->n_sm < tiles) return false;
+    int per_sm = 0;
+    cudaError_t e = cudaErrorInvalidValue;
+    if (c->lg1 == 10 && c->lg2 == 10) e = fused_query<1024, 1024>(&per_sm);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return per_sm >= 1;
+}
+
 }  // namespace
 
 // ======================================================================= create / destroy
@@ -258,7 +306,7 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_bsum); cudaFree(c->d_w);
     cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key); cudaFree(c->d_err); cudaFree(c->d_u);
     cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
-    cudaFree(c->d_trig); cudaFree(c->d_scratch);
+    cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_sync); cudaFree(c->d_fkey); cudaFree(c->d_fstats);
     for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
     for (int i = 0; i < CBMF_MAX_STREAMS; ++i) {
         if (c->aux[i]) { cudaStreamSynchronize(c->aux[i]); cudaStreamDestroy(c->aux[i]); }
@@ -296,7 +344,7 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     if (c->k_lo < 1) c->k_lo = 1;
 
     // templates per launch pair: keep the inter-pass buffer Y inside the L2
-    int64_t sb = (int64_t(64) << 20) / (8 * n);
+    int64_t sb = (int64_t(128) << 20) / (8 * n);
     if (sb < 1) sb = 1;
     if (sb > 256) sb = 256;
     if (const char* e = getenv("CBMF_SUB_BATCH")) {
@@ -331,6 +379,14 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     CUF(cudaStreamSynchronize(c->stream));
 #undef CUF
     { const int rc = alloc_pipeline(c, c->sub_batch, c->n_streams); if (rc) return fail(rc); }
+    c->fused_ok = fused_probe(c);
+    c->fused = false;                      // measured slower than the launch pairs so far
+    if (const char* e = getenv("CBMF_FUSED")) c->fused = c->fused_ok && (strtol(e, nullptr, 10) != 0);
+    if (const char* e = getenv("CBMF_P2_FIRST")) c->p2_first = (strtol(e, nullptr, 10) != 0);
+    if (const char* e = getenv("CBMF_RING")) {
+        const long v = strtol(e, nullptr, 10);
+        if (v >= 2 && v <= 64) c->ring = (int)(v & ~1L);
+    }
     *out = c;
     return CBMF_OK;
 }
@@ -356,6 +412,23 @@ extern "C" int cbmf_set_streams(cbmf_ctx* c, int launch_pairs_in_flight)
 }
 
 extern "C" int cbmf_get_streams(const cbmf_ctx* c) { return c ? c->n_streams : CBMF_EINVAL; }
+
+extern "C" int cbmf_set_fused(cbmf_ctx* c, int on, int ring_templates)
+{
+    if (!c) return CBMF_EINVAL;
+    if (ring_templates != 0 && (ring_templates < 2 || ring_templates > 64 || (ring_templates & 1))) return CBMF_EINVAL;
+    if (on && !c->fused_ok) return CBMF_EINVAL;
+    c->fused = (on != 0);
+    if (ring_templates) c->ring = ring_templates;
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_get_fused(const cbmf_ctx* c, int* ring_templates)
+{
+    if (!c) return CBMF_EINVAL;
+    if (ring_templates) *ring_templates = c->ring;
+    return c->fused ? 1 : 0;
+}
 
 extern "C" int cbmf_get_sub_batch(const cbmf_ctx* c) { return c ? c->sub_batch : CBMF_EINVAL; }
 
@@ -507,6 +580,53 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     c->launches += 1;
 
     c->ev_used[0] = c->ev_used[1] = 0;
+    if (c->fused) {
+        // ---- one persistent cooperative launch for the whole bank (fused.cuh)
+        const int ring = c->ring;
+        if ((size_t)ring > (size_t)c->max_sub_batch * c->max_streams) {
+            if ((rc = alloc_pipeline(c, ring, c->max_streams > 0 ? c->max_streams : 1))) return rc;
+        }
+        if (nt > c->sync_cap) {
+            if (c->d_sync) { CU(cudaFree(c->d_sync)); c->d_sync = nullptr; c->sync_cap = 0; }
+            CU(cudaMalloc(&c->d_sync, sizeof(unsigned int) * (3 * (size_t)nt + 2)));
+            c->sync_cap = nt;
+        }
+        if ((rc = grow(c, c->d_fkey, c->fkey_cap, nt))) return rc;
+        CU(cudaMemsetAsync(c->d_sync, 0, sizeof(unsigned int) * (3 * (size_t)nt + 2), c->stream));
+        CU(cudaMemsetAsync(c->d_fkey, 0, sizeof(unsigned long long) * (size_t)nt, c->stream));
+        FusedArgs fa;
+        fa.w = c->d_w; fa.u = c->d_u; fa.coef = c->d_coef; fa.Y = c->d_Y; fa.cand = c->d_cand;
+        fa.best_key = c->d_fkey;
+        fa.p1_done = c->d_sync; fa.done_ctr = c->d_sync + nt; fa.p2_done = c->d_sync + 2 * nt;
+        fa.p2_next = c->d_sync + 3 * nt; fa.abort_flag = (int*)(c->d_sync + 3 * nt + 1);
+        fa.peaks = c->d_peaks; fa.trig = c->d_trig; fa.trig_cursor = c->d_cursor;
+        fa.trig_cap = (unsigned long long)trig_capacity;
+        if (!c->d_fstats) CU(cudaMalloc(&c->d_fstats, sizeof(unsigned long long) * 6 * (size_t)c->n_sm));
+        fa.stats = c->d_fstats;
+        fa.n_templates = (int)nt; fa.ring = ring; fa.p2_first = c->p2_first;
+        if ((rc = ev_begin(c, 0))) return rc;
+        CU((fused_launch<1024, 1024>(c->stream, c->n_sm, fa)));
+        if ((rc = ev_end(c, 0))) return rc;
+        c->launches += 1;
+        struct { int err; int aborted; unsigned long long found; } st = {0, 0, 0};
+        CU(cudaMemcpyAsync(&st.err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(&st.aborted, fa.abort_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(&st.found, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        if ((rc = ev_collect(c))) return rc;
+        if (st.err) return CBMF_EINVAL;
+        if (st.aborted) { snprintf(c->cuda_err, sizeof(c->cuda_err), "bank_kernel: scheduler wait timed out"); return CBMF_ECUDA; }
+        const int64_t found = (int64_t)st.found;
+        const int64_t kept = found < trig_capacity ? found : trig_capacity;
+        if (n_trig_found) *n_trig_found = found;
+        if (kept > 0 && trig_out) {
+            if ((rc = sort_triggers(c, kept))) return rc;
+            CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, out_kind, c->stream));
+        }
+        CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, out_kind, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
+    }
     const int sb = c->sub_batch;
     // Launch pairs go round-robin over ns streams, each with its own slice of Y / cand / done, so
     // that the tail of one kernel overlaps the head of the next pair.  With per-pass event timing on
@@ -737,6 +857,18 @@ extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_de
     CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return err ? CBMF_EINVAL : CBMF_OK;
+}
+
+extern "C" int cbmf_debug_fused_stats(cbmf_ctx* c, uint64_t* out, int64_t max_blocks, int64_t* n_blocks)
+{
+    if (!c || !out || max_blocks < 0) return CBMF_EINVAL;
+    if (!c->d_fstats) return CBMF_ESTATE;
+    DeviceGuard g(c->device);
+    const int64_t nb = c->n_sm < max_blocks ? c->n_sm : max_blocks;
+    CU(cudaMemcpyAsync(out, c->d_fstats, sizeof(uint64_t) * 6 * (size_t)nb, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (n_blocks) *n_blocks = nb;
+    return CBMF_OK;
 }
 
 extern "C" int cbmf_debug_get_prefix(cbmf_ctx* c, double* p_out)

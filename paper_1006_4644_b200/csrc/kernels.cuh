@@ -5,7 +5,10 @@
 //       in registers (S3, S4), N1-point inverse FFT over k1 -> Y[j1][k2]            (S5, first half)
 //   pass 2 (p2_kernel): for ROWS adjacent rows j1, multiply by W_N^{j1 k2}, N2-point inverse FFT
 //       over k2 -> z[j1 + N1 j2] in registers, |z|^2, arg-max, threshold              (S5-S7)
-//   Y (N complex floats per template in flight) is the only materialised intermediate.
+//   Y (N complex floats per template in flight) is the only materialised intermediate.  It is
+//   stored tile-major, Y[k2 / NC][j1][k2 % NC] with NC = the columns of one pass-1 tile, so that a
+//   pass-1 warp (a few adjacent rows j1 of one tile) stores whole contiguous lines; pass 2 gathers a
+//   row from NC-column segments with asynchronous 16-byte copies.
 //
 // Each per-pass FFT is a Stockham autosort FFT whose butterflies (radix 8/16/32) live in
 // registers and whose digit exchanges go through shared memory.
@@ -98,16 +101,29 @@ __device__ __forceinline__ void twtab_fill(c2* __restrict__ tw, const int tid, c
 // after_last_read() is called once, after this thread's last read of the exchange buffer and
 // before the arithmetic of the last step; pass 2 uses it to start the asynchronous copy of the
 // next row into the same buffer (the hook must synchronise the group before it overwrites).
-template <int L, int NZ1, int SS, bool WARP_SYNC, bool ROWTW, typename Hook = NoHook>
+//
+// SYNC: how the T threads of one FFT (or the threads sharing its exchange buffer) synchronise:
+// the whole block, one warp, or a named barrier (bar_id, bar_threads) for a part of the block.
+enum { SYNC_BLOCK = 0, SYNC_WARP = 1, SYNC_NAMED = 2 };
+__device__ __forceinline__ void named_barrier(const int id, const int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+template <int L, int NZ1, int SS, int SYNC, bool ROWTW, typename Hook = NoHook>
 __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm,
                                          const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook(),
-                                         const c2* __restrict__ tw = nullptr)
+                                         const c2* __restrict__ tw = nullptr, const int bar_id = 0,
+                                         const int bar_threads = 0)
 {
     using C = Cfg<L>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, R2 = C::R2, R3 = C::R3;
     constexpr int LG_R1 = ilog2c(R1);
     auto pad = [](int pos) { return pos + (pos >> LG_R1); };
-    auto sync = []() { if constexpr (WARP_SYNC) __syncwarp(); else __syncthreads(); };
+    auto sync = [&]() {
+        if constexpr (SYNC == SYNC_WARP) __syncwarp();
+        else if constexpr (SYNC == SYNC_NAMED) named_barrier(bar_id, bar_threads);
+        else __syncthreads();
+    };
 
     // ---- step 1: radix R1, no twiddles (Ns = 1); out position i*R1 + q
     {
@@ -243,6 +259,55 @@ __global__ void rcbrt_table_kernel(double* __restrict__ u, int n_half)
     u[k] = r;
 }
 
+// Position of Y[j1][k2] in the tile-major inter-pass buffer of one template.
+template <int L1, int NC>
+__device__ __forceinline__ size_t y_index(const int j1, const int k2)
+{
+    return ((size_t)(k2 / NC) * L1 + j1) * NC + (k2 % NC);
+}
+
+// S3 + S4 for the E/2 possibly non-zero inputs of one thread's column FFT:
+// v[u R1 + r] = w[k] e^{+i Psi(f_k)}, k = (t + T u + (L/R1) r) L2 + k2, inside [k_lo, k_hi], else 0.
+// The bins are taken four at a time: a group no lane of the warp needs is skipped (uniform
+// branch), and inside a group the four phase chains (fp64 Horner, range reduction, SFU sine
+// and cosine) are independent and branch-free, so their latencies overlap.
+//   wt: this thread's column of w, row k1 at wt[k1 * WS];  ut: its column of k^{-1/3}, row k1 at
+//   ut[k1 * US] (shared-memory tiles, or the global table with US = L2).
+template <int L, int L2>
+__device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, const int k2,
+                                              const c2* __restrict__ wt, const int WS,
+                                              const double* __restrict__ ut, const int US,
+                                              const int k_lo, const int k_hi, const double A1, const double A2,
+                                              const double A3, const double A5)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, T = C::T, R1 = C::R1, NZ1 = R1 / 2;
+    constexpr int G = (NZ1 < 4) ? NZ1 : 4;
+#pragma unroll
+    for (int u = 0; u < E / R1; ++u) {
+#pragma unroll
+        for (int rg = 0; rg < NZ1; rg += G) {
+            const int k1a = t + T * u + (L / R1) * rg;
+            const int ka = k1a * L2 + k2, kb = ka + (G - 1) * (L / R1) * L2;
+            if (__any_sync(0xFFFFFFFFu, kb >= k_lo && ka <= k_hi)) {
+#pragma unroll
+                for (int j = 0; j < G; ++j) {
+                    const int k1 = k1a + (L / R1) * j;
+                    const int k = k1 * L2 + k2;
+                    const c2 ph = spa_phasor_u(ut[(size_t)k1 * US], A1, A2, A3, A5);
+                    const c2 wv = (k >= k_lo && k <= k_hi) ? wt[k1 * WS] : czero();
+                    v[u * R1 + rg + j] = cmul(ph, wv);
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < G; ++j) v[u * R1 + rg + j] = czero();
+            }
+        }
+#pragma unroll
+        for (int r = NZ1; r < R1; ++r) v[u * R1 + r] = czero();
+    }
+}
+
 // ------------------------------------------------------------------ pass 1
 enum { LOAD_GEN = 0, LOAD_CPLX = 1, LOAD_REAL = 2 };
 
@@ -303,33 +368,28 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
     if constexpr (TWTAB) twtab_fill<L1>(tw, threadIdx.x, NT);
     if constexpr (MODE != LOAD_GEN) __syncthreads();
 
-    bool first = true;
-    for (int b = blockIdx.y; b < a.batch; b += gridDim.y) {
+    // per-template constants travel through a two-entry shared buffer, fetched one template ahead
+    __shared__ __align__(16) TemplCoef s_coef[2];
+    if constexpr (MODE == LOAD_GEN) {
+        if (threadIdx.x < 4 && (int)blockIdx.y < a.batch)
+            cp_async16(reinterpret_cast<char*>(&s_coef[0]) + 16 * threadIdx.x,
+                       reinterpret_cast<const char*>(a.coef + blockIdx.y) + 16 * threadIdx.x);
+        cp_async_commit();
+        cp_async_wait_all();
+        __syncthreads();
+    }
+
+    int cur = 0;
+    for (int b = blockIdx.y; b < a.batch; b += gridDim.y, cur ^= 1) {
         c2 v[E];
         if constexpr (MODE == LOAD_GEN) {
-            const TemplCoef* tc = a.coef + b;
-            const int k_lo = tc->k_lo, k_hi = tc->k_hi;
-            const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
-            // the phasors of the in-band bins first (they do not need w) ...
-#pragma unroll
-            for (int u = 0; u < E / R1; ++u)
-#pragma unroll
-                for (int r = 0; r < NZ1; ++r) {
-                    const int k = (t + T * u + (L1 / R1) * r) * L2 + k2;
-                    c2 val = czero();
-                    if (k >= k_lo && k <= k_hi) val = spa_phasor_u(__ldg(a.u + k), A1, A2, A3, A5);
-                    v[u * R1 + r] = val;
-                }
-            if (first) { cp_async_wait_all(); __syncthreads(); first = false; }
-            // ... then q~ = w e^{+i Psi}; outside the band the phasor is 0
-#pragma unroll
-            for (int u = 0; u < E / R1; ++u) {
-#pragma unroll
-                for (int r = 0; r < NZ1; ++r)
-                    v[u * R1 + r] = cmul(wt[(t + T * u + (L1 / R1) * r) * NC + c], v[u * R1 + r]);
-#pragma unroll
-                for (int r = NZ1; r < R1; ++r) v[u * R1 + r] = czero();
-            }
+            const int bn = b + gridDim.y;
+            if (threadIdx.x < 4 && bn < a.batch)
+                cp_async16(reinterpret_cast<char*>(&s_coef[cur ^ 1]) + 16 * threadIdx.x,
+                           reinterpret_cast<const char*>(a.coef + bn) + 16 * threadIdx.x);
+            cp_async_commit();
+            const TemplCoef* tc = &s_coef[cur];
+            spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
         } else {
 #pragma unroll
             for (int u = 0; u < E / R1; ++u) {
@@ -347,15 +407,16 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
             }
         }
 
-        fft_core<L1, NZ1, NC, false, false>(v, t, smem + c, 0, 1, NoHook(), TWTAB ? tw : nullptr);
+        fft_core<L1, NZ1, NC, SYNC_BLOCK, false>(v, t, smem + c, 0, 1, NoHook(), TWTAB ? tw : nullptr);
 
-        c2* __restrict__ yb = a.Y + (size_t)b * n_total + (size_t)t * L2 + k2;
+        c2* __restrict__ yb = a.Y + (size_t)b * n_total + y_index<L1, NC>(t, k2);
 #pragma unroll
         for (int u = 0; u < E / RL; ++u) {
 #pragma unroll
             for (int q = 0; q < RL; ++q)
-                yb[(size_t)(T * u + (L1 / RL) * q) * L2] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
+                yb[(size_t)(T * u + (L1 / RL) * q) * NC] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
         }
+        if constexpr (MODE == LOAD_GEN) cp_async_wait_all();   // the next template's constants have landed
         __syncthreads();      // last exchange reads done before the next template's step-1 writes
     }
 }
@@ -394,31 +455,35 @@ template <int L1, int L2>
 __host__ __device__ constexpr int p2_rpw()
 {
     constexpr int per8 = L1 / Cfg<L2>::ROWS / 8;
-    return per8 >= 4 ? 4 : (per8 >= 1 ? per8 : 1);
+    return per8 >= 8 ? 8 : (per8 >= 1 ? per8 : 1);
 }
 template <int L2> __host__ __device__ constexpr int p2_row_stride()
 {
     return Cfg<L2>::PADDED + (Cfg<L2>::T <= 32 ? Cfg<L2>::R1 : 0);      // exchange buffer + G table
 }
 
-// Start the asynchronous copy of one row of Y (L2 complex floats, contiguous) into the row
-// group's shared-memory buffer (unpadded, element k2 at sm[k2]); T threads take part.
-template <int L2>
-__device__ __forceinline__ void p2_prefetch_row(c2* __restrict__ sm, const c2* __restrict__ yrow, const int t)
+// Start the asynchronous copy of row j1 of one template's Y (tile-major: segments of NC columns)
+// into the row group's shared-memory buffer (unpadded, element k2 at sm[k2]); T threads take part.
+template <int L1, int L2>
+__device__ __forceinline__ void p2_prefetch_row(c2* __restrict__ sm, const c2* __restrict__ yb, const int j1, const int t)
 {
-    constexpr int T = Cfg<L2>::T, E = Cfg<L2>::E;
+    constexpr int T = Cfg<L2>::T, E = Cfg<L2>::E, NC = Cfg<L1>::C;
+    static_assert(NC % 2 == 0, "16-byte chunks must not straddle tiles");
 #pragma unroll
-    for (int i = 0; i < E / 2; ++i) cp_async16(sm + 2 * (t + T * i), yrow + 2 * (t + T * i));
+    for (int i = 0; i < E / 2; ++i) {
+        const int k2 = 2 * (t + T * i);
+        cp_async16(sm + k2, yb + y_index<L1, NC>(j1, k2));
+    }
     cp_async_commit();
 }
 
 // Row j1 of template slot b: twiddle, N2 = L2-point inverse FFT over k2 -> z[j1 + L1 j2] in
 // registers, then the epilogue of MODE.  Called by the T threads of one row group.  On entry the
-// copy of the row into sm has been started by p2_prefetch_row; next_row (or nullptr) is the row
-// whose copy is started as soon as the exchange buffer is free again.
+// copy of the row into sm has been started by p2_prefetch_row; next_j1 (or -1) is the row of the
+// same template (yb) whose copy is started as soon as the exchange buffer is free again.
 template <int L1, int L2, int MODE>
 __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int b, const int t,
-                                       c2* __restrict__ sm, const c2* __restrict__ next_row)
+                                       c2* __restrict__ sm, const c2* __restrict__ yb, const int next_j1)
 {
     using C = Cfg<L2>;
     constexpr int E = C::E, T = C::T, R1 = C::R1;
@@ -475,12 +540,12 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
     }
 
     auto start_next = [&]() {
-        if (next_row != nullptr) {          // uniform over the row group
+        if (next_j1 >= 0) {                 // uniform over the row group
             gsync();                        // every thread of the group has read the exchange buffer
-            p2_prefetch_row<L2>(sm, next_row, t);
+            p2_prefetch_row<L1, L2>(sm, yb, next_j1, t);
         }
     };
-    fft_core<L2, R1, 1, WSYNC, true>(v, t, sm, j1, L1, start_next);
+    fft_core<L2, R1, 1, (WSYNC ? SYNC_WARP : SYNC_BLOCK), true>(v, t, sm, j1, L1, start_next);
 
     // v[u*RL + q] = z[j1 + L1 * j2],  j2 = t + T u + (L2/RL) q
     if constexpr (MODE == EPI_STORE) {
@@ -618,12 +683,11 @@ __device__ __forceinline__ void p2_item(const P2Args& a, const int item, const i
     const int t = threadIdx.x % T, row = threadIdx.x / T;
     c2* sm = smem + row * p2_row_stride<L2>();
     const c2* __restrict__ yb = a.Y + (size_t)b * n_total;
-    p2_prefetch_row<L2>(sm, yb + (size_t)((item * RPW) * ROWS + row) * L2, t);
+    p2_prefetch_row<L1, L2>(sm, yb, (item * RPW) * ROWS + row, t);
 #pragma unroll 1
     for (int it = 0; it < RPW; ++it) {
         const int j1 = (item * RPW + it) * ROWS + row;
-        const c2* next_row = (it + 1 < RPW) ? yb + (size_t)(j1 + ROWS) * L2 : nullptr;
-        p2_row<L1, L2, MODE>(a, j1, b, t, sm, next_row);
+        p2_row<L1, L2, MODE>(a, j1, b, t, sm, yb, (it + 1 < RPW) ? j1 + ROWS : -1);
     }
     if constexpr (MODE == EPI_MAX) p2_finish<L1, L2>(a, b, L1 / (ROWS * RPW));
 }

@@ -228,6 +228,32 @@ def test_filter_bank_cfg1_sampled(cbmf):
     assert np.all(tr["snr"] > wl.threshold * (1 - 1e-6))
 
 
+@pytest.mark.parametrize("n_templates,ring", [(1, 2), (37, 2), (64, 6), (129, 4), (96, 16)])
+def test_fused_path_equals_launch_pairs(cbmf, n_templates, ring):
+    """N = 2^20: the persistent fused launch (cbmf_set_fused) gives the same peaks and triggers as the pass-1 / pass-2 launch pairs, for odd bank sizes (one idle
+    half block at the end), banks shorter than the ring, and several ring sizes."""
+    wl = W.config1()
+    bank = np.ascontiguousarray(wl.bank[:n_templates])
+    if n_templates > 1:
+        bank[1] = (80.0, 90.0)                        # empty band inside the bank
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd); g.load_segment(wl.samples)
+    g.set_fused(True, ring)                           # EINVAL here = not available: a B200 has the 128 SMs it needs
+    assert g.get_fused() == (True, ring)
+    l0 = g.launch_count()
+    pk_f, tr_f, nf_f, rc_f = g.filter_bank(bank, wl.threshold)
+    n_launch = g.launch_count() - l0
+    g.set_fused(False)
+    pk_p, tr_p, nf_p, rc_p = g.filter_bank(bank, wl.threshold)
+    g.close()
+    assert n_launch <= 8                              # setup + one bank_kernel + trigger sort
+    assert np.array_equal(pk_f, pk_p)
+    assert nf_f == nf_p and rc_f == rc_p
+    assert np.array_equal(tr_f, tr_p)
+    if n_templates > 1:
+        assert pk_f[1]["idx_peak"] == -1
+
+
 # ------------------------------------------------------------------ edge cases, errors
 
 def test_edge_cases_and_errors(cbmf):
