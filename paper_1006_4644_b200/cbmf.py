@@ -204,11 +204,13 @@ class Context:
         self._check(lib().cbmf_debug_template(self._h, Template(m1, m2), h.ctypes.data), "cbmf_debug_template")
         return h
 
-    def debug_ifft(self, x):
-        """Unnormalised inverse DFT of `batch` vectors [batch, n] complex64 (numpy or CUDA tensor)."""
+    def debug_ifft(self, x, out=None):
+        """Unnormalised inverse DFT of `batch` vectors [batch, n] complex64 (numpy or CUDA tensor;
+        `out`: optional preallocated CUDA tensor of the same shape)."""
         if _is_tensor(x) and x.is_cuda:
             import torch
-            out = torch.empty_like(x)
+            if out is None:
+                out = torch.empty_like(x)
             batch = x.numel() // self.n
             self._check(lib().cbmf_debug_ifft_dev(self._h, x.data_ptr(), out.data_ptr(), self.n, batch),
                         "cbmf_debug_ifft_dev")

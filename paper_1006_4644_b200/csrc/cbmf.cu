@@ -119,7 +119,15 @@ int ilog2(int64_t n) { int l = 0; while ((int64_t(1) << l) < n) ++l; return l; }
 // ---------------------------------------------------------------- launch dispatch over (N1, N2)
 // Templates one pass-1 block works through with its staged w tile (LOAD_GEN): the launch uses
 // ceil(batch / P1_TEMPLATES_PER_BLOCK) blocks per column tile.
-constexpr int P1_TEMPLATES_PER_BLOCK = 4;
+int p1_templates_per_block()
+{
+    static int v = 0;
+    if (v == 0) {
+        v = 4;
+        if (const char* e = getenv("CBMF_P1_TPB")) { const long x = strtol(e, nullptr, 10); if (x >= 1 && x <= 256) v = (int)x; }
+    }
+    return v;
+}
 
 template <int L1, int L2, int MODE>
 cudaError_t launch_p1_L(cudaStream_t s, P1Args a, int batch)
@@ -132,7 +140,8 @@ cudaError_t launch_p1_L(cudaStream_t s, P1Args a, int batch)
         attr_done = true;
     }
     a.batch = batch;
-    const int groups = (MODE == LOAD_GEN) ? (batch + P1_TEMPLATES_PER_BLOCK - 1) / P1_TEMPLATES_PER_BLOCK : batch;
+    const int tpb = p1_templates_per_block();
+    const int groups = (MODE == LOAD_GEN) ? (batch + tpb - 1) / tpb : batch;
     dim3 grid(L2 / Cfg<L1>::C, groups);
     p1_kernel<L1, L2, MODE><<<grid, Cfg<L1>::NT1, smem, s>>>(a);
     return cudaGetLastError();

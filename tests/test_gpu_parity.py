@@ -228,6 +228,58 @@ def test_filter_bank_cfg1_sampled(cbmf):
     assert np.all(tr["snr"] > wl.threshold * (1 - 1e-6))
 
 
+def test_filter_bank_cfg2_sampled(cbmf):
+    """configs[2] at full size (N = 2^20, 65 536 templates U[1,10]^2, one injection at SNR 10): the
+    whole bank on the GPU in one call; every 256th template plus the injection template against
+    the oracle (a double 2^20 transform costs ~0.1 core-second, so the full bank would be hours)."""
+    wl = W.config2()
+    inj = wl.injections[0]
+    idx = sorted(set(range(0, wl.n_templates, 256)) | {inj.template_idx})
+    g, o = _pair(cbmf, wl)
+    pk_g, tr_g, nf_g, rc_g = g.filter_bank(wl.bank, wl.threshold, trig_capacity=1 << 20)
+    assert rc_g == 0 and nf_g == len(tr_g)
+    sel = np.asarray(idx)
+    pk_o, tr_o, _, _ = o.filter_bank(wl.bank[sel], wl.threshold)
+    rho_cache = {}
+
+    def rho_at(t, j):
+        if t not in rho_cache:
+            rho_cache[t] = o.snr_series(*wl.bank[sel[t]])[0]
+        return rho_cache[t][j]
+
+    near = check_peaks(pk_g[sel], pk_o, rho_at)
+    tr_o = tr_o.copy()
+    tr_o["template_idx"] = sel[tr_o["template_idx"]]
+    check_triggers(tr_g[np.isin(tr_g["template_idx"], sel)], tr_o, wl.threshold)
+    g.close(); o.close()
+    p = pk_g[inj.template_idx]
+    assert abs(int(p["idx_peak"]) - inj.sample(wl.fs)) <= 2 and abs(p["snr_max"] - inj.snr) < 3.5
+    assert inj.template_idx not in near and len(near) <= max(2, len(idx) // 50)
+    # whole-bank properties: every template reports a sample of the segment and a sane noise maximum
+    ok = pk_g["idx_peak"] >= 0
+    assert ok.all() and np.all(pk_g["idx_peak"] < wl.n)
+    assert np.all(pk_g["snr_max"] > 3.5) and np.all(pk_g["snr_max"] < 20)
+    assert np.all(pk_g["sigma"] > 0)
+    keys = tr_g["template_idx"].astype(np.int64) * (1 << 32) + tr_g["sample_idx"]
+    assert np.all(np.diff(keys) > 0) and np.all(tr_g["snr"] > wl.threshold * (1 - 1e-6))
+
+
+def test_filter_bank_cfg3_sampled(cbmf):
+    """configs[3] at full size (N = 2^22, f_low = 10 Hz, 4096 templates U[1,5]^2, phases up to
+    1e4 cycles, chirps longer than the segment): the 2 injection templates plus every 128th."""
+    wl = W.config3()
+    idx = sorted(set(range(0, wl.n_templates, 128)) | {i.template_idx for i in wl.injections})
+    pk, tr, near, (ng, no) = _bank_case(cbmf, wl, idx=idx)
+    for inj in wl.injections:
+        p = pk[inj.template_idx]
+        assert abs(int(p["idx_peak"]) - inj.sample(wl.fs)) <= 2
+        assert abs(p["snr_max"] - inj.snr) < 3.5
+        assert inj.template_idx not in near
+    assert len(near) <= 2
+    assert np.all((pk["idx_peak"] >= 0) & (pk["idx_peak"] < wl.n))
+    assert np.all(pk["snr_max"] > 3.5) and np.all(pk["snr_max"] < 20)
+
+
 @pytest.mark.parametrize("n_templates,ring", [(1, 2), (37, 2), (64, 6), (129, 4), (96, 16)])
 def test_fused_path_equals_launch_pairs(cbmf, n_templates, ring):
     """N = 2^20: the persistent fused launch (cbmf_set_fused) gives the same peaks and triggers as the pass-1 / pass-2 launch pairs, for odd bank sizes (one idle
