@@ -67,6 +67,14 @@ __device__ __forceinline__ c2 cmul(c2 a, c2 w)
     unpk(w, wx, wy);
     return fma2(bc(ax), w, mul2(pk(-wy, wx), bc(ay)));
 }
+// a * conj(w) = a.x (w.x, -w.y) + a.y (w.y, w.x)
+__device__ __forceinline__ c2 cmulc(c2 a, c2 w)
+{
+    float ax, ay, wx, wy;
+    unpk(a, ax, ay);
+    unpk(w, wx, wy);
+    return fma2(bc(ay), pk(wy, wx), mul2(pk(wx, -wy), bc(ax)));
+}
 __device__ __forceinline__ c2 csqr(c2 a) { return cmul(a, a); }
 // i * a
 __device__ __forceinline__ c2 mul_i(c2 a) { float x, y; unpk(a, x, y); return pk(-y, x); }
@@ -193,6 +201,45 @@ __device__ __forceinline__ void mul_powers(c2 (&x)[R], c2 g, c2 base)
     }
 #pragma unroll
     for (int lo = (HAS_BASE ? 0 : 1); lo < LO; ++lo) x[lo] = cmul(x[lo], pl[lo]);
+}
+
+// x[r] *= g^(r - R/2) for r = 0..R-1, R = 16 or 32: the twiddles x[r] g^r up to the factor g^(R/2)
+// that is common to all R values.  Where only |DFT(x)|^2 matters (pass 2's arg-max epilogue) that
+// unit-modulus factor can be left out, and the caller restores it for the few samples whose
+// phase is reported.  g^k and its conjugate serve r = R/2 + k and R/2 - k, so R/2 - 1 products
+// build the powers (against R - 2 in mul_powers) and R - 1 apply them.
+template <int R>
+__device__ __forceinline__ void mul_powers_centered(c2 (&x)[R], const c2 g)
+{
+    static_assert(R == 16 || R == 32, "mul_powers_centered: R = 16 or 32");
+    constexpr int H = R / 2;
+    c2 pl[8];
+    pl[1] = g;
+    pl[2] = csqr(g);
+    pl[3] = cmul(pl[2], g);
+    pl[4] = csqr(pl[2]);
+    pl[5] = cmul(pl[4], g);
+    pl[6] = cmul(pl[4], pl[2]);
+    pl[7] = cmul(pl[4], pl[3]);
+#pragma unroll
+    for (int k = 1; k < 8; ++k) {
+        x[H + k] = cmul(x[H + k], pl[k]);
+        x[H - k] = cmulc(x[H - k], pl[k]);
+    }
+    const c2 g8 = csqr(pl[4]);
+    if constexpr (R == 16) {
+        x[0] = cmulc(x[0], g8);
+    } else {
+        x[H + 8] = cmul(x[H + 8], g8);
+        x[H - 8] = cmulc(x[H - 8], g8);
+#pragma unroll
+        for (int k = 9; k < 16; ++k) {
+            const c2 pk_ = cmul(g8, pl[k - 8]);
+            x[H + k] = cmul(x[H + k], pk_);
+            x[H - k] = cmulc(x[H - k], pk_);
+        }
+        x[0] = cmulc(x[0], csqr(g8));
+    }
 }
 
 }  // namespace cbmf

@@ -109,7 +109,10 @@ __device__ __forceinline__ void named_barrier(const int id, const int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
-template <int L, int NZ1, int SS, int SYNC, bool ROWTW, typename Hook = NoHook>
+// CENTER (ROWTW, two-step FFTs): the step-2 twiddles are applied as g^(r - R2/2); every output of
+// this thread then lacks the common factor g^(R2/2), with g = e^{2 pi i (k/(R1 R2) + j1/N)} and
+// k = t mod R1 (see mul_powers_centered and fft_center_factor).
+template <int L, int NZ1, int SS, int SYNC, bool ROWTW, typename Hook = NoHook, bool CENTER = false>
 __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm,
                                          const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook(),
                                          const c2* __restrict__ tw = nullptr, const int bar_id = 0,
@@ -163,6 +166,8 @@ __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __
                 const c2 g = expi_frac(k * (n1 * R3) + j1 * R3, two_over_n);
                 if constexpr (R3 > 1) {
                     mul_powers<R2, true>(x, g, expi_frac(j1 * (i >> LG_R1), two_over_n));
+                } else if constexpr (CENTER) {
+                    mul_powers_centered<R2>(x, g);
                 } else {
                     mul_powers<R2, false>(x, g, pk(1.f, 0.f));
                 }
@@ -221,6 +226,19 @@ __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __
             for (int q = 0; q < R3; ++q) v[u * R3 + q] = x[q];
         }
     }
+}
+
+// The factor g^(R2/2) a CENTER transform leaves out of output element e (= u R2 + q) of thread t
+// of row j1 (n1 = N / L).
+template <int L>
+__device__ __forceinline__ c2 fft_center_factor(const int t, const int e, const int j1, const int n1)
+{
+    using C = Cfg<L>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T;
+    const int k = (t + T * (e / R2)) & (R1 - 1);
+    const long long num = ((long long)k * n1 + j1) * (R2 / 2);           // over N = n1 L
+    const int n_total = n1 * L;
+    return expi_frac((int)(num & (long long)(n_total - 1)), 2.0f / (float)n_total);
 }
 
 // ------------------------------------------------------------------ S3: SPA phasor
@@ -545,7 +563,9 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
             p2_prefetch_row<L1, L2>(sm, yb, next_j1, t);
         }
     };
-    fft_core<L2, R1, 1, (WSYNC ? SYNC_WARP : SYNC_BLOCK), true>(v, t, sm, j1, L1, start_next);
+    // in the arg-max pass only |z|^2 is needed for almost every sample: leave the common factor out
+    constexpr bool CENTER = (MODE == EPI_MAX) && (C::R3 == 1) && (C::R2 == 16 || C::R2 == 32);
+    fft_core<L2, R1, 1, (WSYNC ? SYNC_WARP : SYNC_BLOCK), true, decltype(start_next), CENTER>(v, t, sm, j1, L1, start_next);
 
     // v[u*RL + q] = z[j1 + L1 * j2],  j2 = t + T u + (L2/RL) q
     if constexpr (MODE == EPI_STORE) {
@@ -608,6 +628,7 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
 #pragma unroll
                     for (int e = 1; e < E; ++e)
                         if (e == best_e) zb = v[e];
+                    if constexpr (CENTER) zb = cmul(zb, fft_center_factor<L2>(t, best_e, j1, L1));
                     __stcg(a.cand + (size_t)b * (n_total / E) + (size_t)j1 * T + t, zb);
                 }
             }
@@ -627,7 +648,9 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
                             o.template_idx = a.tmpl_base + b;
                             o.sample_idx = (j2 << LG1) + j1;
                             o.snr = sqrtf(pe) * inv_sigma;
-                            o.phase = atan2f(im(v[e]), re(v[e]));
+                            c2 zt = v[e];
+                            if constexpr (CENTER) zt = cmul(zt, fft_center_factor<L2>(t, e, j1, L1));
+                            o.phase = atan2f(im(zt), re(zt));
                             a.trig[slot] = o;
                         }
                     }
