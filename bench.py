@@ -361,7 +361,7 @@ def run_ours(args):
     if world == 1 and not args.no_cpu:
         import oracle
         cores = oracle.num_threads()
-        n_sample = min(B, max(32, 2 * cores))
+        n_sample = min(B, max(64, 16 * cores))         # ~0.1 core-second per template at N = 2^20
         v, secs, cores = oracle_rate(wl, n_sample)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {n_sample} templates of {wl.name}, filter_bank only, {secs:.2f} s wall"}

@@ -64,6 +64,20 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
+// Bulk asynchronous copy shared -> global (TMA, SASS UBLKCP): one thread hands `bytes` contiguous
+// bytes to the copy engine; no registers and no LSU store slots are involved.
+__device__ __forceinline__ void bulk_store(void* gmem_dst, const void* smem_src, const unsigned bytes)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_src);
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gmem_dst), "r"(s), "r"(bytes)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
+}
+// The copy engine has finished READING shared memory for every bulk store of this thread.
+__device__ __forceinline__ void bulk_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
+// Writes to shared memory by this thread become visible to the copy engine (async proxy).
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
 struct NoHook { __device__ __forceinline__ void operator()() const {} };
 
 // Row stride (in c2) of the step-2 twiddle table TW[k][r] = e^{2 pi i k r / (R1 R2)}, k < R1,
@@ -425,18 +439,28 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
             }
         }
 
+        // the copy engine may still be reading the previous template's output tile out of the exchange buffer
+        if (threadIdx.x == 0) bulk_store_wait_read();
+        __syncthreads();
         fft_core<L1, NZ1, NC, SYNC_BLOCK, false>(v, t, smem + c, 0, 1, NoHook(), TWTAB ? tw : nullptr);
 
-        c2* __restrict__ yb = a.Y + (size_t)b * n_total + y_index<L1, NC>(t, k2);
+        // Y[b][tile] (L1 rows of NC columns) is one contiguous block of the tile-major buffer: build it in
+        // the exchange buffer, unpadded, and hand it to the copy engine in one piece.
+        __syncthreads();                              // every step-2 read of the exchange buffer is done
+        c2* __restrict__ ot = smem + (size_t)t * NC + c;
 #pragma unroll
         for (int u = 0; u < E / RL; ++u) {
 #pragma unroll
             for (int q = 0; q < RL; ++q)
-                yb[(size_t)(T * u + (L1 / RL) * q) * NC] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
+                ot[(size_t)(T * u + (L1 / RL) * q) * NC] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
         }
+        fence_async_smem();
         if constexpr (MODE == LOAD_GEN) cp_async_wait_all();   // the next template's constants have landed
-        __syncthreads();      // last exchange reads done before the next template's step-1 writes
+        __syncthreads();
+        if (threadIdx.x == 0)
+            bulk_store(a.Y + (size_t)b * n_total + (size_t)tile * L1 * NC, smem, (unsigned)(sizeof(c2) * L1 * NC));
     }
+    if (threadIdx.x == 0) bulk_store_wait_read();     // shared memory must outlive the last copy
 }
 
 // ------------------------------------------------------------------ pass 2
