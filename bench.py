@@ -44,6 +44,9 @@ UNIT = "templates/s"
 # FP32 ALU peak of one B200 from unit counts and clocks (B200_PROFILING.md table: 148 SMs,
 # clocks.max.sm 1965 MHz; 128 FP32 lanes per SM, FMA = 2 flop): DESIGN.md §6.
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum per template of the two pass kernels at N = 2^20, from the one
+# `ncu --set full` capture summarised in profiles/r1e_ncu_full_p1_p2.md (224.3 MB and 272.1 MB per launch of 32).
+NCU_DRAM_BYTES_PER_TEMPLATE_2P20 = (224.3e6 / 32, 272.1e6 / 32)
 
 
 def _env_int(name, default):
@@ -71,7 +74,7 @@ def make_workload(name: str, world: int, rank: int):
 class ClockSampler:
     """SM clock and throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
 
-    def __init__(self, index: int, period_s: float = 0.05):
+    def __init__(self, index: int, period_s: float = 0.004):
         self.index, self.period = index, period_s
         self.sm, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()
@@ -344,7 +347,9 @@ def run_ours(args):
                                    "p2_kernel (twiddle + row FFT + |z|^2 + arg-max/threshold)")[which],
         "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "peak_source": "148 SM x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md §6)",
-        "traffic": None,
+        "traffic": (NCU_DRAM_BYTES_PER_TEMPLATE_2P20[which] * tmpl_per_launch) if n == (1 << 20) else None,
+        "traffic_source": "ncu --set full, profiles/r1e_ncu_full_p1_p2.md (per template x templates per launch)",
+        "algorithmic_bytes_per_launch": 8.0 * n * tmpl_per_launch,
         "flops_per_launch": flops_launch, "avg_launch_ms": avg_launch_ms, "templates_per_launch": tmpl_per_launch,
         "pass_ms_per_step": [p_ms[0] / K, p_ms[1] / K],
         "whole_path": {
