@@ -140,6 +140,11 @@ cudaError_t launch_p1_L(cudaStream_t s, P1Args a, int batch)
         attr_done = true;
     }
     a.batch = batch;
+    if (MODE == LOAD_GEN) {
+        // series for k^{-1/3} (spa_correlate): valid where (columns of a tile - 1) / (first in-band bin of a row) <= 2e-3
+        const int k1_lo = a.use_series / L2;          // the caller passes k_lo in use_series
+        a.use_series = (k1_lo >= 1 && (double)(Cfg<L1>::C - 1) <= 2e-3 * (double)k1_lo * (double)L2) ? 1 : 0;
+    }
     const int tpb = p1_templates_per_block();
     const int groups = (MODE == LOAD_GEN) ? (batch + tpb - 1) / tpb : batch;
     dim3 grid(L2 / Cfg<L1>::C, groups);
@@ -654,7 +659,7 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
         cudaStream_t st = (ns > 1) ? c->aux[slot] : c->stream;
         c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err;
+        a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
         if ((rc = ev_begin(c, 0))) return rc;
         CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, st, a1, nb));
         if ((rc = ev_end(c, 0))) return rc;
@@ -771,7 +776,7 @@ extern "C" int cbmf_debug_snr_series(cbmf_ctx* c, cbmf_template t, float* snr_ou
     CU(cudaMemcpyAsync(&tc, c->d_coef, sizeof(tc), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     P1Args a1; memset(&a1, 0, sizeof(a1));
-    a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+    a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
     CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, c->stream, a1, 1));
     P2Args a2; memset(&a2, 0, sizeof(a2));
     a2.Y = c->d_Y; a2.z_out = z;

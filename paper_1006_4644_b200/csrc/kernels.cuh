@@ -305,12 +305,21 @@ __device__ __forceinline__ size_t y_index(const int j1, const int k2)
 // and cosine) are independent and branch-free, so their latencies overlap.
 //   wt: this thread's column of w, row k1 at wt[k1 * WS];  ut: its column of k^{-1/3}, row k1 at
 //   ut[k1 * US] (shared-memory tiles, or the global table with US = L2).
-template <int L, int L2>
+//   SERIES: k^{-1/3} is not loaded per bin but expanded about the first column of the tile,
+//   k = kb + c with kb = k1 L2 + (first k2 of the tile):  k^{-1/3} = kb^{-1/3} (1 + d)^{-1/3},
+//   d = c / kb,  (1 + d)^{-1/3} = 1 - d/3 + 2 d^2/9 - 14 d^3/81 + O(d^4).  ub[k1] = kb^{-1/3} (double)
+//   and inv[k1] = 1/kb (float) sit in shared memory, cf = (float)c; the correction is below 1e-3 and
+//   is evaluated in fp32 (absolute error ~1e-11), the caller guarantees d <= 2e-3 on every in-band
+//   row (d^4 term < 3e-12).  This replaces a scattered 8-byte L2 load per bin, whose latency set the
+//   length of the generator phase, by two shared-memory loads shared by the columns of a row.
+template <int L, int L2, bool SERIES = false>
 __device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, const int k2,
                                               const c2* __restrict__ wt, const int WS,
                                               const double* __restrict__ ut, const int US,
                                               const int k_lo, const int k_hi, const double A1, const double A2,
-                                              const double A3, const double A5)
+                                              const double A3, const double A5,
+                                              const double* __restrict__ ub = nullptr,
+                                              const float* __restrict__ inv = nullptr, const float cf = 0.f)
 {
     using C = Cfg<L>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, NZ1 = R1 / 2;
@@ -326,7 +335,16 @@ __device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, c
                 for (int j = 0; j < G; ++j) {
                     const int k1 = k1a + (L / R1) * j;
                     const int k = k1 * L2 + k2;
-                    const c2 ph = spa_phasor_u(ut[(size_t)k1 * US], A1, A2, A3, A5);
+                    double uk;
+                    if constexpr (SERIES) {
+                        const float d = cf * inv[k1];
+                        const float p = d * fmaf(d, fmaf(d, -14.0f / 81.0f, 2.0f / 9.0f), -1.0f / 3.0f);
+                        const double b0 = ub[k1];
+                        uk = fma(b0, (double)p, b0);
+                    } else {
+                        uk = ut[(size_t)k1 * US];
+                    }
+                    const c2 ph = spa_phasor_u(uk, A1, A2, A3, A5);
                     const c2 wv = (k >= k_lo && k <= k_hi) ? wt[k1 * WS] : czero();
                     v[u * R1 + rg + j] = cmul(ph, wv);
                 }
@@ -352,6 +370,7 @@ struct P1Args {
     c2* __restrict__ Y;                    // [batch][N], Y[j1*N2 + k2]
     int* err_flag;                         // set to 1 on a non-finite real input sample
     int batch;                             // templates (or vectors) in this launch
+    int use_series;                        // LOAD_GEN: k^{-1/3} by the series of spa_correlate (host checks its range)
 };
 
 // The step-2 twiddle table is used where the FFT has two steps (L <= 1024).
@@ -365,7 +384,8 @@ __host__ __device__ constexpr size_t p1_smem_bytes()
 {
     using C = Cfg<L1>;
     return sizeof(c2) * ((size_t)C::PADDED * C::C + (p1_use_twtab<L1>() ? (size_t)twtab_elems<L1>() : 0) +
-                         (MODE == LOAD_GEN ? (size_t)(L1 / 2) * C::C : 0));
+                         (MODE == LOAD_GEN ? (size_t)(L1 / 2) * C::C : 0)) +
+           (MODE == LOAD_GEN ? (sizeof(double) + sizeof(float)) * (size_t)(L1 / 2) : 0);      // ub, inv
 }
 
 // One pass-1 block = one tile of NC adjacent columns k2.  For every template slot b of the
@@ -399,6 +419,16 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
     }
     if constexpr (TWTAB) twtab_fill<L1>(tw, threadIdx.x, NT);
     if constexpr (MODE != LOAD_GEN) __syncthreads();
+    // series tables of spa_correlate: kb^{-1/3} and 1/kb for the first column of the tile, every row k1
+    double* __restrict__ ub = reinterpret_cast<double*>(wt + (size_t)(L1 / 2) * NC);
+    float* __restrict__ inv = reinterpret_cast<float*>(ub + L1 / 2);
+    if constexpr (MODE == LOAD_GEN) {
+        for (int k1 = threadIdx.x; k1 < L1 / 2; k1 += NT) {
+            const int kb = k1 * L2 + tile * NC;
+            ub[k1] = __ldg(a.u + kb);
+            inv[k1] = kb > 0 ? (float)(1.0 / (double)kb) : 0.f;
+        }
+    }
 
     // per-template constants travel through a two-entry shared buffer, fetched one template ahead
     __shared__ __align__(16) TemplCoef s_coef[2];
@@ -421,7 +451,11 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
                            reinterpret_cast<const char*>(a.coef + bn) + 16 * threadIdx.x);
             cp_async_commit();
             const TemplCoef* tc = &s_coef[cur];
-            spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
+            if (a.use_series)
+                spa_correlate<L1, L2, true>(v, t, k2, wt + c, NC, nullptr, 0, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3,
+                                            tc->A5, ub, inv, (float)c);
+            else
+                spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
         } else {
 #pragma unroll
             for (int u = 0; u < E / R1; ++u) {

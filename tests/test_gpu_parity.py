@@ -282,7 +282,7 @@ def test_filter_bank_cfg3_sampled(cbmf):
 
 @pytest.mark.parametrize("n_templates,ring", [(1, 2), (37, 2), (64, 6), (129, 4), (96, 16)])
 def test_fused_path_equals_launch_pairs(cbmf, n_templates, ring):
-    """N = 2^20: the persistent fused launch (cbmf_set_fused) gives the same peaks and triggers as the pass-1 / pass-2 launch pairs, for odd bank sizes (one idle
+    """N = 2^20: the persistent fused launch (cbmf_set_fused) gives the same peaks and triggers (to fp32 rounding) as the pass-1 / pass-2 launch pairs, for odd bank sizes (one idle
     half block at the end), banks shorter than the ring, and several ring sizes."""
     wl = W.config1()
     bank = np.ascontiguousarray(wl.bank[:n_templates])
@@ -299,9 +299,19 @@ def test_fused_path_equals_launch_pairs(cbmf, n_templates, ring):
     pk_p, tr_p, nf_p, rc_p = g.filter_bank(bank, wl.threshold)
     g.close()
     assert n_launch <= 8                              # setup + one bank_kernel + trigger sort
-    assert np.array_equal(pk_f, pk_p)
-    assert nf_f == nf_p and rc_f == rc_p
-    assert np.array_equal(tr_f, tr_p)
+    # the two drivers share the FFT code but not the way k^(-1/3) reaches the generator (table tile in
+    # shared memory vs series about the tile's first column): equal to fp32 rounding, not bit for bit
+    assert rc_f == rc_p
+    assert np.array_equal(pk_f["sigma"], pk_p["sigma"])
+    same = pk_f["idx_peak"] == pk_p["idx_peak"]
+    assert same.mean() >= 0.98                        # near-ties of noise maxima may flip (A12)
+    assert np.allclose(pk_f["snr_max"], pk_p["snr_max"], rtol=2e-5, atol=0)
+    assert np.all(np.abs(wrap_pi(pk_f["phase"][same] - pk_p["phase"][same])) < 5e-4)
+    far = lambda tr: {(int(a), int(b)) for a, b, r in zip(tr["template_idx"], tr["sample_idx"], tr["snr"])
+                      if abs(r - wl.threshold) > 1e-4 * wl.threshold}
+    allk = lambda tr: {(int(a), int(b)) for a, b in zip(tr["template_idx"], tr["sample_idx"])}
+    assert far(tr_f) <= allk(tr_p) and far(tr_p) <= allk(tr_f)
+    assert abs(nf_f - nf_p) <= 2
     if n_templates > 1:
         assert pk_f[1]["idx_peak"] == -1
 
