@@ -137,9 +137,9 @@ int cbmf_debug_fused_stats(cbmf_ctx *ctx, uint64_t *out, int64_t max_blocks, int
 int cbmf_set_sub_batch(cbmf_ctx *ctx, int templates_per_launch);
 int cbmf_get_sub_batch(const cbmf_ctx *ctx);
 /* Launch pairs in flight: sub-batches are issued round-robin on this many internal streams
- * (forked from and joined to the context's stream inside every filter call), so that the tail of
- * one kernel overlaps the next pair.  The inter-pass buffer grows to
- * launch_pairs_in_flight * templates_per_launch * 8 n bytes; results do not depend on it.
+ * (forked from and joined to the context's stream inside every filter call), so that pass-1 blocks
+ * of one pair share the SMs with pass-2 blocks of the others.  Default 4.  The inter-pass buffer
+ * grows to launch_pairs_in_flight * templates_per_launch * 8 n bytes; results do not depend on it.
  * 1 <= launch_pairs_in_flight <= 8. */
 int cbmf_set_streams(cbmf_ctx *ctx, int launch_pairs_in_flight);
 int cbmf_get_streams(const cbmf_ctx *ctx);

@@ -117,16 +117,25 @@ int grow_scratch(cbmf_ctx* c, size_t bytes)
 int ilog2(int64_t n) { int l = 0; while ((int64_t(1) << l) < n) ++l; return l; }
 
 // ---------------------------------------------------------------- launch dispatch over (N1, N2)
-// Templates one pass-1 block works through with its staged w tile (LOAD_GEN): the launch uses
-// ceil(batch / P1_TEMPLATES_PER_BLOCK) blocks per column tile.
-int p1_templates_per_block()
+// Blocks per column tile of a pass-1 launch (LOAD_GEN).  Each block stages its tile of w once and walks
+// through its share of the templates, so FEW, LONG-LIVED blocks are wanted: about one per SM in total.  They
+// then occupy one of the two block slots of an SM for the whole launch and the pass-2 blocks of the other
+// streams take the second slot, which pairs the generator / exchange phases of pass 1 with the FMA-bound
+// row FFTs of pass 2 on every SM (+12 % over short-lived blocks at 4 streams).
+int p1_groups(int n_tiles, int batch)
 {
-    static int v = 0;
-    if (v == 0) {
-        v = 4;
-        if (const char* e = getenv("CBMF_P1_TPB")) { const long x = strtol(e, nullptr, 10); if (x >= 1 && x <= 256) v = (int)x; }
+    static int n_sm = 0;
+    if (n_sm == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) {
+            cudaGetLastError();
+            n_sm = 148;
+        }
     }
-    return v;
+    int g = n_sm / n_tiles;
+    if (g < 1) g = 1;
+    if (g > batch) g = batch;
+    return g;
 }
 
 template <int L1, int L2, int MODE>
@@ -145,8 +154,7 @@ cudaError_t launch_p1_L(cudaStream_t s, P1Args a, int batch)
         const int k1_lo = a.use_series / L2;          // the caller passes k_lo in use_series
         a.use_series = (k1_lo >= 1 && (double)(Cfg<L1>::C - 1) <= 2e-3 * (double)k1_lo * (double)L2) ? 1 : 0;
     }
-    const int tpb = p1_templates_per_block();
-    const int groups = (MODE == LOAD_GEN) ? (batch + tpb - 1) / tpb : batch;
+    const int groups = (MODE == LOAD_GEN) ? p1_groups(L2 / Cfg<L1>::C, batch) : batch;
     dim3 grid(L2 / Cfg<L1>::C, groups);
     p1_kernel<L1, L2, MODE><<<grid, Cfg<L1>::NT1, smem, s>>>(a);
     return cudaGetLastError();
@@ -366,7 +374,7 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
         const long v = strtol(e, nullptr, 10);
         if (v >= 1 && v <= 4096) sb = v;
     }
-    int ns = 2;
+    int ns = 4;
     if (const char* e = getenv("CBMF_STREAMS")) {
         const long v = strtol(e, nullptr, 10);
         if (v >= 1 && v <= CBMF_MAX_STREAMS) ns = (int)v;
