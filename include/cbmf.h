@@ -124,10 +124,10 @@ int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_
  * (n/2 complex floats, interleaved). */
 int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);
 int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
-/* Scheduler statistics of the last fused launch (cbmf_set_fused): per block six 64-bit values,
- * SM cycles spent choosing work, in pass-1 steps, in pass-2 items, the numbers of pass-1 steps
- * and pass-2 items, and the block's total cycles.  out: host, 6 * max_blocks values;
- * *n_blocks = blocks written.  ESTATE before the first fused launch. */
+/* Block statistics of the last fused launch (cbmf_set_fused): per block six 64-bit values, role
+ * (1 = pass 1, 2 = pass 2), SM cycles spent waiting (ring slot / template not ready), cycles
+ * working, steps done (templates / items), total cycles, column tile (-1 for pass 2).  out: host,
+ * 6 * max_blocks values; *n_blocks = blocks written.  ESTATE before the first fused launch. */
 int cbmf_debug_fused_stats(cbmf_ctx *ctx, uint64_t *out, int64_t max_blocks, int64_t *n_blocks);
 
 /* ---- tuning ---- */
@@ -143,12 +143,13 @@ int cbmf_get_sub_batch(const cbmf_ctx *ctx);
  * 1 <= launch_pairs_in_flight <= 8. */
 int cbmf_set_streams(cbmf_ctx *ctx, int launch_pairs_in_flight);
 int cbmf_get_streams(const cbmf_ctx *ctx);
-/* Fused persistent path (csrc/fused.cuh): the whole bank in ONE cooperative launch with one
- * block per SM; pass-1 and pass-2 work is scheduled inside the kernel and the inter-pass buffer
- * is a ring of ring_templates * 8 n bytes that stays in the L2.  Available for n = 2^20 on a
- * device with at least n2/8 = 128 SMs and cooperative launch.  Off by default (the launch
- * pairs above are faster at present); results do not depend on the choice.  ring_templates: even, 2..64, or 0 to keep the current value
- * (default 6).  EINVAL if on = 1 where the fused path is not available.
+/* Fused persistent path (csrc/fused.cuh): the whole bank in ONE cooperative launch with two
+ * blocks per SM, each with one role for the whole bank -- one pass-1 block per column tile (w
+ * staged once) and pass-2 blocks that claim rows from a queue; the inter-pass buffer is a ring of
+ * ring_templates * 8 n bytes.  Available for n = 2^20 on a device with at least n2/8 = 128 SMs
+ * and cooperative launch.  Off by default (the launch pairs above are faster at present,
+ * DESIGN.md §7); results agree with them to fp32 rounding.  ring_templates: 2..64, or 0 to keep
+ * the current value (default 32).  EINVAL if on = 1 where the fused path is not available.
  * cbmf_get_fused returns 1 / 0 (in use or not) and stores the ring size. */
 int cbmf_set_fused(cbmf_ctx *ctx, int on, int ring_templates);
 int cbmf_get_fused(const cbmf_ctx *ctx, int *ring_templates);

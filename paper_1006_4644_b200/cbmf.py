@@ -237,7 +237,7 @@ class Context:
         return w
 
     def debug_fused_stats(self) -> np.ndarray:
-        """[blocks][6] uint64: cycles choosing / in P1 / in P2, P1 steps, P2 items, total cycles."""
+        """[blocks][6] uint64: role (1 / 2), cycles waiting, cycles working, steps, total cycles, tile."""
         out = np.zeros((1024, 6), dtype=np.uint64)
         nb = i64_t(0)
         self._check(lib().cbmf_debug_fused_stats(self._h, out.ctypes.data, 1024, C.byref(nb)), "cbmf_debug_fused_stats")

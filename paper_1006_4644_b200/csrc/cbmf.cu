@@ -55,10 +55,9 @@ struct cbmf_ctx {
     // fused persistent launch (fused.cuh): one cooperative launch per filter_bank call
     bool fused_ok = false;                 // this N and this device can run it
     bool fused = false;                    // use it
-    int ring = 6;                          // templates of Y in flight (even)
-    int p2_first = 1;                      // scheduling preference (fused.cuh)
+    int ring = 32;                         // templates of Y in flight
     int n_sm = 0;
-    unsigned int* d_sync = nullptr;  int64_t sync_cap = 0;        // [3 * cap + 2] counters, see launch_fused
+    unsigned int* d_sync = nullptr;  int64_t sync_cap = 0;        // [3 * cap + 3 + n_sm] counters, see filter_bank_impl
     unsigned long long* d_fkey = nullptr;  int64_t fkey_cap = 0;  // [n_templates] arg-max keys
     unsigned long long* d_fstats = nullptr;                       // [n_sm][6] scheduler statistics of the last fused launch
 
@@ -122,6 +121,14 @@ int ilog2(int64_t n) { int l = 0; while ((int64_t(1) << l) < n) ++l; return l; }
 // then occupy one of the two block slots of an SM for the whole launch and the pass-2 blocks of the other
 // streams take the second slot, which pairs the generator / exchange phases of pass 1 with the FMA-bound
 // row FFTs of pass 2 on every SM (+12 % over short-lived blocks at 4 streams).
+// Series for k^{-1/3} in the generator (spa_correlate): valid where (columns of a tile - 1) / (first bin
+// of the first in-band row) <= 2e-3.
+bool p1_series_ok(int k_lo, int l2, int tile_cols)
+{
+    const int k1_lo = k_lo / l2;
+    return k1_lo >= 1 && (double)(tile_cols - 1) <= 2e-3 * (double)k1_lo * (double)l2;
+}
+
 int p1_groups(int n_tiles, int batch)
 {
     static int n_sm = 0;
@@ -151,8 +158,7 @@ cudaError_t launch_p1_L(cudaStream_t s, P1Args a, int batch)
     a.batch = batch;
     if (MODE == LOAD_GEN) {
         // series for k^{-1/3} (spa_correlate): valid where (columns of a tile - 1) / (first in-band bin of a row) <= 2e-3
-        const int k1_lo = a.use_series / L2;          // the caller passes k_lo in use_series
-        a.use_series = (k1_lo >= 1 && (double)(Cfg<L1>::C - 1) <= 2e-3 * (double)k1_lo * (double)L2) ? 1 : 0;
+        a.use_series = p1_series_ok(a.use_series, L2, Cfg<L1>::C) ? 1 : 0;    // the caller passes k_lo in use_series
     }
     const int groups = (MODE == LOAD_GEN) ? p1_groups(L2 / Cfg<L1>::C, batch) : batch;
     dim3 grid(L2 / Cfg<L1>::C, groups);
@@ -309,12 +315,12 @@ bool fused_probe(cbmf_ctx* c)
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device) != cudaSuccess || !coop) { cudaGetLastError(); return false; }
     if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { cudaGetLastError(); return false; }
     const int tiles = fused_tiles(c->lg1, c->lg2);
-    if (tiles == 0 || c->n_sm < tiles) return false;
+    if (tiles == 0 || c->n_sm < tiles) return false;     // one P1 block per SM, one SM per tile
     int per_sm = 0;
     cudaError_t e = cudaErrorInvalidValue;
     if (c->lg1 == 10 && c->lg2 == 10) e = fused_query<1024, 1024>(&per_sm);
     if (e != cudaSuccess) { cudaGetLastError(); return false; }
-    return per_sm >= 1;
+    return per_sm >= 2;                                   // a P1 and a P2 block on every SM
 }
 
 }  // namespace
@@ -405,10 +411,9 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     c->fused_ok = fused_probe(c);
     c->fused = false;                      // measured slower than the launch pairs so far
     if (const char* e = getenv("CBMF_FUSED")) c->fused = c->fused_ok && (strtol(e, nullptr, 10) != 0);
-    if (const char* e = getenv("CBMF_P2_FIRST")) c->p2_first = (strtol(e, nullptr, 10) != 0);
     if (const char* e = getenv("CBMF_RING")) {
         const long v = strtol(e, nullptr, 10);
-        if (v >= 2 && v <= 64) c->ring = (int)(v & ~1L);
+        if (v >= 2 && v <= 64) c->ring = (int)v;
     }
     *out = c;
     return CBMF_OK;
@@ -439,7 +444,7 @@ extern "C" int cbmf_get_streams(const cbmf_ctx* c) { return c ? c->n_streams : C
 extern "C" int cbmf_set_fused(cbmf_ctx* c, int on, int ring_templates)
 {
     if (!c) return CBMF_EINVAL;
-    if (ring_templates != 0 && (ring_templates < 2 || ring_templates > 64 || (ring_templates & 1))) return CBMF_EINVAL;
+    if (ring_templates != 0 && (ring_templates < 2 || ring_templates > 64)) return CBMF_EINVAL;
     if (on && !c->fused_ok) return CBMF_EINVAL;
     c->fused = (on != 0);
     if (ring_templates) c->ring = ring_templates;
@@ -609,26 +614,30 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
         if ((size_t)ring > (size_t)c->max_sub_batch * c->max_streams) {
             if ((rc = alloc_pipeline(c, ring, c->max_streams > 0 ? c->max_streams : 1))) return rc;
         }
+        const size_t n_sync = 3 * (size_t)nt + 3 + (size_t)c->n_sm;
         if (nt > c->sync_cap) {
             if (c->d_sync) { CU(cudaFree(c->d_sync)); c->d_sync = nullptr; c->sync_cap = 0; }
-            CU(cudaMalloc(&c->d_sync, sizeof(unsigned int) * (3 * (size_t)nt + 2)));
+            CU(cudaMalloc(&c->d_sync, sizeof(unsigned int) * n_sync));
             c->sync_cap = nt;
         }
         if ((rc = grow(c, c->d_fkey, c->fkey_cap, nt))) return rc;
-        CU(cudaMemsetAsync(c->d_sync, 0, sizeof(unsigned int) * (3 * (size_t)nt + 2), c->stream));
+        CU(cudaMemsetAsync(c->d_sync, 0, sizeof(unsigned int) * n_sync, c->stream));
         CU(cudaMemsetAsync(c->d_fkey, 0, sizeof(unsigned long long) * (size_t)nt, c->stream));
+        const int grid = 2 * c->n_sm;
         FusedArgs fa;
         fa.w = c->d_w; fa.u = c->d_u; fa.coef = c->d_coef; fa.Y = c->d_Y; fa.cand = c->d_cand;
         fa.best_key = c->d_fkey;
         fa.p1_done = c->d_sync; fa.done_ctr = c->d_sync + nt; fa.p2_done = c->d_sync + 2 * nt;
-        fa.p2_next = c->d_sync + 3 * nt; fa.abort_flag = (int*)(c->d_sync + 3 * nt + 1);
+        fa.p2_next = c->d_sync + 3 * nt; fa.tile_next = c->d_sync + 3 * nt + 1;
+        fa.abort_flag = (int*)(c->d_sync + 3 * nt + 2); fa.sm_slot = c->d_sync + 3 * nt + 3;
         fa.peaks = c->d_peaks; fa.trig = c->d_trig; fa.trig_cursor = c->d_cursor;
         fa.trig_cap = (unsigned long long)trig_capacity;
-        if (!c->d_fstats) CU(cudaMalloc(&c->d_fstats, sizeof(unsigned long long) * 6 * (size_t)c->n_sm));
+        if (!c->d_fstats) CU(cudaMalloc(&c->d_fstats, sizeof(unsigned long long) * 6 * (size_t)grid));
         fa.stats = c->d_fstats;
-        fa.n_templates = (int)nt; fa.ring = ring; fa.p2_first = c->p2_first;
+        fa.n_templates = (int)nt; fa.ring = ring;
+        fa.use_series = p1_series_ok(c->k_lo, 1 << c->lg2, FusedCfg<1024, 1024>::NC) ? 1 : 0;
         if ((rc = ev_begin(c, 0))) return rc;
-        CU((fused_launch<1024, 1024>(c->stream, c->n_sm, fa)));
+        CU((fused_launch<1024, 1024>(c->stream, grid, fa)));
         if ((rc = ev_end(c, 0))) return rc;
         c->launches += 1;
         struct { int err; int aborted; unsigned long long found; } st = {0, 0, 0};
@@ -887,7 +896,7 @@ extern "C" int cbmf_debug_fused_stats(cbmf_ctx* c, uint64_t* out, int64_t max_bl
     if (!c || !out || max_blocks < 0) return CBMF_EINVAL;
     if (!c->d_fstats) return CBMF_ESTATE;
     DeviceGuard g(c->device);
-    const int64_t nb = c->n_sm < max_blocks ? c->n_sm : max_blocks;
+    const int64_t nb = 2 * c->n_sm < max_blocks ? 2 * c->n_sm : max_blocks;
     CU(cudaMemcpyAsync(out, c->d_fstats, sizeof(uint64_t) * 6 * (size_t)nb, cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (n_blocks) *n_blocks = nb;

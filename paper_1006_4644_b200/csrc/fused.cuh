@@ -1,31 +1,33 @@
 // fused.cuh -- the whole bank in ONE persistent launch.
 //
-// bank_kernel<L1, L2> runs one block of 512 threads per SM (cooperative launch: every block is
-// resident) and walks the bank with two kinds of work, scheduled inside the kernel:
+// bank_kernel<L1, L2> runs two blocks of 256 threads on every SM (cooperative launch: every block
+// is resident for the whole bank) and gives each block ONE role for its lifetime:
 //
-//   P1 (tile, template)   SPA generation + correlate + N1-point column FFTs of NC adjacent
-//                         columns k2 -> Y[slot][j1][k2].  Tile `i` belongs to block `i`, which
-//                         stages w[k] and k^{-1/3} of its columns in shared memory ONCE per
-//                         launch and then takes the templates in order, two at a time (one per
-//                         half of the block, each half with its own exchange buffer and named
-//                         barrier).
-//   P2 (template, rows)   twiddle + N2-point row FFTs + |z|^2 + arg-max / threshold of 64
-//                         adjacent rows j1 (16 warps x 4 rows), claimed from a global queue by
-//                         any block, as soon as all tiles of that template have been written.
+//   P1 block (one per column tile, the first block to arrive on an SM takes a tile):
+//       stages w[k] of its NC columns and the generator / twiddle tables in shared memory ONCE,
+//       then for template b = 0, 1, ...: SPA generation + correlate + N1-point column FFTs ->
+//       output tile in shared memory -> one TMA bulk store into Y[b mod ring] (the body of
+//       p1_kernel), and publishes p1_done[b] once that store has completed.
+//   P2 block (every other block): claims (template, 64 rows) items from a global queue in order,
+//       waits until all tiles of the template have been written, and runs twiddle + N2-point row
+//       FFTs + |z|^2 + arg-max / threshold on them (the body of p2_kernel); the last item of a
+//       template emits its peak record; every item then frees its share of the ring slot.
 //
-// Y is a ring of `ring` templates (8 N bytes each) so that the inter-pass buffer stays in the
-// L2 cache: P1 may write template b only when P2 has finished template b - ring.
+// So every SM that owns a tile runs one P1 block (generator: FP64 / SFU / shared memory; butterflies:
+// FMA pipe) next to one P2 block (FMA-bound), which is the pairing the launch-pair path only gets
+// by chance.  Y is a ring of `ring` templates: P1 may write template b only when P2 has finished
+// template b - ring.
 //
-// Progress: a block never waits while holding work -- it takes a P1 step only when the ring slot
-// is free and claims a P2 item only when its template is complete -- so the earliest unfinished
-// template can always advance.  Every wait is bounded; on a timeout the abort flag stops all blocks
-// and the host reports CBMF_ECUDA instead of hanging.
+// Progress: P1 blocks wait only for ring slots (freed by P2 items of earlier templates), P2 blocks
+// only for P1 of the template they hold (earlier than anything P1 is waiting for): a bounded
+// buffer, no cycle.  Every wait is bounded; on a timeout the abort flag stops all blocks and the
+// host reports CBMF_ECUDA instead of hanging.
 //
-// Ordering (release / acquire at gpu scope): a half block finishes its stores of Y, meets at its
-// barrier, and one thread fences and increments p1_done[b]; the claiming thread reads the counter
-// with ld.acquire and the block barrier hands the ordering to the other threads, which read Y
-// with cp.async.cg (L2, never a stale L1 line).  The same pattern in the other direction frees a
-// ring slot (p2_done[b]).
+// Ordering (release / acquire at gpu scope): the P1 thread that issued the bulk store waits for
+// its completion (cp.async.bulk.wait_group), fences and increments p1_done[b]; the claiming P2
+// thread reads the counter with ld.acquire and the block barrier hands the ordering to the other
+// threads, which read Y with cp.async.cg (L2, never a stale L1 line).  The same pattern in the
+// other direction frees a ring slot (p2_done[b]).
 #pragma once
 #include "kernels.cuh"
 
@@ -42,15 +44,17 @@ struct FusedArgs {
     unsigned int* done_ctr;                // [n_templates], zero on entry: P2 items past the epilogue
     unsigned int* p2_done;                 // [n_templates], zero on entry: P2 items that released the slot
     unsigned int* p2_next;                 // [1], zero on entry: next P2 item of the queue
+    unsigned int* tile_next;               // [1], zero on entry: next column tile without a P1 block
+    unsigned int* sm_slot;                 // [n_sm], zero on entry: blocks that have arrived on each SM
     int* abort_flag;                       // [1], zero on entry
     PeakOut* peaks;                        // [n_templates]
     TrigOut* trig;
     unsigned long long* trig_cursor;
     unsigned long long trig_cap;
     int n_templates;
-    int ring;                              // even, >= 2
-    unsigned long long* stats;             // null, or [grid][6]: cycles deciding / in P1 / in P2, steps P1 / P2, total
-    int p2_first;                          // scheduling: 1 = a ready P2 item is preferred to the next P1 step
+    int ring;                              // >= 2
+    int use_series;                        // generator: k^{-1/3} by the series of spa_correlate
+    unsigned long long* stats;             // null, or [grid][6]: role (1 / 2), cycles waiting, cycles working, steps, total, tile
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
@@ -65,66 +69,155 @@ __device__ __forceinline__ int ld_volatile_s32(const int* p)
     asm volatile("ld.volatile.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ unsigned smid()
+{
+    unsigned v;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(v));
+    return v;
+}
+// At most `n` of this thread's bulk stores are still in flight (their global writes not yet complete).
+template <int N_PENDING>
+__device__ __forceinline__ void bulk_store_wait_done()
+{
+    asm volatile("cp.async.bulk.wait_group %0;\n" ::"n"(N_PENDING) : "memory");
+}
+
+// Release increment of a counter without a return value: earlier writes this thread has observed
+// (here: the completed bulk stores) are visible to whoever acquires the new value.
+__device__ __forceinline__ void red_release_add(unsigned* p, const unsigned v)
+{
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
 template <int L1, int L2>
 struct FusedCfg {
     using C1 = Cfg<L1>;
     using C2 = Cfg<L2>;
-    static constexpr int NT = 512;
-    static constexpr int HALF = 256;                                   // threads of one P1 half
-    static constexpr int NC = HALF / C1::T;                            // columns per tile
+    static constexpr int NT = 256;
+    static constexpr int NC = C1::C;                                   // columns per tile
     static constexpr int NTILES = L2 / NC;
-    static constexpr int ROWS = NT / C2::T;                            // rows in flight in P2
-    static constexpr int RPW = 4;                                      // rows per row group and item
+    static constexpr int ROWS = NT / C2::T;                            // rows in flight in a P2 block
+    static constexpr int RPW = p2_rpw<L1, L2>();                       // rows per warp and item
     static constexpr int ITEM_ROWS = ROWS * RPW;
     static constexpr int ITEMS2 = L1 / ITEM_ROWS;                      // P2 items per template
-    static constexpr size_t EX_HALF = (size_t)C1::PADDED * NC;         // c2 per P1 exchange buffer
-    static constexpr size_t P2_ELEMS = (size_t)p2_row_stride<L2>() * ROWS;
-    static constexpr size_t REGION_A = (2 * EX_HALF > P2_ELEMS) ? 2 * EX_HALF : P2_ELEMS;
-    static constexpr size_t W_ELEMS = (size_t)(L1 / 2) * NC;           // c2 (w tile) and double (u tile)
-    static constexpr size_t TW_ELEMS = (size_t)twtab_elems<L1>();
-    static constexpr size_t SMEM_BYTES = sizeof(c2) * (REGION_A + W_ELEMS + TW_ELEMS) + sizeof(double) * W_ELEMS;
-    static_assert(C1::R3 == 1, "fused kernel: two-step column FFT");
+    static constexpr size_t P1_BYTES = p1_smem_bytes<L1, LOAD_GEN>();
+    static constexpr size_t P2_BYTES = sizeof(c2) * (size_t)p2_row_stride<L2>() * ROWS;
+    static constexpr size_t SMEM_BYTES = P1_BYTES > P2_BYTES ? P1_BYTES : P2_BYTES;
+    static_assert(C1::NT1 == NT && C2::NT2 == NT, "fused kernel: 256-thread blocks in both roles");
     static_assert(C2::T <= 32, "fused kernel: one warp per row");
-    static_assert(C1::T * NC == HALF && L1 % ITEM_ROWS == 0, "fused kernel geometry");
+    static_assert(L1 % ITEM_ROWS == 0, "fused kernel geometry");
 };
 
-// One template of one tile by one half of the block (256 threads, lt = thread index in the half).
+// Bounded wait of one thread until *ctr == want (acquire).  false: timed out or another block aborted.
+__device__ __forceinline__ bool wait_counter(const unsigned* ctr, const unsigned want, int* abort_flag)
+{
+    unsigned spins = 0;
+    while (ld_acquire_u32(ctr) != want) {
+        if (ld_volatile_s32(abort_flag) != 0) return false;
+        if (++spins > (1u << 22)) { atomicExch(abort_flag, 1); return false; }
+        __nanosleep(100);
+    }
+    return true;
+}
+
+// ---------------------------------------------------------------------------------------- P1 role
+// All templates of the bank for column tile `tile` (the loop body is p1_kernel<LOAD_GEN>'s).
 template <int L1, int L2>
-__device__ __forceinline__ void fused_p1(const FusedArgs& a, const int tile, const int b, const int lt,
-                                         const int bar_id, c2* __restrict__ ex, const c2* __restrict__ wt,
-                                         const double* __restrict__ ut, const c2* __restrict__ tw,
-                                         const TemplCoef* __restrict__ tc)
+__device__ __forceinline__ void fused_p1_role(const FusedArgs& a, const int tile, c2* __restrict__ smem,
+                                              unsigned long long& st_wait, unsigned long long& n_steps)
 {
     using F = FusedCfg<L1, L2>;
     using C = Cfg<L1>;
-    constexpr int E = C::E, T = C::T, R1 = C::R1, NC = F::NC, RL = C::R2;
+    constexpr int E = C::E, T = C::T, R1 = C::R1, NC = C::C, NT = F::NT;
+    constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
     constexpr int NZ1 = R1 / 2;                                        // bins k >= N/2 are zero
     constexpr size_t n_total = (size_t)L1 * L2;
-    const int c = lt % NC, t = lt / NC;
+    constexpr bool TWTAB = p1_use_twtab<L1>();
+    __shared__ __align__(16) TemplCoef s_coef[2];
+    __shared__ int s_ok;
+
+    const int tid = threadIdx.x, nt = a.n_templates;
+    const int c = tid % NC, t = tid / NC;
     const int k2 = tile * NC + c;
+    c2* __restrict__ tw = smem + (size_t)C::PADDED * NC;
+    c2* __restrict__ wt = tw + (TWTAB ? twtab_elems<L1>() : 0);
+    double* __restrict__ ub = reinterpret_cast<double*>(wt + (size_t)(L1 / 2) * NC);
+    float* __restrict__ inv = reinterpret_cast<float*>(ub + L1 / 2);
+    {
+        constexpr int CPR = NC / 2, NCHUNK = (L1 / 2) * CPR;
+        for (int ci = tid; ci < NCHUNK; ci += NT) {
+            const int row = ci / CPR, part = ci % CPR;
+            cp_async16(wt + row * NC + 2 * part, a.w + ((size_t)row * L2 + tile * NC + 2 * part));
+        }
+        if (tid < 4) cp_async16(reinterpret_cast<char*>(&s_coef[0]) + 16 * tid, reinterpret_cast<const char*>(a.coef) + 16 * tid);
+        cp_async_commit();
+        if constexpr (TWTAB) twtab_fill<L1>(tw, tid, NT);
+        for (int k1 = tid; k1 < L1 / 2; k1 += NT) {
+            const int kb = k1 * L2 + tile * NC;
+            ub[k1] = __ldg(a.u + kb);
+            inv[k1] = kb > 0 ? (float)(1.0 / (double)kb) : 0.f;
+        }
+        cp_async_wait_all();
+    }
+    __syncthreads();
 
-    c2 v[E];
-    spa_correlate<L1, L2>(v, t, k2, wt + c, NC, ut + c, NC, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
+    int cur = 0, b = 0;
+    for (; b < nt; ++b, cur ^= 1) {
+        if (tid < 4 && b + 1 < nt)
+            cp_async16(reinterpret_cast<char*>(&s_coef[cur ^ 1]) + 16 * tid,
+                       reinterpret_cast<const char*>(a.coef + b + 1) + 16 * tid);
+        cp_async_commit();
+        const TemplCoef* tc = &s_coef[cur];
+        c2 v[E];
+        if (a.use_series)
+            spa_correlate<L1, L2, true>(v, t, k2, wt + c, NC, nullptr, 0, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3,
+                                        tc->A5, ub, inv, (float)c);
+        else
+            spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
 
-    fft_core<L1, NZ1, NC, SYNC_NAMED, false>(v, t, ex + c, 0, 1, NoHook(), tw, bar_id, F::HALF);
+        if (tid == 0) {
+            int ok = 1;
+            if (b >= a.ring) {                       // ring slot of template b: P2 must be through with b - ring
+                const long long t0 = clock64();
+                ok = wait_counter(a.p2_done + (b - a.ring), (unsigned)F::ITEMS2, a.abort_flag) ? 1 : 0;
+                st_wait += (unsigned long long)(clock64() - t0);
+            }
+            bulk_store_wait_read();                  // the previous output tile has left the exchange buffer
+            s_ok = ok;
+        }
+        __syncthreads();
+        if (!s_ok) break;
+        fft_core<L1, NZ1, NC, SYNC_BLOCK, false>(v, t, smem + c, 0, 1, NoHook(), TWTAB ? tw : nullptr);
 
-    c2* __restrict__ yb = a.Y + (size_t)(b % a.ring) * n_total + y_index<L1, NC>(t, k2);
+        __syncthreads();                             // every step-2 read of the exchange buffer is done
+        c2* __restrict__ ot = smem + (size_t)t * NC + c;
 #pragma unroll
-    for (int u = 0; u < E / RL; ++u)
+        for (int u = 0; u < E / RL; ++u)
 #pragma unroll
-        for (int q = 0; q < RL; ++q)
-            yb[(size_t)(T * u + (L1 / RL) * q) * NC] = v[u * RL + q];      // row j1 = t + T u + (L1/RL) q
-    named_barrier(bar_id, F::HALF);      // exchange buffer free again; every store of the half issued
-    if (lt == 0) {
-        __threadfence();
-        atomicAdd(a.p1_done + b, 1u);
+            for (int q = 0; q < RL; ++q)
+                ot[(size_t)(T * u + (L1 / RL) * q) * NC] = v[u * RL + q];      // row j1 = t + T u + (L1/RL) q
+        fence_async_smem();
+        cp_async_wait_all();                         // the next template's constants have landed
+        __syncthreads();
+        if (tid == 0) {
+            if (b > 0) {                             // the store of template b - 1, issued a whole step ago: publish it
+                bulk_store_wait_done<0>();
+                red_release_add(a.p1_done + (b - 1), 1u);
+            }
+            bulk_store(a.Y + (size_t)(b % a.ring) * n_total + (size_t)tile * L1 * NC, smem, (unsigned)(sizeof(c2) * L1 * NC));
+        }
+        ++n_steps;
+    }
+    if (tid == 0) {
+        bulk_store_wait_done<0>();
+        if (b == nt && nt > 0) red_release_add(a.p1_done + (nt - 1), 1u);
     }
 }
 
-// One P2 item: rows [rb * ITEM_ROWS, +ITEM_ROWS) of template b, all 512 threads.
+// ---------------------------------------------------------------------------------------- P2 role
+// One item: rows [rb * ITEM_ROWS, +ITEM_ROWS) of template b, by the 8 warps of the block.
 template <int L1, int L2>
-__device__ __forceinline__ void fused_p2(const FusedArgs& a, const int b, const int rb, c2* __restrict__ smem)
+__device__ __forceinline__ void fused_p2_item(const FusedArgs& a, const int b, const int rb, c2* __restrict__ smem)
 {
     using F = FusedCfg<L1, L2>;
     using C = Cfg<L2>;
@@ -180,106 +273,62 @@ __device__ __forceinline__ void fused_p2(const FusedArgs& a, const int b, const 
 }
 
 template <int L1, int L2>
-__global__ void __launch_bounds__(512, 1) bank_kernel(const FusedArgs a)
+__device__ __forceinline__ void fused_p2_role(const FusedArgs& a, c2* __restrict__ smem,
+                                              unsigned long long& st_wait, unsigned long long& n_steps)
+{
+    using F = FusedCfg<L1, L2>;
+    __shared__ int s_item;
+    const unsigned total = (unsigned)a.n_templates * (unsigned)F::ITEMS2;
+    unsigned next = 0;
+    if (threadIdx.x == 0) next = atomicAdd(a.p2_next, 1u);
+    for (;;) {
+        if (threadIdx.x == 0) {
+            const unsigned cur = next;
+            int item = -1;
+            if (cur < total) {
+                next = atomicAdd(a.p2_next, 1u);     // claim one ahead: its latency hides behind this item
+                const long long t0 = clock64();
+                if (wait_counter(a.p1_done + cur / (unsigned)F::ITEMS2, (unsigned)F::NTILES, a.abort_flag)) item = (int)cur;
+                st_wait += (unsigned long long)(clock64() - t0);
+            }
+            s_item = item;
+        }
+        __syncthreads();
+        const int item = s_item;
+        if (item < 0) break;
+        fused_p2_item<L1, L2>(a, item / F::ITEMS2, item % F::ITEMS2, smem);
+        ++n_steps;
+        __syncthreads();                             // s_item and the row buffers are reused
+    }
+}
+
+// ---------------------------------------------------------------------------------------- kernel
+template <int L1, int L2>
+__global__ void __launch_bounds__(256, 2) bank_kernel(const FusedArgs a)
 {
     extern __shared__ __align__(16) c2 smem[];
     using F = FusedCfg<L1, L2>;
-    using C = Cfg<L1>;
-    constexpr int NC = F::NC;
-    __shared__ int s_act[3];                         // action, template, row block
-
-    c2* __restrict__ wt = smem + F::REGION_A;                                    // [L1/2][NC]
-    c2* __restrict__ tw = wt + F::W_ELEMS;                                       // [R1][R2 + 2]
-    double* __restrict__ ut = reinterpret_cast<double*>(tw + F::TW_ELEMS);       // [L1/2][NC]
-
-    const int tid = threadIdx.x;
-    const int my_tile = ((int)blockIdx.x < F::NTILES) ? (int)blockIdx.x : -1;
-    const int nt = a.n_templates;
-    if (my_tile >= 0) {
-        // stage this block's columns of w and k^{-1/3}: rows of NC * 8 bytes = NC/2 chunks of 16 bytes
-        constexpr int CPR = NC / 2, NCHUNK = (L1 / 2) * CPR;
-        for (int ci = tid; ci < NCHUNK; ci += F::NT) {
-            const int row = ci / CPR, part = ci % CPR;
-            const size_t g = (size_t)row * L2 + my_tile * NC + 2 * part;
-            cp_async16(wt + row * NC + 2 * part, a.w + g);
-            cp_async16(ut + row * NC + 2 * part, a.u + g);
+    __shared__ int s_tile;
+    const long long t_begin = clock64();
+    if (threadIdx.x == 0) {
+        // the first block to arrive on an SM takes a column tile (while there are tiles): one P1 block per SM
+        int tile = -1;
+        if (atomicAdd(a.sm_slot + smid(), 1u) == 0u) {
+            const unsigned tn = atomicAdd(a.tile_next, 1u);
+            if (tn < (unsigned)F::NTILES) tile = (int)tn;
         }
-        cp_async_commit();
-        twtab_fill<L1>(tw, tid, F::NT);
-        cp_async_wait_all();
+        s_tile = tile;
     }
     __syncthreads();
-
-    const unsigned total2 = (unsigned)nt * (unsigned)F::ITEMS2;
-    int next_b1 = (my_tile >= 0) ? 0 : nt;           // next template pair of this block's tile
-    bool q_empty = false;                            // the P2 queue has been seen exhausted
-
-    unsigned long long st_dec = 0, st_p1 = 0, st_p2 = 0, n_p1 = 0, n_p2 = 0;
-    const long long t_begin = clock64();
-    for (;;) {
-        const long long t0 = clock64();
-        if (tid == 0) {
-            int act = 0, tb = 0, rb = 0;             // 0 = exit, 1 = P1 pair, 2 = P2 item, 3 = abort
-            unsigned spins = 0;
-            for (;;) {
-                // (a) the next P1 step of this block's tile, if its ring slots are free (pairs are ring-aligned)
-                bool p1_ok = false;
-                if (next_b1 < nt) {
-                    p1_ok = true;
-                    if (next_b1 >= a.ring) {
-                        p1_ok = ld_acquire_u32(a.p2_done + (next_b1 - a.ring)) == (unsigned)F::ITEMS2;
-                        if (p1_ok && next_b1 + 1 < nt)
-                            p1_ok = ld_acquire_u32(a.p2_done + (next_b1 + 1 - a.ring)) == (unsigned)F::ITEMS2;
-                    }
-                    if (p1_ok && !a.p2_first) { act = 1; tb = next_b1; break; }
-                }
-                // (b) the item at the head of the P2 queue, if its template is complete
-                if (!q_empty) {
-                    const unsigned cur = ld_acquire_u32(a.p2_next);
-                    if (cur >= total2) {
-                        q_empty = true;
-                    } else {
-                        const int b = (int)(cur / (unsigned)F::ITEMS2);
-                        if (ld_acquire_u32(a.p1_done + b) == (unsigned)F::NTILES) {
-                            if (atomicCAS(a.p2_next, cur, cur + 1u) == cur) {
-                                act = 2; tb = b; rb = (int)(cur % (unsigned)F::ITEMS2);
-                                break;
-                            }
-                            continue;                // lost the race: look again at once
-                        }
-                    }
-                }
-                if (p1_ok) { act = 1; tb = next_b1; break; }
-                if (q_empty && next_b1 >= nt) { act = 0; break; }
-                if (ld_volatile_s32(a.abort_flag) != 0) { act = 3; break; }
-                if (++spins > (1u << 22)) { atomicExch(a.abort_flag, 1); act = 3; break; }
-                __nanosleep(200);
-            }
-            s_act[0] = act; s_act[1] = tb; s_act[2] = rb;
-        }
-        __syncthreads();
-        const int act = s_act[0], tb = s_act[1], rb = s_act[2];      // rewritten only after the barrier that ends the step
-        const long long t1 = clock64();
-        st_dec += (unsigned long long)(t1 - t0);
-        if (act == 0 || act == 3) break;
-        if (act == 1) {
-            const int half = tid / F::HALF, lt = tid % F::HALF;
-            const int b = tb + half;
-            if (b < nt)
-                fused_p1<L1, L2>(a, my_tile, b, lt, 1 + half, smem + (size_t)half * F::EX_HALF, wt, ut, tw, a.coef + b);
-            next_b1 = tb + 2;
-            __syncthreads();                         // region A is shared with the P2 role
-            st_p1 += (unsigned long long)(clock64() - t1); ++n_p1;
-        } else {
-            fused_p2<L1, L2>(a, tb, rb, smem);
-            __syncthreads();
-            st_p2 += (unsigned long long)(clock64() - t1); ++n_p2;
-        }
-    }
-    if (a.stats != nullptr && tid == 0) {
+    const int tile = s_tile;
+    unsigned long long st_wait = 0, n_steps = 0;
+    if (tile >= 0) fused_p1_role<L1, L2>(a, tile, smem, st_wait, n_steps);
+    else fused_p2_role<L1, L2>(a, smem, st_wait, n_steps);
+    if (a.stats != nullptr && threadIdx.x == 0) {
         unsigned long long* o = a.stats + 6 * (size_t)blockIdx.x;
-        o[0] = st_dec; o[1] = st_p1; o[2] = st_p2; o[3] = n_p1; o[4] = n_p2;
-        o[5] = (unsigned long long)(clock64() - t_begin);
+        const unsigned long long total = (unsigned long long)(clock64() - t_begin);
+        o[0] = tile >= 0 ? 1ULL : 2ULL; o[1] = st_wait; o[2] = total - st_wait; o[3] = n_steps; o[4] = total;
+        o[5] = (unsigned long long)(long long)tile;
     }
 }
 

@@ -258,10 +258,9 @@ __device__ __forceinline__ c2 fft_center_factor(const int t, const int e, const 
 // ------------------------------------------------------------------ S3: SPA phasor
 // e^{+i Psi_T(f_k)} for bin k >= 1 ("x form" in cycles).  The phase
 // reaches 1e4 cycles, so the polynomial and the reduction to [-1/2, 1/2] cycles run in fp64
-// (the FP64 pipe is otherwise idle); the fraction is then exact to 3e-8 cycles in fp32.
+// (the FP64 pipe is otherwise idle); the fraction is then exact to 2^-32 cycles.
 // u = k^{-1/3} in double comes from the template-independent table built by cbmf_create
-// (rcbrt_table_kernel, 8 bytes per bin, L2-resident).  ph - rint(ph) is taken with the
-// 1.5 * 2^52 trick (two DADD) instead of a conversion.  The reduced angle lies in [-pi, pi],
+// (rcbrt_table_kernel) or from the series of spa_correlate.  The reduced angle lies in [-pi, pi),
 // where the SFU sine/cosine (MUFU.SIN/COS) have absolute error <= 2^-21.4 (CUDA math API,
 // __sinf): a template mismatch of order 1e-13, against the 1e-6 bound of tests/parity.py.
 __device__ __forceinline__ c2 spa_phasor_u(const double u, const double A1, const double A2,
@@ -271,10 +270,20 @@ __device__ __forceinline__ c2 spa_phasor_u(const double u, const double A1, cons
     ph = fma(ph, u, A2);
     ph = fma(ph, u, A1);
     ph = fma(ph, u, -0.125);
-    const double big = 6755399441055744.0;                 // 1.5 * 2^52: (ph + big) - big = rint(ph)
-    const double rn = __dadd_rn(__dadd_rn(ph, big), -big);
-    const float ang = 6.28318530717958647692f * (float)(ph - rn);
+    // |ph| < 2^19 cycles: in ph + 1.5 * 2^20 the unit of the last place is 2^-32, so the low word of the
+    // sum is the phase modulo one cycle as a 32-bit two's-complement fraction (one DADD, no conversion unit)
+    const int frac = __double2loint(__dadd_rn(ph, 1572864.0));
+    const float ang = (float)frac * (6.28318530717958647692f / 4294967296.0f);
     return pk(__cosf(ang), __sinf(ang));
+}
+
+// (double)f for a finite float |f| < 2^100 that is normal or zero, with integer instructions instead of
+// the conversion unit (zero maps to 2^-127 ~ 5.9e-39, which the caller adds to a number of order 1e-2).
+__device__ __forceinline__ double widen_f32(const float f)
+{
+    const unsigned b = __float_as_uint(f);
+    const unsigned hi = (((b & 0x7FFFFFFFu) >> 3) + 0x38000000u) | (b & 0x80000000u);
+    return __hiloint2double((int)hi, (int)(b << 29));
 }
 
 // u[k] = k^{-1/3} in double (k >= 1; u[0] = 0), one Newton step on the library cube root.
@@ -340,7 +349,7 @@ __device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, c
                         const float d = cf * inv[k1];
                         const float p = d * fmaf(d, fmaf(d, -14.0f / 81.0f, 2.0f / 9.0f), -1.0f / 3.0f);
                         const double b0 = ub[k1];
-                        uk = fma(b0, (double)p, b0);
+                        uk = fma(b0, widen_f32(p), b0);
                     } else {
                         uk = ut[(size_t)k1 * US];
                     }

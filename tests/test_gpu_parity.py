@@ -280,10 +280,10 @@ def test_filter_bank_cfg3_sampled(cbmf):
     assert np.all(pk["snr_max"] > 3.5) and np.all(pk["snr_max"] < 20)
 
 
-@pytest.mark.parametrize("n_templates,ring", [(1, 2), (37, 2), (64, 6), (129, 4), (96, 16)])
+@pytest.mark.parametrize("n_templates,ring", [(1, 2), (37, 2), (64, 7), (129, 4), (96, 32)])
 def test_fused_path_equals_launch_pairs(cbmf, n_templates, ring):
-    """N = 2^20: the persistent fused launch (cbmf_set_fused) gives the same peaks and triggers (to fp32 rounding) as the pass-1 / pass-2 launch pairs, for odd bank sizes (one idle
-    half block at the end), banks shorter than the ring, and several ring sizes."""
+    """N = 2^20: the persistent fused launch (cbmf_set_fused) gives the same peaks and triggers (to fp32 rounding) as the pass-1 / pass-2 launch pairs, for a single template,
+    banks shorter and longer than the ring, and several ring sizes."""
     wl = W.config1()
     bank = np.ascontiguousarray(wl.bank[:n_templates])
     if n_templates > 1:
