@@ -131,8 +131,8 @@ int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
 int cbmf_debug_fused_stats(cbmf_ctx *ctx, uint64_t *out, int64_t max_blocks, int64_t *n_blocks);
 
 /* ---- tuning ---- */
-/* Templates per launch pair (pass 1 + pass 2).  Default: 256 MiB of inter-pass buffer
- * (8 n bytes per template) per pair, i.e. 32 templates at n = 2^20; results do not depend on it.
+/* Templates per launch pair (pass 1 + pass 2).  Default: 512 MiB of inter-pass buffer
+ * (8 n bytes per template) per pair, i.e. 64 templates at n = 2^20; results do not depend on it.
  * 1 <= templates_per_launch <= 4096; ENOMEM if the larger buffer cannot be allocated. */
 int cbmf_set_sub_batch(cbmf_ctx *ctx, int templates_per_launch);
 int cbmf_get_sub_batch(const cbmf_ctx *ctx);

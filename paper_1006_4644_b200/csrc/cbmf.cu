@@ -371,9 +371,9 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     c->k_lo = (int)std::ceil(f_low_hz * ((double)n / fs_hz));       // reading A7: inclusive, in double
     if (c->k_lo < 1) c->k_lo = 1;
 
-    // templates per launch pair: 256 MiB of inter-pass buffer per pair (32 templates at N = 2^20).  Measured
+    // templates per launch pair: 512 MiB of inter-pass buffer per pair (64 templates at N = 2^20).  Measured
     // (DESIGN.md §7): larger grids matter more than keeping Y inside the L2 at the present kernel speed.
-    int64_t sb = (int64_t(256) << 20) / (8 * n);
+    int64_t sb = (int64_t(512) << 20) / (8 * n);
     if (sb < 1) sb = 1;
     if (sb > 256) sb = 256;
     if (const char* e = getenv("CBMF_SUB_BATCH")) {

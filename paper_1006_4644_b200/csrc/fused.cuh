@@ -239,10 +239,12 @@ __device__ __forceinline__ void fused_p2_item(const FusedArgs& a, const int b, c
     c2* sm = smem + row * p2_row_stride<L2>();
     const int j1_0 = rb * F::ITEM_ROWS + row;
     p2_prefetch_row<L1, L2>(sm, p.Y, j1_0, t);
+    P2Tw<L1, L2> rtw;
+    rtw.init(j1_0, ROWS, t);
 #pragma unroll 1
     for (int it = 0; it < RPW; ++it) {
         const int j1 = j1_0 + it * ROWS;
-        p2_row<L1, L2, EPI_MAX>(p, j1, 0, t, sm, p.Y, (it + 1 < RPW) ? j1 + ROWS : -1);
+        p2_row<L1, L2, EPI_MAX>(p, j1, 0, t, sm, p.Y, (it + 1 < RPW) ? j1 + ROWS : -1, rtw);
     }
     __syncthreads();                                 // every row of the item has published and left Y
     if (threadIdx.x == 0) {

@@ -130,7 +130,7 @@ template <int L, int NZ1, int SS, int SYNC, bool ROWTW, typename Hook = NoHook, 
 __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm,
                                          const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook(),
                                          const c2* __restrict__ tw = nullptr, const int bar_id = 0,
-                                         const int bar_threads = 0)
+                                         const int bar_threads = 0, const c2* __restrict__ g_row = nullptr)
 {
     using C = Cfg<L>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, R2 = C::R2, R3 = C::R3;
@@ -177,7 +177,8 @@ __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __
             if constexpr (ROWTW) {
                 // e^{2 pi i (k / (R1 R2) + j1 R3 / N)}: numerator over N = n1 L is an exact integer < N
                 const float two_over_n = 2.0f / ((float)n1 * (float)L);
-                const c2 g = expi_frac(k * (n1 * R3) + j1 * R3, two_over_n);
+                // g_row (ROWTW, one step-2 DFT per thread): the caller carries g from row to row by a rotation
+                const c2 g = (g_row != nullptr) ? *g_row : expi_frac(k * (n1 * R3) + j1 * R3, two_over_n);
                 if constexpr (R3 > 1) {
                     mul_powers<R2, true>(x, g, expi_frac(j1 * (i >> LG_R1), two_over_n));
                 } else if constexpr (CENTER) {
@@ -540,7 +541,7 @@ template <int L1, int L2>
 __host__ __device__ constexpr int p2_rpw()
 {
     constexpr int per8 = L1 / Cfg<L2>::ROWS / 8;
-    return per8 >= 8 ? 8 : (per8 >= 1 ? per8 : 1);
+    return per8 >= 16 ? 16 : (per8 >= 1 ? per8 : 1);
 }
 template <int L2> __host__ __device__ constexpr int p2_row_stride()
 {
@@ -562,14 +563,45 @@ __device__ __forceinline__ void p2_prefetch_row(c2* __restrict__ sm, const c2* _
     cp_async_commit();
 }
 
+// Row-to-row twiddle state of one pass-2 thread (EPI_MAX, rows of 1024 points: one warp per row, one
+// DFT per thread and step).  Both row-dependent twiddle seeds are pure phases that advance by a
+// constant angle when the warp moves on by `stride` rows, so after the first row of an item (two
+// sincospi per thread) they are carried by one complex multiply each instead of being recomputed:
+//   G  = e^{2 pi i j1 t / (L1 R1)}        the lane's entry of the (W_N^{j1 L2/R1})^r table,  dG = e^{2 pi i stride t / (L1 R1)}
+//   g  = e^{2 pi i (t n1 + j1) / N}       the step-2 twiddle seed of fft_core (k = t),       dg = e^{2 pi i stride / N}
+// At most 16 rows follow one initialisation: the accumulated rounding is ~1e-6 of the phase.
+template <int L1, int L2>
+struct P2Tw {
+    static constexpr bool ON = (Cfg<L2>::T == 32) && (Cfg<L2>::E == Cfg<L2>::R1) && (Cfg<L2>::E == Cfg<L2>::R2) &&
+                               (Cfg<L2>::R3 == 1);
+    c2 G, dG, g, dg;
+    __device__ __forceinline__ void init(const int j1, const int stride, const int t)
+    {
+        if constexpr (ON) {
+            constexpr int R1 = Cfg<L2>::R1;
+            const float s1 = 2.0f / (float)(L1 * R1), sn = 2.0f / ((float)L1 * (float)L2);
+            G = expi_frac((j1 * t) & (L1 * R1 - 1), s1);
+            dG = expi_frac((stride * t) & (L1 * R1 - 1), s1);
+            g = expi_frac(t * L1 + j1, sn);
+            dg = expi_frac(stride, sn);
+        }
+    }
+    __device__ __forceinline__ void advance()
+    {
+        if constexpr (ON) { G = cmul(G, dG); g = cmul(g, dg); }
+    }
+};
+
 // Row j1 of template slot b: twiddle, N2 = L2-point inverse FFT over k2 -> z[j1 + L1 j2] in
 // registers, then the epilogue of MODE.  Called by the T threads of one row group.  On entry the
 // copy of the row into sm has been started by p2_prefetch_row; next_j1 (or -1) is the row of the
 // same template (yb) whose copy is started as soon as the exchange buffer is free again.
 template <int L1, int L2, int MODE>
 __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int b, const int t,
-                                       c2* __restrict__ sm, const c2* __restrict__ yb, const int next_j1)
+                                       c2* __restrict__ sm, const c2* __restrict__ yb, const int next_j1,
+                                       P2Tw<L1, L2>& rtw)
 {
+    constexpr bool ROT = P2Tw<L1, L2>::ON && (MODE == EPI_MAX);
     using C = Cfg<L2>;
     constexpr int E = C::E, T = C::T, R1 = C::R1;
     constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
@@ -594,7 +626,11 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
     if constexpr (WSYNC) {
         // G[r] = e^{2 pi i j1 r / (L1 R1)}, r < R1: one sincospi per lane, broadcast through shared memory
         c2* __restrict__ G = sm + C::PADDED;
-        for (int r = t; r < R1; r += T) G[r] = expi_frac((j1 * r) & (L1 * R1 - 1), 2.0f / (float)(L1 * R1));
+        if constexpr (ROT) {
+            G[t] = rtw.G;
+        } else {
+            for (int r = t; r < R1; r += T) G[r] = expi_frac((j1 * r) & (L1 * R1 - 1), 2.0f / (float)(L1 * R1));
+        }
         __syncwarp();
 #pragma unroll
         for (int r = 2; r < R1; r += 2) {
@@ -632,7 +668,9 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
     };
     // in the arg-max pass only |z|^2 is needed for almost every sample: leave the common factor out
     constexpr bool CENTER = (MODE == EPI_MAX) && (C::R3 == 1) && (C::R2 == 16 || C::R2 == 32);
-    fft_core<L2, R1, 1, (WSYNC ? SYNC_WARP : SYNC_BLOCK), true, decltype(start_next), CENTER>(v, t, sm, j1, L1, start_next);
+    fft_core<L2, R1, 1, (WSYNC ? SYNC_WARP : SYNC_BLOCK), true, decltype(start_next), CENTER>(
+        v, t, sm, j1, L1, start_next, nullptr, 0, 0, ROT ? &rtw.g : nullptr);
+    if constexpr (ROT) rtw.advance();
 
     // v[u*RL + q] = z[j1 + L1 * j2],  j2 = t + T u + (L2/RL) q
     if constexpr (MODE == EPI_STORE) {
@@ -774,10 +812,12 @@ __device__ __forceinline__ void p2_item(const P2Args& a, const int item, const i
     c2* sm = smem + row * p2_row_stride<L2>();
     const c2* __restrict__ yb = a.Y + (size_t)b * n_total;
     p2_prefetch_row<L1, L2>(sm, yb, (item * RPW) * ROWS + row, t);
+    P2Tw<L1, L2> rtw;
+    if constexpr (MODE == EPI_MAX) rtw.init((item * RPW) * ROWS + row, ROWS, t);
 #pragma unroll 1
     for (int it = 0; it < RPW; ++it) {
         const int j1 = (item * RPW + it) * ROWS + row;
-        p2_row<L1, L2, MODE>(a, j1, b, t, sm, yb, (it + 1 < RPW) ? j1 + ROWS : -1);
+        p2_row<L1, L2, MODE>(a, j1, b, t, sm, yb, (it + 1 < RPW) ? j1 + ROWS : -1, rtw);
     }
     if constexpr (MODE == EPI_MAX) p2_finish<L1, L2>(a, b, L1 / (ROWS * RPW));
 }
