@@ -556,6 +556,19 @@ static int sort_triggers(cbmf_ctx* c, int64_t count)
     if (count <= 1) return CBMF_OK;
     long long np2 = 1;
     while (np2 < count) np2 <<= 1;
+    if (np2 <= TRIG_SMALL) {
+        const size_t smem_small = (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * (size_t)np2;
+        static bool attr_small = false;
+        if (!attr_small) {
+            CU(cudaFuncSetAttribute(trig_sort_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)((sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL)));
+            attr_small = true;
+        }
+        trig_sort_small_kernel<<<1, 1024, smem_small, c->stream>>>(c->d_trig, (int)count, (int)np2);
+        CU(cudaGetLastError());
+        c->launches += 1;
+        return CBMF_OK;
+    }
     const int tile = (int)(np2 < TRIG_TILE ? np2 : TRIG_TILE);
     const size_t smem = sizeof(TrigOut) * (size_t)tile;
     static bool attr_done = false;

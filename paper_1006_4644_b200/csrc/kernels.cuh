@@ -1037,6 +1037,39 @@ __global__ void __launch_bounds__(1024) trig_sort_tile_kernel(TrigOut* trig, lon
     for (int i = threadIdx.x; i < tile; i += blockDim.x) trig[base + i] = s[i];
 }
 
+// Up to TRIG_SMALL records by ONE block: the bitonic network runs on (64-bit key, 16-bit position)
+// pairs -- 12 bytes per compare-exchange operand instead of 32 -- with one thread per compare-exchange
+// (no idle half), and the 16-byte records are permuted once at the end through shared memory.
+constexpr int TRIG_SMALL = 4096;
+__global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, int n, int n_pow2)
+{
+    extern __shared__ __align__(16) unsigned char trig_smem_raw[];
+    unsigned long long* key = reinterpret_cast<unsigned long long*>(trig_smem_raw);          // [n_pow2]
+    TrigOut* rec = reinterpret_cast<TrigOut*>(key + n_pow2);                                  // [n_pow2]
+    unsigned short* pos = reinterpret_cast<unsigned short*>(rec + n_pow2);                    // [n_pow2]
+    for (int i = threadIdx.x; i < n_pow2; i += blockDim.x) {
+        unsigned long long k = ~0ULL;                                  // padding sorts last
+        if (i < n) { const TrigOut o = trig[i]; rec[i] = o; k = trig_key(o); }
+        key[i] = k;
+        pos[i] = (unsigned short)i;
+    }
+    __syncthreads();
+    const int n_pairs = n_pow2 >> 1;
+    for (int kk = 2; kk <= n_pow2; kk <<= 1)
+        for (int jj = kk >> 1; jj > 0; jj >>= 1) {
+            for (int p = threadIdx.x; p < n_pairs; p += blockDim.x) {
+                const int i = ((p & ~(jj - 1)) << 1) | (p & (jj - 1)), x = i | jj;
+                const unsigned long long a = key[i], b = key[x];
+                if ((a > b) == ((i & kk) == 0)) {
+                    key[i] = b; key[x] = a;
+                    const unsigned short t = pos[i]; pos[i] = pos[x]; pos[x] = t;
+                }
+            }
+            __syncthreads();
+        }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = rec[pos[i]];
+}
+
 // ------------------------------------------------------------------ diagnostics
 __global__ void snr_from_z_kernel(const float2* __restrict__ z, float* __restrict__ snr, size_t n, float inv_sigma)
 {
