@@ -45,8 +45,8 @@ UNIT = "templates/s"
 # clocks.max.sm 1965 MHz; 128 FP32 lanes per SM, FMA = 2 flop): DESIGN.md §6.
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per template of the two pass kernels at N = 2^20, from the one
-# `ncu --set full` capture summarised in profiles/r1f_ncu_full_p1_p2.md (217.7 MB and 272.9 MB per launch of 32).
-NCU_DRAM_BYTES_PER_TEMPLATE_2P20 = (217.7e6 / 32, 272.9e6 / 32)
+# `ncu --set full` capture summarised in profiles/r1g_ncu_full_p1_p2.md (485.7 MB and 541.0 MB per launch of 64).
+NCU_DRAM_BYTES_PER_TEMPLATE_2P20 = (485.7e6 / 64, 541.0e6 / 64)
 
 
 def _env_int(name, default):
@@ -348,7 +348,7 @@ def run_ours(args):
         "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "peak_source": "148 SM x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md §6)",
         "traffic": (NCU_DRAM_BYTES_PER_TEMPLATE_2P20[which] * tmpl_per_launch) if n == (1 << 20) else None,
-        "traffic_source": "ncu --set full, profiles/r1f_ncu_full_p1_p2.md (per template x templates per launch)",
+        "traffic_source": "ncu --set full, profiles/r1g_ncu_full_p1_p2.md (per template x templates per launch)",
         "algorithmic_bytes_per_launch": 8.0 * n * tmpl_per_launch,
         "flops_per_launch": flops_launch, "avg_launch_ms": avg_launch_ms, "templates_per_launch": tmpl_per_launch,
         "pass_ms_per_step": [p_ms[0] / K, p_ms[1] / K],
