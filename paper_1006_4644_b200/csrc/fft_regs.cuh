@@ -76,8 +76,6 @@ __device__ __forceinline__ c2 cmulc(c2 a, c2 w)
     return fma2(bc(ay), pk(wy, wx), mul2(pk(wx, -wy), bc(ax)));
 }
 __device__ __forceinline__ c2 csqr(c2 a) { return cmul(a, a); }
-// i * a
-__device__ __forceinline__ c2 mul_i(c2 a) { float x, y; unpk(a, x, y); return pk(-y, x); }
 __device__ __forceinline__ c2 neg2(c2 a) { float x, y; unpk(a, x, y); return pk(-x, -y); }
 
 // cos(2 pi a / 32), a = 0..8, correctly rounded to float.

@@ -6,9 +6,9 @@
 //   pass 2 (p2_kernel): for ROWS adjacent rows j1, multiply by W_N^{j1 k2}, N2-point inverse FFT
 //       over k2 -> z[j1 + N1 j2] in registers, |z|^2, arg-max, threshold              (S5-S7)
 //   Y (N complex floats per template in flight) is the only materialised intermediate.  It is
-//   stored tile-major, Y[k2 / NC][j1][k2 % NC] with NC = the columns of one pass-1 tile, so that a
-//   pass-1 warp (a few adjacent rows j1 of one tile) stores whole contiguous lines; pass 2 gathers a
-//   row from NC-column segments with asynchronous 16-byte copies.
+//   stored tile-major, Y[k2 / NC][j1][k2 % NC] with NC = the columns of one pass-1 tile, so that the
+//   output of a pass-1 block for one template is ONE contiguous piece, written by a TMA bulk store
+//   from shared memory; pass 2 gathers a row from NC-column segments with asynchronous 16-byte copies.
 //
 // Each per-pass FFT is a Stockham autosort FFT whose butterflies (radix 8/16/32) live in
 // registers and whose digit exchanges go through shared memory.
