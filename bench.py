@@ -352,6 +352,9 @@ def run_ours(args):
         "algorithmic_bytes_per_launch": 8.0 * n * tmpl_per_launch,
         "flops_per_launch": flops_launch, "avg_launch_ms": avg_launch_ms, "templates_per_launch": tmpl_per_launch,
         "pass_ms_per_step": [p_ms[0] / K, p_ms[1] / K],
+        "note": ("per-launch figures are taken with every launch ALONE on the GPU (one stream); pass 1 is launched with one "
+                 "block per SM so that pass-2 blocks of the other launch pairs share its SMs in the timed schedule, where "
+                 "the two passes overlap: whole_path gives the fraction of the FP32 peak reached by the whole step"),
         "whole_path": {
             "flops_per_template": f1 + f2, "us_per_template": 1e3 * ms_max / (B * K),
             "achieved_tflops": (f1 + f2) * B * world * K / (ms_max * 1e-3) / 1e12 / world,
