@@ -210,6 +210,17 @@ def test_filter_bank_small_heavy(cbmf, log2n):
     assert pk[0]["idx_peak"] == -1
 
 
+@pytest.mark.parametrize("log2n", [16, 18, 19, 21, 23, 24])
+def test_filter_bank_every_split(cbmf, log2n):
+    """The product kernels (generator + column FFT, row FFT + arg-max epilogue) of every N1 x N2 split that
+    configs 0-3 do not reach: configs[4] workloads (fs = 4096 Hz, f_low = 40 Hz, noise only), three
+    templates each, peaks and triggers against the oracle."""
+    wl = W.sweep_point(log2n, 3)
+    pk, tr, near, _ = _bank_case(cbmf, wl)
+    assert np.all((pk["idx_peak"] >= 0) & (pk["idx_peak"] < wl.n))
+    assert len(near) <= 1
+
+
 def test_filter_bank_cfg1_sampled(cbmf):
     """configs[1] at full size (N = 2^20, 1024 templates, the launch configuration bench.py
     times): the 4 injection templates plus every 64th template against the oracle."""
