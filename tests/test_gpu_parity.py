@@ -403,6 +403,44 @@ def test_trigger_truncation_and_threshold_zero(cbmf):
     g.close(); o.close()
 
 
+@pytest.mark.parametrize("log2n", [12, 16, 20])
+def test_degenerate_segments(cbmf, log2n):
+    """All-zero data: every |z| ties at 0 and the peak must be sample 0 (lowest index on exact ties, A12),
+    SNR 0, no triggers at threshold 6 and all N samples at threshold 0.  A unit impulse: z is the template's
+    whitened impulse response, compared with the oracle as usual."""
+    wl = W.small_case(log2n=log2n, fs=4096.0 if log2n > 12 else 2048.0, n_templates=3, seed=70 + log2n)
+    zero = np.zeros(wl.n, dtype=np.float32)
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd); g.load_segment(zero)
+    pk, tr, nf, rc = g.filter_bank(wl.bank, 6.0)
+    assert rc == 0 and nf == 0 and len(tr) == 0
+    assert np.all(pk["idx_peak"] == 0) and np.all(pk["snr_max"] == 0) and np.all(pk["sigma"] > 0)
+    if log2n <= 16:
+        pk, tr, nf, rc = g.filter_bank(wl.bank[:1], 0.0, trig_capacity=wl.n)      # strict >: nothing above 0
+        assert nf == 0
+    g.close()
+    imp = np.zeros(wl.n, dtype=np.float32); imp[wl.n // 3] = 1000.0
+    wl.samples = imp
+    pk, tr, near, _ = _bank_case(cbmf, wl)
+    assert len(near) <= 1
+
+
+def test_trigger_sort_paths(cbmf):
+    """threshold 0 with one and two templates of 4096 samples: exactly 4096 triggers (the single-block sort,
+    full) and 8192 (tile sort + global merges); both must come back in (template, sample) order."""
+    wl = W.small_case(log2n=12, n_templates=2)
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd); g.load_segment(wl.samples)
+    for nt in (1, 2):
+        pk, tr, nf, rc = g.filter_bank(wl.bank[:nt], 0.0, trig_capacity=nt * wl.n)
+        assert rc == 0 and nf == nt * wl.n
+        assert np.array_equal(tr["template_idx"], np.repeat(np.arange(nt), wl.n))
+        assert np.array_equal(tr["sample_idx"], np.tile(np.arange(wl.n), nt))
+    pk, tr, nf, rc = g.filter_bank(wl.bank[:1], 0.0, trig_capacity=1000)           # 1000 kept of 4096: still sorted
+    assert rc == cbmf.WTRUNC and len(tr) == 1000 and np.all(np.diff(tr["sample_idx"].astype(np.int64)) > 0)
+    g.close()
+
+
 def test_device_pointer_entry_points(cbmf):
     """The *_dev calls (torch CUDA tensors, torch's current stream) give the same bytes."""
     import torch
