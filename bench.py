@@ -292,6 +292,7 @@ def run_ours(args):
         ctx.set_profiling(False)
         sub = ctx.get_sub_batch()
         ctx_streams = ctx.get_streams()
+        fp32_meas = ctx.debug_fp32_peak() if rank == 0 else (None, None)
 
         # ---- e2e leg: host-pointer entry points, pinned host buffers
         psd_h = torch.from_numpy(wl.psd).pin_memory()
@@ -347,6 +348,8 @@ def run_ours(args):
                                    "p2_kernel (twiddle + row FFT + |z|^2 + arg-max/threshold)")[which],
         "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "peak_source": "148 SM x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md §6)",
+        "peak_measured_tflops": {"ffma": fp32_meas[0], "ffma2_packed": fp32_meas[1],
+                                 "how": "cbmf_debug_fp32_peak: dependent FMA chains on every SM, CUDA events (cross-check, not the denominator)"},
         "traffic": (NCU_DRAM_BYTES_PER_TEMPLATE_2P20[which] * tmpl_per_launch) if n == (1 << 20) else None,
         "traffic_source": "ncu --set full, profiles/r1g_ncu_full_p1_p2.md (per template x templates per launch)",
         "algorithmic_bytes_per_launch": 8.0 * n * tmpl_per_launch,

@@ -124,6 +124,10 @@ int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_
  * (n/2 complex floats, interleaved). */
 int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);
 int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
+/* FP32 pipe probe for the roofline denominator: dependent-chain FMA kernels on every
+ * SM, timed with CUDA events on the context's stream; TFLOP/s of scalar FFMA and of packed FFMA2
+ * (fma.rn.f32x2).  Both should read close to SMs x 128 lanes x 2 flop x SM clock. */
+int cbmf_debug_fp32_peak(cbmf_ctx *ctx, double *tflops_ffma, double *tflops_ffma2);
 /* Block statistics of the last fused launch (cbmf_set_fused): per block six 64-bit values, role
  * (1 = pass 1, 2 = pass 2), SM cycles spent waiting (ring slot / template not ready), cycles
  * working, steps done (templates / items), total cycles, column tile (-1 for pass 2).  out: host,

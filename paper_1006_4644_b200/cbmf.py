@@ -55,6 +55,7 @@ def lib() -> C.CDLL:
         "cbmf_debug_get_prefix": (C.c_int, [vp, vp]),
         "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
         "cbmf_debug_fused_stats": (C.c_int, [vp, vp, i64, C.POINTER(i64)]),
+        "cbmf_debug_fp32_peak": (C.c_int, [vp, C.POINTER(dbl), C.POINTER(dbl)]),
         "cbmf_set_sub_batch": (C.c_int, [vp, C.c_int]),
         "cbmf_get_sub_batch": (C.c_int, [vp]),
         "cbmf_set_streams": (C.c_int, [vp, C.c_int]),
@@ -78,7 +79,7 @@ def lib() -> C.CDLL:
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
-           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_debug_fused_stats cbmf_set_sub_batch cbmf_get_sub_batch cbmf_set_streams cbmf_get_streams cbmf_set_fused cbmf_get_fused "
+           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_debug_fused_stats cbmf_debug_fp32_peak cbmf_set_sub_batch cbmf_get_sub_batch cbmf_set_streams cbmf_get_streams cbmf_set_fused cbmf_get_fused "
            "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_strerror "
            "cbmf_last_cuda_error cbmf_version").split()
 
@@ -242,6 +243,12 @@ class Context:
         nb = i64_t(0)
         self._check(lib().cbmf_debug_fused_stats(self._h, out.ctypes.data, 1024, C.byref(nb)), "cbmf_debug_fused_stats")
         return out[: int(nb.value)]
+
+    def debug_fp32_peak(self):
+        """-> (TFLOP/s of scalar FFMA, TFLOP/s of packed FFMA2) measured on this device."""
+        a, b = C.c_double(0), C.c_double(0)
+        self._check(lib().cbmf_debug_fp32_peak(self._h, C.byref(a), C.byref(b)), "cbmf_debug_fp32_peak")
+        return float(a.value), float(b.value)
 
     # -- tuning / introspection
     def set_sub_batch(self, k: int):

@@ -919,6 +919,38 @@ extern "C" int cbmf_debug_fused_stats(cbmf_ctx* c, uint64_t* out, int64_t max_bl
     return CBMF_OK;
 }
 
+extern "C" int cbmf_debug_fp32_peak(cbmf_ctx* c, double* tflops_ffma, double* tflops_ffma2)
+{
+    if (!c || !tflops_ffma || !tflops_ffma2) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    int n_sm = 0;
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, c->device));
+    const int iters = 4000;
+    if (int rc = grow_scratch(c, sizeof(float) * 1024 * (size_t)n_sm)) return rc;
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    double res[2] = {0, 0};
+    for (int packed = 0; packed < 2; ++packed) {
+        for (int rep = 0; rep < 2; ++rep) {           // first launch warms up
+            CU(cudaEventRecord(e0, c->stream));
+            if (packed) fp32_peak_kernel<true><<<n_sm, 1024, 0, c->stream>>>((float*)c->d_scratch, iters, 1.0001f);
+            else fp32_peak_kernel<false><<<n_sm, 1024, 0, c->stream>>>((float*)c->d_scratch, iters, 1.0001f);
+            CU(cudaGetLastError());
+            CU(cudaEventRecord(e1, c->stream));
+            CU(cudaEventSynchronize(e1));
+            c->launches += 1;
+        }
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        const double flops = 2.0 * (packed ? 2.0 : 1.0) * 8.0 * 4.0 * (double)iters * 1024.0 * (double)n_sm;
+        res[packed] = flops / ((double)ms * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *tflops_ffma = res[0]; *tflops_ffma2 = res[1];
+    return CBMF_OK;
+}
+
 extern "C" int cbmf_debug_get_prefix(cbmf_ctx* c, double* p_out)
 {
     if (!c || !p_out) return CBMF_EINVAL;

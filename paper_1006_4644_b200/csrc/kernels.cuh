@@ -1070,6 +1070,33 @@ __global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, in
     for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = rec[pos[i]];
 }
 
+// ------------------------------------------------------------------ FP32 pipe probe (roofline cross-check)
+// Eight independent FMA chains per thread, 1024 threads per block, one block per SM.  PACKED = false: scalar
+// FFMA (2 flop per lane and instruction); PACKED = true: FFMA2 (4 flop).  flops = 2 * (PACKED ? 2 : 1) * 8 * 4
+// per thread and iteration.
+template <bool PACKED>
+__global__ void __launch_bounds__(1024, 1) fp32_peak_kernel(float* __restrict__ out, const int iters, const float s)
+{
+    float a[8];
+    c2 p[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { a[i] = (float)threadIdx.x * 1e-3f + (float)i; p[i] = pk(a[i], a[i] + 1.f); }
+    const c2 ps = pk(s, s * 0.5f), pc = pk(0.25f, 0.125f);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if constexpr (PACKED) p[i] = fma2(p[i], ps, pc);
+                else a[i] = fmaf(a[i], s, 0.25f);
+            }
+    }
+    float acc = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc += a[i] + re(p[i]) + im(p[i]);
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
 // ------------------------------------------------------------------ diagnostics
 __global__ void snr_from_z_kernel(const float2* __restrict__ z, float* __restrict__ snr, size_t n, float inv_sigma)
 {
