@@ -94,7 +94,8 @@ int cbmf_load_segment_dev(cbmf_ctx *ctx, const float *samples_dev, int64_t n_sam
  *                            written are an unspecified subset and the call returns
  *                            CBMF_WTRUNC.
  * snr_threshold >= 0.  n_templates may be 0.  ESTATE before PSD and segment are set;
- * EINVAL on a non-positive or non-finite mass or a negative / NaN threshold. */
+ * EINVAL on a non-positive or non-finite mass, on a template whose phase exceeds 2^19 cycles
+ * inside the band (total mass far below 0.3 Msun at f_low = 10 Hz), or a negative / NaN threshold. */
 int cbmf_filter_bank(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_templates,
                      float snr_threshold, cbmf_peak *peaks_out,
                      cbmf_trigger *trig_out, int64_t trig_capacity, int64_t *n_trig_found);

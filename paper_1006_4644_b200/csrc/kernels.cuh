@@ -976,6 +976,16 @@ __global__ void template_setup_kernel(const SetupArgs a)
     c.A3 = b2 * s * s * s * i2pi;
     c.A5 = b0 * s * s * s * s * s * i2pi;
     if (c.k_hi >= c.k_lo) {
+        // the generator reduces the phase modulo one cycle with a 2^-32 fixed-point trick that needs
+        // |Psi| / 2 pi < 2^19 cycles on the band; |Psi| is largest at k_lo (total masses far below 0.3 Msun at 10 Hz)
+        const double ul = 1.0 / cbrt((double)c.k_lo);
+        const double ph_lo = fabs(ul * (c.A1 + ul * (c.A2 + ul * (c.A3 + ul * ul * c.A5)))) + 1.0;
+        if (!(ph_lo < 524288.0)) {
+            *a.err_flag = 1;
+            c.k_hi = -1;
+            a.coef[i] = c;
+            return;
+        }
         const double sig = sqrt(a.prefix[c.k_hi]);
         c.sigma = (float)sig;
         c.inv_sigma = (float)(1.0 / sig);

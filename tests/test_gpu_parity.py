@@ -367,7 +367,7 @@ def test_edge_cases_and_errors(cbmf):
     pk, tr, nf, rc = g.filter_bank(np.zeros((0, 2)), 6.0)
     assert len(pk) == 0 and len(tr) == 0 and nf == 0 and rc == 0
     # bad masses / threshold
-    for b in ([[1.4, -1.0]], [[0.0, 1.0]], [[np.nan, 1.0]], [[np.inf, 1.0]]):
+    for b in ([[1.4, -1.0]], [[0.0, 1.0]], [[np.nan, 1.0]], [[np.inf, 1.0]], [[1e-3, 1e-3]]):   # last: phase > 2^19 cycles
         with pytest.raises(cbmf.CbmfError) as e:
             g.filter_bank(np.array(b), 6.0)
         assert e.value.rc == cbmf.EINVAL
