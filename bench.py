@@ -44,9 +44,6 @@ UNIT = "templates/s"
 # FP32 ALU peak of one B200 from unit counts and clocks (B200_PROFILING.md table: 148 SMs,
 # clocks.max.sm 1965 MHz; 128 FP32 lanes per SM, FMA = 2 flop): DESIGN.md §6.
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum per template of the two pass kernels at N = 2^20, from the one
-# `ncu --set full` capture summarised in profiles/r1g_ncu_full_p1_p2.md (485.7 MB and 541.0 MB per launch of 64).
-NCU_DRAM_BYTES_PER_TEMPLATE_2P20 = (485.7e6 / 64, 541.0e6 / 64)
 
 
 def _env_int(name, default):
@@ -59,7 +56,7 @@ def _env_int(name, default):
 def make_workload(name: str, world: int, rank: int):
     """Seeded synthetic workload; for world > 1 the bank is world x the config's size and
     this rank takes slice `rank` (weak scaling)."""
-    from paper_1006_4644_b200 import workloads as W
+    from testsupport import workloads as W
     from paper_1006_4644_b200.sharding import shard_range
     wl = W.by_name(name)
     per_rank = wl.n_templates
@@ -143,7 +140,7 @@ def pass_flops(n: int, lg1: int, lg2: int, n_b_mean: float):
 
 def mean_band_bins(wl) -> float:
     """Mean number of in-band bins k_lo..k_hi over the bank (host arithmetic on inputs only)."""
-    from paper_1006_4644_b200.workloads import T_SUN_S
+    from testsupport.workloads import T_SUN_S
     mt = wl.bank[:, 0] + wl.bank[:, 1]
     f_isco = 1.0 / (6.0 ** 1.5 * np.pi * mt * T_SUN_S)
     k_lo = math.ceil(wl.f_low * wl.n / wl.fs)
@@ -207,25 +204,57 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------- our arm
-def run_ours(args):
-    import torch
-    import torch.distributed as dist
-    from paper_1006_4644_b200 import cbmf
+def kernel_source_hash() -> str:
+    """sha256 over the kernel sources the traffic figure belongs to (csrc/*.cu, *.cuh, include/cbmf.h)."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    files = sorted(glob.glob(os.path.join(ROOT, "paper_1006_4644_b200", "csrc", "*.cu*"))) + \
+        [os.path.join(ROOT, "include", "cbmf.h")]
+    for f in files:
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
 
-    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
 
-    wl = make_workload(args.workload, world, rank)
+def load_traffic(n: int):
+    """DRAM bytes per template of the two pass kernels from the tracked ncu summary profiles/traffic.json
+    (written by bench_traffic.py from one `ncu --set full` capture).  None unless the capture was taken on
+    exactly the kernel sources of this tree (hash) and at this N."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            t = json.load(fh)
+    except Exception:
+        return None, "profiles/traffic.json missing"
+    if t.get("kernel_source_hash") != kernel_source_hash():
+        return None, f"profiles/traffic.json was captured on other kernel sources ({t.get('kernel_source_hash')})"
+    if int(t.get("n", 0)) != n:
+        return None, f"profiles/traffic.json is for n = {t.get('n')}"
+    return t, t.get("source", "profiles/traffic.json")
+
+
+def fp32_probe(device: int):
+    """Measured FFMA / FFMA2 TFLOP/s from the stand-alone probe bench_fp32_probe.cu (not the product library)."""
+    import ctypes
+    import subprocess
+    src, lib = os.path.join(ROOT, "bench_fp32_probe.cu"), os.path.join(ROOT, "bench_fp32_probe.so")
+    try:
+        if not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+            subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-Xcompiler", "-fPIC",
+                            "-shared", "-o", lib, src], check=True, capture_output=True)
+        L = ctypes.CDLL(lib)
+        a, b = ctypes.c_double(0), ctypes.c_double(0)
+        rc = L.fp32_probe(int(device), ctypes.byref(a), ctypes.byref(b))
+        return (a.value, b.value) if rc == 0 else (None, None)
+    except Exception:
+        return None, None
+
+
+def measure(torch, dist, cbmf, wl, dev, local, world, K, Wm, cap, args, with_e2e=True, with_passes=True):
+    """All legs of one workload on this rank.  -> dict of raw measurements."""
     B, n = wl.n_templates, wl.n
-    cap = args.trig_capacity
     stream = torch.cuda.Stream(device=dev)
-    K, Wm = args.steps, args.warmup
-
+    out = {}
     with torch.cuda.stream(stream):
         ctx = cbmf.Context(n, wl.fs, wl.f_low, device=local, stream=stream.cuda_stream)
         if args.sub_batch:
@@ -244,14 +273,13 @@ def run_ours(args):
             ctx.load_segment(smp_d)
             return ctx.filter_bank_into(bank_d, wl.threshold, peaks_d, trig_d, cap)
 
-        def timed(fn, k, with_flush=True):
+        def timed(fn, k):
             """k steps, each bracketed by CUDA events on the context's stream; L2 flushed
             (untimed) before every step.  -> (sum of step times in ms, last result)"""
             evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
             res = None
             for i in range(k):
-                if with_flush:
-                    flush.fill_(i & 0xFF)
+                flush.fill_(i & 0xFF)
                 evs[i][0].record(stream)
                 res = fn()
                 evs[i][1].record(stream)
@@ -263,6 +291,12 @@ def run_ours(args):
                 dist.barrier()
             torch.cuda.synchronize()
 
+        def max_over_ranks(x):
+            t = torch.tensor([x], dtype=torch.float64, device=dev)
+            if world > 1:
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+
         # ---- device-resident leg: `value`
         for _ in range(Wm):
             flush.fill_(1)
@@ -272,66 +306,126 @@ def run_ours(args):
         with ClockSampler(local) as clk:
             ms_total, (nf, rc) = timed(step_dev, K)
         barrier()
-        launches = ctx.launch_count() - l0
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_max = float(t.item())
-        value = B * world * K / (ms_max * 1e-3)
+        out["launches"] = ctx.launch_count() - l0
+        out["ms_max"] = max_over_ranks(ms_total)
+        out["clocks"] = clk.summary()
+        out["nf"] = int(nf)
+        out["split"] = ctx.get_split()
+        out["sub_batch"], out["streams"] = ctx.get_sub_batch(), ctx.get_streams()
+        out["peaks"] = peaks_d.cpu().numpy().view(cbmf.PEAK_DTYPE).copy()
 
-        # ---- roofline leg: per-launch events inside K more steps
-        ctx.set_profiling(True)
-        p_ms, p_n = [0.0, 0.0], [0, 0]
-        for i in range(K):
-            flush.fill_(i & 0xFF)
-            step_dev()
-            for w in (0, 1):
-                ms, nl = ctx.last_pass_time(w)
-                p_ms[w] += ms
-                p_n[w] += nl
-        ctx.set_profiling(False)
-        sub = ctx.get_sub_batch()
-        ctx_streams = ctx.get_streams()
-        fp32_meas = ctx.debug_fp32_peak() if rank == 0 else (None, None)
+        # ---- roofline legs: per-launch events inside K more steps, every launch alone (mode 1) and in the
+        # real overlapped schedule (mode 2)
+        if with_passes:
+            for mode, key in ((1, "alone"), (2, "overlapped")):
+                ctx.set_profiling(mode)
+                p_ms, p_n = [0.0, 0.0], [0, 0]
+                for i in range(K):
+                    flush.fill_(i & 0xFF)
+                    step_dev()
+                    for w in (0, 1):
+                        ms, nl = ctx.last_pass_time(w)
+                        p_ms[w] += ms
+                        p_n[w] += nl
+                ctx.set_profiling(0)
+                out["pass_" + key] = (p_ms, p_n)
 
         # ---- e2e leg: host-pointer entry points, pinned host buffers
-        psd_h = torch.from_numpy(wl.psd).pin_memory()
-        smp_h = torch.from_numpy(wl.samples).pin_memory()
-        bank_h = torch.from_numpy(np.ascontiguousarray(wl.bank)).pin_memory()
-        peaks_h = torch.empty(B * 16, dtype=torch.uint8).pin_memory()
-        trig_h = torch.empty(cap * 16, dtype=torch.uint8).pin_memory()
+        if with_e2e:
+            psd_h = torch.from_numpy(wl.psd).pin_memory()
+            smp_h = torch.from_numpy(wl.samples).pin_memory()
+            bank_h = torch.from_numpy(np.ascontiguousarray(wl.bank)).pin_memory()
+            peaks_h = torch.empty(B * 16, dtype=torch.uint8).pin_memory()
+            trig_h = torch.empty(cap * 16, dtype=torch.uint8).pin_memory()
 
-        def step_host():
-            ctx.set_psd(psd_h)
-            ctx.load_segment(smp_h)
-            return ctx.filter_bank_into(bank_h, wl.threshold, peaks_h, trig_h, cap)
+            def step_host():
+                ctx.set_psd(psd_h)
+                ctx.load_segment(smp_h)
+                return ctx.filter_bank_into(bank_h, wl.threshold, peaks_h, trig_h, cap)
 
-        for _ in range(Wm):
-            step_host()
-        barrier()
-        e_ms, (nf_h, rc_h) = timed(step_host, K)
-        barrier()
-        te = torch.tensor([e_ms], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e_value = B * world * K / (float(te.item()) * 1e-3)
-        h2d = psd_h.numel() * 8 + smp_h.numel() * 4 + bank_h.numel() * 8
-        d2h = B * 16 + min(nf_h, cap) * 16 + 4 + 4 + 4 + 8      # peaks, triggers, 3 status words, trigger count
-
-        peaks = np.frombuffer(peaks_h.numpy().tobytes(), dtype=cbmf.PEAK_DTYPE)
+            for _ in range(Wm):
+                step_host()
+            barrier()
+            e_ms, (nf_h, rc_h) = timed(step_host, K)
+            barrier()
+            out["e_ms_max"] = max_over_ranks(e_ms)
+            out["h2d"] = psd_h.numel() * 8 + smp_h.numel() * 4 + bank_h.numel() * 8
+            # peaks, kept triggers, the early template-status word (8 B) and the trigger count (8 B)
+            out["d2h"] = B * 16 + min(nf_h, cap) * 16 + 4 + 4 + 8 + 8
         ctx.close()
+    return out
+
+
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start the N ranks ourselves
+    (one process per GPU, rendezvous on 127.0.0.1) and pass rank 0's line through."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1006_4644_b200 import cbmf
+
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = make_workload(args.workload, world, rank)
+    B, n = wl.n_templates, wl.n
+    cap = args.trig_capacity
+    K, Wm = args.steps, args.warmup
+    m = measure(torch, dist, cbmf, wl, dev, local, world, K, Wm, cap, args)
+    ms_max = m["ms_max"]
+    value = B * world * K / (ms_max * 1e-3)
+    e_value = B * world * K / (m["e_ms_max"] * 1e-3)
+    fp32_meas = fp32_probe(local) if rank == 0 else (None, None)
+
+    # ---- sustained record: a few steps of configs[2] (65 536 templates, ~0.2 s per step): the state a
+    # 1-2 million-template bank (PAPER.md:27) runs in, with its own clocks
+    sustained = None
+    if args.workload == "cfg1" and not args.no_sustained:
+        wl2 = make_workload("cfg2", world, rank)
+        Ks = max(2, min(K, args.sustained_steps))
+        m2 = measure(torch, dist, cbmf, wl2, dev, local, world, Ks, 3, 1 << 20, args, with_e2e=False, with_passes=False)
+        lg1s, lg2s = m2["split"]
+        f1s, f2s = pass_flops(wl2.n, lg1s, lg2s, mean_band_bins(wl2))
+        v2 = wl2.n_templates * world * Ks / (m2["ms_max"] * 1e-3)
+        sustained = {
+            "workload": "cfg2", "templates_per_step_per_gpu": wl2.n_templates, "steps": Ks, "warmup": 3,
+            "value": v2, "unit": UNIT, "ms_per_step": m2["ms_max"] / Ks, "clocks": m2["clocks"],
+            "gpu_launches": int(m2["launches"]), "triggers_found": m2["nf"],
+            "whole_path": {"flops_per_template": f1s + f2s, "us_per_template": 1e3 * m2["ms_max"] / (wl2.n_templates * Ks),
+                           "frac_of_fp32_peak": (f1s + f2s) * v2 / world / 1e12 / FP32_PEAK_TFLOPS,
+                           "dense_equivalent_frac": (5.0 * wl2.n * (lg1s + lg2s) + 6.0 * wl2.n + 48.0 * (wl2.n / 2)) * v2 / world / 1e12 / FP32_PEAK_TFLOPS,
+                           "note": "frac_of_fp32_peak counts the generator on the in-band bins only (mean n_b/N = 0.10 in cfg2); "
+                                   "dense_equivalent_frac counts it on all N/2 bins (SURVEY.md §8(d))"},
+        }
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline numbers for the dominant pass
-    lg = int(math.log2(n))
-    lg1 = lg // 2
-    lg2 = lg - lg1
+    # ---- roofline numbers for the dominant pass (FFT split as the library chose it)
+    lg1, lg2 = m["split"]
     n_b = mean_band_bins(wl)
     f1, f2 = pass_flops(n, lg1, lg2, n_b)
+    p_ms, p_n = m["pass_alone"]
+    o_ms, o_n = m["pass_overlapped"]
     which = 0 if p_ms[0] >= p_ms[1] else 1
     avg_launch_ms = p_ms[which] / max(p_n[which], 1)
     tmpl_per_launch = B * K / max(p_n[which], 1)
@@ -343,27 +437,32 @@ def run_ours(args):
             peaks_file = json.load(fh)
     except Exception:
         pass
+    traffic, traffic_src = load_traffic(n)
+    tr_per_tmpl = None if traffic is None else traffic["dram_bytes_per_template"][which]
     roofline = {
         "bound": "alu", "kernel": ("p1_kernel (SPA generate + correlate + column FFT)",
                                    "p2_kernel (twiddle + row FFT + |z|^2 + arg-max/threshold)")[which],
         "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "peak_source": "148 SM x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md §6)",
         "peak_measured_tflops": {"ffma": fp32_meas[0], "ffma2_packed": fp32_meas[1],
-                                 "how": "cbmf_debug_fp32_peak: dependent FMA chains on every SM, CUDA events (cross-check, not the denominator)"},
-        "traffic": (NCU_DRAM_BYTES_PER_TEMPLATE_2P20[which] * tmpl_per_launch) if n == (1 << 20) else None,
-        "traffic_source": "ncu --set full, profiles/r1g_ncu_full_p1_p2.md (per template x templates per launch)",
+                                 "how": "bench_fp32_probe.cu: dependent FMA chains on every SM, CUDA events (cross-check, not the denominator)"},
+        "traffic": None if tr_per_tmpl is None else tr_per_tmpl * tmpl_per_launch,
+        "traffic_source": traffic_src,
         "algorithmic_bytes_per_launch": 8.0 * n * tmpl_per_launch,
         "flops_per_launch": flops_launch, "avg_launch_ms": avg_launch_ms, "templates_per_launch": tmpl_per_launch,
         "pass_ms_per_step": [p_ms[0] / K, p_ms[1] / K],
-        "note": ("per-launch figures are taken with every launch ALONE on the GPU (one stream); pass 1 is launched with one "
-                 "block per SM so that pass-2 blocks of the other launch pairs share its SMs in the timed schedule, where "
-                 "the two passes overlap: whole_path gives the fraction of the FP32 peak reached by the whole step"),
+        "pass_launch_ms_overlapped": [o_ms[0] / max(o_n[0], 1), o_ms[1] / max(o_n[1], 1)],
+        "note": ("`achieved` and pass_ms_per_step are taken with every launch ALONE on the GPU (one stream); pass 1 is launched "
+                 "with few long-lived blocks so that pass-2 blocks of the other launch pairs share its SMs in the timed "
+                 "schedule, where the passes overlap (pass_launch_ms_overlapped: mean duration of a launch in that schedule, "
+                 "events on its own stream); whole_path gives the fraction of the FP32 peak reached by the whole step"),
         "whole_path": {
             "flops_per_template": f1 + f2, "us_per_template": 1e3 * ms_max / (B * K),
-            "achieved_tflops": (f1 + f2) * B * world * K / (ms_max * 1e-3) / 1e12 / world,
+            "achieved_tflops": (f1 + f2) * B * K / (ms_max * 1e-3) / 1e12,
             "frac_of_fp32_peak": (f1 + f2) * B * K / (ms_max * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
             "inter_pass_bytes_per_template": 16 * n,
             "hbm_gbs_measured_peak": peaks_file.get("hbm_gbs"),
+            "hbm_frac_if_y_spills": (16.0 * n * value / world / 1e9 / peaks_file["hbm_gbs"]) if peaks_file.get("hbm_gbs") else None,
         },
     }
 
@@ -382,16 +481,18 @@ def run_ours(args):
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name, "n": n, "fs_hz": wl.fs, "f_low_hz": wl.f_low,
-                   "templates_per_step_per_gpu": B, "threshold": wl.threshold, "sub_batch": sub, "streams": ctx_streams,
+                   "templates_per_step_per_gpu": B, "threshold": wl.threshold, "sub_batch": m["sub_batch"],
+                   "streams": m["streams"], "fft_split_log2": [lg1, lg2],
                    "l2": "flushed (256 MiB fill) before every timed step",
                    "step": "set_psd + load_segment + filter_bank (S0-S8)",
                    "parallelism": f"bank sharded over {world} GPU(s), segment replicated"},
         "segment_seconds_per_wall_second": (n / wl.fs) / (ms_max / K * 1e-3),
-        "triggers_found": int(nf), "peak_snr_max": float(peaks["snr_max"].max()),
-        "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
-        "gpu_launches": int(launches),
-        "clocks": clk.summary(),
+        "triggers_found": m["nf"], "peak_snr_max": float(m["peaks"]["snr_max"].max()),
+        "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": int(m["h2d"]), "d2h_bytes_per_step": int(m["d2h"])},
+        "gpu_launches": int(m["launches"]),
+        "clocks": m["clocks"],
         "roofline": roofline,
+        "sustained": sustained,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line))
@@ -411,6 +512,8 @@ def main():
     ap.add_argument("--streams", type=int, default=0, help="launch pairs in flight (0 = library default)")
     ap.add_argument("--trig-capacity", type=int, default=1 << 16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the cfg2 `sustained` record of the default run")
+    ap.add_argument("--sustained-steps", type=int, default=3)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -63,7 +63,11 @@ typedef struct { int32_t template_idx; int32_t sample_idx; float snr; float phas
 /* Create a context for segments of n samples (n a power of two, 2^12 <= n <= 2^24) at
  * sample rate fs_hz, with lower cutoff f_low_hz (0 < f_low < fs/2), on CUDA device
  * `device`.  cuda_stream is a cudaStream_t (e.g. torch's current stream) or NULL for the
- * default stream.  Errors: EINVAL, ECUDA, ENOMEM. */
+ * default stream.  Contexts are independent, also across devices of one process: all
+ * per-device state (kernel attributes, SM count) lives in the context, and the library
+ * reads no environment variable.  The floor 2^12 (SURVEY.md §8(b) proposes 2^10) is that of
+ * the two-pass FFT split, N1, N2 >= 64; the paper's segments are 2^18..2^21
+ * (PAPER.md:249-254).  Errors: EINVAL, ECUDA, ENOMEM. */
 int cbmf_create(cbmf_ctx **out, int device, int64_t n, double fs_hz, double f_low_hz,
                 void *cuda_stream);
 int cbmf_destroy(cbmf_ctx *ctx);
@@ -90,12 +94,19 @@ int cbmf_load_segment_dev(cbmf_ctx *ctx, const float *samples_dev, int64_t n_sam
  *   trig_out[trig_capacity]  triggers sorted by (template_idx, sample_idx); may be NULL
  *                            with capacity 0 (triggers are still counted).
  *   n_trig_found             total number of samples above threshold over the whole bank;
- *                            if it exceeds trig_capacity the first trig_capacity entries
- *                            written are an unspecified subset and the call returns
- *                            CBMF_WTRUNC.
+ *                            if it exceeds trig_capacity the list is TRUNCATED: trig_out holds
+ *                            the first trig_capacity triggers in (template_idx, sample_idx)
+ *                            order (what the full sorted list would start with) and the call
+ *                            returns CBMF_WTRUNC.  A truncated call may filter the leading part
+ *                            of the bank a second time to collect them.
+ * The trigger test is |z[j]|^2 > (snr_threshold * sigma)^2 evaluated in fp32 (monotone in rho,
+ * SURVEY.md reading A13); it is authoritative: the reported snr = sqrt(|z|^2) / sigma is rounded
+ * separately and may differ from the threshold by one unit in the last place either way.
  * snr_threshold >= 0.  n_templates may be 0.  ESTATE before PSD and segment are set;
  * EINVAL on a non-positive or non-finite mass, on a template whose phase exceeds 2^19 cycles
- * inside the band (total mass far below 0.3 Msun at f_low = 10 Hz), or a negative / NaN threshold. */
+ * inside the band (total mass far below 0.3 Msun at f_low = 10 Hz), or a negative / NaN threshold.
+ * The masses are checked on the device BEFORE any filtering: a bank with an invalid template
+ * fails at once, nothing is written, and cbmf_last_bad_template() names the first offender. */
 int cbmf_filter_bank(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_templates,
                      float snr_threshold, cbmf_peak *peaks_out,
                      cbmf_trigger *trig_out, int64_t trig_capacity, int64_t *n_trig_found);
@@ -105,6 +116,9 @@ int cbmf_filter_bank_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_t n
                          float snr_threshold, cbmf_peak *peaks_out_dev,
                          cbmf_trigger *trig_out_dev, int64_t trig_capacity,
                          int64_t *n_trig_found);
+/* Bank index of the first invalid template of the last cbmf_filter_bank* call that returned
+ * EINVAL for that reason, else -1. */
+int64_t cbmf_last_bad_template(const cbmf_ctx *ctx);
 
 /* ---- diagnostics: used by the parity tests and the kernel sweep, never by filter_bank ---- */
 
@@ -125,15 +139,6 @@ int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_
  * (n/2 complex floats, interleaved). */
 int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);
 int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
-/* FP32 pipe probe for the roofline denominator: dependent-chain FMA kernels on every
- * SM, timed with CUDA events on the context's stream; TFLOP/s of scalar FFMA and of packed FFMA2
- * (fma.rn.f32x2).  Both should read close to SMs x 128 lanes x 2 flop x SM clock. */
-int cbmf_debug_fp32_peak(cbmf_ctx *ctx, double *tflops_ffma, double *tflops_ffma2);
-/* Block statistics of the last fused launch (cbmf_set_fused): per block six 64-bit values, role
- * (1 = pass 1, 2 = pass 2), SM cycles spent waiting (ring slot / template not ready), cycles
- * working, steps done (templates / items), total cycles, column tile (-1 for pass 2).  out: host,
- * 6 * max_blocks values; *n_blocks = blocks written.  ESTATE before the first fused launch. */
-int cbmf_debug_fused_stats(cbmf_ctx *ctx, uint64_t *out, int64_t max_blocks, int64_t *n_blocks);
 
 /* ---- tuning ---- */
 /* Templates per launch pair (pass 1 + pass 2).  Default: 512 MiB of inter-pass buffer
@@ -148,27 +153,21 @@ int cbmf_get_sub_batch(const cbmf_ctx *ctx);
  * 1 <= launch_pairs_in_flight <= 8. */
 int cbmf_set_streams(cbmf_ctx *ctx, int launch_pairs_in_flight);
 int cbmf_get_streams(const cbmf_ctx *ctx);
-/* Fused persistent path (csrc/fused.cuh): the whole bank in ONE cooperative launch with two
- * blocks per SM, each with one role for the whole bank -- one pass-1 block per column tile (w
- * staged once) and pass-2 blocks that claim rows from a queue; the inter-pass buffer is a ring of
- * ring_templates * 8 n bytes.  Available for n = 2^20 on a device with at least n2/8 = 128 SMs
- * and cooperative launch.  Off by default (the launch pairs above are faster at present,
- * DESIGN.md §7); results agree with them to fp32 rounding.  ring_templates: 2..64, or 0 to keep
- * the current value (default 32).  EINVAL if on = 1 where the fused path is not available.
- * cbmf_get_fused returns 1 / 0 (in use or not) and stores the ring size. */
-int cbmf_set_fused(cbmf_ctx *ctx, int on, int ring_templates);
-int cbmf_get_fused(const cbmf_ctx *ctx, int *ring_templates);
-
 /* ---- introspection ---- */
+/* The FFT split chosen at create: n = 2^log2_n1 * 2^log2_n2, pass 1 = column FFTs of 2^log2_n1
+ * points, pass 2 = row FFTs of 2^log2_n2 points (bench.py's per-pass flop counts). */
+int cbmf_get_split(const cbmf_ctx *ctx, int *log2_n1, int *log2_n2);
 /* Kernels launched by this context since creation (bench.py's gpu_launches). */
 int64_t cbmf_launch_count(const cbmf_ctx *ctx);
 /* Device time (ms, CUDA events on the context's stream) and launch count of the two FFT-pass
  * kernels inside the last cbmf_filter_bank* call; used for the roofline line of bench.py.
- * which = 0: pass 1 (generate + column FFT), 1: pass 2 (row FFT + epilogue).  On the fused
- * path which = 0 is the one bank_kernel launch (both passes) and which = 1 reports nothing. */
+ * which = 0: pass 1 (generate + column FFT), 1: pass 2 (row FFT + epilogue). */
 int cbmf_last_pass_time(const cbmf_ctx *ctx, int which, double *ms_out, int64_t *launches_out);
-/* Enable (1) / disable (0) the per-pass event timing above (default off: no events recorded). */
-int cbmf_set_profiling(cbmf_ctx *ctx, int on);
+/* Per-pass event timing above: 0 off (default, no events recorded); 1 every pass launch ALONE, all
+ * on the context's stream; 2 the real schedule (launch pairs on the internal streams), every launch
+ * bracketed by events on its own stream, so a duration includes the time the kernel shares its SMs
+ * with the launches of the other pairs.  EINVAL for any other value. */
+int cbmf_set_profiling(cbmf_ctx *ctx, int mode);
 const char *cbmf_strerror(int rc);
 const char *cbmf_last_cuda_error(const cbmf_ctx *ctx);
 const char *cbmf_version(void);

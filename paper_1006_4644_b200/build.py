@@ -7,6 +7,7 @@ with the gpurun snapshot; on a box that has nvcc it is rebuilt when a source is 
 """
 from __future__ import annotations
 
+import glob
 import os
 import shutil
 import subprocess
@@ -17,8 +18,7 @@ _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 LIB = os.path.join(_PKG, "libcbmf.so")
 SOURCES = [os.path.join(CSRC, "cbmf.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "fft_regs.cuh"),
-                  os.path.join(_ROOT, "include", "cbmf.h")]
+DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(_ROOT, "include", "cbmf.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -54,14 +54,12 @@ def lib() -> C.CDLL:
         "cbmf_debug_generate_dev": (C.c_int, [vp, vp, i64, vp]),
         "cbmf_debug_get_prefix": (C.c_int, [vp, vp]),
         "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
-        "cbmf_debug_fused_stats": (C.c_int, [vp, vp, i64, C.POINTER(i64)]),
-        "cbmf_debug_fp32_peak": (C.c_int, [vp, C.POINTER(dbl), C.POINTER(dbl)]),
         "cbmf_set_sub_batch": (C.c_int, [vp, C.c_int]),
         "cbmf_get_sub_batch": (C.c_int, [vp]),
         "cbmf_set_streams": (C.c_int, [vp, C.c_int]),
         "cbmf_get_streams": (C.c_int, [vp]),
-        "cbmf_set_fused": (C.c_int, [vp, C.c_int, C.c_int]),
-        "cbmf_get_fused": (C.c_int, [vp, C.POINTER(C.c_int)]),
+        "cbmf_get_split": (C.c_int, [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+        "cbmf_last_bad_template": (i64, [vp]),
         "cbmf_launch_count": (i64, [vp]),
         "cbmf_last_pass_time": (C.c_int, [vp, C.c_int, C.POINTER(dbl), C.POINTER(i64)]),
         "cbmf_set_profiling": (C.c_int, [vp, C.c_int]),
@@ -79,7 +77,8 @@ def lib() -> C.CDLL:
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
-           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_debug_fused_stats cbmf_debug_fp32_peak cbmf_set_sub_batch cbmf_get_sub_batch cbmf_set_streams cbmf_get_streams cbmf_set_fused cbmf_get_fused "
+           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch "
+           "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
            "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_strerror "
            "cbmf_last_cuda_error cbmf_version").split()
 
@@ -95,19 +94,41 @@ def _is_tensor(a) -> bool:
     return hasattr(a, "data_ptr") and hasattr(a, "is_cuda")
 
 
-def _ptr(a, dtype=None):
-    """-> (address, on_device).  numpy arrays and tensors must be contiguous (and of `dtype`)."""
+_TORCH_NAME = {"float64": "torch.float64", "float32": "torch.float32", "uint8": "torch.uint8",
+               "complex64": "torch.complex64"}
+
+
+def _ptr(a, dtype=None, device=None, itemsize=None):
+    """-> (address, on_device).  numpy arrays and tensors must be contiguous and of `dtype` (a numpy dtype
+    name; for output records `itemsize` = 16 also admits raw uint8 buffers); a CUDA tensor must live on
+    device index `device`.  A wrong dtype would be misread by the kernels, so it is an error here."""
     if a is None:
         return None, False
     if _is_tensor(a):
         if not a.is_contiguous():
             raise ValueError("tensor must be contiguous")
+        if dtype is not None:
+            ok = str(a.dtype) == _TORCH_NAME.get(dtype, "torch." + dtype)
+            if not ok and itemsize is not None:
+                ok = str(a.dtype) == "torch.uint8" and a.numel() % itemsize == 0
+            if not ok:
+                raise ValueError(f"expected a {dtype} tensor, got {a.dtype}")
+        if a.is_cuda and device is not None and a.device.index != device:
+            raise ValueError(f"tensor lives on cuda:{a.device.index}, the context on cuda:{device}")
         return a.data_ptr(), bool(a.is_cuda)
     if not isinstance(a, np.ndarray) or not a.flags["C_CONTIGUOUS"]:
         raise ValueError("expected a C-contiguous numpy array or a torch tensor")
-    if dtype is not None and a.dtype != dtype:
-        raise ValueError(f"expected dtype {dtype}, got {a.dtype}")
+    if dtype is not None:
+        ok = a.dtype == np.dtype(dtype) if dtype in ("float64", "float32", "uint8", "complex64") else a.dtype == dtype
+        if not ok and itemsize is not None:
+            ok = a.dtype.itemsize == itemsize or (a.dtype == np.uint8 and a.size % itemsize == 0)
+        if not ok:
+            raise ValueError(f"expected dtype {dtype}, got {a.dtype}")
     return a.ctypes.data, False
+
+
+def _nbytes(a) -> int:
+    return int(a.numel() * a.element_size()) if _is_tensor(a) else int(a.nbytes)
 
 
 class Context:
@@ -142,14 +163,19 @@ class Context:
 
     def _check(self, rc: int, what: str) -> int:
         if rc < 0:
-            raise CbmfError(rc, what, lib().cbmf_last_cuda_error(self._h).decode() if rc == ECUDA else "")
+            detail = lib().cbmf_last_cuda_error(self._h).decode() if rc == ECUDA else ""
+            if rc == EINVAL and what == "cbmf_filter_bank":
+                bad = int(lib().cbmf_last_bad_template(self._h))
+                if bad >= 0:
+                    detail = f"first invalid template: index {bad}"
+            raise CbmfError(rc, what, detail)
         return rc
 
     # -- the three calls of the path
     def set_psd(self, psd):
         if isinstance(psd, np.ndarray):
             psd = np.ascontiguousarray(psd, dtype=np.float64)
-        p, dev = _ptr(psd)
+        p, dev = _ptr(psd, "float64", self.device)
         n_bins = int(psd.numel() if _is_tensor(psd) else psd.size)
         f = lib().cbmf_set_psd_dev if dev else lib().cbmf_set_psd
         self._check(f(self._h, p, n_bins), "cbmf_set_psd")
@@ -157,7 +183,7 @@ class Context:
     def load_segment(self, samples):
         if isinstance(samples, np.ndarray):
             samples = np.ascontiguousarray(samples, dtype=np.float32)
-        p, dev = _ptr(samples)
+        p, dev = _ptr(samples, "float32", self.device)
         n = int(samples.numel() if _is_tensor(samples) else samples.size)
         f = lib().cbmf_load_segment_dev if dev else lib().cbmf_load_segment
         self._check(f(self._h, p, n), "cbmf_load_segment")
@@ -179,12 +205,16 @@ class Context:
     def filter_bank_into(self, bank, snr_threshold: float, peaks_out, trig_out, trig_capacity: int):
         """Caller-owned buffers (all host -- numpy / pinned tensors -- or all CUDA tensors):
         bank float64 [B,2], peaks_out 16 B/template, trig_out 16 B/entry.  -> (n_found, rc)."""
-        pb, dev = _ptr(bank)
-        pp, devp = _ptr(peaks_out)
-        pt, devt = _ptr(trig_out)
+        pb, dev = _ptr(bank, "float64", self.device)
+        pp, devp = _ptr(peaks_out, "peak records", self.device, itemsize=16)
+        pt, devt = _ptr(trig_out, "trigger records", self.device, itemsize=16)
         if devp != dev or (trig_out is not None and devt != dev):
             raise ValueError("bank, peaks_out and trig_out must all be host or all be device arrays")
         nt = int((bank.numel() if _is_tensor(bank) else bank.size) // 2)
+        if _nbytes(peaks_out) < 16 * nt:
+            raise ValueError("peaks_out is smaller than 16 bytes per template")
+        if trig_out is not None and _nbytes(trig_out) < 16 * int(trig_capacity):
+            raise ValueError("trig_out is smaller than 16 bytes per trigger of trig_capacity")
         nf = C.c_int64(0)
         f = lib().cbmf_filter_bank_dev if dev else lib().cbmf_filter_bank
         rc = f(self._h, pb, nt, float(snr_threshold), pp, pt, int(trig_capacity), C.byref(nf))
@@ -237,19 +267,6 @@ class Context:
         self._check(lib().cbmf_debug_get_weights(self._h, w.ctypes.data), "cbmf_debug_get_weights")
         return w
 
-    def debug_fused_stats(self) -> np.ndarray:
-        """[blocks][6] uint64: role (1 / 2), cycles waiting, cycles working, steps, total cycles, tile."""
-        out = np.zeros((1024, 6), dtype=np.uint64)
-        nb = i64_t(0)
-        self._check(lib().cbmf_debug_fused_stats(self._h, out.ctypes.data, 1024, C.byref(nb)), "cbmf_debug_fused_stats")
-        return out[: int(nb.value)]
-
-    def debug_fp32_peak(self):
-        """-> (TFLOP/s of scalar FFMA, TFLOP/s of packed FFMA2) measured on this device."""
-        a, b = C.c_double(0), C.c_double(0)
-        self._check(lib().cbmf_debug_fp32_peak(self._h, C.byref(a), C.byref(b)), "cbmf_debug_fp32_peak")
-        return float(a.value), float(b.value)
-
     # -- tuning / introspection
     def set_sub_batch(self, k: int):
         self._check(lib().cbmf_set_sub_batch(self._h, int(k)), "cbmf_set_sub_batch")
@@ -263,20 +280,21 @@ class Context:
     def get_streams(self) -> int:
         return int(lib().cbmf_get_streams(self._h))
 
-    def set_fused(self, on: bool, ring: int = 0):
-        self._check(lib().cbmf_set_fused(self._h, int(bool(on)), int(ring)), "cbmf_set_fused")
+    def get_split(self):
+        """-> (log2 N1, log2 N2): pass 1 = column FFTs of N1 points, pass 2 = row FFTs of N2 points."""
+        a, b = C.c_int(0), C.c_int(0)
+        self._check(lib().cbmf_get_split(self._h, C.byref(a), C.byref(b)), "cbmf_get_split")
+        return int(a.value), int(b.value)
 
-    def get_fused(self):
-        """-> (in use, ring size in templates)"""
-        ring = C.c_int(0)
-        r = int(lib().cbmf_get_fused(self._h, C.byref(ring)))
-        return bool(r > 0), int(ring.value)
+    def last_bad_template(self) -> int:
+        return int(lib().cbmf_last_bad_template(self._h))
 
     def launch_count(self) -> int:
         return int(lib().cbmf_launch_count(self._h))
 
-    def set_profiling(self, on: bool):
-        self._check(lib().cbmf_set_profiling(self._h, int(bool(on))), "cbmf_set_profiling")
+    def set_profiling(self, mode: int):
+        """0 off, 1 every pass launch alone on the context's stream, 2 in the real overlapped schedule."""
+        self._check(lib().cbmf_set_profiling(self._h, int(mode)), "cbmf_set_profiling")
 
     def last_pass_time(self, which: int):
         ms, nl = C.c_double(0), C.c_int64(0)

@@ -6,13 +6,13 @@
 // of kernels.cuh.  There is no CPU fallback and nothing here touches oracle/.
 #include "../../include/cbmf.h"
 #include "kernels.cuh"
-#include "fused.cuh"
 
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <unordered_set>
 #include <vector>
 
 using namespace cbmf;
@@ -52,17 +52,16 @@ struct cbmf_ctx {
     TrigOut* d_trig = nullptr;    int64_t trig_cap = 0;       // entries (power of two)
     void* d_scratch = nullptr;    size_t scratch_bytes = 0;   // debug paths / load_segment
 
-    // fused persistent launch (fused.cuh): one cooperative launch per filter_bank call
-    bool fused_ok = false;                 // this N and this device can run it
-    bool fused = false;                    // use it
-    int ring = 32;                         // templates of Y in flight
-    int n_sm = 0;
-    unsigned int* d_sync = nullptr;  int64_t sync_cap = 0;        // [3 * cap + 3 + n_sm] counters, see filter_bank_impl
-    unsigned long long* d_fkey = nullptr;  int64_t fkey_cap = 0;  // [n_templates] arg-max keys
-    unsigned long long* d_fstats = nullptr;                       // [n_sm][6] scheduler statistics of the last fused launch
+    int n_sm = 0;                          // SMs of this context's device
+    // kernels whose dynamic shared-memory opt-in has been set on THIS device (cudaFuncSetAttribute is per
+    // device, so the cache belongs to the context, not to the process)
+    std::unordered_set<const void*> attr_set;
+    unsigned int* d_tcount = nullptr;  int64_t tcount_cap = 0;    // [n_templates] triggers per template
+    long long* d_bad = nullptr;            // [1] index of the first invalid template of the last bank, or LLONG_MAX
+    int64_t last_bad = -1;
 
     int64_t launches = 0;
-    bool profiling = false;
+    int profiling = 0;                     // 0 off, 1 every launch alone on the context's stream, 2 in the real schedule
     std::vector<cudaEvent_t> ev[2];        // per pass: start/stop pairs of the last filter call
     size_t ev_used[2] = {0, 0};
     double last_ms[2] = {0, 0};
@@ -129,38 +128,37 @@ bool p1_series_ok(int k_lo, int l2, int tile_cols)
     return k1_lo >= 1 && (double)(tile_cols - 1) <= 2e-3 * (double)k1_lo * (double)l2;
 }
 
-int p1_groups(int n_tiles, int batch)
+int p1_groups(int n_sm, int n_tiles, int batch)
 {
-    static int n_sm = 0;
-    if (n_sm == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) {
-            cudaGetLastError();
-            n_sm = 148;
-        }
-    }
     int g = n_sm / n_tiles;
     if (g < 1) g = 1;
     if (g > batch) g = batch;
     return g;
 }
 
-template <int L1, int L2, int MODE>
-cudaError_t launch_p1_L(cudaStream_t s, P1Args a, int batch)
+// Opt a kernel in to `bytes` of dynamic shared memory on the context's device, once per context.
+template <typename K>
+cudaError_t ensure_smem_attr(cbmf_ctx* c, K kernel, size_t bytes)
 {
-    static bool attr_done = false;
+    const void* key = reinterpret_cast<const void*>(kernel);
+    if (c->attr_set.count(key)) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) c->attr_set.insert(key);
+    return e;
+}
+
+template <int L1, int L2, int MODE>
+cudaError_t launch_p1_L(cbmf_ctx* c, cudaStream_t s, P1Args a, int batch)
+{
     const size_t smem = p1_smem_bytes<L1, MODE>();
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(p1_kernel<L1, L2, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    cudaError_t e = ensure_smem_attr(c, p1_kernel<L1, L2, MODE>, smem);
+    if (e != cudaSuccess) return e;
     a.batch = batch;
     if (MODE == LOAD_GEN) {
         // series for k^{-1/3} (spa_correlate): valid where (columns of a tile - 1) / (first in-band bin of a row) <= 2e-3
         a.use_series = p1_series_ok(a.use_series, L2, Cfg<L1>::C) ? 1 : 0;    // the caller passes k_lo in use_series
     }
-    const int groups = (MODE == LOAD_GEN) ? p1_groups(L2 / Cfg<L1>::C, batch) : batch;
+    const int groups = (MODE == LOAD_GEN) ? p1_groups(c->n_sm, L2 / Cfg<L1>::C, batch) : batch;
     dim3 grid(L2 / Cfg<L1>::C, groups);
     p1_kernel<L1, L2, MODE><<<grid, Cfg<L1>::NT1, smem, s>>>(a);
     return cudaGetLastError();
@@ -170,15 +168,11 @@ template <int L1, int L2, int MODE>
 constexpr int p2_items() { return L1 / (Cfg<L2>::ROWS * (MODE == EPI_MAX ? p2_rpw<L1, L2>() : 1)); }
 
 template <int L1, int L2, int MODE>
-cudaError_t launch_p2_L(cudaStream_t s, const P2Args& a, int batch)
+cudaError_t launch_p2_L(cbmf_ctx* c, cudaStream_t s, const P2Args& a, int batch)
 {
-    static bool attr_done = false;
     const size_t smem = sizeof(c2) * (size_t)p2_row_stride<L2>() * Cfg<L2>::ROWS;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(p2_kernel<L1, L2, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    cudaError_t e = ensure_smem_attr(c, p2_kernel<L1, L2, MODE>, smem);
+    if (e != cudaSuccess) return e;
     dim3 grid(p2_items<L1, L2, MODE>(), batch);
     p2_kernel<L1, L2, MODE><<<grid, Cfg<L2>::NT2, smem, s>>>(a);
     return cudaGetLastError();
@@ -204,14 +198,14 @@ cudaError_t launch_p2_L(cudaStream_t s, const P2Args& a, int batch)
     }
 
 template <int MODE>
-cudaError_t launch_p1(int lg1, int lg2, cudaStream_t s, const P1Args& a, int batch)
+cudaError_t launch_p1(cbmf_ctx* c, cudaStream_t s, const P1Args& a, int batch)
 {
-    CBMF_DISPATCH(lg1, lg2, (launch_p1_L<L1, L2, MODE>(s, a, batch)))
+    CBMF_DISPATCH(c->lg1, c->lg2, (launch_p1_L<L1, L2, MODE>(c, s, a, batch)))
 }
 template <int MODE>
-cudaError_t launch_p2(int lg1, int lg2, cudaStream_t s, const P2Args& a, int batch)
+cudaError_t launch_p2(cbmf_ctx* c, cudaStream_t s, const P2Args& a, int batch)
 {
-    CBMF_DISPATCH(lg1, lg2, (launch_p2_L<L1, L2, MODE>(s, a, batch)))
+    CBMF_DISPATCH(c->lg1, c->lg2, (launch_p2_L<L1, L2, MODE>(c, s, a, batch)))
 }
 
 // candidate slots per template of the arg-max pass: one per (row j1, thread of the row group) = N / E2
@@ -224,20 +218,20 @@ size_t cand_per_template(const cbmf_ctx* c)
 }
 
 // pass-timing events (cbmf_set_profiling): one start/stop pair per launch
-int ev_begin(cbmf_ctx* c, int which)
+int ev_begin(cbmf_ctx* c, int which, cudaStream_t st)
 {
     if (!c->profiling) return CBMF_OK;
     auto& v = c->ev[which];
     if (c->ev_used[which] + 2 > v.size()) {
         for (int i = 0; i < 2; ++i) { cudaEvent_t e; CU(cudaEventCreate(&e)); v.push_back(e); }
     }
-    CU(cudaEventRecord(v[c->ev_used[which]], c->stream));
+    CU(cudaEventRecord(v[c->ev_used[which]], st));
     return CBMF_OK;
 }
-int ev_end(cbmf_ctx* c, int which)
+int ev_end(cbmf_ctx* c, int which, cudaStream_t st)
 {
     if (!c->profiling) return CBMF_OK;
-    CU(cudaEventRecord(c->ev[which][c->ev_used[which] + 1], c->stream));
+    CU(cudaEventRecord(c->ev[which][c->ev_used[which] + 1], st));
     c->ev_used[which] += 2;
     return CBMF_OK;
 }
@@ -286,43 +280,6 @@ int alloc_pipeline(cbmf_ctx* c, int sb, int ns)
     return CBMF_OK;
 }
 
-// ---------------------------------------------------------------- fused persistent launch
-template <int L1, int L2>
-cudaError_t fused_query(int* blocks_per_sm)
-{
-    using F = FusedCfg<L1, L2>;
-    cudaError_t e = cudaFuncSetAttribute(bank_kernel<L1, L2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, bank_kernel<L1, L2>, F::NT, F::SMEM_BYTES);
-}
-template <int L1, int L2>
-cudaError_t fused_launch(cudaStream_t s, int grid, FusedArgs a)
-{
-    using F = FusedCfg<L1, L2>;
-    void* params[] = {(void*)&a};
-    return cudaLaunchCooperativeKernel((const void*)bank_kernel<L1, L2>, dim3((unsigned)grid), dim3(F::NT), params,
-                                       F::SMEM_BYTES, s);
-}
-// Sizes for which bank_kernel is instantiated: (lg1, lg2) -> tiles, or 0.
-int fused_tiles(int lg1, int lg2)
-{
-    if (lg1 == 10 && lg2 == 10) return FusedCfg<1024, 1024>::NTILES;
-    return 0;
-}
-bool fused_probe(cbmf_ctx* c)
-{
-    int coop = 0;
-    if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device) != cudaSuccess || !coop) { cudaGetLastError(); return false; }
-    if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { cudaGetLastError(); return false; }
-    const int tiles = fused_tiles(c->lg1, c->lg2);
-    if (tiles == 0 || c->n_sm < tiles) return false;     // one P1 block per SM, one SM per tile
-    int per_sm = 0;
-    cudaError_t e = cudaErrorInvalidValue;
-    if (c->lg1 == 10 && c->lg2 == 10) e = fused_query<1024, 1024>(&per_sm);
-    if (e != cudaSuccess) { cudaGetLastError(); return false; }
-    return per_sm >= 2;                                   // a P1 and a P2 block on every SM
-}
-
 }  // namespace
 
 // ======================================================================= create / destroy
@@ -334,7 +291,7 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_bsum); cudaFree(c->d_w);
     cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key); cudaFree(c->d_err); cudaFree(c->d_u);
     cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
-    cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_sync); cudaFree(c->d_fkey); cudaFree(c->d_fstats);
+    cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_tcount); cudaFree(c->d_bad);
     for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
     for (int i = 0; i < CBMF_MAX_STREAMS; ++i) {
         if (c->aux[i]) { cudaStreamSynchronize(c->aux[i]); cudaStreamDestroy(c->aux[i]); }
@@ -351,6 +308,7 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
 {
     if (!out) return CBMF_EINVAL;
     *out = nullptr;
+    // 2^12 <= n: the two-pass split needs N1, N2 >= 64 (DESIGN.md §3 records the floor against SURVEY.md §8(b)'s 2^10)
     if (n < (int64_t(1) << 12) || n > (int64_t(1) << 24) || (n & (n - 1)) != 0) return CBMF_EINVAL;
     if (!(fs_hz > 0) || !std::isfinite(fs_hz)) return CBMF_EINVAL;
     if (!(f_low_hz > 0) || !(f_low_hz < 0.5 * fs_hz)) return CBMF_EINVAL;
@@ -379,15 +337,7 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     int64_t sb = (int64_t(512) << 20) / (8 * n);
     if (sb < 1) sb = 1;
     if (sb > 256) sb = 256;
-    if (const char* e = getenv("CBMF_SUB_BATCH")) {
-        const long v = strtol(e, nullptr, 10);
-        if (v >= 1 && v <= 4096) sb = v;
-    }
-    int ns = 4;
-    if (const char* e = getenv("CBMF_STREAMS")) {
-        const long v = strtol(e, nullptr, 10);
-        if (v >= 1 && v <= CBMF_MAX_STREAMS) ns = (int)v;
-    }
+    const int ns = 4;                      // launch pairs in flight (cbmf_set_streams)
     c->sub_batch = (int)sb;
     c->n_streams = ns;
 
@@ -404,6 +354,8 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     CUF(cudaMalloc(&c->d_u, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_err, sizeof(int)));
     CUF(cudaMalloc(&c->d_cursor, sizeof(unsigned long long)));
+    CUF(cudaMalloc(&c->d_bad, sizeof(long long)));
+    CUF(cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, device));
     CUF(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
     rcbrt_table_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(c->d_u, (int)nh);
     CUF(cudaGetLastError());
@@ -411,13 +363,6 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     CUF(cudaStreamSynchronize(c->stream));
 #undef CUF
     { const int rc = alloc_pipeline(c, c->sub_batch, c->n_streams); if (rc) return fail(rc); }
-    c->fused_ok = fused_probe(c);
-    c->fused = false;                      // measured slower than the launch pairs so far
-    if (const char* e = getenv("CBMF_FUSED")) c->fused = c->fused_ok && (strtol(e, nullptr, 10) != 0);
-    if (const char* e = getenv("CBMF_RING")) {
-        const long v = strtol(e, nullptr, 10);
-        if (v >= 2 && v <= 64) c->ring = (int)v;
-    }
     *out = c;
     return CBMF_OK;
 }
@@ -444,24 +389,17 @@ extern "C" int cbmf_set_streams(cbmf_ctx* c, int launch_pairs_in_flight)
 
 extern "C" int cbmf_get_streams(const cbmf_ctx* c) { return c ? c->n_streams : CBMF_EINVAL; }
 
-extern "C" int cbmf_set_fused(cbmf_ctx* c, int on, int ring_templates)
+extern "C" int cbmf_get_sub_batch(const cbmf_ctx* c) { return c ? c->sub_batch : CBMF_EINVAL; }
+
+extern "C" int cbmf_get_split(const cbmf_ctx* c, int* log2_n1, int* log2_n2)
 {
     if (!c) return CBMF_EINVAL;
-    if (ring_templates != 0 && (ring_templates < 2 || ring_templates > 64)) return CBMF_EINVAL;
-    if (on && !c->fused_ok) return CBMF_EINVAL;
-    c->fused = (on != 0);
-    if (ring_templates) c->ring = ring_templates;
+    if (log2_n1) *log2_n1 = c->lg1;
+    if (log2_n2) *log2_n2 = c->lg2;
     return CBMF_OK;
 }
 
-extern "C" int cbmf_get_fused(const cbmf_ctx* c, int* ring_templates)
-{
-    if (!c) return CBMF_EINVAL;
-    if (ring_templates) *ring_templates = c->ring;
-    return c->fused ? 1 : 0;
-}
-
-extern "C" int cbmf_get_sub_batch(const cbmf_ctx* c) { return c ? c->sub_batch : CBMF_EINVAL; }
+extern "C" int64_t cbmf_last_bad_template(const cbmf_ctx* c) { return c ? c->last_bad : -1; }
 
 // ======================================================================= S0: set_psd
 static int set_psd_impl(cbmf_ctx* c, const double* psd_dev)
@@ -518,10 +456,10 @@ static int load_segment_impl(cbmf_ctx* c, const float* samples_dev)
     CU(cudaMemcpyAsync(c->d_coef, &tc, sizeof(tc), cudaMemcpyHostToDevice, c->stream));
     P1Args a1; memset(&a1, 0, sizeof(a1));
     a1.in_r = samples_dev; a1.Y = c->d_Y; a1.err_flag = c->d_err;
-    CU(launch_p1<LOAD_REAL>(c->lg1, c->lg2, c->stream, a1, 1));
+    CU(launch_p1<LOAD_REAL>(c, c->stream, a1, 1));
     P2Args a2; memset(&a2, 0, sizeof(a2));
     a2.Y = c->d_Y; a2.coef = c->d_coef; a2.w_out = c->d_w; a2.wfac = c->d_wfac;
-    CU(launch_p2<EPI_WSTORE>(c->lg1, c->lg2, c->stream, a2, 1));
+    CU(launch_p2<EPI_WSTORE>(c, c->stream, a2, 1));
     c->launches += 2;
     int err = 0;
     CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -561,12 +499,8 @@ static int sort_triggers(cbmf_ctx* c, int64_t count)
     while (np2 < count) np2 <<= 1;
     if (np2 <= TRIG_SMALL) {
         const size_t smem_small = (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * (size_t)np2;
-        static bool attr_small = false;
-        if (!attr_small) {
-            CU(cudaFuncSetAttribute(trig_sort_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)((sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL)));
-            attr_small = true;
-        }
+        CU(ensure_smem_attr(c, trig_sort_small_kernel,
+                            (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL));
         trig_sort_small_kernel<<<1, 1024, smem_small, c->stream>>>(c->d_trig, (int)count, (int)np2);
         CU(cudaGetLastError());
         c->launches += 1;
@@ -574,12 +508,7 @@ static int sort_triggers(cbmf_ctx* c, int64_t count)
     }
     const int tile = (int)(np2 < TRIG_TILE ? np2 : TRIG_TILE);
     const size_t smem = sizeof(TrigOut) * (size_t)tile;
-    static bool attr_done = false;
-    if (!attr_done) {
-        CU(cudaFuncSetAttribute(trig_sort_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)(sizeof(TrigOut) * TRIG_TILE)));
-        attr_done = true;
-    }
+    CU(ensure_smem_attr(c, trig_sort_tile_kernel, sizeof(TrigOut) * TRIG_TILE));
     const unsigned tiles = (unsigned)(np2 / tile);
     trig_sort_tile_kernel<<<tiles, 1024, smem, c->stream>>>(c->d_trig, count, tile, 0);
     CU(cudaGetLastError());
@@ -598,88 +527,17 @@ static int sort_triggers(cbmf_ctx* c, int64_t count)
     return CBMF_OK;
 }
 
-// bank_dev: [n][2] doubles on the device.  Outputs go to host or device pointers (out_kind).
-static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr,
-                            void* peaks_out, void* trig_out, int64_t trig_capacity,
-                            int64_t* n_trig_found, cudaMemcpyKind out_kind)
+// Pass-1 / pass-2 launch pairs for templates [0, nt) whose constants are in c->d_coef; peaks to c->d_peaks,
+// triggers to c->d_trig (dev_cap entries; the total is counted in c->d_cursor whatever the capacity).
+static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap)
 {
-    if (n_trig_found) *n_trig_found = 0;
-    if (nt == 0) return CBMF_OK;
     int rc;
-    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
-    if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
-    // device trigger buffer: capacity rounded up to a power of two (bitonic padding), >= 1
-    int64_t tcap = 1;
-    while (tcap < trig_capacity) tcap <<= 1;
-    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
-
-    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
-    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
-    SetupArgs sa;
-    sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
-    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = thr; sa.err_flag = c->d_err;
-    template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
-    CU(cudaGetLastError());
-    c->launches += 1;
-
-    c->ev_used[0] = c->ev_used[1] = 0;
-    if (c->fused) {
-        // ---- one persistent cooperative launch for the whole bank (fused.cuh)
-        const int ring = c->ring;
-        if ((size_t)ring > (size_t)c->max_sub_batch * c->max_streams) {
-            if ((rc = alloc_pipeline(c, ring, c->max_streams > 0 ? c->max_streams : 1))) return rc;
-        }
-        const size_t n_sync = 3 * (size_t)nt + 3 + (size_t)c->n_sm;
-        if (nt > c->sync_cap) {
-            if (c->d_sync) { CU(cudaFree(c->d_sync)); c->d_sync = nullptr; c->sync_cap = 0; }
-            CU(cudaMalloc(&c->d_sync, sizeof(unsigned int) * n_sync));
-            c->sync_cap = nt;
-        }
-        if ((rc = grow(c, c->d_fkey, c->fkey_cap, nt))) return rc;
-        CU(cudaMemsetAsync(c->d_sync, 0, sizeof(unsigned int) * n_sync, c->stream));
-        CU(cudaMemsetAsync(c->d_fkey, 0, sizeof(unsigned long long) * (size_t)nt, c->stream));
-        const int grid = 2 * c->n_sm;
-        FusedArgs fa;
-        fa.w = c->d_w; fa.u = c->d_u; fa.coef = c->d_coef; fa.Y = c->d_Y; fa.cand = c->d_cand;
-        fa.best_key = c->d_fkey;
-        fa.p1_done = c->d_sync; fa.done_ctr = c->d_sync + nt; fa.p2_done = c->d_sync + 2 * nt;
-        fa.p2_next = c->d_sync + 3 * nt; fa.tile_next = c->d_sync + 3 * nt + 1;
-        fa.abort_flag = (int*)(c->d_sync + 3 * nt + 2); fa.sm_slot = c->d_sync + 3 * nt + 3;
-        fa.peaks = c->d_peaks; fa.trig = c->d_trig; fa.trig_cursor = c->d_cursor;
-        fa.trig_cap = (unsigned long long)trig_capacity;
-        if (!c->d_fstats) CU(cudaMalloc(&c->d_fstats, sizeof(unsigned long long) * 6 * (size_t)grid));
-        fa.stats = c->d_fstats;
-        fa.n_templates = (int)nt; fa.ring = ring;
-        fa.use_series = p1_series_ok(c->k_lo, 1 << c->lg2, FusedCfg<1024, 1024>::NC) ? 1 : 0;
-        if ((rc = ev_begin(c, 0))) return rc;
-        CU((fused_launch<1024, 1024>(c->stream, grid, fa)));
-        if ((rc = ev_end(c, 0))) return rc;
-        c->launches += 1;
-        struct { int err; int aborted; unsigned long long found; } st = {0, 0, 0};
-        CU(cudaMemcpyAsync(&st.err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaMemcpyAsync(&st.aborted, fa.abort_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaMemcpyAsync(&st.found, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
-        if ((rc = ev_collect(c))) return rc;
-        if (st.err) return CBMF_EINVAL;
-        if (st.aborted) { snprintf(c->cuda_err, sizeof(c->cuda_err), "bank_kernel: scheduler wait timed out"); return CBMF_ECUDA; }
-        const int64_t found = (int64_t)st.found;
-        const int64_t kept = found < trig_capacity ? found : trig_capacity;
-        if (n_trig_found) *n_trig_found = found;
-        if (kept > 0 && trig_out) {
-            if ((rc = sort_triggers(c, kept))) return rc;
-            CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, out_kind, c->stream));
-        }
-        CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, out_kind, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
-        return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
-    }
     const int sb = c->sub_batch;
     // Launch pairs go round-robin over ns streams, each with its own slice of Y / cand / done, so
     // that the tail of one kernel overlaps the head of the next pair.  With per-pass event timing on
-    // (cbmf_set_profiling) everything stays on the context's stream: each launch is timed alone.
-    const int ns = (c->profiling || nt <= sb) ? 1 : c->n_streams;
+    // (cbmf_set_profiling mode 1) everything stays on the context's stream: each launch is timed alone;
+    // mode 2 keeps the real schedule and brackets every launch with events on its own stream.
+    const int ns = (c->profiling == 1 || nt <= sb) ? 1 : c->n_streams;
     const size_t ncand = cand_per_template(c);
     if (ns > 1) {
         CU(cudaEventRecord(c->ev_fork, c->stream));
@@ -693,19 +551,20 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
         c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         P1Args a1; memset(&a1, 0, sizeof(a1));
         a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
-        if ((rc = ev_begin(c, 0))) return rc;
-        CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, st, a1, nb));
-        if ((rc = ev_end(c, 0))) return rc;
+        if ((rc = ev_begin(c, 0, st))) return rc;
+        CU(launch_p1<LOAD_GEN>(c, st, a1, nb));
+        if ((rc = ev_end(c, 0, st))) return rc;
         P2Args a2; memset(&a2, 0, sizeof(a2));
         a2.Y = Y; a2.coef = c->d_coef + t0;
         a2.cand = c->d_cand + (size_t)slot * c->max_sub_batch * ncand;
         a2.best_key = c->d_key + (size_t)slot * c->max_sub_batch;
         a2.done_ctr = c->d_done + (size_t)slot * c->max_sub_batch; a2.peaks = c->d_peaks + t0; a2.trig = c->d_trig;
-        a2.trig_cursor = c->d_cursor; a2.trig_cap = (unsigned long long)trig_capacity;
+        a2.trig_cursor = c->d_cursor; a2.trig_cap = (unsigned long long)dev_cap;
+        a2.trig_count = c->d_tcount + t0;
         a2.tmpl_base = (int)t0;
-        if ((rc = ev_begin(c, 1))) return rc;
-        CU(launch_p2<EPI_MAX>(c->lg1, c->lg2, st, a2, nb));
-        if ((rc = ev_end(c, 1))) return rc;
+        if ((rc = ev_begin(c, 1, st))) return rc;
+        CU(launch_p2<EPI_MAX>(c, st, a2, nb));
+        if ((rc = ev_end(c, 1, st))) return rc;
         c->launches += 2;
     }
     if (ns > 1) {
@@ -714,19 +573,80 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
             CU(cudaStreamWaitEvent(c->stream, c->ev_join[s], 0));
         }
     }
+    return CBMF_OK;
+}
 
-    // status word + trigger count back to the host, then sort what was kept
-    struct { int err; unsigned long long found; } st = {0, 0};
-    CU(cudaMemcpyAsync(&st.err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaMemcpyAsync(&st.found, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+// bank_dev: [n][2] doubles on the device.  Outputs go to host or device pointers (out_kind).
+static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr,
+                            void* peaks_out, void* trig_out, int64_t trig_capacity,
+                            int64_t* n_trig_found, cudaMemcpyKind out_kind)
+{
+    if (n_trig_found) *n_trig_found = 0;
+    c->last_bad = -1;
+    if (nt == 0) return CBMF_OK;
+    int rc;
+    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_tcount, c->tcount_cap, nt))) return rc;
+    // device trigger buffer: capacity rounded up to a power of two (bitonic padding), >= 1
+    int64_t tcap = 1;
+    while (tcap < trig_capacity) tcap <<= 1;
+    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
+
+    const long long no_bad = 0x7FFFFFFFFFFFFFFFLL;
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
+    CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
+    CU(cudaMemcpyAsync(c->d_bad, &no_bad, sizeof(long long), cudaMemcpyHostToDevice, c->stream));
+    SetupArgs sa;
+    sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
+    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
+    sa.threshold = thr; sa.err_flag = c->d_err; sa.bad_idx = c->d_bad;
+    template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    // an invalid template fails the call here, before any filtering, and is named (cbmf_last_bad_template)
+    long long bad = no_bad;
+    CU(cudaMemcpyAsync(&bad, c->d_bad, sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (bad != no_bad) { c->last_bad = (int64_t)bad; return CBMF_EINVAL; }
+
+    c->ev_used[0] = c->ev_used[1] = 0;
+    if ((rc = run_bank_passes(c, nt, c->trig_cap))) return rc;
+
+    // trigger count back to the host, then sort what was kept
+    unsigned long long found_u = 0;
+    CU(cudaMemcpyAsync(&found_u, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if ((rc = ev_collect(c))) return rc;
-    if (st.err) return CBMF_EINVAL;                 // a non-positive / non-finite mass (device check)
-    const int64_t found = (int64_t)st.found;
-    const int64_t kept = found < trig_capacity ? found : trig_capacity;
+    const int64_t found = (int64_t)found_u;
     if (n_trig_found) *n_trig_found = found;
+    const int64_t kept = found < trig_capacity ? found : trig_capacity;
     if (kept > 0 && trig_out) {
-        if ((rc = sort_triggers(c, kept))) return rc;
+        int64_t on_device = found;
+        if (found > c->trig_cap) {
+            // Truncated and the device list is incomplete.  The contract (cbmf.h) keeps the FIRST trig_capacity
+            // triggers in (template, sample) order, so the whole lists of the leading templates are needed:
+            // find the shortest bank prefix [0, t_cut] holding at least trig_capacity triggers from the
+            // per-template counts and filter that prefix again into a buffer that takes all of its triggers.
+            std::vector<unsigned int> cnt((size_t)nt);
+            CU(cudaMemcpyAsync(cnt.data(), c->d_tcount, sizeof(unsigned int) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+            int64_t cum = 0, t_cut = 0;
+            for (; t_cut < nt; ++t_cut) { cum += cnt[(size_t)t_cut]; if (cum >= trig_capacity) break; }
+            int64_t need = 1;
+            while (need < cum) need <<= 1;
+            if ((rc = grow(c, c->d_trig, c->trig_cap, need))) return rc;
+            CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
+            CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
+            const int prof = c->profiling;
+            c->profiling = 0;                           // the repeat is not part of the per-pass timing
+            rc = run_bank_passes(c, t_cut + 1, c->trig_cap);
+            c->profiling = prof;
+            if (rc) return rc;
+            on_device = cum;
+        }
+        if ((rc = sort_triggers(c, on_device))) return rc;
         CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, out_kind, c->stream));
     }
     CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, out_kind, c->stream));
@@ -784,7 +704,7 @@ static int setup_one(cbmf_ctx* c, cbmf_template t)
     SetupArgs sa;
     sa.bank = c->d_bank; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = 1;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = 0.f; sa.err_flag = c->d_err;
+    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr;
     template_setup_kernel<<<1, 32, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     c->launches += 1;
@@ -810,10 +730,10 @@ extern "C" int cbmf_debug_snr_series(cbmf_ctx* c, cbmf_template t, float* snr_ou
     CU(cudaStreamSynchronize(c->stream));
     P1Args a1; memset(&a1, 0, sizeof(a1));
     a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
-    CU(launch_p1<LOAD_GEN>(c->lg1, c->lg2, c->stream, a1, 1));
+    CU(launch_p1<LOAD_GEN>(c, c->stream, a1, 1));
     P2Args a2; memset(&a2, 0, sizeof(a2));
     a2.Y = c->d_Y; a2.z_out = z;
-    CU(launch_p2<EPI_STORE>(c->lg1, c->lg2, c->stream, a2, 1));
+    CU(launch_p2<EPI_STORE>(c, c->stream, a2, 1));
     snr_from_z_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>((const float2*)z, snr, n, tc.inv_sigma);
     CU(cudaGetLastError());
     c->launches += 3;
@@ -849,10 +769,10 @@ extern "C" int cbmf_debug_ifft_dev(cbmf_ctx* c, const float* in_dev, float* out_
         const int nb = (int)((batch - b0 < sb) ? (batch - b0) : sb);
         P1Args a1; memset(&a1, 0, sizeof(a1));
         a1.in_c = (const c2*)in_dev + (size_t)b0 * n; a1.Y = c->d_Y; a1.err_flag = c->d_err;
-        CU(launch_p1<LOAD_CPLX>(c->lg1, c->lg2, c->stream, a1, nb));
+        CU(launch_p1<LOAD_CPLX>(c, c->stream, a1, nb));
         P2Args a2; memset(&a2, 0, sizeof(a2));
         a2.Y = c->d_Y; a2.z_out = (c2*)out_dev + (size_t)b0 * n;
-        CU(launch_p2<EPI_STORE>(c->lg1, c->lg2, c->stream, a2, nb));
+        CU(launch_p2<EPI_STORE>(c, c->stream, a2, nb));
         c->launches += 2;
     }
     CU(cudaStreamSynchronize(c->stream));
@@ -893,7 +813,7 @@ extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_de
     SetupArgs sa;
     sa.bank = (const double*)bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = 0.f; sa.err_flag = c->d_err;
+    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr;
     template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     const int nh = (int)(c->n / 2);
@@ -905,50 +825,6 @@ extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_de
     CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return err ? CBMF_EINVAL : CBMF_OK;
-}
-
-extern "C" int cbmf_debug_fused_stats(cbmf_ctx* c, uint64_t* out, int64_t max_blocks, int64_t* n_blocks)
-{
-    if (!c || !out || max_blocks < 0) return CBMF_EINVAL;
-    if (!c->d_fstats) return CBMF_ESTATE;
-    DeviceGuard g(c->device);
-    const int64_t nb = 2 * c->n_sm < max_blocks ? 2 * c->n_sm : max_blocks;
-    CU(cudaMemcpyAsync(out, c->d_fstats, sizeof(uint64_t) * 6 * (size_t)nb, cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    if (n_blocks) *n_blocks = nb;
-    return CBMF_OK;
-}
-
-extern "C" int cbmf_debug_fp32_peak(cbmf_ctx* c, double* tflops_ffma, double* tflops_ffma2)
-{
-    if (!c || !tflops_ffma || !tflops_ffma2) return CBMF_EINVAL;
-    DeviceGuard g(c->device);
-    int n_sm = 0;
-    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, c->device));
-    const int iters = 4000;
-    if (int rc = grow_scratch(c, sizeof(float) * 1024 * (size_t)n_sm)) return rc;
-    cudaEvent_t e0, e1;
-    CU(cudaEventCreate(&e0));
-    CU(cudaEventCreate(&e1));
-    double res[2] = {0, 0};
-    for (int packed = 0; packed < 2; ++packed) {
-        for (int rep = 0; rep < 2; ++rep) {           // first launch warms up
-            CU(cudaEventRecord(e0, c->stream));
-            if (packed) fp32_peak_kernel<true><<<n_sm, 1024, 0, c->stream>>>((float*)c->d_scratch, iters, 1.0001f);
-            else fp32_peak_kernel<false><<<n_sm, 1024, 0, c->stream>>>((float*)c->d_scratch, iters, 1.0001f);
-            CU(cudaGetLastError());
-            CU(cudaEventRecord(e1, c->stream));
-            CU(cudaEventSynchronize(e1));
-            c->launches += 1;
-        }
-        float ms = 0.f;
-        CU(cudaEventElapsedTime(&ms, e0, e1));
-        const double flops = 2.0 * (packed ? 2.0 : 1.0) * 8.0 * 4.0 * (double)iters * 1024.0 * (double)n_sm;
-        res[packed] = flops / ((double)ms * 1e-3) / 1e12;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    *tflops_ffma = res[0]; *tflops_ffma2 = res[1];
-    return CBMF_OK;
 }
 
 extern "C" int cbmf_debug_get_prefix(cbmf_ctx* c, double* p_out)
@@ -984,8 +860,8 @@ extern "C" int cbmf_last_pass_time(const cbmf_ctx* c, int which, double* ms_out,
 
 extern "C" int cbmf_set_profiling(cbmf_ctx* c, int on)
 {
-    if (!c) return CBMF_EINVAL;
-    c->profiling = (on != 0);
+    if (!c || on < 0 || on > 2) return CBMF_EINVAL;
+    c->profiling = on;
     return CBMF_OK;
 }
 

@@ -521,6 +521,7 @@ struct P2Args {
     TrigOut* trig;                         // bounded trigger list
     unsigned long long* trig_cursor;       // total found so far
     unsigned long long trig_cap;
+    unsigned int* trig_count;              // [batch] triggers found per template (for a deterministic truncated list)
     int tmpl_base;                         // bank index of template 0 of this sub-batch
     // EPI_STORE
     c2* __restrict__ z_out;                // [batch][N], natural order
@@ -739,6 +740,12 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
             }
         }
         if (m > thr2 && inv_sigma > 0.f) {
+            // one slot range per thread: count, reserve, write (order inside the list is restored by the sort)
+            unsigned n_mine = 0;
+#pragma unroll
+            for (int e = 0; e < E; ++e) n_mine += (pw(e) > thr2) ? 1u : 0u;
+            unsigned long long slot = atomicAdd(a.trig_cursor, (unsigned long long)n_mine);
+            atomicAdd(a.trig_count + b, n_mine);
 #pragma unroll
             for (int q = 0; q < RL; ++q)
 #pragma unroll
@@ -746,7 +753,6 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
                     const int e = u * RL + q;
                     const float pe = pw(e);
                     if (pe > thr2) {
-                        const unsigned long long slot = atomicAdd(a.trig_cursor, 1ULL);
                         if (slot < a.trig_cap) {
                             const int j2 = t + T * u + (L2 / RL) * q;
                             TrigOut o;
@@ -758,6 +764,7 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
                             o.phase = atan2f(im(zt), re(zt));
                             a.trig[slot] = o;
                         }
+                        ++slot;
                     }
                 }
         }
@@ -937,6 +944,7 @@ struct SetupArgs {
     double df;
     float threshold;
     int* err_flag;
+    long long* bad_idx;                  // smallest index of an invalid template (atomicMin), may be null
 };
 
 __global__ void template_setup_kernel(const SetupArgs a)
@@ -950,6 +958,7 @@ __global__ void template_setup_kernel(const SetupArgs a)
     c.sigma = c.inv_sigma = 0.f; c.thr2 = 0.f; c.nz_class = 0; c.pad_[0] = c.pad_[1] = 0;
     if (!(m1 > 0.0) || !(m2 > 0.0) || isinf(m1) || isinf(m2)) {
         *a.err_flag = 1;
+        if (a.bad_idx) atomicMin(a.bad_idx, (long long)i);
         a.coef[i] = c;
         return;
     }
@@ -982,6 +991,7 @@ __global__ void template_setup_kernel(const SetupArgs a)
         const double ph_lo = fabs(ul * (c.A1 + ul * (c.A2 + ul * (c.A3 + ul * ul * c.A5)))) + 1.0;
         if (!(ph_lo < 524288.0)) {
             *a.err_flag = 1;
+            if (a.bad_idx) atomicMin(a.bad_idx, (long long)i);
             c.k_hi = -1;
             a.coef[i] = c;
             return;
@@ -1078,33 +1088,6 @@ __global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, in
             __syncthreads();
         }
     for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = rec[pos[i]];
-}
-
-// ------------------------------------------------------------------ FP32 pipe probe (roofline cross-check)
-// Eight independent FMA chains per thread, 1024 threads per block, one block per SM.  PACKED = false: scalar
-// FFMA (2 flop per lane and instruction); PACKED = true: FFMA2 (4 flop).  flops = 2 * (PACKED ? 2 : 1) * 8 * 4
-// per thread and iteration.
-template <bool PACKED>
-__global__ void __launch_bounds__(1024, 1) fp32_peak_kernel(float* __restrict__ out, const int iters, const float s)
-{
-    float a[8];
-    c2 p[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) { a[i] = (float)threadIdx.x * 1e-3f + (float)i; p[i] = pk(a[i], a[i] + 1.f); }
-    const c2 ps = pk(s, s * 0.5f), pc = pk(0.25f, 0.125f);
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int r = 0; r < 4; ++r)
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                if constexpr (PACKED) p[i] = fma2(p[i], ps, pc);
-                else a[i] = fmaf(a[i], s, 0.25f);
-            }
-    }
-    float acc = 0.f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) acc += a[i] + re(p[i]) + im(p[i]);
-    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 
 // ------------------------------------------------------------------ diagnostics

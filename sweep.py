@@ -9,7 +9,7 @@ m1, m2 uniform in [1, 3] Msun.  For every point, on one GPU, device-resident dat
   generate  the SPA generator alone writing q~ = w e^{i Psi} to HBM (cbmf_debug_generate_dev)
   filter    the whole hot path (cbmf_filter_bank_dev: S2-S8) in templates/s
 
-    python -m paper_1006_4644_b200.sweep [--log2n 16 ... 24] [--batches 1 8 64 512] [--repeats 5]
+    python sweep.py [--log2n 16 ... 24] [--batches 1 8 64 512] [--repeats 5]
 
 One JSON line per point on stdout; `--markdown` prints a table instead.  Points whose buffers
 would exceed --max-gib (input + output of the FFT comparison) run with the largest batch that fits
@@ -19,9 +19,14 @@ from __future__ import annotations
 
 import argparse
 import json
+import os
 import sys
 
 import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
 
 
 def _time(fn, stream, repeats):
@@ -42,7 +47,8 @@ def _time(fn, stream, repeats):
 
 def run_point(log2n: int, batch: int, repeats: int, max_gib: float):
     import torch
-    from . import cbmf, workloads as W
+    from paper_1006_4644_b200 import cbmf
+    from testsupport import workloads as W
     n = 1 << log2n
     dev = torch.device("cuda", 0)
     stream = torch.cuda.Stream(device=dev)

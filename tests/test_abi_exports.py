@@ -46,12 +46,46 @@ def test_argument_errors_need_no_gpu():
 
 
 def test_product_does_not_import_oracle():
-    """The product path never routes through the oracle (③): no import of oracle/ anywhere
-    in the package, and no CPU fallback module."""
+    """The product path never routes through the oracle (③): no import of oracle/ or of the test-support
+    generators anywhere in the package, no CPU fallback module, no library FFT (north_star: cuFFT is never
+    on the product path), no environment variables read behind the C ABI, and the method's arithmetic only
+    in csrc/ (the Python side holds marshalling and index bookkeeping)."""
     pkg = os.path.join(ROOT, "paper_1006_4644_b200")
-    for dirpath, _, files in os.walk(pkg):
+    py_files = []
+    for dirpath, dirs, files in os.walk(pkg):
+        dirs[:] = [d for d in dirs if d != "__pycache__"]
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
-                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert not re.search(r"^\s*(import|from)\s+(oracle|testsupport)\b", txt, flags=re.M), f
                 assert "mf_oracle" not in txt and "liboracle" not in txt, f
+                assert not re.search(r"torch\.fft|cufft|numpy\.fft|np\.fft|scipy\.fft", txt, flags=re.I), f
+                assert "getenv" not in txt, f
+                if f.endswith(".py"):
+                    py_files.append(f)
+                    # the 2PN phase coefficients (3715/756, 15293365/508032) belong to csrc/ only
+                    assert "3715" not in txt and "15293365" not in txt and "4.925490947641267e-6" not in txt, f
+    assert sorted(py_files) == ["__init__.py", "build.py", "cbmf.py", "sharding.py"], py_files
+    assert sorted(os.listdir(os.path.join(pkg, "csrc"))) == ["cbmf.cu", "fft_regs.cuh", "kernels.cuh"]
+
+
+def test_binding_rejects_wrong_dtypes():
+    """cbmf.py checks dtype / size of every array it hands to the C ABI (a float32 PSD tensor would be
+    read as float64 by the kernel).  Pure host checks: they raise before any library call."""
+    import numpy as np
+    import pytest
+    import torch
+    from paper_1006_4644_b200 import cbmf
+    with pytest.raises(ValueError):
+        cbmf._ptr(torch.zeros(9, dtype=torch.float32), "float64")
+    with pytest.raises(ValueError):
+        cbmf._ptr(torch.zeros(8, dtype=torch.float64), "float32")
+    with pytest.raises(ValueError):
+        cbmf._ptr(np.zeros(8, dtype=np.float32), "float64")
+    with pytest.raises(ValueError):
+        cbmf._ptr(torch.zeros(24, dtype=torch.uint8), "peak records", itemsize=16)     # not a multiple of 16 bytes
+    with pytest.raises(ValueError):
+        cbmf._ptr(torch.zeros((4, 4), dtype=torch.float64).t(), "float64")               # not contiguous
+    assert cbmf._ptr(torch.zeros(32, dtype=torch.uint8), "peak records", itemsize=16)[1] is False
+    assert cbmf._ptr(np.zeros(2, dtype=cbmf.PEAK_DTYPE), "peak records", itemsize=16)[1] is False
+    assert cbmf._ptr(torch.zeros(8, dtype=torch.float64), "float64")[1] is False

@@ -13,7 +13,9 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_1006_4644_b200 import workloads as W
+from testsupport import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -489,3 +491,17 @@ def test_psd_infinite_weight_zero():
     df = w.fs / w.n
     assert sigma ** 2 == pytest.approx(4 * df * np.sum((k * df) ** (-7 / 3) / psd[k]), rel=1e-13)
     assert np.all(np.isfinite(rho))
+
+
+def test_oracle_under_sanitizers(tmp_path):
+    """the oracle built with -fsanitize=address,undefined runs two pins (P1 and the bank
+    loop with an empty band and a truncated list) without a report (tests/asan_driver.c)."""
+    import subprocess
+    exe = str(tmp_path / "asan_driver")
+    cmd = ["gcc", "-O1", "-g", "-std=c11", "-fopenmp", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+           "-fno-omit-frame-pointer", "-o", exe, os.path.join(ROOT, "tests", "asan_driver.c"),
+           os.path.join(ROOT, "oracle", "mf_oracle.c"), "-lm"]
+    subprocess.run(cmd, check=True)
+    env = dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", OMP_NUM_THREADS="2")
+    r = subprocess.run([exe], capture_output=True, text=True, env=env, timeout=120)
+    assert r.returncode == 0 and "asan driver ok" in r.stdout, (r.returncode, r.stdout, r.stderr[-2000:])
