@@ -154,11 +154,13 @@ cudaError_t launch_p1_L(cbmf_ctx* c, cudaStream_t s, P1Args a, int batch)
     cudaError_t e = ensure_smem_attr(c, p1_kernel<L1, L2, MODE>, smem);
     if (e != cudaSuccess) return e;
     a.batch = batch;
-    if (MODE == LOAD_GEN) {
-        // series for k^{-1/3} (spa_correlate): valid where (columns of a tile - 1) / (first in-band bin of a row) <= 2e-3
+    constexpr bool GEN = (MODE == LOAD_GEN || MODE == LOAD_GEN_DUMP);
+    if (GEN) {
+        // expansion about the first column of a tile (spa_generate_rows, spa_correlate): valid where
+        // (columns of a tile - 1) / (first in-band bin of a row) <= 2e-3
         a.use_series = p1_series_ok(a.use_series, L2, Cfg<L1>::C) ? 1 : 0;    // the caller passes k_lo in use_series
     }
-    const int groups = (MODE == LOAD_GEN) ? p1_groups(c->n_sm, L2 / Cfg<L1>::C, batch) : batch;
+    const int groups = GEN ? p1_groups(c->n_sm, L2 / Cfg<L1>::C, batch) : batch;
     dim3 grid(L2 / Cfg<L1>::C, groups);
     p1_kernel<L1, L2, MODE><<<grid, Cfg<L1>::NT1, smem, s>>>(a);
     return cudaGetLastError();
@@ -750,12 +752,21 @@ extern "C" int cbmf_debug_template(cbmf_ctx* c, cbmf_template t, float* h_out)
     DeviceGuard g(c->device);
     int rc;
     if ((rc = setup_one(c, t))) return rc;
-    const int nh = (int)(c->n / 2);
-    if ((rc = grow_scratch(c, sizeof(float2) * (size_t)(nh + 1)))) return rc;
-    debug_template_kernel<<<(nh + 1 + 255) / 256, 256, 0, c->stream>>>(c->d_coef, c->d_u, (float2*)c->d_scratch, nh, c->df);
+    // the PRODUCT generator (pass 1 of filter_bank) with unit weights, its inputs dumped instead of transformed
+    const size_t n = (size_t)c->n, nh = n / 2;
+    if ((rc = grow_scratch(c, sizeof(c2) * (nh + n) + sizeof(float2) * (nh + 1)))) return rc;
+    c2* ones = (c2*)c->d_scratch;
+    c2* q = ones + nh;
+    float2* h = (float2*)(q + n);
+    fill_ones_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(ones, (int)nh);
     CU(cudaGetLastError());
-    c->launches += 1;
-    CU(cudaMemcpyAsync(h_out, c->d_scratch, sizeof(float2) * (size_t)(nh + 1), cudaMemcpyDeviceToHost, c->stream));
+    P1Args a1; memset(&a1, 0, sizeof(a1));
+    a1.w = ones; a1.u = c->d_u; a1.coef = c->d_coef; a1.Y = q; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+    CU(launch_p1<LOAD_GEN_DUMP>(c, c->stream, a1, 1));
+    debug_template_kernel<<<(unsigned)((nh + 1 + 255) / 256), 256, 0, c->stream>>>(q, h, (int)nh, c->df);
+    CU(cudaGetLastError());
+    c->launches += 3;
+    CU(cudaMemcpyAsync(h_out, h, sizeof(float2) * (nh + 1), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return CBMF_OK;
 }

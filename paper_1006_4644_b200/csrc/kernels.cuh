@@ -15,6 +15,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 #include "fft_regs.cuh"
 
 namespace cbmf {
@@ -126,11 +127,33 @@ __device__ __forceinline__ void named_barrier(const int id, const int nthreads)
 // CENTER (ROWTW, two-step FFTs): the step-2 twiddles are applied as g^(r - R2/2); every output of
 // this thread then lacks the common factor g^(R2/2), with g = e^{2 pi i (k/(R1 R2) + j1/N)} and
 // k = t mod R1 (see mul_powers_centered and fft_center_factor).
-template <int L, int NZ1, int SS, int SYNC, bool ROWTW, typename Hook = NoHook, bool CENTER = false>
-__device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm,
-                                         const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook(),
-                                         const c2* __restrict__ tw = nullptr, const int bar_id = 0,
-                                         const int bar_threads = 0, const c2* __restrict__ g_row = nullptr)
+// Step 1 alone (radix R1, no twiddles, Ns = 1; output position i*R1 + q in the exchange buffer): callers that
+// prune by the number of non-zero inputs instantiate only this part per NZ1 and share fft_core_tail.
+template <int L, int NZ1, int SS>
+__device__ __forceinline__ void fft_core_step1(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, T = C::T, R1 = C::R1;
+    constexpr int LG_R1 = ilog2c(R1);
+    auto pad = [](int pos) { return pos + (pos >> LG_R1); };
+    constexpr int NB = E / R1;
+#pragma unroll
+    for (int u = 0; u < NB; ++u) {
+        c2 x[R1];
+#pragma unroll
+        for (int r = 0; r < R1; ++r) x[r] = v[u * R1 + r];
+        DftP<R1, NZ1>::run(x);
+        const int i = t + T * u;
+#pragma unroll
+        for (int q = 0; q < R1; ++q) sm[(i * (R1 + 1) + q) * SS] = x[q];       // = pad(i R1 + q)
+    }
+}
+
+template <int L, int SS, int SYNC, bool ROWTW, typename Hook = NoHook, bool CENTER = false>
+__device__ __forceinline__ void fft_core_tail(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm,
+                                              const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook(),
+                                              const c2* __restrict__ tw = nullptr, const int bar_id = 0,
+                                              const int bar_threads = 0, const c2* __restrict__ g_row = nullptr)
 {
     using C = Cfg<L>;
     constexpr int E = C::E, T = C::T, R1 = C::R1, R2 = C::R2, R3 = C::R3;
@@ -141,30 +164,17 @@ __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __
         else if constexpr (SYNC == SYNC_NAMED) named_barrier(bar_id, bar_threads);
         else __syncthreads();
     };
-
-    // ---- step 1: radix R1, no twiddles (Ns = 1); out position i*R1 + q
-    {
-        constexpr int NB = E / R1;
-#pragma unroll
-        for (int u = 0; u < NB; ++u) {
-            c2 x[R1];
-#pragma unroll
-            for (int r = 0; r < R1; ++r) x[r] = v[u * R1 + r];
-            DftP<R1, NZ1>::run(x);
-            const int i = t + T * u;
-#pragma unroll
-            for (int q = 0; q < R1; ++q) sm[pad(i * R1 + q) * SS] = x[q];
-        }
-    }
     sync();
     // ---- step 2: radix R2, Ns = R1
     {
         constexpr int NB = E / R2, NS = R1;
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
-            const int i = t + T * u;
+            // L/R2 is a multiple of R1, so pad(i + (L/R2) r) = pad(i) + r (L/R2)(1 + 1/R1): one base, constant offsets
+            static_assert((L / R2) % R1 == 0, "step-2 stride");
+            const int pi = pad(t + T * u);
 #pragma unroll
-            for (int r = 0; r < R2; ++r) v[u * R2 + r] = sm[pad(i + (L / R2) * r) * SS];
+            for (int r = 0; r < R2; ++r) v[u * R2 + r] = sm[(pi + r * ((L / R2) + (L / R2) / R1)) * SS];
         }
         if constexpr (R3 == 1) after_last_read();
 #pragma unroll
@@ -211,9 +221,9 @@ __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __
             for (int u = 0; u < NB; ++u) {
                 const int i = t + T * u;
                 const int k = i & (NS - 1);
-                const int base = (i >> LG_R1) * (NS * R2) + k;
+                const int pb = pad((i >> LG_R1) * (NS * R2) + k);
 #pragma unroll
-                for (int q = 0; q < R2; ++q) sm[pad(base + q * NS) * SS] = v[u * R2 + q];
+                for (int q = 0; q < R2; ++q) sm[(pb + q * (NS + 1)) * SS] = v[u * R2 + q];      // NS = R1: pad(base + q R1) = pad(base) + q (R1 + 1)
             }
         }
     }
@@ -223,9 +233,10 @@ __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __
         constexpr int NB = E / R3, NS = R1 * R2;
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
-            const int i = t + T * u;
+            static_assert(R3 == 1 || (L / R3) % R1 == 0, "step-3 stride");
+            const int pi = pad(t + T * u);
 #pragma unroll
-            for (int r = 0; r < R3; ++r) v[u * R3 + r] = sm[pad(i + (L / R3) * r) * SS];
+            for (int r = 0; r < R3; ++r) v[u * R3 + r] = sm[(pi + r * ((L / R3) + (L / R3) / R1)) * SS];
         }
         after_last_read();
 #pragma unroll
@@ -241,6 +252,16 @@ __device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __
             for (int q = 0; q < R3; ++q) v[u * R3 + q] = x[q];
         }
     }
+}
+
+template <int L, int NZ1, int SS, int SYNC, bool ROWTW, typename Hook = NoHook, bool CENTER = false>
+__device__ __forceinline__ void fft_core(c2 (&v)[Cfg<L>::E], const int t, c2* __restrict__ sm,
+                                         const int j1 = 0, const int n1 = 1, Hook after_last_read = Hook(),
+                                         const c2* __restrict__ tw = nullptr, const int bar_id = 0,
+                                         const int bar_threads = 0, const c2* __restrict__ g_row = nullptr)
+{
+    fft_core_step1<L, NZ1, SS>(v, t, sm);
+    fft_core_tail<L, SS, SYNC, ROWTW, Hook, CENTER>(v, t, sm, j1, n1, after_last_read, tw, bar_id, bar_threads, g_row);
 }
 
 // The factor g^(R2/2) a CENTER transform leaves out of output element e (= u R2 + q) of thread t
@@ -368,8 +389,86 @@ __device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, c
     }
 }
 
+// ------------------------------------------------------------------ S3 by rows (pass 1, two-step column FFTs)
+// The NC columns of a pass-1 tile are consecutive bins k = kb + c of one row k1 (kb = k1 L2 + first column of the
+// tile), so the phase in cycles, phi(k) = Psi_T(f_k) / 2 pi = -1/8 + A1 u + A2 u^2 + A3 u^3 + A5 u^5 with
+// u = k^{-1/3}, is expanded about kb (D = d/dk, Du = -u^4 / 3):
+//     phi(kb + c) = phi0 + c D phi + c^2 D2 phi / 2 + c^3 D3 phi / 6 + O(c^4 D4 phi),
+//     D  phi = -(u^4 / 3)    (A1 +  2 A2 u +   3 A3 u^2 +   5 A5 u^4)
+//     D2 phi =  (u^7 / 9)    (4 A1 + 10 A2 u +  18 A3 u^2 +  40 A5 u^4)
+//     D3 phi = -(u^10 / 27) (28 A1 + 80 A2 u + 162 A3 u^2 + 440 A5 u^4)
+// and evaluated ONCE per (template, row) instead of once per bin.  phi0 and D phi (up to 1e4 and a few cycles) are
+// taken in fp64 and reduced modulo one cycle to 32-bit fixed point (units of 2^-32 cycle, the low word of
+// x + 1.5 * 2^20 as in spa_phasor_u); D2 phi / 2 and D3 phi / 6 are below 1e-2 and 1e-7 cycles and are taken in
+// fp32.  A bin then costs three wrapping integer multiply-adds (the reduction modulo one cycle is free), one
+// conversion and the SFU sine / cosine.  The caller guarantees c / kb <= 2e-3 on every in-band row
+// (p1_series_ok), where the neglected quartic term is below 3.2 (c/kb)^4 phi < 1e-6 cycle for phi < 1e4 cycles.
+struct __align__(16) RowCoef { unsigned p0, p1; int p2, p3; };
+
+__device__ __forceinline__ RowCoef spa_row_coef(const double u, const double A1, const double A2, const double A3,
+                                                const double A5)
+{
+    const double u2 = u * u;
+    double ph = fma(u2, A5, A3);
+    ph = fma(ph, u, A2);
+    ph = fma(ph, u, A1);
+    ph = fma(ph, u, -0.125);
+    double q1 = fma(u2, 5.0 * A5, 3.0 * A3);
+    q1 = fma(q1, u, 2.0 * A2);
+    q1 = fma(q1, u, A1);
+    const double d1 = (-1.0 / 3.0) * (u2 * u2) * q1;
+    const float uf = (float)u, uf2 = uf * uf, uf3 = uf2 * uf;
+    const float a1 = (float)A1, a2 = (float)A2, a3 = (float)A3, a5 = (float)A5;
+    float q2 = fmaf(uf2, 40.f * a5, 18.f * a3);
+    q2 = fmaf(q2, uf, 10.f * a2);
+    q2 = fmaf(q2, uf, 4.f * a1);
+    float q3 = fmaf(uf2, 440.f * a5, 162.f * a3);
+    q3 = fmaf(q3, uf, 80.f * a2);
+    q3 = fmaf(q3, uf, 28.f * a1);
+    const float uf7 = uf3 * uf3 * uf;
+    const float d2 = (4294967296.0f / 18.0f) * (uf7 * q2);             // D2 phi / 2 in units of 2^-32 cycle
+    const float d3 = (-4294967296.0f / 162.0f) * ((uf7 * uf3) * q3);   // D3 phi / 6
+    RowCoef r;
+    r.p0 = (unsigned)__double2loint(__dadd_rn(ph, 1572864.0));
+    r.p1 = (unsigned)__double2loint(__dadd_rn(d1, 1572864.0));
+    r.p2 = __float2int_rn(d2);
+    r.p3 = __float2int_rn(d3);
+    return r;
+}
+
+// S3 + S4 from row records: v[r] = w[k] e^{+i Psi(f_k)}, k = (t + T r) L2 + k2, for r < NZ (the DFT that follows
+// reads no other input); zero outside [k_lo, k_hi].  (c1, c2_, c3) = (c, c^2, c^3) of this thread's column c.
+// Row record k1 sits at rc_lo[k1] for k1 < RS and at rc_hi[k1 - RS] above (RS a multiple of T: the choice is made at
+// compile time for every r).
+template <int L, int L2, int NZ, int RS>
+__device__ __forceinline__ void spa_generate_rows(c2 (&v)[Cfg<L>::E], const int t, const int k2,
+                                                  const c2* __restrict__ wt, const int WS,
+                                                  const RowCoef* __restrict__ rc_lo, const RowCoef* __restrict__ rc_hi,
+                                                  const int k_lo, const int k_hi,
+                                                  const int c1, const int c2_, const int c3)
+{
+    using C = Cfg<L>;
+    constexpr int T = C::T, R1 = C::R1;
+    static_assert(C::E == R1, "one step-1 DFT per thread");
+    static_assert(RS % T == 0, "row-record split on a multiple of T");
+#pragma unroll
+    for (int r = 0; r < NZ; ++r) {
+        const int k1 = t + T * r;
+        const int k = k1 * L2 + k2;
+        const uint4 q = *reinterpret_cast<const uint4*>((T * r < RS) ? rc_lo + k1 : rc_hi + (k1 - RS));
+        const unsigned ph = q.x + (unsigned)c1 * q.y + (unsigned)c2_ * q.z + (unsigned)c3 * q.w;
+        const float ang = (float)(int)ph * (6.28318530717958647692f / 4294967296.0f);
+        const c2 wv = (k >= k_lo && k <= k_hi) ? wt[k1 * WS] : czero();
+        v[r] = cmul(pk(__cosf(ang), __sinf(ang)), wv);
+    }
+#pragma unroll
+    for (int r = NZ; r < R1; ++r) v[r] = czero();
+}
+
 // ------------------------------------------------------------------ pass 1
-enum { LOAD_GEN = 0, LOAD_CPLX = 1, LOAD_REAL = 2 };
+// LOAD_GEN_DUMP (diagnostic): the generator of LOAD_GEN, bit for bit, but the generated inputs q~[k] are written to
+// Y[b][k] in natural order and no FFT is run -- cbmf_debug_template reads the PRODUCT generator through it.
+enum { LOAD_GEN = 0, LOAD_CPLX = 1, LOAD_REAL = 2, LOAD_GEN_DUMP = 3 };
 
 struct P1Args {
     const c2* __restrict__ w;              // [N/2] weighted data spectrum (LOAD_GEN)
@@ -386,31 +485,51 @@ struct P1Args {
 // The step-2 twiddle table is used where the FFT has two steps (L <= 1024).
 template <int L> __host__ __device__ constexpr bool p1_use_twtab() { return Cfg<L>::R3 == 1; }
 
+// The generator by rows (spa_generate_rows) serves the two-step column FFTs; the 2048- / 4096-point ones have no
+// shared memory left for its tables and keep the per-bin series (spa_correlate).
+template <int L> __host__ __device__ constexpr bool p1_by_rows() { return Cfg<L>::R3 == 1; }
+// Row records k1 < p1_rc_split live in their own array, the others in the (L/R1) NC elements the padded exchange
+// buffer has beyond the unpadded output tile.  At L = 1024 that keeps a block at 112.5 KiB, so that TWO blocks fit
+// one SM (measured: 2 KiB more costs 16 % of the bank throughput).
+template <int L> __host__ __device__ constexpr int p1_rc_split()
+{
+    constexpr int tail_rows = (Cfg<L>::PADDED - L) * Cfg<L>::C * (int)sizeof(c2) / 16;       // 16 = sizeof(RowCoef)
+    constexpr int want = (L >= 1024) ? L / 2 - tail_rows : L / 2;
+    return (want / Cfg<L>::T) * Cfg<L>::T + ((want % Cfg<L>::T) ? Cfg<L>::T : 0);
+}
+
 // Shared memory of one pass-1 block: the exchange buffer of NC column FFTs, the step-2 twiddle
 // table and, for LOAD_GEN, the tile w[k1][k2 in tile], k1 < N1/2 (the upper half of the
 // spectrum is zero), staged once per block and reused by every template the block works through.
-template <int L1, int MODE>
+template <int L1, int MODE_>
 __host__ __device__ constexpr size_t p1_smem_bytes()
 {
     using C = Cfg<L1>;
+    constexpr int MODE = (MODE_ == LOAD_GEN_DUMP) ? LOAD_GEN : MODE_;
     return sizeof(c2) * ((size_t)C::PADDED * C::C + (p1_use_twtab<L1>() ? (size_t)twtab_elems<L1>() : 0) +
                          (MODE == LOAD_GEN ? (size_t)(L1 / 2) * C::C : 0)) +
-           (MODE == LOAD_GEN ? (sizeof(double) + sizeof(float)) * (size_t)(L1 / 2) : 0);      // ub, inv
+           (MODE == LOAD_GEN ? (p1_by_rows<L1>() ? sizeof(RowCoef) * (size_t)p1_rc_split<L1>()                     // rc_lo
+                                                 : (sizeof(double) + sizeof(float)) * (size_t)(L1 / 2))            // ub, inv
+                             : 0);
 }
 
 // One pass-1 block = one tile of NC adjacent columns k2.  For every template slot b of the
 // launch with b = blockIdx.y (mod gridDim.y): N1 = L1-point inverse FFT over k1 of
 // x[k1*L2 + k2] -> Y[b][j1*L2 + k2].
-template <int L1, int L2, int MODE>
-__global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p1_kernel(const P1Args a)
+template <int L1, int L2, int MODE_>
+__global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<L1>::NT1 <= 256 ? 2 : 1))) p1_kernel(const P1Args a)
 {
     extern __shared__ __align__(16) c2 smem[];
     using C = Cfg<L1>;
+    constexpr int MODE = (MODE_ == LOAD_GEN_DUMP) ? LOAD_GEN : MODE_;
+    constexpr bool DUMP = (MODE_ == LOAD_GEN_DUMP);
     constexpr int E = C::E, T = C::T, R1 = C::R1, NC = C::C, NT = C::NT1;
     constexpr int RL = (C::R3 > 1) ? C::R3 : C::R2;
     constexpr int NZ1 = (MODE == LOAD_GEN) ? R1 / 2 : R1;    // bins k >= N/2 are zero
     constexpr size_t n_total = (size_t)L1 * L2;
     constexpr bool TWTAB = p1_use_twtab<L1>();
+    constexpr bool BYROWS = (MODE == LOAD_GEN) && p1_by_rows<L1>();
+    constexpr int RS = p1_rc_split<L1>();                  // row records k1 < RS: own array; the rest: exchange-buffer tail
 
     const int tile = blockIdx.x;
     const int c = threadIdx.x % NC, t = threadIdx.x / NC;
@@ -429,43 +548,128 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
     }
     if constexpr (TWTAB) twtab_fill<L1>(tw, threadIdx.x, NT);
     if constexpr (MODE != LOAD_GEN) __syncthreads();
-    // series tables of spa_correlate: kb^{-1/3} and 1/kb for the first column of the tile, every row k1
-    double* __restrict__ ub = reinterpret_cast<double*>(wt + (size_t)(L1 / 2) * NC);
+
+    // ---- generator state
+    // by rows (two-step FFTs): one RowCoef per row k1 < L1/2 of the CURRENT template -- rows below RS in their own
+    // array after the w tile, the others in the tail of the exchange buffer that the unpadded output tile leaves
+    // free (so that two pass-1 blocks still fit one SM); every thread keeps kb^{-1/3} of the RPT rows it fills.
+    // per-bin series (three-step FFTs): tables kb^{-1/3} (double) and 1/kb of the first column, every row.
+    RowCoef* __restrict__ rc_lo = reinterpret_cast<RowCoef*>(wt + (size_t)(L1 / 2) * NC);              // [RS]
+    RowCoef* __restrict__ rc_hi = reinterpret_cast<RowCoef*>(smem + (size_t)L1 * NC);                   // [L1/2 - RS]
+    double* __restrict__ ub = reinterpret_cast<double*>(wt + (size_t)(L1 / 2) * NC);                    // (!BYROWS)
     float* __restrict__ inv = reinterpret_cast<float*>(ub + L1 / 2);
+    // Row records are WARP-LOCAL: a warp holds T_W = 32 / NC values of t and needs the rows k1 = t + T r, r < R1/2, of
+    // exactly those; its 32 lanes fill them (RPT = T_W (R1/2) / 32 rows each: lane (t, c) takes r = RPT c + i), so a
+    // __syncwarp orders fill and use and no block barrier is involved.  kb^{-1/3} of a lane's rows stays in registers.
+    static_assert(!BYROWS || (NC <= 32 && ((R1 / 2) % NC == 0 || NC % (R1 / 2) == 0)), "rows of a warp divide among its lanes");
+    constexpr int RPT_W = ((R1 / 2) / NC > 1) ? (R1 / 2) / NC : 1;      // lanes c >= R1/2 of a wide tile stay idle
+    double u_mine[RPT_W];
     if constexpr (MODE == LOAD_GEN) {
-        for (int k1 = threadIdx.x; k1 < L1 / 2; k1 += NT) {
-            const int kb = k1 * L2 + tile * NC;
-            ub[k1] = __ldg(a.u + kb);
-            inv[k1] = kb > 0 ? (float)(1.0 / (double)kb) : 0.f;
+        if constexpr (BYROWS) {
+#pragma unroll
+            for (int i = 0; i < RPT_W; ++i) {
+                const int k1 = t + T * (RPT_W * c + i);
+                u_mine[i] = (RPT_W * c + i < R1 / 2) ? __ldg(a.u + (k1 * L2 + tile * NC)) : 0.0;
+            }
+        } else {
+            for (int k1 = threadIdx.x; k1 < L1 / 2; k1 += NT) {
+                const int kb = k1 * L2 + tile * NC;
+                ub[k1] = __ldg(a.u + kb);
+                inv[k1] = kb > 0 ? (float)(1.0 / (double)kb) : 0.f;
+            }
         }
     }
+    // row records of one template: those rows of this warp that touch the template's band
+    auto fill_rows = [&](const TemplCoef* __restrict__ tn) {
+        const int k_lo = tn->k_lo, k_hi = tn->k_hi;
+        const double A1 = tn->A1, A2 = tn->A2, A3 = tn->A3, A5 = tn->A5;
+#pragma unroll
+        for (int i = 0; i < RPT_W; ++i) {
+            const int k1 = t + T * (RPT_W * c + i);
+            const int kb = k1 * L2 + tile * NC;
+            if (RPT_W * c + i < R1 / 2 && kb + NC - 1 >= k_lo && kb <= k_hi) {
+                const RowCoef r = spa_row_coef(u_mine[i], A1, A2, A3, A5);
+                if (k1 < RS) rc_lo[k1] = r; else rc_hi[k1 - RS] = r;
+            }
+        }
+        __syncwarp();
+    };
 
     // per-template constants travel through a two-entry shared buffer, fetched one template ahead
     __shared__ __align__(16) TemplCoef s_coef[2];
+    const int G = gridDim.y;
+    auto fetch_coef = [&](const int slot, const int bb) {
+        if (threadIdx.x < 4 && bb < a.batch)
+            cp_async16(reinterpret_cast<char*>(&s_coef[slot]) + 16 * threadIdx.x,
+                       reinterpret_cast<const char*>(a.coef + bb) + 16 * threadIdx.x);
+    };
+    const bool by_rows = BYROWS && a.use_series;          // uniform over the launch
     if constexpr (MODE == LOAD_GEN) {
-        if (threadIdx.x < 4 && (int)blockIdx.y < a.batch)
-            cp_async16(reinterpret_cast<char*>(&s_coef[0]) + 16 * threadIdx.x,
-                       reinterpret_cast<const char*>(a.coef + blockIdx.y) + 16 * threadIdx.x);
+        fetch_coef(0, blockIdx.y);
         cp_async_commit();
         cp_async_wait_all();
         __syncthreads();
     }
 
     int cur = 0;
-    for (int b = blockIdx.y; b < a.batch; b += gridDim.y, cur ^= 1) {
+    for (int b = blockIdx.y; b < a.batch; b += G, cur ^= 1) {
         c2 v[E];
+        bool step1_done = false;
         if constexpr (MODE == LOAD_GEN) {
-            const int bn = b + gridDim.y;
-            if (threadIdx.x < 4 && bn < a.batch)
-                cp_async16(reinterpret_cast<char*>(&s_coef[cur ^ 1]) + 16 * threadIdx.x,
-                           reinterpret_cast<const char*>(a.coef + bn) + 16 * threadIdx.x);
+            fetch_coef(cur ^ 1, b + G);
             cp_async_commit();
             const TemplCoef* tc = &s_coef[cur];
-            if (a.use_series)
-                spa_correlate<L1, L2, true>(v, t, k2, wt + c, NC, nullptr, 0, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3,
-                                            tc->A5, ub, inv, (float)c);
-            else
-                spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
+            if constexpr (BYROWS) {
+                if (by_rows) {
+                    // this template's row records (the previous ones were last read by this warp in the previous
+                    // iteration; the exchange-buffer tail is free between the step-2 reads and the step-1 writes);
+                    // the copy engine drains the previous output tile meanwhile
+                    fill_rows(tc);
+                    const int k_lo = tc->k_lo, k_hi = tc->k_hi;
+                    // inputs v[r] = x[t + T r] beyond the band are zero: prune the step-1 DFT to NZ of them (uniform)
+                    const int nz = (k_hi < 0) ? 0 : ((k_hi / L2) / T + 1);
+                    auto run = [&](auto nz_tag) {
+                        constexpr int NZ = decltype(nz_tag)::value;
+                        spa_generate_rows<L1, L2, NZ, RS>(v, t, k2, wt + c, NC, rc_lo, rc_hi, k_lo, k_hi, c, c * c, c * c * c);
+                        if constexpr (!DUMP) {
+                            // the copy engine may still be reading the previous output tile out of the exchange buffer
+                            if (threadIdx.x == 0) bulk_store_wait_read();
+                            __syncthreads();
+                            fft_core_step1<L1, NZ, NC>(v, t, smem + c);
+                        }
+                    };
+                    if constexpr (R1 >= 32) {
+                        if (nz <= 2) run(std::integral_constant<int, 2>());
+                        else if (nz <= 4) run(std::integral_constant<int, 4>());
+                        else if (nz <= 6) run(std::integral_constant<int, 6>());
+                        else if (nz <= 8) run(std::integral_constant<int, 8>());
+                        else if (nz <= 10) run(std::integral_constant<int, 10>());
+                        else if (nz <= 12) run(std::integral_constant<int, 12>());
+                        else if (nz <= 14) run(std::integral_constant<int, 14>());
+                        else run(std::integral_constant<int, 16>());
+                    } else if constexpr (R1 >= 16) {
+                        if (nz <= 2) run(std::integral_constant<int, 2>());
+                        else if (nz <= 4) run(std::integral_constant<int, 4>());
+                        else if (nz <= 6) run(std::integral_constant<int, 6>());
+                        else run(std::integral_constant<int, 8>());
+                    } else {
+                        if (nz <= 2) run(std::integral_constant<int, 2>());
+                        else run(std::integral_constant<int, R1 / 2>());
+                    }
+                    step1_done = true;
+                }
+            }
+            if (!step1_done) {
+                if constexpr (!BYROWS) {
+                    if (a.use_series)
+                        spa_correlate<L1, L2, true>(v, t, k2, wt + c, NC, nullptr, 0, tc->k_lo, tc->k_hi, tc->A1, tc->A2,
+                                                    tc->A3, tc->A5, ub, inv, (float)c);
+                    else
+                        spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
+                } else {
+                    spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
+                }
+            }
         } else {
 #pragma unroll
             for (int u = 0; u < E / R1; ++u) {
@@ -483,13 +687,25 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
             }
         }
 
-        // the copy engine may still be reading the previous template's output tile out of the exchange buffer
-        if (threadIdx.x == 0) bulk_store_wait_read();
-        __syncthreads();
-        fft_core<L1, NZ1, NC, SYNC_BLOCK, false>(v, t, smem + c, 0, 1, NoHook(), TWTAB ? tw : nullptr);
+        if constexpr (DUMP) {
+#pragma unroll
+            for (int r = 0; r < R1; ++r)
+                a.Y[(size_t)b * n_total + (size_t)(t + T * r) * L2 + k2] = v[r];
+            cp_async_wait_all();
+            __syncthreads();
+            continue;
+        }
+        if (!step1_done) {
+            // the copy engine may still be reading the previous template's output tile out of the exchange buffer
+            if (threadIdx.x == 0) bulk_store_wait_read();
+            __syncthreads();
+            fft_core_step1<L1, NZ1, NC>(v, t, smem + c);
+        }
+        fft_core_tail<L1, NC, SYNC_BLOCK, false>(v, t, smem + c, 0, 1, NoHook(), TWTAB ? tw : nullptr);
 
         // Y[b][tile] (L1 rows of NC columns) is one contiguous block of the tile-major buffer: build it in
         // the exchange buffer, unpadded, and hand it to the copy engine in one piece.
+        if constexpr (MODE == LOAD_GEN) cp_async_wait_all();   // the next template's constants have landed
         __syncthreads();                              // every step-2 read of the exchange buffer is done
         c2* __restrict__ ot = smem + (size_t)t * NC + c;
 #pragma unroll
@@ -499,7 +715,6 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 256 ? 2 : 1)) p
                 ot[(size_t)(T * u + (L1 / RL) * q) * NC] = v[u * RL + q];     // row j1 = t + T u + (L1/RL) q
         }
         fence_async_smem();
-        if constexpr (MODE == LOAD_GEN) cp_async_wait_all();   // the next template's constants have landed
         __syncthreads();
         if (threadIdx.x == 0)
             bulk_store(a.Y + (size_t)b * n_total + (size_t)tile * L1 * NC, smem, (unsigned)(sizeof(c2) * L1 * NC));
@@ -1097,19 +1312,25 @@ __global__ void snr_from_z_kernel(const float2* __restrict__ z, float* __restric
     if (i < n) snr[i] = sqrtf(fmaf(z[i].x, z[i].x, z[i].y * z[i].y)) * inv_sigma;
 }
 
-// h~[k] = f_k^{-7/6} e^{-i Psi_T(f_k)} on the band, zero elsewhere, k = 0..N/2
-__global__ void debug_template_kernel(const TemplCoef* __restrict__ tc, const double* __restrict__ u,
-                                      float2* __restrict__ h, int n_half, double df)
+// h~[k] = f_k^{-7/6} conj(q[k]) for k < N/2 (q = the product generator's e^{+i Psi_T} on the band, zero elsewhere,
+// dumped by p1_kernel<LOAD_GEN_DUMP> with unit weights); h~[N/2] = 0.
+__global__ void debug_template_kernel(const c2* __restrict__ q, float2* __restrict__ h, int n_half, double df)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k > n_half) return;
     float2 o = make_float2(0.f, 0.f);
-    if (k >= tc->k_lo && k <= tc->k_hi) {
-        const c2 ph = spa_phasor_u(u[k], tc->A1, tc->A2, tc->A3, tc->A5);
+    if (k >= 1 && k < n_half) {
+        const c2 e = q[k];
         const float amp = (float)pow((double)k * df, -7.0 / 6.0);
-        o = make_float2(amp * re(ph), -amp * im(ph));
+        o = make_float2(amp * re(e), -amp * im(e));
     }
     h[k] = o;
+}
+
+__global__ void fill_ones_kernel(c2* __restrict__ w, int n)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) w[k] = pk(1.0f, 0.0f);
 }
 
 // generator alone: q~[b][k] = w[k] e^{+i Psi_b(f_k)}, k < N/2  (config-4 generator throughput)
