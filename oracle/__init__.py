@@ -69,6 +69,8 @@ def lib():
         L.orc_snr_series.argtypes = [C.c_void_p, C.c_double, C.c_double, dp, dp, dp]
         L.orc_filter_bank.argtypes = [C.c_void_p, dp, C.c_int64, C.c_double, C.POINTER(Peak),
                                       C.POINTER(Trigger), C.c_int64, C.POINTER(C.c_int64)]
+        L.orc_cluster_triggers.argtypes = [C.POINTER(Trigger), C.c_int64, C.c_int64, C.c_int64,
+                                           C.POINTER(Trigger), C.c_int64, C.POINTER(C.c_int64)]
         L.orc_num_threads.restype = C.c_int
         L.orc_set_num_threads.argtypes = [C.c_int]
         _lib = L
@@ -108,6 +110,19 @@ def band(n: int, fs: float, f_low: float, m1: float, m2: float):
     if rc:
         raise OracleError(rc, "orc_band")
     return klo.value, khi.value
+
+
+def cluster_triggers(trig: np.ndarray, n_samples: int, window: int, capacity: int | None = None):
+    """NEXT-1 twin: -> (events[TRIG_DTYPE], n_events, rc).  trig: TRIG_DTYPE records."""
+    t = np.ascontiguousarray(trig, dtype=TRIG_DTYPE)
+    cap = len(t) if capacity is None else int(capacity)
+    out = np.zeros(max(cap, 1), dtype=TRIG_DTYPE)
+    n = C.c_int64()
+    rc = lib().orc_cluster_triggers(t.ctypes.data_as(C.POINTER(Trigger)), len(t), int(n_samples), int(window),
+                                    out.ctypes.data_as(C.POINTER(Trigger)), cap, C.byref(n))
+    if rc < 0:
+        raise OracleError(rc, "orc_cluster_triggers")
+    return out[:min(n.value, cap)], n.value, rc
 
 
 def num_threads() -> int:

@@ -21,7 +21,9 @@
  * listed in DESIGN.md.
  *
  * Parity pins (tests/test_oracle_pins.py): every exported function is pinned;
- * none is "parity unpinned".
+ * none is "parity unpinned".  (orc_cluster_triggers, the SURVEY.md §8(f) NEXT-1
+ * twin added in round 2, is pinned by hand-built trigger lists whose clusters
+ * follow from the definition by inspection: test_cluster_*.)
  *
  * Threads: OpenMP across templates only (orc_filter_bank).
  */
@@ -399,6 +401,81 @@ int orc_filter_bank(const orc_ctx *c, const double *bank_m1m2, int64_t n_templat
     if (n_trig_found) *n_trig_found = total;
     if (err) return err;
     return (total > written && trig_out) ? ORC_WTRUNC : ORC_OK;
+}
+
+/* ------------------------------------------------- trigger clustering */
+
+/* "Reduce the [c(t_0)] set, in order to detect local maximum" (PAPER.md:103,
+ * the step after the threshold; done on the CPU).  The paper
+ * gives no rule and no window; reading A24:
+ *   two above-threshold samples of the SAME template belong to one event if
+ *   they are linked by a chain of above-threshold samples of that template in
+ *   which consecutive links are at most `window` samples apart, distances
+ *   taken on the circle of n_samples (the filter output is circular, A11);
+ *   an event is reported as its sample of largest SNR, the smallest sample
+ *   index among equal maxima; events are listed by (template, that sample).
+ * Written as the definition: pairwise distances and the transitive closure
+ * (O(n^2) per template), no sorting assumption on the input.
+ * out may be NULL (count only); at most out_capacity events are written
+ * (rc = ORC_WTRUNC if there are more), *n_out is always the full count. */
+int orc_cluster_triggers(const orc_trigger *trig, int64_t n_trig, int64_t n_samples,
+                         int64_t window, orc_trigger *out, int64_t out_capacity, int64_t *n_out)
+{
+    if ((!trig && n_trig) || n_trig < 0 || n_samples <= 0 || window < 0 || out_capacity < 0 || !n_out)
+        return ORC_EINVAL;
+    *n_out = 0;
+    if (n_trig == 0) return ORC_OK;
+    for (int64_t i = 0; i < n_trig; ++i)
+        if (trig[i].sample_idx < 0 || trig[i].sample_idx >= n_samples || trig[i].template_idx < 0) return ORC_EINVAL;
+    int64_t *label = (int64_t *)malloc(sizeof(int64_t) * (size_t)n_trig);
+    orc_trigger *ev = (orc_trigger *)malloc(sizeof(orc_trigger) * (size_t)n_trig);
+    if (!label || !ev) { free(label); free(ev); return ORC_ENOMEM; }
+    for (int64_t i = 0; i < n_trig; ++i) label[i] = i;
+    /* transitive closure: lower the labels of linked pairs until nothing changes */
+    for (int changed = 1; changed;) {
+        changed = 0;
+        for (int64_t i = 0; i < n_trig; ++i)
+            for (int64_t j = i + 1; j < n_trig; ++j) {
+                if (trig[i].template_idx != trig[j].template_idx || label[i] == label[j]) continue;
+                int64_t d = trig[i].sample_idx - trig[j].sample_idx;
+                if (d < 0) d = -d;
+                if (n_samples - d < d) d = n_samples - d;          /* distance on the circle */
+                if (d <= window) {
+                    int64_t m = label[i] < label[j] ? label[i] : label[j];
+                    label[i] = label[j] = m;
+                    changed = 1;
+                }
+            }
+    }
+    /* one event per label: largest SNR, smallest sample index among equals */
+    int64_t n_ev = 0;
+    for (int64_t i = 0; i < n_trig; ++i) {
+        if (label[i] != i) continue;                               /* i is the smallest member: the label */
+        orc_trigger best = trig[i];
+        for (int64_t j = 0; j < n_trig; ++j) {
+            if (label[j] != i) continue;
+            if (trig[j].snr > best.snr || (trig[j].snr == best.snr && trig[j].sample_idx < best.sample_idx))
+                best = trig[j];
+        }
+        ev[n_ev++] = best;
+    }
+    /* order by (template, sample): plain insertion sort */
+    for (int64_t i = 1; i < n_ev; ++i) {
+        orc_trigger x = ev[i];
+        int64_t j = i - 1;
+        while (j >= 0 && (ev[j].template_idx > x.template_idx ||
+                          (ev[j].template_idx == x.template_idx && ev[j].sample_idx > x.sample_idx))) {
+            ev[j + 1] = ev[j];
+            --j;
+        }
+        ev[j + 1] = x;
+    }
+    int64_t w = 0;
+    for (int64_t i = 0; i < n_ev; ++i)
+        if (out && w < out_capacity) out[w++] = ev[i];
+    *n_out = n_ev;
+    free(label); free(ev);
+    return (out && n_ev > w) ? ORC_WTRUNC : ORC_OK;
 }
 
 /* Threads orc_filter_bank will use (for bench.py's cpu_baseline "cores"). */

@@ -505,3 +505,103 @@ def test_oracle_under_sanitizers(tmp_path):
     env = dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", OMP_NUM_THREADS="2")
     r = subprocess.run([exe], capture_output=True, text=True, env=env, timeout=120)
     assert r.returncode == 0 and "asan driver ok" in r.stdout, (r.returncode, r.stdout, r.stderr[-2000:])
+
+
+# ------------------------------------------------------------------ NEXT-1: trigger clustering
+# Pins: hand-built trigger lists whose events follow from the definition (reading A24) by inspection.
+
+def _tr(rows):
+    a = np.zeros(len(rows), dtype=oracle.TRIG_DTYPE)
+    for i, (t, j, r) in enumerate(rows):
+        a[i] = (t, j, r, 0.1 * i)
+    return a
+
+
+def _ev(ev):
+    return [(int(e["template_idx"]), int(e["sample_idx"]), float(e["snr"])) for e in ev]
+
+
+def test_cluster_single_run_keeps_its_maximum():
+    tr = _tr([(0, 100, 6.5), (0, 101, 7.5), (0, 102, 9.0), (0, 103, 8.0), (0, 104, 6.1)])
+    ev, n, rc = oracle.cluster_triggers(tr, 1 << 12, 2)
+    assert rc == 0 and n == 1 and _ev(ev) == [(0, 102, 9.0)]
+    assert ev[0]["phase"] == tr[2]["phase"]                        # the whole record of the maximum is kept
+
+
+def test_cluster_gap_rule_is_inclusive_at_window():
+    base = [(0, 10, 7.0), (0, 15, 8.0)]                            # 5 samples apart
+    assert oracle.cluster_triggers(_tr(base), 4096, 5)[1] == 1     # gap == window: one event
+    ev, n, _ = oracle.cluster_triggers(_tr(base), 4096, 4)         # gap > window: two events
+    assert n == 2 and _ev(ev) == [(0, 10, 7.0), (0, 15, 8.0)]
+    assert oracle.cluster_triggers(_tr(base), 4096, 0)[1] == 2     # window 0: every sample its own event
+
+
+def test_cluster_chain_links_far_ends():
+    """Samples 0, 3, 6, 9 with window 3 are one event although 0 and 9 are 9 apart (chain rule)."""
+    tr = _tr([(2, 0, 6.1), (2, 3, 6.2), (2, 6, 6.9), (2, 9, 6.3), (2, 20, 7.7)])
+    ev, n, _ = oracle.cluster_triggers(tr, 4096, 3)
+    assert n == 2 and _ev(ev) == [(2, 6, 6.9), (2, 20, 7.7)]
+
+
+def test_cluster_wraps_around_the_segment_end():
+    """The filter output is circular (A11): N-2 and 1 are 3 samples apart."""
+    n_s = 1024
+    tr = _tr([(0, 1, 6.5), (0, 500, 7.0), (0, n_s - 2, 8.5)])
+    ev, n, _ = oracle.cluster_triggers(tr, n_s, 3)
+    assert n == 2 and _ev(ev) == [(0, 500, 7.0), (0, n_s - 2, 8.5)]
+    ev, n, _ = oracle.cluster_triggers(tr, n_s, 2)
+    assert n == 3
+    # a ring of triggers that closes on itself is ONE event
+    ring = _tr([(0, j, 6.0 + 0.001 * j) for j in range(0, n_s, 4)])
+    ev, n, _ = oracle.cluster_triggers(ring, n_s, 4)
+    assert n == 1 and _ev(ev) == [(0, n_s - 4, 6.0 + 0.001 * (n_s - 4))]
+
+
+def test_cluster_ties_take_the_smallest_sample():
+    tr = _tr([(0, 40, 7.0), (0, 41, 9.0), (0, 42, 9.0), (0, 43, 8.0)])
+    ev, n, _ = oracle.cluster_triggers(tr, 4096, 1)
+    assert _ev(ev) == [(0, 41, 9.0)]
+    n_s = 256                                                      # tie across the wrap: sample 0 < sample N-1
+    tr = _tr([(0, n_s - 1, 9.0), (0, 0, 9.0)])
+    assert _ev(oracle.cluster_triggers(tr, n_s, 1)[0]) == [(0, 0, 9.0)]
+
+
+def test_cluster_templates_never_merge_and_order_is_template_then_sample():
+    tr = _tr([(3, 100, 6.5), (1, 100, 7.0), (1, 101, 7.5), (3, 101, 6.6), (0, 4000, 8.0), (1, 900, 6.2)])   # unsorted input
+    ev, n, rc = oracle.cluster_triggers(tr, 4096, 8)
+    assert rc == 0 and _ev(ev) == [(0, 4000, 8.0), (1, 101, 7.5), (1, 900, 6.2), (3, 101, 6.6)]
+
+
+def test_cluster_empty_count_only_truncation_and_errors():
+    ev, n, rc = oracle.cluster_triggers(_tr([]), 1024, 5)
+    assert n == 0 and rc == 0 and len(ev) == 0
+    tr = _tr([(0, 10, 7.0), (0, 100, 8.0), (1, 5, 6.5)])
+    ev, n, rc = oracle.cluster_triggers(tr, 1024, 5, capacity=2)
+    assert n == 3 and rc == oracle.WTRUNC and _ev(ev) == [(0, 10, 7.0), (0, 100, 8.0)]
+    ev, n, rc = oracle.cluster_triggers(tr, 1024, 5, capacity=0)
+    assert n == 3 and len(ev) == 0
+    with pytest.raises(oracle.OracleError):
+        oracle.cluster_triggers(_tr([(0, 2000, 7.0)]), 1024, 5)    # sample outside the segment
+    with pytest.raises(oracle.OracleError):
+        oracle.cluster_triggers(tr, 1024, -1)
+
+
+def test_cluster_of_a_real_trigger_list_cfg0():
+    """configs[0] through the oracle: the SNR-12 injection gives a run of adjacent above-threshold samples in
+    the matching template; with a window of 16 samples it is ONE event at the peak sample, and the number of
+    events equals the number of runs counted directly from the series."""
+    w = W.config0()
+    o = oracle.Oracle(w.n, w.fs, w.f_low)
+    o.set_psd(w.psd)
+    o.load_segment(w.samples)
+    pk, tr, nf, _ = o.filter_bank(w.bank, w.threshold)
+    ev, n, rc = oracle.cluster_triggers(tr, w.n, 16)
+    mine = ev[ev["template_idx"] == 16]
+    assert len(mine) == 1 and int(mine[0]["sample_idx"]) == int(pk[16]["idx_peak"]) and mine[0]["snr"] == pk[16]["snr_max"]
+    # count runs directly: per template, sorted samples, a new run where the circular gap exceeds the window
+    runs = 0
+    for t in np.unique(tr["template_idx"]):
+        s = np.sort(tr["sample_idx"][tr["template_idx"] == t])
+        gaps = np.diff(np.concatenate([s, [s[0] + w.n]]))
+        runs += max(1, int(np.sum(gaps > 16)))
+    assert n == runs
