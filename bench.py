@@ -349,6 +349,22 @@ def measure(torch, dist, cbmf, wl, dev, local, world, K, Wm, cap, args, with_e2e
             e_ms, (nf_h, rc_h) = timed(step_host, K)
             barrier()
             out["e_ms_max"] = max_over_ranks(e_ms)
+            # the same step with the host-side reduction of PAPER.md:103 behind it, clustered while the GPU filters
+            # the following sub-batches: must not cost anything
+            ev_h = torch.empty(cap * 16, dtype=torch.uint8).pin_memory()
+
+            def step_host_clustered():
+                ctx.set_psd(psd_h)
+                ctx.load_segment(smp_h)
+                return ctx.filter_bank_clustered_into(bank_h, wl.threshold, args.cluster_window, peaks_h, ev_h, cap)
+
+            for _ in range(Wm):
+                step_host_clustered()
+            barrier()
+            c_ms, (n_ev, nf_c, rc_c) = timed(step_host_clustered, K)
+            barrier()
+            out["c_ms_max"] = max_over_ranks(c_ms)
+            out["n_events"] = int(n_ev)
             out["h2d"] = psd_h.numel() * 8 + smp_h.numel() * 4 + bank_h.numel() * 8
             # peaks, kept triggers, the early template-status word (8 B) and the trigger count (8 B)
             out["d2h"] = B * 16 + min(nf_h, cap) * 16 + 4 + 4 + 8 + 8
@@ -489,6 +505,10 @@ def run_ours(args):
         "segment_seconds_per_wall_second": (n / wl.fs) / (ms_max / K * 1e-3),
         "triggers_found": m["nf"], "peak_snr_max": float(m["peaks"]["snr_max"].max()),
         "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": int(m["h2d"]), "d2h_bytes_per_step": int(m["d2h"])},
+        "e2e_clustered": {"value": B * world * K / (m["c_ms_max"] * 1e-3), "unit": UNIT, "events": m["n_events"],
+                          "window_samples": args.cluster_window,
+                          "what": "cbmf_filter_bank_clustered: raw triggers reduced to events on the host while the GPU "
+                                  "filters the next sub-batches (NEXT-1, PAPER.md:103, :131)"},
         "gpu_launches": int(m["launches"]),
         "clocks": m["clocks"],
         "roofline": roofline,
@@ -512,6 +532,7 @@ def main():
     ap.add_argument("--streams", type=int, default=0, help="launch pairs in flight (0 = library default)")
     ap.add_argument("--trig-capacity", type=int, default=1 << 16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cluster-window", type=int, default=64, help="event window in samples for the e2e_clustered leg")
     ap.add_argument("--no-sustained", action="store_true", help="skip the cfg2 `sustained` record of the default run")
     ap.add_argument("--sustained-steps", type=int, default=3)
     args = ap.parse_args()

@@ -120,6 +120,31 @@ int cbmf_filter_bank_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_t n
  * EINVAL for that reason, else -1. */
 int64_t cbmf_last_bad_template(const cbmf_ctx *ctx);
 
+/* ---- trigger clustering ----
+ * "Reduce the [c(t_0)] set, in order to detect local maximum"; "The clusterization phase is made
+ * only by CPU.  This chose permits us to hide this computing part behind the next iteration".
+ * The paper states no rule; reading A24: above-threshold samples of ONE template form an event
+ * while consecutive ones are at most window_samples apart, the segment taken as a circle (the filter output is
+ * circular); an event is reported as its sample of largest snr (the whole trigger record), the smallest
+ * sample_idx among equal maxima; events are ordered by (template_idx, sample_idx). */
+
+/* Host function, no device work: trig[n_trig] must be sorted strictly by (template_idx, sample_idx) with
+ * 0 <= sample_idx < n_samples, as cbmf_filter_bank returns it.  Writes at most event_capacity events (the first ones
+ * in order; rc = CBMF_WTRUNC if there are more), *n_events = the full count.  EINVAL on an unsorted list, an index
+ * out of range, window_samples < 0 or a NULL n_events. */
+int cbmf_cluster_triggers(const cbmf_trigger *trig, int64_t n_trig, int64_t n_samples, int64_t window_samples,
+                          cbmf_trigger *events_out, int64_t event_capacity, int64_t *n_events);
+
+/* cbmf_filter_bank with the reduction behind it, overlapped as PAPER.md:131 describes: the bank runs as a stream of
+ * launch pairs (sub-batches); each pair's raw triggers are copied to pinned host memory right behind it and the
+ * host sorts and clusters them while the GPU filters the following pairs.  All pointers are HOST pointers.
+ * peaks_out[n_templates] as in cbmf_filter_bank; events_out[event_capacity] the events of the whole bank in
+ * (template_idx, sample_idx) order, truncated like the trigger list (CBMF_WTRUNC); *n_events the full event count;
+ * *n_trig_found (may be NULL) the number of raw above-threshold samples.  Same errors as cbmf_filter_bank. */
+int cbmf_filter_bank_clustered(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_templates, float snr_threshold,
+                               int64_t window_samples, cbmf_peak *peaks_out, cbmf_trigger *events_out,
+                               int64_t event_capacity, int64_t *n_events, int64_t *n_trig_found);
+
 /* ---- diagnostics: used by the parity tests and the kernel sweep, never by filter_bank ---- */
 
 /* rho[j] (n floats) and optionally z[j] (2n floats, interleaved re,im) for one template,

@@ -47,6 +47,8 @@ def lib() -> C.CDLL:
         "cbmf_load_segment_dev": (C.c_int, [vp, vp, i64]),
         "cbmf_filter_bank": (C.c_int, [vp, vp, i64, flt, vp, vp, i64, C.POINTER(i64)]),
         "cbmf_filter_bank_dev": (C.c_int, [vp, vp, i64, flt, vp, vp, i64, C.POINTER(i64)]),
+        "cbmf_cluster_triggers": (C.c_int, [vp, i64, i64, i64, vp, i64, C.POINTER(i64)]),
+        "cbmf_filter_bank_clustered": (C.c_int, [vp, vp, i64, flt, i64, vp, vp, i64, C.POINTER(i64), C.POINTER(i64)]),
         "cbmf_debug_snr_series": (C.c_int, [vp, Template, vp, vp]),
         "cbmf_debug_template": (C.c_int, [vp, Template, vp]),
         "cbmf_debug_ifft": (C.c_int, [vp, vp, vp, i64, i64]),
@@ -75,7 +77,8 @@ def lib() -> C.CDLL:
 
 
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
-           "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_debug_snr_series "
+           "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_cluster_triggers "
+           "cbmf_filter_bank_clustered cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
            "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
@@ -221,6 +224,38 @@ class Context:
         self._check(rc, "cbmf_filter_bank")
         return nf.value, rc
 
+    def filter_bank_clustered(self, bank, snr_threshold: float, window_samples: int, event_capacity: int = 1 << 16):
+        """Host arrays in, host arrays out: -> (peaks[PEAK_DTYPE], events[TRIG_DTYPE], n_events, n_trig_found, rc).
+        The host clusters each sub-batch's triggers while the GPU filters the next ones."""
+        b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+        nt = b.shape[0]
+        peaks = np.zeros(nt, dtype=PEAK_DTYPE)
+        ev = np.zeros(max(int(event_capacity), 1), dtype=TRIG_DTYPE)
+        ne, nf = C.c_int64(0), C.c_int64(0)
+        rc = lib().cbmf_filter_bank_clustered(self._h, b.ctypes.data if nt else None, nt, float(snr_threshold),
+                                              int(window_samples), peaks.ctypes.data if nt else None,
+                                              ev.ctypes.data if event_capacity else None, int(event_capacity),
+                                              C.byref(ne), C.byref(nf))
+        self._check(rc, "cbmf_filter_bank")
+        return peaks, ev[:min(ne.value, int(event_capacity))], ne.value, nf.value, rc
+
+    def filter_bank_clustered_into(self, bank, snr_threshold: float, window_samples: int, peaks_out, events_out,
+                                   event_capacity: int):
+        """Caller-owned HOST buffers (numpy / pinned tensors).  -> (n_events, n_trig_found, rc)"""
+        pb, dev = _ptr(bank, "float64")
+        pp, devp = _ptr(peaks_out, "peak records", itemsize=16)
+        pe, deve = _ptr(events_out, "trigger records", itemsize=16)
+        if dev or devp or deve:
+            raise ValueError("cbmf_filter_bank_clustered takes host arrays (the clustering runs on the host)")
+        nt = int((bank.numel() if _is_tensor(bank) else bank.size) // 2)
+        if _nbytes(peaks_out) < 16 * nt or (events_out is not None and _nbytes(events_out) < 16 * int(event_capacity)):
+            raise ValueError("output buffer too small")
+        ne, nf = C.c_int64(0), C.c_int64(0)
+        rc = lib().cbmf_filter_bank_clustered(self._h, pb, nt, float(snr_threshold), int(window_samples), pp, pe,
+                                              int(event_capacity), C.byref(ne), C.byref(nf))
+        self._check(rc, "cbmf_filter_bank")
+        return ne.value, nf.value, rc
+
     # -- diagnostics
     def debug_snr_series(self, m1: float, m2: float, want_z: bool = True):
         snr = np.empty(self.n, dtype=np.float32)
@@ -300,6 +335,20 @@ class Context:
         ms, nl = C.c_double(0), C.c_int64(0)
         self._check(lib().cbmf_last_pass_time(self._h, int(which), C.byref(ms), C.byref(nl)), "cbmf_last_pass_time")
         return ms.value, nl.value
+
+
+def cluster_triggers(trig, n_samples: int, window_samples: int, event_capacity: int | None = None):
+    """cbmf_cluster_triggers (host only): trig = TRIG_DTYPE records sorted by (template, sample).
+    -> (events[TRIG_DTYPE], n_events, rc)"""
+    t = np.ascontiguousarray(trig, dtype=TRIG_DTYPE)
+    cap = len(t) if event_capacity is None else int(event_capacity)
+    ev = np.zeros(max(cap, 1), dtype=TRIG_DTYPE)
+    n = C.c_int64(0)
+    rc = lib().cbmf_cluster_triggers(t.ctypes.data if len(t) else None, len(t), int(n_samples), int(window_samples),
+                                     ev.ctypes.data if cap else None, cap, C.byref(n))
+    if rc < 0:
+        raise CbmfError(rc, "cbmf_cluster_triggers")
+    return ev[:min(n.value, cap)], n.value, rc
 
 
 def version() -> str:

@@ -6,11 +6,13 @@
 // of kernels.cuh.  There is no CPU fallback and nothing here touches oracle/.
 #include "../../include/cbmf.h"
 #include "kernels.cuh"
+#include "cluster.h"
 
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <new>
 #include <unordered_set>
 #include <vector>
@@ -59,6 +61,14 @@ struct cbmf_ctx {
     unsigned int* d_tcount = nullptr;  int64_t tcount_cap = 0;    // [n_templates] triggers per template
     long long* d_bad = nullptr;            // [1] index of the first invalid template of the last bank, or LLONG_MAX
     int64_t last_bad = -1;
+
+    // clustered bank call (cbmf_filter_bank_clustered): per launch pair a device trigger region and cursor, copied
+    // to a ring of pinned host slots while later pairs run
+    TrigOut* d_ptrig = nullptr;            // [CBMF_MAX_STREAMS][PAIR_TRIG_CAP]
+    unsigned long long* d_pcursor = nullptr;   // [CBMF_MAX_STREAMS]
+    TrigOut* h_ptrig = nullptr;            // pinned [PIPE_RING][PAIR_TRIG_CAP]
+    unsigned long long* h_pcursor = nullptr;   // pinned [PIPE_RING]
+    cudaEvent_t ev_pipe[32] = {};
 
     int64_t launches = 0;
     int profiling = 0;                     // 0 off, 1 every launch alone on the context's stream, 2 in the real schedule
@@ -294,6 +304,8 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key); cudaFree(c->d_err); cudaFree(c->d_u);
     cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
     cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_tcount); cudaFree(c->d_bad);
+    cudaFree(c->d_ptrig); cudaFree(c->d_pcursor); cudaFreeHost(c->h_ptrig); cudaFreeHost(c->h_pcursor);
+    for (cudaEvent_t e : c->ev_pipe) if (e) cudaEventDestroy(e);
     for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
     for (int i = 0; i < CBMF_MAX_STREAMS; ++i) {
         if (c->aux[i]) { cudaStreamSynchronize(c->aux[i]); cudaStreamDestroy(c->aux[i]); }
@@ -692,6 +704,161 @@ extern "C" int cbmf_filter_bank(cbmf_ctx* c, const cbmf_template* bank, int64_t 
     CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
     return filter_bank_impl(c, c->d_bank, nt, thr, peaks_out, trig_out, trig_capacity, n_trig_found,
                             cudaMemcpyDeviceToHost);
+}
+
+// ======================================================================= NEXT-1: clustered bank call
+// The bank loop of cbmf_filter_bank with the host-side reduction of PAPER.md:103 / :131 behind it: every launch pair
+// (sub-batch) writes its raw triggers to its own device region; a copy to pinned host memory follows the pair on its
+// stream; the host enqueues pairs up to PIPE_RING ahead and, pair by pair as their copies complete, sorts and
+// clusters the triggers (cluster.h) WHILE the GPU filters the following pairs.
+namespace {
+constexpr int PIPE_RING = 32;                 // pairs enqueued ahead of the one the host is clustering
+constexpr int PAIR_TRIG_CAP = 4096;           // raw triggers kept per launch pair (64 KiB per copy)
+
+int pipe_alloc(cbmf_ctx* c)
+{
+    if (c->d_ptrig) return CBMF_OK;
+    CU(cudaMalloc(&c->d_ptrig, sizeof(TrigOut) * (size_t)CBMF_MAX_STREAMS * PAIR_TRIG_CAP));
+    CU(cudaMalloc(&c->d_pcursor, sizeof(unsigned long long) * CBMF_MAX_STREAMS));
+    CU(cudaMallocHost(&c->h_ptrig, sizeof(TrigOut) * (size_t)PIPE_RING * PAIR_TRIG_CAP));
+    CU(cudaMallocHost(&c->h_pcursor, sizeof(unsigned long long) * PIPE_RING));
+    for (int i = 0; i < PIPE_RING; ++i) CU(cudaEventCreateWithFlags(&c->ev_pipe[i], cudaEventDisableTiming));
+    return CBMF_OK;
+}
+}  // namespace
+
+extern "C" int cbmf_cluster_triggers(const cbmf_trigger* trig, int64_t n_trig, int64_t n_samples, int64_t window_samples,
+                                     cbmf_trigger* events_out, int64_t event_capacity, int64_t* n_events)
+{
+    if ((!trig && n_trig) || n_trig < 0 || n_samples <= 0 || window_samples < 0 || event_capacity < 0 || !n_events)
+        return CBMF_EINVAL;
+    if (event_capacity > 0 && !events_out) return CBMF_EINVAL;
+    *n_events = 0;
+    std::vector<HostTrig> ev;
+    if (!cluster_sorted(reinterpret_cast<const HostTrig*>(trig), n_trig, n_samples, window_samples, ev)) return CBMF_EINVAL;
+    const int64_t n = (int64_t)ev.size(), kept = n < event_capacity ? n : event_capacity;
+    if (kept) memcpy(events_out, ev.data(), sizeof(HostTrig) * (size_t)kept);
+    *n_events = n;
+    return n > event_capacity ? CBMF_WTRUNC : CBMF_OK;
+}
+
+extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank, int64_t nt, float thr,
+                                          int64_t window_samples, cbmf_peak* peaks_out, cbmf_trigger* events_out,
+                                          int64_t event_capacity, int64_t* n_events, int64_t* n_trig_found)
+{
+    int rc = filter_args_ok(c, bank, nt, thr, peaks_out, events_out, event_capacity);
+    if (rc) return rc;
+    if (window_samples < 0 || !n_events) return CBMF_EINVAL;
+    *n_events = 0;
+    if (n_trig_found) *n_trig_found = 0;
+    c->last_bad = -1;
+    if (nt == 0) return CBMF_OK;
+    DeviceGuard g(c->device);
+    if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
+    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_tcount, c->tcount_cap, nt))) return rc;
+    if ((rc = pipe_alloc(c))) return rc;
+    CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
+
+    const long long no_bad = 0x7FFFFFFFFFFFFFFFLL;
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
+    CU(cudaMemcpyAsync(c->d_bad, &no_bad, sizeof(long long), cudaMemcpyHostToDevice, c->stream));
+    SetupArgs sa;
+    sa.bank = c->d_bank; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
+    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
+    sa.threshold = thr; sa.err_flag = c->d_err; sa.bad_idx = c->d_bad;
+    template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    long long bad = no_bad;
+    CU(cudaMemcpyAsync(&bad, c->d_bad, sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (bad != no_bad) { c->last_bad = (int64_t)bad; return CBMF_EINVAL; }
+
+    const int sb = c->sub_batch, ns = c->n_streams;
+    const size_t ncand = cand_per_template(c);
+    const int64_t n_pairs = (nt + sb - 1) / sb;
+    CU(cudaEventRecord(c->ev_fork, c->stream));
+    for (int s = 0; s < ns; ++s) CU(cudaStreamWaitEvent(c->aux[s], c->ev_fork, 0));
+
+    std::vector<HostTrig> events;
+    std::vector<int64_t> overflow;              // pairs whose raw list did not fit PAIR_TRIG_CAP: filtered again below
+    int64_t found_total = 0;
+    auto enqueue = [&](int64_t pair) -> int {
+        const int64_t t0 = pair * sb;
+        const int nb = (int)((nt - t0 < sb) ? (nt - t0) : sb);
+        const int slot = (int)(pair % ns), ring = (int)(pair % PIPE_RING);
+        cudaStream_t st = c->aux[slot];
+        c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
+        CU(cudaMemsetAsync(c->d_pcursor + slot, 0, sizeof(unsigned long long), st));
+        P1Args a1; memset(&a1, 0, sizeof(a1));
+        a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+        CU(launch_p1<LOAD_GEN>(c, st, a1, nb));
+        P2Args a2; memset(&a2, 0, sizeof(a2));
+        a2.Y = Y; a2.coef = c->d_coef + t0;
+        a2.cand = c->d_cand + (size_t)slot * c->max_sub_batch * ncand;
+        a2.best_key = c->d_key + (size_t)slot * c->max_sub_batch;
+        a2.done_ctr = c->d_done + (size_t)slot * c->max_sub_batch; a2.peaks = c->d_peaks + t0;
+        a2.trig = c->d_ptrig + (size_t)slot * PAIR_TRIG_CAP;
+        a2.trig_cursor = c->d_pcursor + slot; a2.trig_cap = PAIR_TRIG_CAP;
+        a2.trig_count = c->d_tcount + t0;
+        a2.tmpl_base = (int)t0;
+        CU(launch_p2<EPI_MAX>(c, st, a2, nb));
+        c->launches += 2;
+        CU(cudaMemcpyAsync(c->h_pcursor + ring, c->d_pcursor + slot, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(c->h_ptrig + (size_t)ring * PAIR_TRIG_CAP, a2.trig, sizeof(TrigOut) * PAIR_TRIG_CAP,
+                           cudaMemcpyDeviceToHost, st));
+        CU(cudaEventRecord(c->ev_pipe[ring], st));
+        return CBMF_OK;
+    };
+    auto key_less = [](const HostTrig& a, const HostTrig& b) {
+        return a.template_idx != b.template_idx ? a.template_idx < b.template_idx : a.sample_idx < b.sample_idx;
+    };
+    int64_t next_enq = 0;
+    for (int64_t done = 0; done < n_pairs; ++done) {
+        // ns pairs share the ring slot's stream order; keep the ring one short of full so a slot is never re-armed
+        // before the host has consumed it
+        while (next_enq < n_pairs && next_enq - done < PIPE_RING - 1)
+            if ((rc = enqueue(next_enq++))) return rc;
+        const int ring = (int)(done % PIPE_RING);
+        CU(cudaEventSynchronize(c->ev_pipe[ring]));
+        const int64_t found = (int64_t)c->h_pcursor[ring];
+        found_total += found;
+        if (found > PAIR_TRIG_CAP) { overflow.push_back(done); continue; }
+        HostTrig* t = reinterpret_cast<HostTrig*>(c->h_ptrig + (size_t)ring * PAIR_TRIG_CAP);
+        std::sort(t, t + found, key_less);
+        if (!cluster_sorted(t, found, c->n, window_samples, events)) return CBMF_ECUDA;      // cannot happen: device indices are in range
+    }
+    for (int s = 0; s < ns; ++s) {
+        CU(cudaEventRecord(c->ev_join[s], c->aux[s]));
+        CU(cudaStreamWaitEvent(c->stream, c->ev_join[s], 0));
+    }
+    CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (!overflow.empty()) {
+        // a pair with more raw triggers than its region holds (a loud transient): filter its templates again through
+        // the plain call with a list that takes all of them, then cluster
+        PeakOut pk;
+        std::vector<HostTrig> raw((size_t)c->n);
+        for (int64_t pair : overflow) {
+            const int64_t t0 = pair * sb, nb = (nt - t0 < sb) ? (nt - t0) : sb;
+            for (int64_t i = 0; i < nb; ++i) {                     // template by template: at most n triggers each
+                int64_t nf = 0;
+                rc = filter_bank_impl(c, c->d_bank + 2 * (t0 + i), 1, thr, &pk, raw.data(), c->n, &nf, cudaMemcpyDeviceToHost);
+                if (rc < 0) return rc;
+                for (int64_t j = 0; j < nf; ++j) raw[(size_t)j].template_idx = (int32_t)(t0 + i);
+                if (!cluster_sorted(raw.data(), nf, c->n, window_samples, events)) return CBMF_ECUDA;
+            }
+        }
+        std::stable_sort(events.begin(), events.end(), key_less);
+    }
+    const int64_t n_ev = (int64_t)events.size(), kept = n_ev < event_capacity ? n_ev : event_capacity;
+    if (kept) memcpy(events_out, events.data(), sizeof(HostTrig) * (size_t)kept);
+    *n_events = n_ev;
+    if (n_trig_found) *n_trig_found = found_total;
+    return n_ev > event_capacity ? CBMF_WTRUNC : CBMF_OK;
 }
 
 // ======================================================================= diagnostics
