@@ -125,6 +125,46 @@ def cluster_triggers(trig: np.ndarray, n_samples: int, window: int, capacity: in
     return out[:min(n.value, cap)], n.value, rc
 
 
+def stream_segments(n_total: int, n: int, discard: int):
+    """Segment starts of NEXT-2 (reading A25): hop = n - discard, as many whole segments as fit."""
+    if not (0 <= discard < n) or n_total < n:
+        raise ValueError("bad stream geometry")
+    hop = n - discard
+    return [s * hop for s in range((n_total - n) // hop + 1)]
+
+
+def filter_stream(n: int, fs: float, f_low: float, psd: np.ndarray, stream: np.ndarray, bank: np.ndarray,
+                  snr_threshold: float, discard: int):
+    """NEXT-2 twin (PAPER.md:247-255 table 4.1, :157): a continuous float32 stream is cut into segments of n samples
+    that overlap by `discard` samples; every segment is matched-filtered on its own (circular, as orc_snr_series
+    defines it) and the first `discard` output samples, which the wrap-around of templates up to that length
+    corrupts, are left out of the peak and of the trigger list.  Written as the definition: per segment and template
+    the full series from orc_snr_series, then numpy's argmax / comparison on the slice [discard, n).
+    -> (peaks[S, B] PEAK_DTYPE with idx_peak relative to the segment start, triggers TRIG_DTYPE (sample_idx relative
+        to the segment start, sorted by (template, sample) inside each segment), seg_offsets int64[S + 1],
+        seg_starts list)"""
+    starts = stream_segments(len(stream), n, discard)
+    b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+    o = Oracle(n, fs, f_low)
+    o.set_psd(psd)
+    peaks = np.zeros((len(starts), len(b)), dtype=PEAK_DTYPE)
+    trig, offs = [], [0]
+    for si, s0 in enumerate(starts):
+        o.load_segment(np.ascontiguousarray(stream[s0:s0 + n], dtype=np.float32))
+        for ti, (m1, m2) in enumerate(b):
+            rho, z, sigma = o.snr_series(m1, m2)
+            if not sigma > 0:
+                peaks[si, ti] = (0.0, -1, 0.0, 0.0)
+                continue
+            j = discard + int(np.argmax(rho[discard:]))               # first maximum = smallest index
+            peaks[si, ti] = (rho[j], j, np.angle(z[j]), sigma)
+            for jj in discard + np.nonzero(rho[discard:] > snr_threshold)[0]:
+                trig.append((ti, int(jj), rho[jj], np.angle(z[jj])))
+        offs.append(len(trig))
+    o.close()
+    return peaks, np.array(trig, dtype=TRIG_DTYPE), np.array(offs, dtype=np.int64), starts
+
+
 def num_threads() -> int:
     return lib().orc_num_threads()
 
