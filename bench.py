@@ -372,6 +372,44 @@ def measure(torch, dist, cbmf, wl, dev, local, world, K, Wm, cap, args, with_e2e
     return out
 
 
+# PAPER.md:249-254, table 4.1: vector size, low-frequency cut, max templates processed in real time (GTX 275)
+PAPER_ONLINE = ((18, 30.0, 3435), (19, 23.0, 4095), (20, 15.0, 4478), (21, 14.0, 4279))
+
+
+def online_capacity(torch, cbmf, local, n_templates=2048, n_segments=4):
+    """NEXT-2: the paper's online figure through cbmf_filter_stream: [1.4, 1.4] Msun templates,
+    fs = 4096 Hz, the paper's vector sizes and cut-offs, segments overlapping by half (what its table implies:
+    4478 = 128 s / 28.6 ms at 2^20); capacity = templates that fit into the hop time of one segment."""
+    from testsupport import workloads as W
+    fs, rows = 4096.0, []
+    for log2n, f_low, paper in PAPER_ONLINE:
+        n = 1 << log2n
+        hop = n // 2
+        n_total = n + (n_segments - 1) * hop
+        big = 1 << int(math.ceil(math.log2(n_total)))
+        psd_big = W.onesided_psd("A", big, fs, f_low)
+        stream = W.to_time_domain(W.noise_spectrum(big, fs, f_low, psd_big, 900 + log2n), big, fs)[:n_total]
+        stream_h = torch.from_numpy(np.ascontiguousarray(stream)).pin_memory()
+        bank = W.draw_bank(910 + log2n, n_templates, 1.35, 1.45)
+        st = torch.cuda.Stream(device=torch.device("cuda", local))
+        with torch.cuda.stream(st):
+            ctx = cbmf.Context(n, fs, f_low, device=local, stream=st.cuda_stream)
+            ctx.set_psd(W.onesided_psd("A", n, fs, f_low))
+            ctx.filter_stream(stream_h, bank, 6.0, hop)                       # warm-up
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st)
+            pk, tr, offs, nf, rc = ctx.filter_stream(stream_h, bank, 6.0, hop)
+            b.record(st)
+            st.synchronize()
+            ms_seg = a.elapsed_time(b) / n_segments
+            ctx.close()
+        rows.append({"n_log2": log2n, "f_low_hz": f_low, "hop_s": hop / fs, "templates": n_templates, "segments": n_segments,
+                     "ms_per_segment": ms_seg, "us_per_template": 1e3 * ms_seg / n_templates,
+                     "max_templates_in_real_time": int(n_templates * (hop / fs) / (ms_seg * 1e-3)),
+                     "paper_gtx275": paper, "triggers": int(nf)})
+    return rows
+
+
 def spawn_ranks(args) -> int:
     """`python bench.py --gpus N` with N > 1 and no torchrun environment: start the N ranks ourselves
     (one process per GPU, rendezvous on 127.0.0.1) and pass rank 0's line through."""
@@ -430,6 +468,8 @@ def run_ours(args):
                            "note": "frac_of_fp32_peak counts the generator on the in-band bins only (mean n_b/N = 0.10 in cfg2); "
                                    "dense_equivalent_frac counts it on all N/2 bins (SURVEY.md §8(d))"},
         }
+
+    online = online_capacity(torch, cbmf, local) if (world == 1 and args.workload == "cfg1" and not args.no_online) else None
 
     if rank != 0:
         if world > 1:
@@ -513,6 +553,7 @@ def run_ours(args):
         "clocks": m["clocks"],
         "roofline": roofline,
         "sustained": sustained,
+        "online_capacity": online,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line))
@@ -533,6 +574,7 @@ def main():
     ap.add_argument("--trig-capacity", type=int, default=1 << 16)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cluster-window", type=int, default=64, help="event window in samples for the e2e_clustered leg")
+    ap.add_argument("--no-online", action="store_true", help="skip the online_capacity record (cbmf_filter_stream, PAPER.md table 4.1)")
     ap.add_argument("--no-sustained", action="store_true", help="skip the cfg2 `sustained` record of the default run")
     ap.add_argument("--sustained-steps", type=int, default=3)
     args = ap.parse_args()

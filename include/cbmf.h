@@ -145,6 +145,31 @@ int cbmf_filter_bank_clustered(cbmf_ctx *ctx, const cbmf_template *bank, int64_t
                                int64_t window_samples, cbmf_peak *peaks_out, cbmf_trigger *events_out,
                                int64_t event_capacity, int64_t *n_events, int64_t *n_trig_found);
 
+/* ---- segment streaming ----
+ * The online use of PAPER.md:247-255 (table 4.1: templates processed in real time) with the data kept on the device
+ * (PAPER.md:157-165).  A continuous stream samples[n_total] (HOST pointer, float32; pinned memory lets the copies
+ * overlap) is cut into segments of n samples (the context's n) that overlap by `discard` samples: segment s starts
+ * at s * (n - discard), and as many whole segments as fit are processed (*n_segments).  Every segment is filtered
+ * on its own, circularly, exactly as cbmf_load_segment + cbmf_filter_bank do; the first `discard` output samples of a
+ * segment, which the wrap-around of templates up to that length corrupts, take no part in its peaks or triggers
+ * (overlap-save; reading A25: the paper's table implies discard = n/2).  The template constants are
+ * set up once; while the bank runs on segment s, segment s + 1 is copied to the device and transformed on a second
+ * stream into a second weight buffer.
+ *   peaks_out[n_segments * n_templates]  segment-major; idx_peak counts from the start of ITS segment (>= discard)
+ *   trig_out[trig_capacity]              the triggers of segment 0, then 1, ...; inside a segment sorted by
+ *                                        (template_idx, sample_idx), sample_idx counted from the segment start
+ *   seg_offsets_out[n_segments + 1]      (may be NULL) segment s owns trig_out[seg_offsets_out[s] .. [s + 1])
+ *   n_trig_found                         (may be NULL) all above-threshold samples of all segments; when that exceeds
+ *                                        trig_capacity the list stops at the capacity (whole leading triggers of the
+ *                                        segment that crosses it, later segments empty) and rc = CBMF_WTRUNC
+ * Global sample index of a peak or trigger = s * (n - discard) + its index.  The call leaves no loaded segment in
+ * the context (ESTATE for cbmf_filter_bank until the next cbmf_load_segment).  ESTATE without a PSD; EINVAL for
+ * discard outside [0, n), n_total < n, a NaN / Inf sample, an invalid template (cbmf_last_bad_template). */
+int cbmf_filter_stream(cbmf_ctx *ctx, const float *samples, int64_t n_total, const cbmf_template *bank,
+                       int64_t n_templates, float snr_threshold, int64_t discard, cbmf_peak *peaks_out,
+                       cbmf_trigger *trig_out, int64_t trig_capacity, int64_t *seg_offsets_out,
+                       int64_t *n_trig_found, int64_t *n_segments);
+
 /* ---- diagnostics: used by the parity tests and the kernel sweep, never by filter_bank ---- */
 
 /* rho[j] (n floats) and optionally z[j] (2n floats, interleaved re,im) for one template,

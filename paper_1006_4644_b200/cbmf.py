@@ -49,6 +49,7 @@ def lib() -> C.CDLL:
         "cbmf_filter_bank_dev": (C.c_int, [vp, vp, i64, flt, vp, vp, i64, C.POINTER(i64)]),
         "cbmf_cluster_triggers": (C.c_int, [vp, i64, i64, i64, vp, i64, C.POINTER(i64)]),
         "cbmf_filter_bank_clustered": (C.c_int, [vp, vp, i64, flt, i64, vp, vp, i64, C.POINTER(i64), C.POINTER(i64)]),
+        "cbmf_filter_stream": (C.c_int, [vp, vp, i64, vp, i64, flt, i64, vp, vp, i64, vp, C.POINTER(i64), C.POINTER(i64)]),
         "cbmf_debug_snr_series": (C.c_int, [vp, Template, vp, vp]),
         "cbmf_debug_template": (C.c_int, [vp, Template, vp]),
         "cbmf_debug_ifft": (C.c_int, [vp, vp, vp, i64, i64]),
@@ -78,7 +79,7 @@ def lib() -> C.CDLL:
 
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_cluster_triggers "
-           "cbmf_filter_bank_clustered cbmf_debug_snr_series "
+           "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
            "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
@@ -255,6 +256,30 @@ class Context:
                                               int(event_capacity), C.byref(ne), C.byref(nf))
         self._check(rc, "cbmf_filter_bank")
         return ne.value, nf.value, rc
+
+    def filter_stream(self, samples, bank, snr_threshold: float, discard: int, trig_capacity: int = 1 << 16):
+        """cbmf_filter_stream on a host float32 stream (numpy or pinned tensor).
+        -> (peaks[S, B] PEAK_DTYPE, triggers TRIG_DTYPE, seg_offsets int64[S + 1], n_found, rc)"""
+        if isinstance(samples, np.ndarray):
+            samples = np.ascontiguousarray(samples, dtype=np.float32)
+        ps, dev = _ptr(samples, "float32")
+        if dev:
+            raise ValueError("cbmf_filter_stream takes a host stream")
+        n_total = int(samples.numel() if _is_tensor(samples) else samples.size)
+        b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+        nt = b.shape[0]
+        hop = self.n - int(discard)
+        n_seg = (n_total - self.n) // hop + 1 if (0 < hop <= self.n and n_total >= self.n) else 1
+        peaks = np.zeros((max(n_seg, 1), nt), dtype=PEAK_DTYPE)
+        trig = np.zeros(max(int(trig_capacity), 1), dtype=TRIG_DTYPE)
+        offs = np.zeros(max(n_seg, 1) + 1, dtype=np.int64)
+        nf, ns = C.c_int64(0), C.c_int64(0)
+        rc = lib().cbmf_filter_stream(self._h, ps, n_total, b.ctypes.data if nt else None, nt, float(snr_threshold),
+                                      int(discard), peaks.ctypes.data if nt else None,
+                                      trig.ctypes.data if trig_capacity else None, int(trig_capacity),
+                                      offs.ctypes.data, C.byref(nf), C.byref(ns))
+        self._check(rc, "cbmf_filter_bank")
+        return peaks[:ns.value], trig[:int(offs[ns.value])], offs[:ns.value + 1], nf.value, rc
 
     # -- diagnostics
     def debug_snr_series(self, m1: float, m2: float, want_z: bool = True):

@@ -64,6 +64,18 @@ struct cbmf_ctx {
 
     // clustered bank call (cbmf_filter_bank_clustered): per launch pair a device trigger region and cursor, copied
     // to a ring of pinned host slots while later pairs run
+    TemplCoef* d_segcoef = nullptr;        // [1] band constants of the load_segment epilogue
+    int after_enqueue = 0;                 // cbmf_filter_stream: call after_enqueue_fn once the bank's launches are enqueued
+    int64_t after_enqueue_seg = 0;
+    int (*after_enqueue_fn)(void*, int64_t) = nullptr;
+    void* after_enqueue_arg = nullptr;
+    // segment streaming (cbmf_filter_stream): second weight buffer, staging and scratch of the loader stream
+    c2* d_w2 = nullptr;                    // [N/2]
+    c2* d_segY = nullptr;                  // [N]
+    float* d_segin = nullptr;              // [N]
+    int* d_segerr = nullptr;               // [1]
+    cudaStream_t seg_stream = nullptr;
+    cudaEvent_t ev_seg_ready[2] = {};
     TrigOut* d_ptrig = nullptr;            // [CBMF_MAX_STREAMS][PAIR_TRIG_CAP]
     unsigned long long* d_pcursor = nullptr;   // [CBMF_MAX_STREAMS]
     TrigOut* h_ptrig = nullptr;            // pinned [PIPE_RING][PAIR_TRIG_CAP]
@@ -179,14 +191,14 @@ cudaError_t launch_p1_L(cbmf_ctx* c, cudaStream_t s, P1Args a, int batch)
 template <int L1, int L2, int MODE>
 constexpr int p2_items() { return L1 / (Cfg<L2>::ROWS * (MODE == EPI_MAX ? p2_rpw<L1, L2>() : 1)); }
 
-template <int L1, int L2, int MODE>
+template <int L1, int L2, int MODE, bool MASK = false>
 cudaError_t launch_p2_L(cbmf_ctx* c, cudaStream_t s, const P2Args& a, int batch)
 {
     const size_t smem = sizeof(c2) * (size_t)p2_row_stride<L2>() * Cfg<L2>::ROWS;
-    cudaError_t e = ensure_smem_attr(c, p2_kernel<L1, L2, MODE>, smem);
+    cudaError_t e = ensure_smem_attr(c, p2_kernel<L1, L2, MODE, MASK>, smem);
     if (e != cudaSuccess) return e;
     dim3 grid(p2_items<L1, L2, MODE>(), batch);
-    p2_kernel<L1, L2, MODE><<<grid, Cfg<L2>::NT2, smem, s>>>(a);
+    p2_kernel<L1, L2, MODE, MASK><<<grid, Cfg<L2>::NT2, smem, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -214,10 +226,10 @@ cudaError_t launch_p1(cbmf_ctx* c, cudaStream_t s, const P1Args& a, int batch)
 {
     CBMF_DISPATCH(c->lg1, c->lg2, (launch_p1_L<L1, L2, MODE>(c, s, a, batch)))
 }
-template <int MODE>
+template <int MODE, bool MASK = false>
 cudaError_t launch_p2(cbmf_ctx* c, cudaStream_t s, const P2Args& a, int batch)
 {
-    CBMF_DISPATCH(c->lg1, c->lg2, (launch_p2_L<L1, L2, MODE>(c, s, a, batch)))
+    CBMF_DISPATCH(c->lg1, c->lg2, (launch_p2_L<L1, L2, MODE, MASK>(c, s, a, batch)))
 }
 
 // candidate slots per template of the arg-max pass: one per (row j1, thread of the row group) = N / E2
@@ -304,6 +316,9 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key); cudaFree(c->d_err); cudaFree(c->d_u);
     cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
     cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_tcount); cudaFree(c->d_bad);
+    cudaFree(c->d_segcoef); cudaFree(c->d_w2); cudaFree(c->d_segY); cudaFree(c->d_segin); cudaFree(c->d_segerr);
+    if (c->seg_stream) { cudaStreamSynchronize(c->seg_stream); cudaStreamDestroy(c->seg_stream); }
+    for (cudaEvent_t e : c->ev_seg_ready) if (e) cudaEventDestroy(e);
     cudaFree(c->d_ptrig); cudaFree(c->d_pcursor); cudaFreeHost(c->h_ptrig); cudaFreeHost(c->h_pcursor);
     for (cudaEvent_t e : c->ev_pipe) if (e) cudaEventDestroy(e);
     for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
@@ -459,22 +474,32 @@ extern "C" int cbmf_set_psd(cbmf_ctx* c, const double* psd, int64_t n_bins)
 
 // ======================================================================= S1: load_segment
 // d~[k] = dt conj(IDFT(d)[k]) for real d, so the forward transform reuses the inverse kernels.
+// Enqueue only: samples_dev -> w_out on stream st, with Y_scratch (n complex) as the inter-pass buffer and *err_flag
+// set on a non-finite sample.
+static int enqueue_load_segment(cbmf_ctx* c, const float* samples_dev, c2* w_out, c2* Y_scratch, cudaStream_t st, int* err_flag)
+{
+    // k_lo travels to the EPI_WSTORE epilogue in a one-entry TemplCoef of its own (a bank may be reading d_coef)
+    if (!c->d_segcoef) {
+        CU(cudaMalloc(&c->d_segcoef, sizeof(TemplCoef)));
+        TemplCoef tc; memset(&tc, 0, sizeof(tc)); tc.k_lo = c->k_lo; tc.k_hi = (int)(c->n / 2 - 1);
+        CU(cudaMemcpy(c->d_segcoef, &tc, sizeof(tc), cudaMemcpyHostToDevice));
+    }
+    CU(cudaMemsetAsync(err_flag, 0, sizeof(int), st));
+    P1Args a1; memset(&a1, 0, sizeof(a1));
+    a1.in_r = samples_dev; a1.Y = Y_scratch; a1.err_flag = err_flag;
+    CU(launch_p1<LOAD_REAL>(c, st, a1, 1));
+    P2Args a2; memset(&a2, 0, sizeof(a2));
+    a2.Y = Y_scratch; a2.coef = c->d_segcoef; a2.w_out = w_out; a2.wfac = c->d_wfac;
+    CU(launch_p2<EPI_WSTORE>(c, st, a2, 1));
+    c->launches += 2;
+    return CBMF_OK;
+}
+
 static int load_segment_impl(cbmf_ctx* c, const float* samples_dev)
 {
     c->have_seg = false;
-    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
-    // k_lo travels to the EPI_WSTORE epilogue in a one-entry TemplCoef
-    int rc = grow(c, c->d_coef, c->coef_cap, 1);
+    int rc = enqueue_load_segment(c, samples_dev, c->d_w, c->d_Y, c->stream, c->d_err);
     if (rc) return rc;
-    TemplCoef tc; memset(&tc, 0, sizeof(tc)); tc.k_lo = c->k_lo; tc.k_hi = (int)(c->n / 2 - 1);
-    CU(cudaMemcpyAsync(c->d_coef, &tc, sizeof(tc), cudaMemcpyHostToDevice, c->stream));
-    P1Args a1; memset(&a1, 0, sizeof(a1));
-    a1.in_r = samples_dev; a1.Y = c->d_Y; a1.err_flag = c->d_err;
-    CU(launch_p1<LOAD_REAL>(c, c->stream, a1, 1));
-    P2Args a2; memset(&a2, 0, sizeof(a2));
-    a2.Y = c->d_Y; a2.coef = c->d_coef; a2.w_out = c->d_w; a2.wfac = c->d_wfac;
-    CU(launch_p2<EPI_WSTORE>(c, c->stream, a2, 1));
-    c->launches += 2;
     int err = 0;
     CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
@@ -543,8 +568,9 @@ static int sort_triggers(cbmf_ctx* c, int64_t count)
 
 // Pass-1 / pass-2 launch pairs for templates [0, nt) whose constants are in c->d_coef; peaks to c->d_peaks,
 // triggers to c->d_trig (dev_cap entries; the total is counted in c->d_cursor whatever the capacity).
-static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap)
+static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap, const c2* w = nullptr, int j_min = 0)
 {
+    if (!w) w = c->d_w;
     int rc;
     const int sb = c->sub_batch;
     // Launch pairs go round-robin over ns streams, each with its own slice of Y / cand / done, so
@@ -564,7 +590,7 @@ static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap)
         cudaStream_t st = (ns > 1) ? c->aux[slot] : c->stream;
         c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+        a1.w = w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
         if ((rc = ev_begin(c, 0, st))) return rc;
         CU(launch_p1<LOAD_GEN>(c, st, a1, nb));
         if ((rc = ev_end(c, 0, st))) return rc;
@@ -576,8 +602,10 @@ static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap)
         a2.trig_cursor = c->d_cursor; a2.trig_cap = (unsigned long long)dev_cap;
         a2.trig_count = c->d_tcount + t0;
         a2.tmpl_base = (int)t0;
+        a2.j_min = j_min;
         if ((rc = ev_begin(c, 1, st))) return rc;
-        CU(launch_p2<EPI_MAX>(c, st, a2, nb));
+        if (j_min > 0) CU((launch_p2<EPI_MAX, true>(c, st, a2, nb)));
+        else CU(launch_p2<EPI_MAX>(c, st, a2, nb));
         if ((rc = ev_end(c, 1, st))) return rc;
         c->launches += 2;
     }
@@ -587,30 +615,24 @@ static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap)
             CU(cudaStreamWaitEvent(c->stream, c->ev_join[s], 0));
         }
     }
+    if (c->after_enqueue && c->after_enqueue_fn) {
+        c->after_enqueue = 0;                   // once per bank (a truncated list repeats the passes)
+        if ((rc = c->after_enqueue_fn(c->after_enqueue_arg, c->after_enqueue_seg))) return rc;
+    }
     return CBMF_OK;
 }
 
-// bank_dev: [n][2] doubles on the device.  Outputs go to host or device pointers (out_kind).
-static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr,
-                            void* peaks_out, void* trig_out, int64_t trig_capacity,
-                            int64_t* n_trig_found, cudaMemcpyKind out_kind)
+// Template constants of a bank (S2) into c->d_coef, with the early check: an invalid template fails the call here,
+// before any filtering, and is named (cbmf_last_bad_template).  bank_dev: [n][2] doubles on the device.
+static int bank_setup(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr)
 {
-    if (n_trig_found) *n_trig_found = 0;
-    c->last_bad = -1;
-    if (nt == 0) return CBMF_OK;
     int rc;
+    c->last_bad = -1;
     if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
     if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
     if ((rc = grow(c, c->d_tcount, c->tcount_cap, nt))) return rc;
-    // device trigger buffer: capacity rounded up to a power of two (bitonic padding), >= 1
-    int64_t tcap = 1;
-    while (tcap < trig_capacity) tcap <<= 1;
-    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
-
     const long long no_bad = 0x7FFFFFFFFFFFFFFFLL;
     CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
-    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
-    CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
     CU(cudaMemcpyAsync(c->d_bad, &no_bad, sizeof(long long), cudaMemcpyHostToDevice, c->stream));
     SetupArgs sa;
     sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
@@ -619,14 +641,27 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     c->launches += 1;
-    // an invalid template fails the call here, before any filtering, and is named (cbmf_last_bad_template)
     long long bad = no_bad;
     CU(cudaMemcpyAsync(&bad, c->d_bad, sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (bad != no_bad) { c->last_bad = (int64_t)bad; return CBMF_EINVAL; }
+    return CBMF_OK;
+}
 
+// One bank pass over the segment whose weights are w (default: the context's), samples j < j_min excluded: filter,
+// count, sort and deliver.  Outputs go to host or device pointers (out_kind); *found_out = all triggers found.
+static int bank_filter(cbmf_ctx* c, int64_t nt, const c2* w, int j_min, void* peaks_out, void* trig_out,
+                       int64_t trig_capacity, int64_t* found_out, cudaMemcpyKind out_kind)
+{
+    int rc;
+    // device trigger buffer: capacity rounded up to a power of two (bitonic padding), >= 1
+    int64_t tcap = 1;
+    while (tcap < trig_capacity) tcap <<= 1;
+    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
+    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
+    CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
     c->ev_used[0] = c->ev_used[1] = 0;
-    if ((rc = run_bank_passes(c, nt, c->trig_cap))) return rc;
+    if ((rc = run_bank_passes(c, nt, c->trig_cap, w, j_min))) return rc;
 
     // trigger count back to the host, then sort what was kept
     unsigned long long found_u = 0;
@@ -634,7 +669,7 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     CU(cudaStreamSynchronize(c->stream));
     if ((rc = ev_collect(c))) return rc;
     const int64_t found = (int64_t)found_u;
-    if (n_trig_found) *n_trig_found = found;
+    if (found_out) *found_out = found;
     const int64_t kept = found < trig_capacity ? found : trig_capacity;
     if (kept > 0 && trig_out) {
         int64_t on_device = found;
@@ -655,7 +690,7 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
             CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
             const int prof = c->profiling;
             c->profiling = 0;                           // the repeat is not part of the per-pass timing
-            rc = run_bank_passes(c, t_cut + 1, c->trig_cap);
+            rc = run_bank_passes(c, t_cut + 1, c->trig_cap, w, j_min);
             c->profiling = prof;
             if (rc) return rc;
             on_device = cum;
@@ -666,6 +701,18 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, out_kind, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
+}
+
+static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr,
+                            void* peaks_out, void* trig_out, int64_t trig_capacity,
+                            int64_t* n_trig_found, cudaMemcpyKind out_kind)
+{
+    if (n_trig_found) *n_trig_found = 0;
+    c->last_bad = -1;
+    if (nt == 0) return CBMF_OK;
+    int rc;
+    if ((rc = bank_setup(c, bank_dev, nt, thr))) return rc;
+    return bank_filter(c, nt, c->d_w, 0, peaks_out, trig_out, trig_capacity, n_trig_found, out_kind);
 }
 
 static int filter_args_ok(cbmf_ctx* c, const void* bank, int64_t nt, float thr, void* peaks,
@@ -755,27 +802,10 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
     if (nt == 0) return CBMF_OK;
     DeviceGuard g(c->device);
     if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
-    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
-    if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
-    if ((rc = grow(c, c->d_tcount, c->tcount_cap, nt))) return rc;
     if ((rc = pipe_alloc(c))) return rc;
     CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
-
-    const long long no_bad = 0x7FFFFFFFFFFFFFFFLL;
-    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    if ((rc = bank_setup(c, c->d_bank, nt, thr))) return rc;
     CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
-    CU(cudaMemcpyAsync(c->d_bad, &no_bad, sizeof(long long), cudaMemcpyHostToDevice, c->stream));
-    SetupArgs sa;
-    sa.bank = c->d_bank; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
-    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = thr; sa.err_flag = c->d_err; sa.bad_idx = c->d_bad;
-    template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
-    CU(cudaGetLastError());
-    c->launches += 1;
-    long long bad = no_bad;
-    CU(cudaMemcpyAsync(&bad, c->d_bad, sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    if (bad != no_bad) { c->last_bad = (int64_t)bad; return CBMF_EINVAL; }
 
     const int sb = c->sub_batch, ns = c->n_streams;
     const size_t ncand = cand_per_template(c);
@@ -859,6 +889,86 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
     *n_events = n_ev;
     if (n_trig_found) *n_trig_found = found_total;
     return n_ev > event_capacity ? CBMF_WTRUNC : CBMF_OK;
+}
+
+// ======================================================================= NEXT-2: segment streaming
+extern "C" int cbmf_filter_stream(cbmf_ctx* c, const float* samples, int64_t n_total, const cbmf_template* bank,
+                                  int64_t nt, float thr, int64_t discard, cbmf_peak* peaks_out,
+                                  cbmf_trigger* trig_out, int64_t trig_capacity, int64_t* seg_offsets_out,
+                                  int64_t* n_trig_found, int64_t* n_segments)
+{
+    if (!c || !samples || !n_segments || nt < 0 || trig_capacity < 0) return CBMF_EINVAL;
+    if (nt > 0 && (!bank || !peaks_out)) return CBMF_EINVAL;
+    if (trig_capacity > 0 && !trig_out) return CBMF_EINVAL;
+    if (!(thr >= 0.f) || nt > 0x7FFFFFFF) return CBMF_EINVAL;
+    if (discard < 0 || discard >= c->n || n_total < c->n) return CBMF_EINVAL;
+    if (!c->have_psd) return CBMF_ESTATE;
+    const int64_t n = c->n, hop = n - discard, n_seg = (n_total - n) / hop + 1;
+    *n_segments = n_seg;
+    if (n_trig_found) *n_trig_found = 0;
+    if (seg_offsets_out) seg_offsets_out[0] = 0;
+    c->last_bad = -1;
+    c->have_seg = false;                       // the context's own segment slot is used as buffer 0 of the stream
+    DeviceGuard g(c->device);
+    int rc;
+    if (!c->d_w2) {
+        CU(cudaMalloc(&c->d_w2, sizeof(c2) * (size_t)(n / 2)));
+        CU(cudaMalloc(&c->d_segY, sizeof(c2) * (size_t)n));
+        CU(cudaMalloc(&c->d_segin, sizeof(float) * (size_t)n));
+        CU(cudaMalloc(&c->d_segerr, sizeof(int)));
+        CU(cudaStreamCreateWithFlags(&c->seg_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&c->ev_seg_ready[i], cudaEventDisableTiming));
+    }
+    if (nt > 0) {
+        if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
+        CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
+        if ((rc = bank_setup(c, c->d_bank, nt, thr))) return rc;     // the constants serve every segment
+    }
+    c2* wbuf[2] = {c->d_w, c->d_w2};
+    auto load = [&](int64_t s) -> int {       // segment s: host -> device -> w[s % 2], all on the loader stream
+        CU(cudaMemcpyAsync(c->d_segin, samples + s * hop, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, c->seg_stream));
+        int r = enqueue_load_segment(c, c->d_segin, wbuf[s & 1], c->d_segY, c->seg_stream, c->d_segerr);
+        if (r) return r;
+        CU(cudaEventRecord(c->ev_seg_ready[s & 1], c->seg_stream));
+        return CBMF_OK;
+    };
+    CU(cudaStreamSynchronize(c->stream));
+    if ((rc = load(0))) return rc;
+    int64_t written = 0, found_total = 0;
+    bool truncated = false;
+    for (int64_t s = 0; s < n_seg; ++s) {
+        // the loader has had the previous bank's time to finish: its error flag first (a NaN / Inf sample)
+        int err = 0;
+        CU(cudaMemcpyAsync(&err, c->d_segerr, sizeof(int), cudaMemcpyDeviceToHost, c->seg_stream));
+        CU(cudaStreamSynchronize(c->seg_stream));
+        if (err) return CBMF_EINVAL;
+        // Segment s + 1 is loaded and transformed on the loader stream WHILE the bank runs on segment s
+        // (keep the data on the device; the other buffer was last read by the bank of segment s - 1,
+        // which has been collected).  The bank of segment s is enqueued first so that it owns the SMs.
+        if (nt == 0) { if (s + 1 < n_seg && (rc = load(s + 1))) return rc; if (seg_offsets_out) seg_offsets_out[s + 1] = 0; continue; }
+        const int64_t room = trig_capacity - written;
+        int64_t found = 0;
+        CU(cudaStreamWaitEvent(c->stream, c->ev_seg_ready[s & 1], 0));      // the bank forks from the context's stream
+        // bank_filter enqueues the whole bank and then waits for it; the next load must be enqueued in between, so
+        // hand it over as a hook that run_bank_passes calls after its last launch
+        c->after_enqueue = (s + 1 < n_seg) ? 1 : 0;
+        c->after_enqueue_seg = s + 1;
+        struct Hook { decltype(load)* f; } hk{&load};
+        c->after_enqueue_fn = [](void* p, int64_t seg) -> int { return (*static_cast<Hook*>(p)->f)(seg); };
+        c->after_enqueue_arg = &hk;
+        rc = bank_filter(c, nt, wbuf[s & 1], (int)discard, peaks_out + s * nt, trig_out ? trig_out + written : nullptr,
+                         room > 0 ? room : 0, &found, cudaMemcpyDeviceToHost);
+        c->after_enqueue = 0;
+        c->after_enqueue_fn = nullptr;
+        if (rc < 0) return rc;
+        if (rc == CBMF_WTRUNC) truncated = true;
+        found_total += found;
+        written += (found < room) ? found : (room > 0 ? room : 0);
+        if (seg_offsets_out) seg_offsets_out[s + 1] = written;
+    }
+    CU(cudaStreamSynchronize(c->seg_stream));
+    if (n_trig_found) *n_trig_found = found_total;
+    return truncated ? CBMF_WTRUNC : CBMF_OK;
 }
 
 // ======================================================================= diagnostics

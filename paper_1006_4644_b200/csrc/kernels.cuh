@@ -738,6 +738,7 @@ struct P2Args {
     unsigned long long trig_cap;
     unsigned int* trig_count;              // [batch] triggers found per template (for a deterministic truncated list)
     int tmpl_base;                         // bank index of template 0 of this sub-batch
+    int j_min;                             // MASK: samples j < j_min take no part in the peak or the trigger list
     // EPI_STORE
     c2* __restrict__ z_out;                // [batch][N], natural order
     // EPI_WSTORE (load_segment): w[k] = conj(Z[k]) * wfac[k] for k < N/2
@@ -812,7 +813,7 @@ struct P2Tw {
 // registers, then the epilogue of MODE.  Called by the T threads of one row group.  On entry the
 // copy of the row into sm has been started by p2_prefetch_row; next_j1 (or -1) is the row of the
 // same template (yb) whose copy is started as soon as the exchange buffer is free again.
-template <int L1, int L2, int MODE>
+template <int L1, int L2, int MODE, bool MASK = false>
 __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int b, const int t,
                                        c2* __restrict__ sm, const c2* __restrict__ yb, const int next_j1,
                                        P2Tw<L1, L2>& rtw)
@@ -921,12 +922,23 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
         // leaves z in its own candidate slot (j1, t) for the block that finishes the template.
         const TemplCoef* tc = a.coef + b;
         const float thr2 = tc->thr2, inv_sigma = tc->inv_sigma;
-        auto pw = [&](int e) { float x, y; unpk(v[e], x, y); return fmaf(x, x, y * y); };
+        // MASK (segment streaming): sample j = j1 + L1 j2 counts only if j >= j_min, i.e. j2 >= j2_min on this row;
+        // an excluded sample reads as -1, below every |z|^2 and every threshold
+        const int j2_min = MASK ? max(0, (a.j_min - j1 + L1 - 1) >> LG1) : 0;
+        auto pw = [&](int e) {
+            float x, y;
+            unpk(v[e], x, y);
+            float p = fmaf(x, x, y * y);
+            if constexpr (MASK) {
+                if (t + T * (e / RL) + (L2 / RL) * (e % RL) < j2_min) p = -1.0f;
+            }
+            return p;
+        };
         float m = pw(0);
 #pragma unroll
         for (int e = 1; e < E; ++e) m = fmaxf(m, pw(e));
         const unsigned mbits = __float_as_uint(m);
-        if (mbits >= best_bits) {
+        if (mbits >= best_bits && (!MASK || m >= 0.f)) {
             // only the lanes holding the group's largest value go on (usually one per warp)
             unsigned gm = mbits;
             if constexpr (WSYNC) gm = __reduce_max_sync(__activemask(), mbits);
@@ -1023,7 +1035,7 @@ __device__ __forceinline__ void p2_finish(const P2Args& a, const int b, const in
 }
 
 // One item of pass 2: ROWS * RPW rows of template slot b.
-template <int L1, int L2, int MODE>
+template <int L1, int L2, int MODE, bool MASK = false>
 __device__ __forceinline__ void p2_item(const P2Args& a, const int item, const int b, c2* __restrict__ smem)
 {
     using C = Cfg<L2>;
@@ -1039,16 +1051,16 @@ __device__ __forceinline__ void p2_item(const P2Args& a, const int item, const i
 #pragma unroll 1
     for (int it = 0; it < RPW; ++it) {
         const int j1 = (item * RPW + it) * ROWS + row;
-        p2_row<L1, L2, MODE>(a, j1, b, t, sm, yb, (it + 1 < RPW) ? j1 + ROWS : -1, rtw);
+        p2_row<L1, L2, MODE, MASK>(a, j1, b, t, sm, yb, (it + 1 < RPW) ? j1 + ROWS : -1, rtw);
     }
     if constexpr (MODE == EPI_MAX) p2_finish<L1, L2>(a, b, L1 / (ROWS * RPW));
 }
 
-template <int L1, int L2, int MODE>
+template <int L1, int L2, int MODE, bool MASK = false>
 __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
 {
     extern __shared__ __align__(16) c2 smem[];
-    p2_item<L1, L2, MODE>(a, blockIdx.x, blockIdx.y, smem);
+    p2_item<L1, L2, MODE, MASK>(a, blockIdx.x, blockIdx.y, smem);
 }
 
 // ------------------------------------------------------------------ S0: PSD tables (fp64)
