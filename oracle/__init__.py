@@ -69,6 +69,7 @@ def lib():
         L.orc_snr_series.argtypes = [C.c_void_p, C.c_double, C.c_double, dp, dp, dp]
         L.orc_filter_bank.argtypes = [C.c_void_p, dp, C.c_int64, C.c_double, C.POINTER(Peak),
                                       C.POINTER(Trigger), C.c_int64, C.POINTER(C.c_int64)]
+        L.orc_chisq.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int64, C.c_int, dp, dp, C.POINTER(C.c_int64)]
         L.orc_cluster_triggers.argtypes = [C.POINTER(Trigger), C.c_int64, C.c_int64, C.c_int64,
                                            C.POINTER(Trigger), C.c_int64, C.POINTER(C.c_int64)]
         L.orc_num_threads.restype = C.c_int
@@ -229,6 +230,17 @@ class Oracle:
         if rc:
             raise OracleError(rc, "orc_snr_series")
         return rho, z, s.value
+
+    def chisq(self, m1: float, m2: float, j: int, p: int):
+        """NEXT-4 twin (ref. [24]): -> (chi^2, z_l complex128[p], band edges int64[p + 1])"""
+        chi = C.c_double()
+        zl = np.zeros(p, dtype=np.complex128)
+        edges = np.zeros(p + 1, dtype=np.int64)
+        rc = lib().orc_chisq(self._h, m1, m2, int(j), int(p), C.byref(chi), _dp(zl.view(np.float64)),
+                             edges.ctypes.data_as(C.POINTER(C.c_int64)))
+        if rc:
+            raise OracleError(rc, "orc_chisq")
+        return chi.value, zl, edges
 
     def filter_bank(self, bank: np.ndarray, snr_threshold: float, trig_capacity: int = 1 << 20):
         """-> (peaks[PEAK_DTYPE], triggers[TRIG_DTYPE], n_found, rc)"""

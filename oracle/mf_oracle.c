@@ -23,7 +23,9 @@
  * Parity pins (tests/test_oracle_pins.py): every exported function is pinned;
  * none is "parity unpinned".  (orc_cluster_triggers, the SURVEY.md §8(f) NEXT-1
  * twin added in round 2, is pinned by hand-built trigger lists whose clusters
- * follow from the definition by inspection: test_cluster_*.)
+ * follow from the definition by inspection: test_cluster_*; orc_chisq, the
+ * NEXT-4 twin, by sum_l z_l = z, chi^2 = 0 for data proportional to the
+ * template, <chi^2> = 2p - 2 in noise and equal band powers: test_chisq_*.)
  *
  * Threads: OpenMP across templates only (orc_filter_bank).
  */
@@ -401,6 +403,77 @@ int orc_filter_bank(const orc_ctx *c, const double *bank_m1m2, int64_t n_templat
     if (n_trig_found) *n_trig_found = total;
     if (err) return err;
     return (total > written && trig_out) ? ORC_WTRUNC : ORC_OK;
+}
+
+/* ------------------------------------------------- chi-squared veto */
+
+/* Allen's chi-squared time-frequency discriminator ("a optimized
+ * chi-squared [24] test routine", ref. [24] = PAPER.md:321, Phys. Rev. D 71,
+ * 062001) for one template at ONE output sample j.  Reading A26:
+ *   the template's band [k_lo, k_hi] is cut into p contiguous sub-bands of
+ *   (as nearly as the grid allows) equal expected SNR^2: with the running sum
+ *   S(k) = 4 df sum_{k'=k_lo..k} f_k'^{-7/3}/S_n[k'] (S(k_hi) = sigma^2), band l =
+ *   0..p-1 holds the bins k with  l sigma^2/p <= S(k-1) < (l+1) sigma^2/p
+ *   (S(k_lo - 1) = 0), i.e. a bin belongs to the band in which it STARTS;
+ *   z_l[j] = 4 df sum_{k in band l} d~[k] h~*[k]/S_n[k] e^{+2 pi i jk/n}  (so sum_l z_l = z[j]),
+ *   sigma_l^2 = 4 df sum_{k in band l} f_k^{-7/3}/S_n[k],  p_l = sigma_l^2/sigma^2,
+ *   chi^2 = sum_l |z_l - p_l z|^2 / (p_l sigma^2)   (bands with p_l = 0 contribute nothing).
+ * With unit-variance quadratures (A4) chi^2 has 2p - 2 degrees of freedom in
+ * Gaussian noise and vanishes for data proportional to the template.
+ * Written as the definition: direct sums over the bins, the phase of e^{2 pi i jk/n}
+ * from the exact integer jk mod n.  zl_out (2p doubles, may be NULL) receives z_l. */
+int orc_chisq(const orc_ctx *c, double m1, double m2, int64_t j, int p,
+              double *chisq_out, double *zl_out_or_null, int64_t *edges_out_or_null /* p+1 */)
+{
+    if (!c || !chisq_out || p < 1 || p > 4096) return ORC_EINVAL;
+    if (!c->psd || !c->dtil) return ORC_ESTATE;
+    if (j < 0 || j >= c->n) return ORC_EINVAL;
+    int64_t n = c->n, klo, khi;
+    int rc = orc_band(n, c->fs, c->f_low, m1, m2, &klo, &khi);
+    if (rc) return rc;
+    *chisq_out = 0.0;
+    if (khi < klo) return ORC_OK;
+    double sigma2 = 0.0;
+    rc = orc_sigma2(c, m1, m2, &sigma2);
+    if (rc) return rc;
+    double *zr = (double *)calloc((size_t)p, sizeof(double)), *zi = (double *)calloc((size_t)p, sizeof(double));
+    double *s2 = (double *)calloc((size_t)p, sizeof(double));
+    if (!zr || !zi || !s2) { free(zr); free(zi); free(s2); return ORC_ENOMEM; }
+    if (edges_out_or_null) for (int l = 0; l <= p; ++l) edges_out_or_null[l] = khi + 1;
+    double run = 0.0;                                   /* S(k - 1) */
+    int last = -1;
+    for (int64_t k = klo; k <= khi; ++k) {
+        int l = (int)floor(run / sigma2 * (double)p);
+        if (l > p - 1) l = p - 1;
+        if (edges_out_or_null && l != last) { for (int q = last + 1; q <= l; ++q) edges_out_or_null[q] = k; last = l; }
+        double f = (double)k * c->df;
+        double term = 4.0 * c->df * pow(f, -7.0 / 3.0) / c->psd[k];
+        double amp = pow(f, -7.0 / 6.0), psi = orc_psi(m1, m2, f);
+        double hr = amp * cos(psi), hi = amp * sin(psi);           /* conj(h~) = amp e^{+i psi} */
+        double dr = c->dtil[2 * k], di = c->dtil[2 * k + 1];
+        double wgt = 4.0 * c->df / c->psd[k];
+        double qr = wgt * (dr * hr - di * hi), qi = wgt * (dr * hi + di * hr);
+        int64_t jk = (int64_t)(((unsigned long long)j * (unsigned long long)k) % (unsigned long long)n);
+        double ang = 2.0 * ORC_PI * (double)jk / (double)n;
+        double cr = cos(ang), ci = sin(ang);
+        zr[l] += qr * cr - qi * ci;
+        zi[l] += qr * ci + qi * cr;
+        s2[l] += term;
+        run += term;
+    }
+    double ztr = 0.0, zti = 0.0;
+    for (int l = 0; l < p; ++l) { ztr += zr[l]; zti += zi[l]; }
+    double chi = 0.0;
+    for (int l = 0; l < p; ++l) {
+        double pl = s2[l] / sigma2;
+        if (!(pl > 0)) continue;
+        double er = zr[l] - pl * ztr, ei = zi[l] - pl * zti;
+        chi += (er * er + ei * ei) / (pl * sigma2);
+    }
+    if (zl_out_or_null) for (int l = 0; l < p; ++l) { zl_out_or_null[2 * l] = zr[l]; zl_out_or_null[2 * l + 1] = zi[l]; }
+    *chisq_out = chi;
+    free(zr); free(zi); free(s2);
+    return ORC_OK;
 }
 
 /* ------------------------------------------------- trigger clustering */

@@ -688,3 +688,69 @@ def test_stream_valid_half_is_free_of_wrap_around():
     assert int(np.argmax(a)) == int(np.argmax(b))
     # while the discarded part IS corrupted by what wraps around from the segment's end (the chirp itself)
     assert np.max(np.abs(rho1[:hop // 4] - rho2[hop:hop + hop // 4])) > 3 * np.max(np.abs(a - b))
+
+
+# ------------------------------------------------------------------ NEXT-4: chi-squared veto (ref. [24])
+
+def _orc(w):
+    o = oracle.Oracle(w.n, w.fs, w.f_low)
+    o.set_psd(w.psd)
+    o.load_segment(w.samples)
+    return o
+
+
+def test_chisq_bands_sum_to_the_filter_output_and_have_equal_power():
+    w = W.config0()
+    o = _orc(w)
+    m1, m2 = 1.4, 1.4
+    rho, z, sigma = o.snr_series(m1, m2)
+    klo, khi = oracle.band(w.n, w.fs, w.f_low, m1, m2)
+    f = np.arange(w.n // 2 + 1) * (w.fs / w.n)
+    for p in (1, 2, 8, 16):
+        for j in (0, 40960, 12345, w.n - 1):
+            chi, zl, edges = o.chisq(m1, m2, j, p)
+            assert abs(zl.sum() - z[j]) <= 1e-9 * abs(z).max()            # sum_l z_l = z[j] (pinned series, P13)
+            assert edges[0] == klo and edges[p] == khi + 1 and np.all(np.diff(edges) > 0)
+        # equal expected SNR^2 per band, to the granularity of one bin
+        term = 4.0 * (w.fs / w.n) * f[klo:khi + 1] ** (-7.0 / 3.0) / w.psd[klo:khi + 1]
+        s2 = np.array([term[edges[l] - klo:edges[l + 1] - klo].sum() for l in range(p)])
+        assert abs(s2.sum() - sigma ** 2) <= 1e-12 * sigma ** 2
+        assert np.max(np.abs(s2 - sigma ** 2 / p)) <= term.max() * 1.0000001
+    assert o.chisq(m1, m2, 40960, 1)[0] == 0.0                            # p = 1: identically zero
+
+
+def test_chisq_vanishes_for_data_proportional_to_the_template():
+    w = W.config0(noise=False)                                            # noise-free exact-parameter injection
+    o = _orc(w)
+    j = w.injections[0].sample(w.fs)
+    for p in (2, 8, 16):
+        chi, zl, _ = o.chisq(1.4, 1.4, j, p)
+        assert chi < 1e-9                                                 # against rho^2 = 144
+    # another template on the same data: the bands disagree
+    assert o.chisq(2.2, 1.1, j, 8)[0] > 1.0
+
+
+def test_chisq_has_2p_minus_2_degrees_of_freedom_in_noise():
+    w = W.sweep_point(16, 4)                                              # noise only, N = 2^16
+    o = _orc(w)
+    p = 8
+    js = np.arange(0, w.n, 97)[:400]
+    chis = np.array([o.chisq(w.bank[0, 0], w.bank[0, 1], int(j), p)[0] for j in js])
+    assert abs(chis.mean() - (2 * p - 2)) < 0.08 * (2 * p - 2)            # mean of a chi^2_14: 14 +- 0.26 over 400
+    assert abs(chis.var() - 2 * (2 * p - 2)) < 0.35 * 2 * (2 * p - 2)
+
+
+def test_chisq_rejects_a_glitch_that_rings_the_template():
+    """A loud impulse gives a large SNR in every template but its power is spread evenly over frequency, not as
+    f^-7/3: chi^2 per degree of freedom is far above 1, while the chirp of configs[0] in noise stays near 1."""
+    w = W.config0()
+    o = _orc(w)
+    j_inj = w.injections[0].sample(w.fs)
+    chi_sig = o.chisq(1.4, 1.4, j_inj, 16)[0]
+    assert chi_sig < 2.0 * 30
+    s = w.samples.copy(); s[30000] += 4.0e4
+    o.load_segment(s)
+    pk, _, _, _ = o.filter_bank(w.bank[16:17], 6.0)
+    assert pk[0]["snr_max"] > 12.0
+    chi_glitch = o.chisq(1.4, 1.4, int(pk[0]["idx_peak"]), 16)[0]
+    assert chi_glitch > 10 * 30
