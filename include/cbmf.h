@@ -170,6 +170,22 @@ int cbmf_filter_stream(cbmf_ctx *ctx, const float *samples, int64_t n_total, con
                        cbmf_trigger *trig_out, int64_t trig_capacity, int64_t *seg_offsets_out,
                        int64_t *n_trig_found, int64_t *n_segments);
 
+/* ---- chi-squared veto ----
+ * Allen's chi-squared time-frequency discriminator ("a optimized chi-squared [24] test routine";
+ * ref. [24] at PAPER.md:321: Phys. Rev. D 71, 062001), for every template of `bank` at ONE output sample of the
+ * loaded segment, sample_idx[t] (e.g. idx_peak of cbmf_filter_bank; a negative index gives chi^2 = 0, as does an
+ * empty band).  Reading A26: the band [k_lo, k_hi] of a template is cut into p_bands contiguous
+ * sub-bands of equal expected SNR^2 on the grid (bin k belongs to band floor(p P[k-1] / sigma^2), P the S0 prefix
+ * table); z_l = the filter output restricted to band l (sum_l z_l = z[sample]), p_l = sigma_l^2 / sigma^2,
+ *     chi^2 = sum_l |z_l - p_l z|^2 / (p_l sigma^2),
+ * which has 2 p_bands - 2 degrees of freedom in Gaussian noise (quadratures of unit variance) and vanishes for data
+ * proportional to the template.  One sample needs no FFT: the band sums are taken directly on the device in fp64
+ * from the same w[k] and SPA phase the filter uses.  All pointers are HOST pointers; chisq_out[n_templates];
+ * zl_out (may be NULL): n_templates * p_bands complex doubles (re, im), the z_l.  1 <= p_bands <= 256,
+ * n_templates <= 65535.  ESTATE before PSD and segment; EINVAL for an index >= n or an invalid template. */
+int cbmf_chisq(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_templates, const int32_t *sample_idx,
+               int p_bands, float *chisq_out, double *zl_out);
+
 /* ---- diagnostics: used by the parity tests and the kernel sweep, never by filter_bank ---- */
 
 /* rho[j] (n floats) and optionally z[j] (2n floats, interleaved re,im) for one template,

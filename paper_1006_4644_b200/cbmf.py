@@ -50,6 +50,7 @@ def lib() -> C.CDLL:
         "cbmf_cluster_triggers": (C.c_int, [vp, i64, i64, i64, vp, i64, C.POINTER(i64)]),
         "cbmf_filter_bank_clustered": (C.c_int, [vp, vp, i64, flt, i64, vp, vp, i64, C.POINTER(i64), C.POINTER(i64)]),
         "cbmf_filter_stream": (C.c_int, [vp, vp, i64, vp, i64, flt, i64, vp, vp, i64, vp, C.POINTER(i64), C.POINTER(i64)]),
+        "cbmf_chisq": (C.c_int, [vp, vp, i64, vp, C.c_int, vp, vp]),
         "cbmf_debug_snr_series": (C.c_int, [vp, Template, vp, vp]),
         "cbmf_debug_template": (C.c_int, [vp, Template, vp]),
         "cbmf_debug_ifft": (C.c_int, [vp, vp, vp, i64, i64]),
@@ -79,7 +80,7 @@ def lib() -> C.CDLL:
 
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_cluster_triggers "
-           "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_debug_snr_series "
+           "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_chisq cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
            "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
@@ -280,6 +281,19 @@ class Context:
                                       offs.ctypes.data, C.byref(nf), C.byref(ns))
         self._check(rc, "cbmf_filter_bank")
         return peaks[:ns.value], trig[:int(offs[ns.value])], offs[:ns.value + 1], nf.value, rc
+
+    def chisq(self, bank, sample_idx, p_bands: int, want_bands: bool = False):
+        """cbmf_chisq: chi^2 of every template at its own sample.  -> chisq float32[B] (, z_l complex128[B, p])"""
+        b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+        idx = np.ascontiguousarray(sample_idx, dtype=np.int32)
+        if len(idx) != len(b):
+            raise ValueError("one sample index per template")
+        chi = np.zeros(len(b), dtype=np.float32)
+        zl = np.zeros((len(b), int(p_bands)), dtype=np.complex128) if want_bands else None
+        rc = lib().cbmf_chisq(self._h, b.ctypes.data if len(b) else None, len(b), idx.ctypes.data if len(b) else None,
+                              int(p_bands), chi.ctypes.data if len(b) else None, zl.ctypes.data if want_bands else None)
+        self._check(rc, "cbmf_filter_bank")
+        return (chi, zl) if want_bands else chi
 
     # -- diagnostics
     def debug_snr_series(self, m1: float, m2: float, want_z: bool = True):

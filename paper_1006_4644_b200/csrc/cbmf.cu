@@ -971,6 +971,44 @@ extern "C" int cbmf_filter_stream(cbmf_ctx* c, const float* samples, int64_t n_t
     return truncated ? CBMF_WTRUNC : CBMF_OK;
 }
 
+// ======================================================================= NEXT-4: chi-squared veto
+extern "C" int cbmf_chisq(cbmf_ctx* c, const cbmf_template* bank, int64_t nt, const int32_t* sample_idx, int p_bands,
+                          float* chisq_out, double* zl_out)
+{
+    if (!c || nt < 0 || (nt > 0 && (!bank || !sample_idx || !chisq_out))) return CBMF_EINVAL;
+    if (p_bands < 1 || p_bands > CHISQ_MAX_BANDS || nt > 65535) return CBMF_EINVAL;
+    if (!c->have_psd || !c->have_seg) return CBMF_ESTATE;
+    for (int64_t i = 0; i < nt; ++i) if (sample_idx[i] >= c->n) return CBMF_EINVAL;       // < 0: no sample, chi^2 = 0
+    if (nt == 0) return CBMF_OK;
+    DeviceGuard g(c->device);
+    int rc;
+    if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
+    CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
+    if ((rc = bank_setup(c, c->d_bank, nt, 0.f))) return rc;
+    const int p = p_bands;
+    const size_t b_edges = sizeof(int) * (size_t)nt * (p + 1), b_idx = sizeof(int) * (size_t)nt;
+    const size_t b_zl = sizeof(double) * 2 * (size_t)nt * p, b_chi = sizeof(float) * (size_t)nt;
+    if ((rc = grow_scratch(c, b_zl + b_edges + b_idx + b_chi + 64))) return rc;
+    double* d_zl = (double*)c->d_scratch;
+    int* d_edges = (int*)(d_zl + 2 * (size_t)nt * p);
+    int* d_idx = d_edges + (size_t)nt * (p + 1);
+    float* d_chi = (float*)(d_idx + nt);
+    CU(cudaMemcpyAsync(d_idx, sample_idx, b_idx, cudaMemcpyHostToDevice, c->stream));
+    const int ne = (int)nt * (p + 1);
+    chisq_edges_kernel<<<(ne + 127) / 128, 128, 0, c->stream>>>(c->d_coef, c->d_prefix, p, d_edges, (int)nt);
+    CU(cudaGetLastError());
+    chisq_bands_kernel<<<dim3((unsigned)p, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_u, c->d_coef, d_edges, d_idx, p,
+                                                                                 c->log2n, d_zl);
+    CU(cudaGetLastError());
+    chisq_finish_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(c->d_coef, c->d_prefix, d_edges, d_zl, p, d_chi, (int)nt);
+    CU(cudaGetLastError());
+    c->launches += 3;
+    CU(cudaMemcpyAsync(chisq_out, d_chi, b_chi, cudaMemcpyDeviceToHost, c->stream));
+    if (zl_out) CU(cudaMemcpyAsync(zl_out, d_zl, b_zl, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return CBMF_OK;
+}
+
 // ======================================================================= diagnostics
 // One template's coefficients into d_coef[0] (threshold 0).
 static int setup_one(cbmf_ctx* c, cbmf_template t)

@@ -1317,6 +1317,104 @@ __global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, in
     for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = rec[pos[i]];
 }
 
+// ------------------------------------------------------------------ NEXT-4: chi-squared veto (ref. [24])
+// Allen's time-frequency discriminator at ONE output sample j per template.  The band [k_lo, k_hi] is cut into p
+// contiguous sub-bands of equal expected SNR^2 on the prefix table P (S0): bin k belongs to band
+// floor(p P[k-1] / sigma^2), i.e. band l starts at the first bin with P[k-1] >= l sigma^2 / p (reading A26).
+//   z_l = sum_{k in band l} w[k] e^{+i Psi(f_k)} e^{+2 pi i jk/N},  sigma_l^2 = P[last bin of l] - P[first bin - 1],
+//   chi^2 = sum_l |z_l - p_l z|^2 / (p_l sigma^2),  p_l = sigma_l^2 / sigma^2,  z = sum_l z_l.
+// A single sample needs no FFT: the sums are taken directly, one block per (band, template), in double.
+constexpr int CHISQ_MAX_BANDS = 256;
+
+__global__ void chisq_edges_kernel(const TemplCoef* __restrict__ coef, const double* __restrict__ prefix, int p,
+                                   int* __restrict__ edges /* [n][p + 1] */, int n_templates)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_templates * (p + 1)) return;
+    const int b = i / (p + 1), l = i % (p + 1);
+    const TemplCoef* tc = coef + b;
+    const int k_lo = tc->k_lo, k_hi = tc->k_hi;
+    int e = k_hi + 1;
+    if (k_hi >= k_lo && l < p) {
+        const double sigma2 = prefix[k_hi];
+        // smallest k in [k_lo, k_hi] with floor(p P[k-1] / sigma2) >= l  (P[k_lo - 1] = 0); monotone in k
+        int lo = k_lo, hi = k_hi + 1;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const double run = (mid > k_lo) ? prefix[mid - 1] : 0.0;
+            int band = (int)floor(run / sigma2 * (double)p);
+            if (band > p - 1) band = p - 1;
+            if (band >= l) hi = mid; else lo = mid + 1;
+        }
+        e = lo;
+    }
+    edges[i] = e;
+}
+
+__global__ void __launch_bounds__(256) chisq_bands_kernel(const c2* __restrict__ w, const double* __restrict__ u,
+                                                          const TemplCoef* __restrict__ coef,
+                                                          const int* __restrict__ edges, const int* __restrict__ sample_idx,
+                                                          int p, int log2n, double* __restrict__ zl /* [n][p][2] */)
+{
+    const int l = blockIdx.x, b = blockIdx.y;
+    const TemplCoef* tc = coef + b;
+    const int k0 = edges[b * (p + 1) + l], k1 = edges[b * (p + 1) + l + 1];
+    const long long j = sample_idx[b];
+    const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+    const unsigned long long mask = (1ULL << log2n) - 1ULL;
+    const float two_over_n = 2.0f / (float)(1ULL << log2n);
+    double sr = 0.0, si = 0.0;
+    if (j >= 0) {
+        for (int k = k0 + threadIdx.x; k < k1; k += blockDim.x) {
+            const c2 q = cmul(__ldg(w + k), spa_phasor_u(__ldg(u + k), A1, A2, A3, A5));
+            const c2 r = cmul(q, expi_frac((int)(((unsigned long long)j * (unsigned long long)k) & mask), two_over_n));
+            sr += (double)re(r);
+            si += (double)im(r);
+        }
+    }
+    __shared__ double s_r[8], s_i[8];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        sr += __shfl_down_sync(0xFFFFFFFFu, sr, off);
+        si += __shfl_down_sync(0xFFFFFFFFu, si, off);
+    }
+    if ((threadIdx.x & 31) == 0) { s_r[threadIdx.x >> 5] = sr; s_i[threadIdx.x >> 5] = si; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tr = 0.0, ti = 0.0;
+        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { tr += s_r[i]; ti += s_i[i]; }
+        zl[((size_t)b * p + l) * 2] = tr;
+        zl[((size_t)b * p + l) * 2 + 1] = ti;
+    }
+}
+
+__global__ void chisq_finish_kernel(const TemplCoef* __restrict__ coef, const double* __restrict__ prefix,
+                                    const int* __restrict__ edges, const double* __restrict__ zl, int p,
+                                    float* __restrict__ chisq, int n_templates)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_templates) return;
+    const TemplCoef* tc = coef + b;
+    float out = 0.f;
+    if (tc->k_hi >= tc->k_lo) {
+        const double sigma2 = prefix[tc->k_hi];
+        double zr = 0.0, zi = 0.0;
+        for (int l = 0; l < p; ++l) { zr += zl[((size_t)b * p + l) * 2]; zi += zl[((size_t)b * p + l) * 2 + 1]; }
+        double chi = 0.0;
+        for (int l = 0; l < p; ++l) {
+            const int e0 = edges[b * (p + 1) + l], e1 = edges[b * (p + 1) + l + 1];
+            if (e1 <= e0) continue;
+            const double s2 = prefix[e1 - 1] - ((e0 > tc->k_lo) ? prefix[e0 - 1] : 0.0);
+            const double pl = s2 / sigma2;
+            if (!(pl > 0.0)) continue;
+            const double er = zl[((size_t)b * p + l) * 2] - pl * zr, ei = zl[((size_t)b * p + l) * 2 + 1] - pl * zi;
+            chi += (er * er + ei * ei) / (pl * sigma2);
+        }
+        out = (float)chi;
+    }
+    chisq[b] = out;
+}
+
 // ------------------------------------------------------------------ diagnostics
 __global__ void snr_from_z_kernel(const float2* __restrict__ z, float* __restrict__ snr, size_t n, float inv_sigma)
 {
