@@ -58,6 +58,9 @@ def lib():
         L.orc_f_isco.restype = C.c_double
         L.orc_psi.argtypes = [C.c_double] * 3
         L.orc_psi.restype = C.c_double
+        L.orc_psi_pn.argtypes = [C.c_double] * 3 + [C.c_int]
+        L.orc_psi_pn.restype = C.c_double
+        L.orc_set_pn_order.argtypes = [C.c_void_p, C.c_int]
         L.orc_band.argtypes = [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double,
                                C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.orc_create.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.c_double, C.c_double]
@@ -99,6 +102,11 @@ def fft(x: np.ndarray, sign: int) -> np.ndarray:
 
 def psi(m1: float, m2: float, f: float) -> float:
     return lib().orc_psi(float(m1), float(m2), float(f))
+
+
+def psi_pn(m1: float, m2: float, f: float, half_order: int) -> float:
+    """SPA phase at 2PN (half_order 4) or 2.5PN (5): NEXT-3."""
+    return lib().orc_psi_pn(float(m1), float(m2), float(f), int(half_order))
 
 
 def f_isco(m1: float, m2: float) -> float:
@@ -194,6 +202,11 @@ class Oracle:
             self.close()
         except Exception:
             pass
+
+    def set_pn_order(self, half_order: int):
+        rc = lib().orc_set_pn_order(self._h, int(half_order))
+        if rc:
+            raise OracleError(rc, "orc_set_pn_order")
 
     def set_psd(self, psd: np.ndarray):
         p = np.ascontiguousarray(psd, dtype=np.float64)

@@ -58,6 +58,7 @@ typedef struct orc_ctx {
     double *psd;        /* n/2+1 one-sided S_n, or NULL */
     double *dtil;       /* 2*(n/2+1): d~[k] = dt * sum_j d[j] e^{-2 pi i jk/n}, or NULL */
     double *tw_re, *tw_im;   /* cos/sin(2 pi k / n), k < n/2, each evaluated directly */
+    int pn_half_order;       /* 4: 2PN phase (BASELINE.json configs[0], default); 5: + the 2.5PN term (NEXT-3) */
 } orc_ctx;
 
 /* ------------------------------------------------------------------ FFT */
@@ -147,6 +148,28 @@ double orc_psi(double m1, double m2, double f)
     return -ORC_PI / 4.0 + 3.0 / (128.0 * eta * v5) * br;
 }
 
+/* NEXT-3: the paper's stated order, "Post Newtonian approximation of order 2.5 in phase
+ * and 0 in amplitude".  The paper prints no formula; the 2.5PN term of the stationary-phase
+ * (TaylorF2) phase is taken from the literature -- Arun, Iyer, Sathyaprakash & Sundararajan, Phys. Rev. D 71,
+ * 084008 (2005), eq. (3.4); the same expression is eq. (3.18) of Buonanno, Iyer, Ochsner, Pan & Sathyaprakash,
+ * Phys. Rev. D 80, 084043 (2009):
+ *   Psi_2.5PN(f) = Psi_2PN(f) + 3/(128 eta v^5) * pi (38645/756 - 65 eta/9) (1 + 3 ln(v / v_lso)) v^5,
+ *   v = (pi M f)^{1/3},  v_lso = 6^{-1/2}  (so 3 ln(v/v_lso) = ln(f / f_ISCO)).
+ * half_order = 4 returns orc_psi.  Pin: tests/test_oracle_pins.py derives every coefficient up to v^5, this one
+ * included, from the 2.5PN energy function and flux by series division and two integrations (test_p3b_*). */
+double orc_psi_pn(double m1, double m2, double f, int half_order)
+{
+    double psi = orc_psi(m1, m2, f);
+    if (half_order >= 5) {
+        double M = (m1 + m2) * ORC_TSUN;
+        double eta = m1 * m2 / ((m1 + m2) * (m1 + m2));
+        double v = cbrt(ORC_PI * M * f);
+        double vlso = 1.0 / sqrt(6.0);
+        psi += 3.0 / (128.0 * eta) * ORC_PI * (38645.0 / 756.0 - 65.0 * eta / 9.0) * (1.0 + 3.0 * log(v / vlso));
+    }
+    return psi;
+}
+
 /* Band of a template on the DFT grid, SURVEY.md §8(c) item 2 / readings A6-A7:
  * k_lo = ceil(f_low N/fs), k_hi = min(floor(f_ISCO N/fs), N/2-1); empty if k_hi<k_lo. */
 int orc_band(int64_t n, double fs, double f_low, double m1, double m2,
@@ -180,6 +203,7 @@ int orc_create(orc_ctx **out, int64_t n, double fs_hz, double f_low_hz)
     if (!c) return ORC_ENOMEM;
     c->n = n; c->fs = fs_hz; c->f_low = f_low_hz;
     c->dt = 1.0 / fs_hz; c->df = fs_hz / (double)n;
+    c->pn_half_order = 4;
     c->tw_re = (double *)malloc(sizeof(double) * (size_t)(n / 2));
     c->tw_im = (double *)malloc(sizeof(double) * (size_t)(n / 2));
     if (!c->tw_re || !c->tw_im) { orc_destroy(c); return ORC_ENOMEM; }
@@ -188,6 +212,14 @@ int orc_create(orc_ctx **out, int64_t n, double fs_hz, double f_low_hz)
         c->tw_re[k] = cos(a); c->tw_im[k] = sin(a);
     }
     *out = c;
+    return ORC_OK;
+}
+
+/* Phase order of the templates of this context: 4 (2PN, default) or 5 (2.5PN, NEXT-3). */
+int orc_set_pn_order(orc_ctx *c, int half_order)
+{
+    if (!c || (half_order != 4 && half_order != 5)) return ORC_EINVAL;
+    c->pn_half_order = half_order;
     return ORC_OK;
 }
 
@@ -244,7 +276,7 @@ int orc_template(const orc_ctx *c, double m1, double m2, double *h_out)
     for (int64_t k = klo; k <= khi; ++k) {
         double f = (double)k * c->df;
         double amp = pow(f, -7.0 / 6.0);
-        double psi = orc_psi(m1, m2, f);
+        double psi = orc_psi_pn(m1, m2, f, c->pn_half_order);
         h_out[2 * k] = amp * cos(psi);
         h_out[2 * k + 1] = -amp * sin(psi);
     }
@@ -282,7 +314,7 @@ static int filter_z(const orc_ctx *c, double m1, double m2, double *z,
     for (int64_t k = klo; k <= khi; ++k) {
         double f = (double)k * c->df;
         double amp = pow(f, -7.0 / 6.0);
-        double psi = orc_psi(m1, m2, f);
+        double psi = orc_psi_pn(m1, m2, f, c->pn_half_order);
         /* conj(h~) = amp e^{+i psi} */
         double hr = amp * cos(psi), hi = amp * sin(psi);
         double dr = c->dtil[2 * k], di = c->dtil[2 * k + 1];
@@ -448,7 +480,7 @@ int orc_chisq(const orc_ctx *c, double m1, double m2, int64_t j, int p,
         if (edges_out_or_null && l != last) { for (int q = last + 1; q <= l; ++q) edges_out_or_null[q] = k; last = l; }
         double f = (double)k * c->df;
         double term = 4.0 * c->df * pow(f, -7.0 / 3.0) / c->psd[k];
-        double amp = pow(f, -7.0 / 6.0), psi = orc_psi(m1, m2, f);
+        double amp = pow(f, -7.0 / 6.0), psi = orc_psi_pn(m1, m2, f, c->pn_half_order);
         double hr = amp * cos(psi), hi = amp * sin(psi);           /* conj(h~) = amp e^{+i psi} */
         double dr = c->dtil[2 * k], di = c->dtil[2 * k + 1];
         double wgt = 4.0 * c->df / c->psd[k];

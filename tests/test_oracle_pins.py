@@ -754,3 +754,69 @@ def test_chisq_rejects_a_glitch_that_rings_the_template():
     assert pk[0]["snr_max"] > 12.0
     chi_glitch = o.chisq(1.4, 1.4, int(pk[0]["idx_peak"]), 16)[0]
     assert chi_glitch > 10 * 30
+
+
+# ------------------------------------------------------------------ NEXT-3: the 2.5PN phase term
+
+def _taylorf2_from_energy_balance(eta):
+    """Coefficients psi_n, n = 0..5, of Psi(f) = 3/(128 eta v^5) sum_n psi_n v^n (n = 5: the coefficient of ln f,
+    i.e. of 3 ln v), DERIVED here from the post-Newtonian energy function and flux by the stationary-phase relation
+    d^2 Psi / df^2 = 2 pi dt/df = -(2 pi^2 M^2 / 3) e'(v) / (v^2 F(v)),  v = (pi M f)^(1/3):
+    series division of e'(v) by F(v), then two integrations in f term by term (the v^5 term integrates to ln f).
+    Energy and flux to 2.5PN (Blanchet, Living Rev. Relativity 9, 4 (2006), eqs. (194) and (231), circular orbits):
+      e(v)  = -(eta v^2 / 2) [1 - (9 + eta)/12 v^2 - (81 - 57 eta + eta^2)/24 v^4]
+      F(v)  = (32/5) eta^2 v^10 [1 - (1247/336 + 35 eta/12) v^2 + 4 pi v^3
+              + (-44711/9072 + 9271 eta/504 + 65 eta^2/18) v^4 - (8191/672 + 583 eta/24) pi v^5]."""
+    from fractions import Fraction as Fr
+    import math
+    pi = math.pi
+    a2, a4 = -(9 + eta) / 12.0, -(81 - 57 * eta + eta ** 2) / 24.0
+    num = [1.0, 0.0, 2 * a2, 0.0, 3 * a4, 0.0]                                  # -e'(v) / (eta v)
+    den = [1.0, 0.0, -(1247 / 336 + 35 * eta / 12), 4 * pi,
+           -44711 / 9072 + 9271 * eta / 504 + 65 * eta ** 2 / 18, -(8191 / 672 + 583 * eta / 24) * pi]
+    s = []                                                                      # S(v) = num / den, power series
+    for n in range(6):
+        s.append(num[n] - sum(s[k] * den[n - k] for k in range(n)))
+    # Psi'' = K v^-11 S(v), K = 5 pi^2 M^2 / (48 eta); integrating f^alpha twice, alpha = (n - 11)/3:
+    # psi_n = 40 s_n / ((n - 8)(n - 5)) for n != 5, and the ln f coefficient is -(40/9) s_5 (see DESIGN.md §3 A27)
+    out = [40.0 * s[n] / ((n - 8) * (n - 5)) for n in range(5)]
+    out.append(-(40.0 / 9.0) * s[5])
+    return out
+
+
+@pytest.mark.parametrize("m1,m2", [(1.4, 1.4), (1.0, 3.0), (10.0, 1.2)])
+def test_p3b_phase_coefficients_follow_from_energy_balance(m1, m2):
+    """Pins BOTH the 2PN coefficients of orc_psi (already fixed by the survey's 40-digit values) and the 2.5PN term of
+    orc_psi_pn: extract the oracle's coefficients numerically and compare with the energy-balance derivation."""
+    eta = m1 * m2 / (m1 + m2) ** 2
+    want = _taylorf2_from_energy_balance(eta)
+    assert abs(want[0] - 1.0) < 1e-14 and abs(want[1]) < 1e-14
+    assert abs(want[2] - (3715 / 756 + 55 * eta / 9)) < 1e-12
+    assert abs(want[3] + 16 * np.pi) < 1e-12
+    assert abs(want[4] - (15293365 / 508032 + 27145 * eta / 504 + 3085 * eta ** 2 / 72)) < 1e-11
+    assert abs(want[5] - np.pi * (38645 / 756 - 65 * eta / 9)) < 1e-11
+    # the oracle's 2.5PN term, extracted as a function: [Psi_2.5 - Psi_2] * 128 eta / 3 = C (1 + ln(f / f_isco))
+    M = (m1 + m2) * 4.925490947641267e-6
+    fi = oracle.f_isco(m1, m2)
+    for f in (10.0, 40.0, 133.0, 900.0):
+        extra = (oracle.psi_pn(m1, m2, f, 5) - oracle.psi_pn(m1, m2, f, 4)) * 128 * eta / 3
+        assert abs(extra - want[5] * (1 + np.log(f / fi))) < 1e-9 * abs(want[5]) * 10
+        assert oracle.psi_pn(m1, m2, f, 4) == oracle.psi(m1, m2, f)
+    # and the full oracle phase against the derived series, evaluated independently
+    for f in (20.0, 100.0, 400.0):
+        v = (np.pi * M * f) ** (1 / 3)
+        series = -np.pi / 4 + 3 / (128 * eta * v ** 5) * (sum(want[n] * v ** n for n in range(5))
+                                                         + want[5] * v ** 5 * (1 + 3 * np.log(v * np.sqrt(6.0))))
+        assert abs(series - oracle.psi_pn(m1, m2, f, 5)) < 1e-9 * abs(series)
+
+
+def test_p3b_chirp_time_with_the_25pn_term():
+    """-(1/2 pi) dPsi/df = time to coalescence: the 2.5PN term adds C/(2 pi f) * 3/(128 eta), a few tenths of a second
+    at 40 Hz for 1.4 + 1.4 (the 2.5PN chirp-time term is negative in tau, i.e. the chirp is shorter)."""
+    m1 = m2 = 1.4
+    eta = 0.25
+    f, h = 40.0, 1e-3
+    tau = lambda order: -(oracle.psi_pn(m1, m2, f + h, order) - oracle.psi_pn(m1, m2, f - h, order)) / (2 * h) / (2 * np.pi)
+    c5 = np.pi * (38645 / 756 - 65 * eta / 9)
+    assert abs((tau(5) - tau(4)) + 3 / (128 * eta) * c5 / (2 * np.pi * f)) < 1e-6
+    assert -0.25 < tau(5) - tau(4) < -0.05
