@@ -206,6 +206,19 @@ int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_
 int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);
 int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
 
+/* ---- waveform order ----
+ * Phase order of the SPA templates, in half post-Newtonian orders: 4 = 2PN (default: BASELINE.json configs[0], the
+ * Psi_T of the header comment), 5 = 2.5PN, the order the paper states ("Post Newtonian approximation of order 2.5 in
+ * phase and 0 in amplitude"; its Fig. 4 title says "PN2").  The paper prints no formula; the 2.5PN term
+ * is the published one (Arun, Iyer, Sathyaprakash & Sundararajan, Phys. Rev. D 71, 084008 (2005), eq. 3.4 =
+ * Buonanno et al., Phys. Rev. D 80, 084043 (2009), eq. 3.18):
+ *     Psi += 3/(128 eta v^5) * pi (38645/756 - 65 eta/9) (1 + 3 ln(v / v_lso)) v^5,   v_lso = 6^{-1/2}.
+ * Applies to every later call (filter, stream, chisq, debug); amplitude, band and sigma do not change, so PSD and
+ * segment stay loaded.  EINVAL for any other value.  (The paper's own variant -- time-domain generation, forward
+ * FFT and normalisation by a reduction -- is not built: DESIGN.md §10.) */
+int cbmf_set_pn_order(cbmf_ctx *ctx, int half_order);
+int cbmf_get_pn_order(const cbmf_ctx *ctx);
+
 /* ---- tuning ---- */
 /* Templates per launch pair (pass 1 + pass 2).  Default: 512 MiB of inter-pass buffer
  * (8 n bytes per template) per pair, i.e. 64 templates at n = 2^20; results do not depend on it.

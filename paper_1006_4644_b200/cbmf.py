@@ -58,6 +58,8 @@ def lib() -> C.CDLL:
         "cbmf_debug_generate_dev": (C.c_int, [vp, vp, i64, vp]),
         "cbmf_debug_get_prefix": (C.c_int, [vp, vp]),
         "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
+        "cbmf_set_pn_order": (C.c_int, [vp, C.c_int]),
+        "cbmf_get_pn_order": (C.c_int, [vp]),
         "cbmf_set_sub_batch": (C.c_int, [vp, C.c_int]),
         "cbmf_get_sub_batch": (C.c_int, [vp]),
         "cbmf_set_streams": (C.c_int, [vp, C.c_int]),
@@ -82,7 +84,7 @@ EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_seg
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_cluster_triggers "
            "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_chisq cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
-           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_sub_batch cbmf_get_sub_batch "
+           "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_pn_order cbmf_get_pn_order cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
            "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_strerror "
            "cbmf_last_cuda_error cbmf_version").split()
@@ -340,6 +342,13 @@ class Context:
         w = np.empty(self.n // 2, dtype=np.complex64)
         self._check(lib().cbmf_debug_get_weights(self._h, w.ctypes.data), "cbmf_debug_get_weights")
         return w
+
+    def set_pn_order(self, half_order: int):
+        """4 = 2PN phase (default), 5 = 2.5PN (the paper's stated order, NEXT-3)."""
+        self._check(lib().cbmf_set_pn_order(self._h, int(half_order)), "cbmf_set_pn_order")
+
+    def get_pn_order(self) -> int:
+        return int(lib().cbmf_get_pn_order(self._h))
 
     # -- tuning / introspection
     def set_sub_batch(self, k: int):

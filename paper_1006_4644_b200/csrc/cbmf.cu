@@ -29,6 +29,7 @@ struct cbmf_ctx {
     double fs = 0, f_low = 0, df = 0, dt = 0;
     int k_lo = 0;
     bool have_psd = false, have_seg = false;
+    int pn_half_order = 4;                 // phase order of the templates: 4 = 2PN, 5 = 2.5PN (cbmf_set_pn_order)
     int sub_batch = 0;                     // templates per pass-1/pass-2 launch pair
     int max_sub_batch = 0;
     int n_streams = 1;                     // launch pairs in flight (each on its own stream and Y slice)
@@ -41,6 +42,7 @@ struct cbmf_ctx {
     double* d_prefix = nullptr;            // [N/2]
     double* d_bsum = nullptr;              // [ceil(N/2 / SCAN_TILE)] scan block totals / offsets
     double* d_u = nullptr;                 // [N/2] k^{-1/3}
+    double* d_lnk = nullptr;               // [N/2] ln k, built on the first cbmf_set_pn_order(5)
     c2* d_w = nullptr;                     // [N/2]
     c2* d_Y = nullptr;                     // [slots][N]
     c2* d_cand = nullptr;                  // [slots][N / E2] arg-max candidates, one per (row, thread)
@@ -314,7 +316,7 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     cudaStreamSynchronize(c->stream);
     cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_bsum); cudaFree(c->d_w);
     cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key); cudaFree(c->d_err); cudaFree(c->d_u);
-    cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
+    cudaFree(c->d_lnk); cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
     cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_tcount); cudaFree(c->d_bad);
     cudaFree(c->d_segcoef); cudaFree(c->d_w2); cudaFree(c->d_segY); cudaFree(c->d_segin); cudaFree(c->d_segerr);
     if (c->seg_stream) { cudaStreamSynchronize(c->seg_stream); cudaStreamDestroy(c->seg_stream); }
@@ -419,6 +421,23 @@ extern "C" int cbmf_set_streams(cbmf_ctx* c, int launch_pairs_in_flight)
 extern "C" int cbmf_get_streams(const cbmf_ctx* c) { return c ? c->n_streams : CBMF_EINVAL; }
 
 extern "C" int cbmf_get_sub_batch(const cbmf_ctx* c) { return c ? c->sub_batch : CBMF_EINVAL; }
+
+extern "C" int cbmf_set_pn_order(cbmf_ctx* c, int half_order)
+{
+    if (!c || (half_order != 4 && half_order != 5)) return CBMF_EINVAL;
+    if (half_order == 5 && !c->d_lnk) {
+        DeviceGuard g(c->device);
+        const size_t nh = (size_t)c->n / 2;
+        CU(cudaMalloc(&c->d_lnk, sizeof(double) * nh));
+        lnk_table_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(c->d_lnk, (int)nh);
+        CU(cudaGetLastError());
+        c->launches += 1;
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    c->pn_half_order = half_order;
+    return CBMF_OK;
+}
+extern "C" int cbmf_get_pn_order(const cbmf_ctx* c) { return c ? c->pn_half_order : CBMF_EINVAL; }
 
 extern "C" int cbmf_get_split(const cbmf_ctx* c, int* log2_n1, int* log2_n2)
 {
@@ -590,7 +609,7 @@ static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap, const c2* w
         cudaStream_t st = (ns > 1) ? c->aux[slot] : c->stream;
         c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+        a1.w = w; a1.u = c->d_u; a1.lnk = c->d_lnk; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
         if ((rc = ev_begin(c, 0, st))) return rc;
         CU(launch_p1<LOAD_GEN>(c, st, a1, nb));
         if ((rc = ev_end(c, 0, st))) return rc;
@@ -637,7 +656,7 @@ static int bank_setup(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr
     SetupArgs sa;
     sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = thr; sa.err_flag = c->d_err; sa.bad_idx = c->d_bad;
+    sa.threshold = thr; sa.err_flag = c->d_err; sa.bad_idx = c->d_bad; sa.pn_half_order = c->pn_half_order;
     template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     c->launches += 1;
@@ -824,7 +843,7 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
         c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         CU(cudaMemsetAsync(c->d_pcursor + slot, 0, sizeof(unsigned long long), st));
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+        a1.w = c->d_w; a1.u = c->d_u; a1.lnk = c->d_lnk; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
         CU(launch_p1<LOAD_GEN>(c, st, a1, nb));
         P2Args a2; memset(&a2, 0, sizeof(a2));
         a2.Y = Y; a2.coef = c->d_coef + t0;
@@ -997,7 +1016,7 @@ extern "C" int cbmf_chisq(cbmf_ctx* c, const cbmf_template* bank, int64_t nt, co
     const int ne = (int)nt * (p + 1);
     chisq_edges_kernel<<<(ne + 127) / 128, 128, 0, c->stream>>>(c->d_coef, c->d_prefix, p, d_edges, (int)nt);
     CU(cudaGetLastError());
-    chisq_bands_kernel<<<dim3((unsigned)p, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_u, c->d_coef, d_edges, d_idx, p,
+    chisq_bands_kernel<<<dim3((unsigned)p, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_u, c->d_lnk, c->d_coef, d_edges, d_idx, p,
                                                                                  c->log2n, d_zl);
     CU(cudaGetLastError());
     chisq_finish_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(c->d_coef, c->d_prefix, d_edges, d_zl, p, d_chi, (int)nt);
@@ -1021,7 +1040,7 @@ static int setup_one(cbmf_ctx* c, cbmf_template t)
     SetupArgs sa;
     sa.bank = c->d_bank; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = 1;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr;
+    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr; sa.pn_half_order = c->pn_half_order;
     template_setup_kernel<<<1, 32, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     c->launches += 1;
@@ -1046,7 +1065,7 @@ extern "C" int cbmf_debug_snr_series(cbmf_ctx* c, cbmf_template t, float* snr_ou
     CU(cudaMemcpyAsync(&tc, c->d_coef, sizeof(tc), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     P1Args a1; memset(&a1, 0, sizeof(a1));
-    a1.w = c->d_w; a1.u = c->d_u; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+    a1.w = c->d_w; a1.u = c->d_u; a1.lnk = c->d_lnk; a1.coef = c->d_coef; a1.Y = c->d_Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
     CU(launch_p1<LOAD_GEN>(c, c->stream, a1, 1));
     P2Args a2; memset(&a2, 0, sizeof(a2));
     a2.Y = c->d_Y; a2.z_out = z;
@@ -1076,7 +1095,7 @@ extern "C" int cbmf_debug_template(cbmf_ctx* c, cbmf_template t, float* h_out)
     fill_ones_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(ones, (int)nh);
     CU(cudaGetLastError());
     P1Args a1; memset(&a1, 0, sizeof(a1));
-    a1.w = ones; a1.u = c->d_u; a1.coef = c->d_coef; a1.Y = q; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+    a1.w = ones; a1.u = c->d_u; a1.lnk = c->d_lnk; a1.coef = c->d_coef; a1.Y = q; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
     CU(launch_p1<LOAD_GEN_DUMP>(c, c->stream, a1, 1));
     debug_template_kernel<<<(unsigned)((nh + 1 + 255) / 256), 256, 0, c->stream>>>(q, h, (int)nh, c->df);
     CU(cudaGetLastError());
@@ -1139,12 +1158,12 @@ extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_de
     SetupArgs sa;
     sa.bank = (const double*)bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr;
+    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr; sa.pn_half_order = c->pn_half_order;
     template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     const int nh = (int)(c->n / 2);
     int gx = (nh + 255) / 256; if (gx > 592) gx = 592;
-    generate_only_kernel<<<dim3(gx, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_u, c->d_coef, (c2*)q_out_dev, nh);
+    generate_only_kernel<<<dim3(gx, (unsigned)nt), 256, 0, c->stream>>>(c->d_w, c->d_u, c->d_lnk, c->d_coef, (c2*)q_out_dev, nh);
     CU(cudaGetLastError());
     c->launches += 2;
     int err = 0;

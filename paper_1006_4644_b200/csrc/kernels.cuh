@@ -22,13 +22,14 @@ namespace cbmf {
 
 // ------------------------------------------------------------------ per-template constants (S2)
 struct __align__(16) TemplCoef {
-    // phase in cycles: Psi/(2 pi) = -1/8 + u (A1 + u (A2 + u (A3 + u^2 A5))),  u = k^{-1/3}
+    // phase in cycles: Psi/(2 pi) = A0 + u (A1 + u (A2 + u (A3 + u^2 A5))) + AL ln k,  u = k^{-1/3};
+    // 2PN (BASELINE.json configs[0]): A0 = -1/8, AL = 0;  2.5PN (cbmf_set_pn_order, NEXT-3): AL ln k + const
     double A1, A2, A3, A5;
     int k_lo, k_hi;              // inclusive band on the DFT grid; empty if k_hi < k_lo
     float sigma, inv_sigma;      // sqrt(P[k_hi]), 1/sigma (0 for an empty band)
     float thr2;                  // (threshold * sigma)^2 : |z|^2 > thr2  <=>  rho > threshold
-    int nz_class;                // reserved
-    int pad_[2];
+    float A0;                    // constant term, reduced to [-1/2, 1/2) cycles
+    double AL;                   // coefficient of ln k (0 at 2PN)
 };
 static_assert(sizeof(TemplCoef) == 64, "TemplCoef layout");
 
@@ -285,13 +286,22 @@ __device__ __forceinline__ c2 fft_center_factor(const int t, const int e, const 
 // (rcbrt_table_kernel) or from the series of spa_correlate.  The reduced angle lies in [-pi, pi),
 // where the SFU sine/cosine (MUFU.SIN/COS) have absolute error <= 2^-21.4 (CUDA math API,
 // __sinf): a template mismatch of order 1e-13, against the 1e-6 bound of tests/parity.py.
-__device__ __forceinline__ c2 spa_phasor_u(const double u, const double A1, const double A2,
-                                           const double A3, const double A5)
+struct SpaCoef { double A1, A2, A3, A5, AL; float A0; };
+__device__ __forceinline__ SpaCoef spa_coef(const TemplCoef* __restrict__ tc)
 {
-    double ph = fma(u * u, A5, A3);
-    ph = fma(ph, u, A2);
-    ph = fma(ph, u, A1);
-    ph = fma(ph, u, -0.125);
+    SpaCoef s;
+    s.A1 = tc->A1; s.A2 = tc->A2; s.A3 = tc->A3; s.A5 = tc->A5; s.AL = tc->AL; s.A0 = tc->A0;
+    return s;
+}
+
+// lnk: the table ln k of lnk_table_kernel (read only where AL != 0, i.e. at 2.5PN; may be null at 2PN)
+__device__ __forceinline__ c2 spa_phasor_u(const double u, const int k, const SpaCoef& a, const double* __restrict__ lnk)
+{
+    double ph = fma(u * u, a.A5, a.A3);
+    ph = fma(ph, u, a.A2);
+    ph = fma(ph, u, a.A1);
+    ph = fma(ph, u, (double)a.A0);
+    if (a.AL != 0.0) ph = fma(a.AL, __ldg(lnk + k), ph);          // 2.5PN only (uniform over a template)
     // |ph| < 2^19 cycles: in ph + 1.5 * 2^20 the unit of the last place is 2^-32, so the low word of the
     // sum is the phase modulo one cycle as a 32-bit two's-complement fraction (one DADD, no conversion unit)
     const int frac = __double2loint(__dadd_rn(ph, 1572864.0));
@@ -309,6 +319,13 @@ __device__ __forceinline__ double widen_f32(const float f)
 }
 
 // u[k] = k^{-1/3} in double (k >= 1; u[0] = 0), one Newton step on the library cube root.
+// lnk[k] = ln k in double (k >= 1; lnk[0] = 0): the 2.5PN phase term (cbmf_set_pn_order).
+__global__ void lnk_table_kernel(double* __restrict__ lnk, int n_half)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n_half) lnk[k] = k > 0 ? log((double)k) : 0.0;
+}
+
 __global__ void rcbrt_table_kernel(double* __restrict__ u, int n_half)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -347,8 +364,8 @@ template <int L, int L2, bool SERIES = false>
 __device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, const int k2,
                                               const c2* __restrict__ wt, const int WS,
                                               const double* __restrict__ ut, const int US,
-                                              const int k_lo, const int k_hi, const double A1, const double A2,
-                                              const double A3, const double A5,
+                                              const int k_lo, const int k_hi, const SpaCoef& sc,
+                                              const double* __restrict__ lnk,
                                               const double* __restrict__ ub = nullptr,
                                               const float* __restrict__ inv = nullptr, const float cf = 0.f)
 {
@@ -375,7 +392,7 @@ __device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, c
                     } else {
                         uk = ut[(size_t)k1 * US];
                     }
-                    const c2 ph = spa_phasor_u(uk, A1, A2, A3, A5);
+                    const c2 ph = spa_phasor_u(uk, k, sc, lnk);
                     const c2 wv = (k >= k_lo && k <= k_hi) ? wt[k1 * WS] : czero();
                     v[u * R1 + rg + j] = cmul(ph, wv);
                 }
@@ -405,18 +422,18 @@ __device__ __forceinline__ void spa_correlate(c2 (&v)[Cfg<L>::E], const int t, c
 // (p1_series_ok), where the neglected quartic term is below 3.2 (c/kb)^4 phi < 1e-6 cycle for phi < 1e4 cycles.
 struct __align__(16) RowCoef { unsigned p0, p1; int p2, p3; };
 
-__device__ __forceinline__ RowCoef spa_row_coef(const double u, const double A1, const double A2, const double A3,
-                                                const double A5)
+__device__ __forceinline__ RowCoef spa_row_coef(const double u, const int kb, const SpaCoef& a, const double* __restrict__ lnk)
 {
+    const double A1 = a.A1, A2 = a.A2, A3 = a.A3, A5 = a.A5;
     const double u2 = u * u;
     double ph = fma(u2, A5, A3);
     ph = fma(ph, u, A2);
     ph = fma(ph, u, A1);
-    ph = fma(ph, u, -0.125);
+    ph = fma(ph, u, (double)a.A0);
     double q1 = fma(u2, 5.0 * A5, 3.0 * A3);
     q1 = fma(q1, u, 2.0 * A2);
     q1 = fma(q1, u, A1);
-    const double d1 = (-1.0 / 3.0) * (u2 * u2) * q1;
+    double d1 = (-1.0 / 3.0) * (u2 * u2) * q1;
     const float uf = (float)u, uf2 = uf * uf, uf3 = uf2 * uf;
     const float a1 = (float)A1, a2 = (float)A2, a3 = (float)A3, a5 = (float)A5;
     float q2 = fmaf(uf2, 40.f * a5, 18.f * a3);
@@ -426,8 +443,17 @@ __device__ __forceinline__ RowCoef spa_row_coef(const double u, const double A1,
     q3 = fmaf(q3, uf, 80.f * a2);
     q3 = fmaf(q3, uf, 28.f * a1);
     const float uf7 = uf3 * uf3 * uf;
-    const float d2 = (4294967296.0f / 18.0f) * (uf7 * q2);             // D2 phi / 2 in units of 2^-32 cycle
-    const float d3 = (-4294967296.0f / 162.0f) * ((uf7 * uf3) * q3);   // D3 phi / 6
+    float d2 = (4294967296.0f / 18.0f) * (uf7 * q2);             // D2 phi / 2 in units of 2^-32 cycle
+    float d3 = (-4294967296.0f / 162.0f) * ((uf7 * uf3) * q3);   // D3 phi / 6
+    if (a.AL != 0.0) {
+        // 2.5PN: + AL ln k, with D = AL / k, D2 / 2 = -AL / (2 k^2), D3 / 6 = AL / (3 k^3)  (k^-1 = u^3)
+        const double ik = u * u2;
+        ph = fma(a.AL, __ldg(lnk + kb), ph);
+        d1 = fma(a.AL, ik, d1);
+        const float alf = (float)a.AL, ikf = (float)ik;
+        d2 = fmaf(-0.5f * 4294967296.0f * alf, ikf * ikf, d2);
+        d3 = fmaf((4294967296.0f / 3.0f) * alf, ikf * ikf * ikf, d3);
+    }
     RowCoef r;
     r.p0 = (unsigned)__double2loint(__dadd_rn(ph, 1572864.0));
     r.p1 = (unsigned)__double2loint(__dadd_rn(d1, 1572864.0));
@@ -473,6 +499,7 @@ enum { LOAD_GEN = 0, LOAD_CPLX = 1, LOAD_REAL = 2, LOAD_GEN_DUMP = 3 };
 struct P1Args {
     const c2* __restrict__ w;              // [N/2] weighted data spectrum (LOAD_GEN)
     const double* __restrict__ u;          // [N/2] k^{-1/3} (LOAD_GEN)
+    const double* __restrict__ lnk;        // [N/2] ln k (LOAD_GEN at 2.5PN, else null)
     const TemplCoef* __restrict__ coef;    // [batch] (LOAD_GEN)
     const c2* __restrict__ in_c;           // [batch][N] (LOAD_CPLX)
     const float* __restrict__ in_r;        // [batch][N] (LOAD_REAL)
@@ -582,13 +609,13 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<
     // row records of one template: those rows of this warp that touch the template's band
     auto fill_rows = [&](const TemplCoef* __restrict__ tn) {
         const int k_lo = tn->k_lo, k_hi = tn->k_hi;
-        const double A1 = tn->A1, A2 = tn->A2, A3 = tn->A3, A5 = tn->A5;
+        const SpaCoef sc = spa_coef(tn);
 #pragma unroll
         for (int i = 0; i < RPT_W; ++i) {
             const int k1 = t + T * (RPT_W * c + i);
             const int kb = k1 * L2 + tile * NC;
             if (RPT_W * c + i < R1 / 2 && kb + NC - 1 >= k_lo && kb <= k_hi) {
-                const RowCoef r = spa_row_coef(u_mine[i], A1, A2, A3, A5);
+                const RowCoef r = spa_row_coef(u_mine[i], kb, sc, a.lnk);
                 if (k1 < RS) rc_lo[k1] = r; else rc_hi[k1 - RS] = r;
             }
         }
@@ -662,12 +689,12 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<
             if (!step1_done) {
                 if constexpr (!BYROWS) {
                     if (a.use_series)
-                        spa_correlate<L1, L2, true>(v, t, k2, wt + c, NC, nullptr, 0, tc->k_lo, tc->k_hi, tc->A1, tc->A2,
-                                                    tc->A3, tc->A5, ub, inv, (float)c);
+                        spa_correlate<L1, L2, true>(v, t, k2, wt + c, NC, nullptr, 0, tc->k_lo, tc->k_hi, spa_coef(tc), a.lnk, ub, inv,
+                                                    (float)c);
                     else
-                        spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
+                        spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, spa_coef(tc), a.lnk);
                 } else {
-                    spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, tc->A1, tc->A2, tc->A3, tc->A5);
+                    spa_correlate<L1, L2>(v, t, k2, wt + c, NC, a.u + k2, L2, tc->k_lo, tc->k_hi, spa_coef(tc), a.lnk);
                 }
             }
         } else {
@@ -1170,6 +1197,7 @@ struct SetupArgs {
     double n_over_fs;                    // N / fs  (= 1/df)
     double df;
     float threshold;
+    int pn_half_order;                   // 4: 2PN phase (default), 5: + the 2.5PN term
     int* err_flag;
     long long* bad_idx;                  // smallest index of an invalid template (atomicMin), may be null
 };
@@ -1182,7 +1210,7 @@ __global__ void template_setup_kernel(const SetupArgs a)
     TemplCoef c;
     c.A1 = c.A2 = c.A3 = c.A5 = 0.0;
     c.k_lo = a.k_lo; c.k_hi = -1;
-    c.sigma = c.inv_sigma = 0.f; c.thr2 = 0.f; c.nz_class = 0; c.pad_[0] = c.pad_[1] = 0;
+    c.sigma = c.inv_sigma = 0.f; c.thr2 = 0.f; c.A0 = -0.125f; c.AL = 0.0;
     if (!(m1 > 0.0) || !(m2 > 0.0) || isinf(m1) || isinf(m2)) {
         *a.err_flag = 1;
         if (a.bad_idx) atomicMin(a.bad_idx, (long long)i);
@@ -1211,11 +1239,20 @@ __global__ void template_setup_kernel(const SetupArgs a)
     c.A2 = b3 * s * s * i2pi;
     c.A3 = b2 * s * s * s * i2pi;
     c.A5 = b0 * s * s * s * s * s * i2pi;
+    if (a.pn_half_order >= 5) {
+        // NEXT-3 ("order 2.5 in phase"): Psi += c0 pi (38645/756 - 65 eta/9) (1 + 3 ln(v / v_lso)),
+        // v_lso = 6^{-1/2} (Arun et al., PRD 71, 084008 (2005), eq. 3.4; Buonanno et al., PRD 80, 084043 (2009),
+        // eq. 3.18).  3 ln(v / v_lso) = ln(f / f_ISCO) = ln k + ln(df / f_ISCO): a ln k term and a constant.
+        const double B5 = c0 * PI * (38645.0 / 756.0 - 65.0 * eta / 9.0) * i2pi;
+        c.AL = B5;
+        const double a0 = -0.125 + B5 * (1.0 + log(a.df / f_isco));
+        c.A0 = (float)(a0 - rint(a0));
+    }
     if (c.k_hi >= c.k_lo) {
         // the generator reduces the phase modulo one cycle with a 2^-32 fixed-point trick that needs
         // |Psi| / 2 pi < 2^19 cycles on the band; |Psi| is largest at k_lo (total masses far below 0.3 Msun at 10 Hz)
         const double ul = 1.0 / cbrt((double)c.k_lo);
-        const double ph_lo = fabs(ul * (c.A1 + ul * (c.A2 + ul * (c.A3 + ul * ul * c.A5)))) + 1.0;
+        const double ph_lo = fabs(ul * (c.A1 + ul * (c.A2 + ul * (c.A3 + ul * ul * c.A5)))) + fabs(c.AL) * log((double)a.n_half) + 1.0;
         if (!(ph_lo < 524288.0)) {
             *a.err_flag = 1;
             if (a.bad_idx) atomicMin(a.bad_idx, (long long)i);
@@ -1352,6 +1389,7 @@ __global__ void chisq_edges_kernel(const TemplCoef* __restrict__ coef, const dou
 }
 
 __global__ void __launch_bounds__(256) chisq_bands_kernel(const c2* __restrict__ w, const double* __restrict__ u,
+                                                          const double* __restrict__ lnk,
                                                           const TemplCoef* __restrict__ coef,
                                                           const int* __restrict__ edges, const int* __restrict__ sample_idx,
                                                           int p, int log2n, double* __restrict__ zl /* [n][p][2] */)
@@ -1360,13 +1398,13 @@ __global__ void __launch_bounds__(256) chisq_bands_kernel(const c2* __restrict__
     const TemplCoef* tc = coef + b;
     const int k0 = edges[b * (p + 1) + l], k1 = edges[b * (p + 1) + l + 1];
     const long long j = sample_idx[b];
-    const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+    const SpaCoef sc = spa_coef(tc);
     const unsigned long long mask = (1ULL << log2n) - 1ULL;
     const float two_over_n = 2.0f / (float)(1ULL << log2n);
     double sr = 0.0, si = 0.0;
     if (j >= 0) {
         for (int k = k0 + threadIdx.x; k < k1; k += blockDim.x) {
-            const c2 q = cmul(__ldg(w + k), spa_phasor_u(__ldg(u + k), A1, A2, A3, A5));
+            const c2 q = cmul(__ldg(w + k), spa_phasor_u(__ldg(u + k), k, sc, lnk));
             const c2 r = cmul(q, expi_frac((int)(((unsigned long long)j * (unsigned long long)k) & mask), two_over_n));
             sr += (double)re(r);
             si += (double)im(r);
@@ -1445,16 +1483,17 @@ __global__ void fill_ones_kernel(c2* __restrict__ w, int n)
 
 // generator alone: q~[b][k] = w[k] e^{+i Psi_b(f_k)}, k < N/2  (config-4 generator throughput)
 __global__ void __launch_bounds__(256) generate_only_kernel(const c2* __restrict__ w, const double* __restrict__ u,
+                                                            const double* __restrict__ lnk,
                                                             const TemplCoef* __restrict__ coef,
                                                             c2* __restrict__ q, int n_half)
 {
     const int b = blockIdx.y;
     const TemplCoef* tc = coef + b;
-    const double A1 = tc->A1, A2 = tc->A2, A3 = tc->A3, A5 = tc->A5;
+    const SpaCoef sc = spa_coef(tc);
     const int k_lo = tc->k_lo, k_hi = tc->k_hi;
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_half; k += gridDim.x * blockDim.x) {
         c2 o = czero();
-        if (k >= k_lo && k <= k_hi) o = cmul(__ldg(w + k), spa_phasor_u(__ldg(u + k), A1, A2, A3, A5));
+        if (k >= k_lo && k <= k_hi) o = cmul(__ldg(w + k), spa_phasor_u(__ldg(u + k), k, sc, lnk));
         q[(size_t)b * n_half + k] = o;
     }
 }
