@@ -247,6 +247,9 @@ int cbmf_last_pass_time(const cbmf_ctx *ctx, int which, double *ms_out, int64_t 
  * bracketed by events on its own stream, so a duration includes the time the kernel shares its SMs
  * with the launches of the other pairs.  EINVAL for any other value. */
 int cbmf_set_profiling(cbmf_ctx *ctx, int mode);
+/* Launch timeline of the last profiled cbmf_filter_bank* call: for pass `which`, start and end of every launch in ms
+ * since the first pass-1 launch (start_end_ms[2 i], [2 i + 1]; at most max_launches pairs; *n_launches = all). */
+int cbmf_debug_timeline(const cbmf_ctx *ctx, int which, float *start_end_ms, int64_t max_launches, int64_t *n_launches);
 const char *cbmf_strerror(int rc);
 const char *cbmf_last_cuda_error(const cbmf_ctx *ctx);
 const char *cbmf_version(void);

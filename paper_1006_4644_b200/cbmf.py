@@ -69,6 +69,7 @@ def lib() -> C.CDLL:
         "cbmf_launch_count": (i64, [vp]),
         "cbmf_last_pass_time": (C.c_int, [vp, C.c_int, C.POINTER(dbl), C.POINTER(i64)]),
         "cbmf_set_profiling": (C.c_int, [vp, C.c_int]),
+        "cbmf_debug_timeline": (C.c_int, [vp, C.c_int, vp, i64, C.POINTER(i64)]),
         "cbmf_strerror": (C.c_char_p, [C.c_int]),
         "cbmf_last_cuda_error": (C.c_char_p, [vp]),
         "cbmf_version": (C.c_char_p, []),
@@ -86,7 +87,7 @@ EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_seg
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
            "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_pn_order cbmf_get_pn_order cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
-           "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_strerror "
+           "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_debug_timeline cbmf_strerror "
            "cbmf_last_cuda_error cbmf_version").split()
 
 
@@ -378,6 +379,13 @@ class Context:
     def set_profiling(self, mode: int):
         """0 off, 1 every pass launch alone on the context's stream, 2 in the real overlapped schedule."""
         self._check(lib().cbmf_set_profiling(self._h, int(mode)), "cbmf_set_profiling")
+
+    def debug_timeline(self, which: int) -> np.ndarray:
+        """[launches, 2] float32: start / end (ms since the first pass-1 launch) of every launch of pass `which`."""
+        out = np.zeros((4096, 2), dtype=np.float32)
+        n = C.c_int64(0)
+        self._check(lib().cbmf_debug_timeline(self._h, int(which), out.ctypes.data, 4096, C.byref(n)), "cbmf_debug_timeline")
+        return out[:min(int(n.value), 4096)]
 
     def last_pass_time(self, which: int):
         ms, nl = C.c_double(0), C.c_int64(0)

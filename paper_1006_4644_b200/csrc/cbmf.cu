@@ -61,7 +61,8 @@ struct cbmf_ctx {
     // device, so the cache belongs to the context, not to the process)
     std::unordered_set<const void*> attr_set;
     unsigned int* d_tcount = nullptr;  int64_t tcount_cap = 0;    // [n_templates] triggers per template
-    long long* d_bad = nullptr;            // [1] index of the first invalid template of the last bank, or LLONG_MAX
+    long long* d_bad = nullptr;            // = d_cursor + 1: index of the first invalid template of the last bank, or NO_BAD_TEMPLATE
+    unsigned char* h_stage = nullptr;  size_t stage_bytes = 0;    // pinned staging of a bank call's results
     int64_t last_bad = -1;
 
     // clustered bank call (cbmf_filter_bank_clustered): per launch pair a device trigger region and cursor, copied
@@ -88,6 +89,7 @@ struct cbmf_ctx {
     int profiling = 0;                     // 0 off, 1 every launch alone on the context's stream, 2 in the real schedule
     std::vector<cudaEvent_t> ev[2];        // per pass: start/stop pairs of the last filter call
     size_t ev_used[2] = {0, 0};
+    std::vector<float> timeline[2];        // per pass: (start, end) in ms of every launch of the last profiled call
     double last_ms[2] = {0, 0};
     int64_t last_launches[2] = {0, 0};
     char cuda_err[256] = {0};
@@ -266,12 +268,15 @@ int ev_collect(cbmf_ctx* c)
     for (int w = 0; w < 2; ++w) {
         c->last_ms[w] = 0; c->last_launches[w] = 0;
         if (!c->profiling) continue;
+        c->timeline[w].clear();
         for (size_t i = 0; i + 1 < c->ev_used[w]; i += 2) {
-            float ms = 0.f;
+            float ms = 0.f, t0 = 0.f;
             CU(cudaEventElapsedTime(&ms, c->ev[w][i], c->ev[w][i + 1]));
             c->last_ms[w] += ms; c->last_launches[w] += 1;
+            if (c->ev_used[0] >= 2) CU(cudaEventElapsedTime(&t0, c->ev[0][0], c->ev[w][i]));    // since the first pass-1 launch
+            c->timeline[w].push_back(t0);
+            c->timeline[w].push_back(t0 + ms);
         }
-        c->ev_used[w] = 0;
     }
     return CBMF_OK;
 }
@@ -317,7 +322,7 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     cudaFree(c->d_wfac); cudaFree(c->d_term); cudaFree(c->d_prefix); cudaFree(c->d_bsum); cudaFree(c->d_w);
     cudaFree(c->d_Y); cudaFree(c->d_cand); cudaFree(c->d_done); cudaFree(c->d_key); cudaFree(c->d_err); cudaFree(c->d_u);
     cudaFree(c->d_lnk); cudaFree(c->d_cursor); cudaFree(c->d_coef); cudaFree(c->d_bank); cudaFree(c->d_peaks);
-    cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_tcount); cudaFree(c->d_bad);
+    cudaFree(c->d_trig); cudaFree(c->d_scratch); cudaFree(c->d_tcount); cudaFreeHost(c->h_stage);
     cudaFree(c->d_segcoef); cudaFree(c->d_w2); cudaFree(c->d_segY); cudaFree(c->d_segin); cudaFree(c->d_segerr);
     if (c->seg_stream) { cudaStreamSynchronize(c->seg_stream); cudaStreamDestroy(c->seg_stream); }
     for (cudaEvent_t e : c->ev_seg_ready) if (e) cudaEventDestroy(e);
@@ -384,8 +389,9 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     CUF(cudaMalloc(&c->d_w, sizeof(c2) * nh));
     CUF(cudaMalloc(&c->d_u, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_err, sizeof(int)));
-    CUF(cudaMalloc(&c->d_cursor, sizeof(unsigned long long)));
-    CUF(cudaMalloc(&c->d_bad, sizeof(long long)));
+    // status block of a bank call: {trigger cursor, first invalid template}: one reset copy, one read-back
+    CUF(cudaMalloc(&c->d_cursor, 2 * sizeof(unsigned long long)));
+    c->d_bad = reinterpret_cast<long long*>(c->d_cursor + 1);
     CUF(cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, device));
     CUF(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
     rcbrt_table_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(c->d_u, (int)nh);
@@ -609,7 +615,7 @@ static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap, const c2* w
         cudaStream_t st = (ns > 1) ? c->aux[slot] : c->stream;
         c2* Y = c->d_Y + (size_t)slot * c->max_sub_batch * (size_t)c->n;
         P1Args a1; memset(&a1, 0, sizeof(a1));
-        a1.w = w; a1.u = c->d_u; a1.lnk = c->d_lnk; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo;
+        a1.w = w; a1.u = c->d_u; a1.lnk = c->d_lnk; a1.coef = c->d_coef + t0; a1.Y = Y; a1.err_flag = c->d_err; a1.use_series = c->k_lo; a1.bad = c->d_bad;
         if ((rc = ev_begin(c, 0, st))) return rc;
         CU(launch_p1<LOAD_GEN>(c, st, a1, nb));
         if ((rc = ev_end(c, 0, st))) return rc;
@@ -622,6 +628,7 @@ static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap, const c2* w
         a2.trig_count = c->d_tcount + t0;
         a2.tmpl_base = (int)t0;
         a2.j_min = j_min;
+        a2.bad = c->d_bad;
         if ((rc = ev_begin(c, 1, st))) return rc;
         if (j_min > 0) CU((launch_p2<EPI_MAX, true>(c, st, a2, nb)));
         else CU(launch_p2<EPI_MAX>(c, st, a2, nb));
@@ -650,10 +657,11 @@ static int bank_setup(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr
     if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
     if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
     if ((rc = grow(c, c->d_tcount, c->tcount_cap, nt))) return rc;
-    const long long no_bad = 0x7FFFFFFFFFFFFFFFLL;
+    const long long no_bad = NO_BAD_TEMPLATE;
     CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
     CU(cudaMemcpyAsync(c->d_bad, &no_bad, sizeof(long long), cudaMemcpyHostToDevice, c->stream));
     SetupArgs sa;
+    sa.tcount = nullptr;
     sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
     sa.threshold = thr; sa.err_flag = c->d_err; sa.bad_idx = c->d_bad; sa.pn_half_order = c->pn_half_order;
@@ -722,6 +730,10 @@ static int bank_filter(cbmf_ctx* c, int64_t nt, const c2* w, int j_min, void* pe
     return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
 }
 
+// The plain bank call.  Everything is enqueued behind one another -- status reset, template setup, the launch pairs
+// (which return at once if the setup found an invalid template), a single-block sort of up to TRIG_SMALL triggers with
+// the count read on the device, the result copies -- and the host waits ONCE; only a bank with more triggers than
+// that, or than the list holds, goes through the general collection (bank_filter's tail) afterwards.
 static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr,
                             void* peaks_out, void* trig_out, int64_t trig_capacity,
                             int64_t* n_trig_found, cudaMemcpyKind out_kind)
@@ -730,8 +742,96 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     c->last_bad = -1;
     if (nt == 0) return CBMF_OK;
     int rc;
-    if ((rc = bank_setup(c, bank_dev, nt, thr))) return rc;
-    return bank_filter(c, nt, c->d_w, 0, peaks_out, trig_out, trig_capacity, n_trig_found, out_kind);
+    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_tcount, c->tcount_cap, nt))) return rc;
+    int64_t tcap = 1;
+    while (tcap < trig_capacity) tcap <<= 1;
+    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
+    const bool to_host = (out_kind == cudaMemcpyDeviceToHost);
+    const int64_t n_fast = trig_capacity < TRIG_SMALL ? trig_capacity : TRIG_SMALL;      // triggers the fast path delivers
+    const size_t b_status = 16, b_peaks = sizeof(PeakOut) * (size_t)nt, b_trig = sizeof(TrigOut) * (size_t)n_fast;
+    if (b_status + b_peaks + b_trig > c->stage_bytes) {
+        if (c->h_stage) { CU(cudaFreeHost(c->h_stage)); c->h_stage = nullptr; c->stage_bytes = 0; }
+        CU(cudaMallocHost(&c->h_stage, b_status + b_peaks + b_trig));
+        c->stage_bytes = b_status + b_peaks + b_trig;
+    }
+    unsigned long long* h_status = reinterpret_cast<unsigned long long*>(c->h_stage);
+    unsigned char* h_peaks = c->h_stage + b_status;
+    unsigned char* h_trig = h_peaks + b_peaks;
+
+    h_status[0] = 0ULL; h_status[1] = (unsigned long long)NO_BAD_TEMPLATE;
+    CU(cudaMemcpyAsync(c->d_cursor, h_status, b_status, cudaMemcpyHostToDevice, c->stream));      // cursor = 0, bad = none
+    SetupArgs sa;
+    sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
+    sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
+    sa.threshold = thr; sa.err_flag = c->d_err; sa.bad_idx = c->d_bad; sa.tcount = c->d_tcount; sa.pn_half_order = c->pn_half_order;
+    template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    c->ev_used[0] = c->ev_used[1] = 0;
+    if ((rc = run_bank_passes(c, nt, c->trig_cap))) return rc;
+    const int sort_limit = (int)(c->trig_cap < TRIG_SMALL ? c->trig_cap : TRIG_SMALL);
+    CU(ensure_smem_attr(c, trig_sort_small_dev_kernel,
+                        (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL));
+    trig_sort_small_dev_kernel<<<1, 1024, (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL,
+                                 c->stream>>>(c->d_trig, c->d_cursor, c->d_bad, sort_limit);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    CU(cudaMemcpyAsync(h_status, c->d_cursor, b_status, cudaMemcpyDeviceToHost, c->stream));
+    if (to_host) {
+        CU(cudaMemcpyAsync(h_peaks, c->d_peaks, b_peaks, cudaMemcpyDeviceToHost, c->stream));
+        if (b_trig && trig_out) CU(cudaMemcpyAsync(h_trig, c->d_trig, b_trig, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    if ((rc = ev_collect(c))) return rc;
+    if ((long long)h_status[1] != NO_BAD_TEMPLATE) { c->last_bad = (int64_t)h_status[1]; return CBMF_EINVAL; }
+    const int64_t found = (int64_t)h_status[0];
+    if (n_trig_found) *n_trig_found = found;
+    const int64_t kept = found < trig_capacity ? found : trig_capacity;
+    if (found <= sort_limit && found <= trig_capacity) {
+        // the common case: the sorted list is complete
+        if (to_host) {
+            memcpy(peaks_out, h_peaks, b_peaks);
+            if (kept > 0 && trig_out) memcpy(trig_out, h_trig, sizeof(TrigOut) * (size_t)kept);
+        } else {
+            if (kept > 0 && trig_out) CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, out_kind, c->stream));
+            CU(cudaMemcpyAsync(peaks_out, c->d_peaks, b_peaks, out_kind, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+        }
+        return CBMF_OK;
+    }
+    // many triggers: the general collection (sort of any size, truncated lists)
+    if (kept > 0 && trig_out) {
+        int64_t on_device = found;
+        if (found > c->trig_cap) {
+            // Truncated and the device list is incomplete.  The contract (cbmf.h) keeps the FIRST trig_capacity
+            // triggers in (template, sample) order, so the whole lists of the leading templates are needed:
+            // find the shortest bank prefix [0, t_cut] holding at least trig_capacity triggers from the
+            // per-template counts and filter that prefix again into a buffer that takes all of its triggers.
+            std::vector<unsigned int> cnt((size_t)nt);
+            CU(cudaMemcpyAsync(cnt.data(), c->d_tcount, sizeof(unsigned int) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+            int64_t cum = 0, t_cut = 0;
+            for (; t_cut < nt; ++t_cut) { cum += cnt[(size_t)t_cut]; if (cum >= trig_capacity) break; }
+            int64_t need = 1;
+            while (need < cum) need <<= 1;
+            if ((rc = grow(c, c->d_trig, c->trig_cap, need))) return rc;
+            CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
+            CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
+            const int prof = c->profiling;
+            c->profiling = 0;                           // the repeat is not part of the per-pass timing
+            rc = run_bank_passes(c, t_cut + 1, c->trig_cap);
+            c->profiling = prof;
+            if (rc) return rc;
+            on_device = cum;
+        }
+        if ((rc = sort_triggers(c, on_device))) return rc;
+        CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, out_kind, c->stream));
+    }
+    CU(cudaMemcpyAsync(peaks_out, c->d_peaks, b_peaks, out_kind, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
 }
 
 static int filter_args_ok(cbmf_ctx* c, const void* bank, int64_t nt, float thr, void* peaks,
@@ -1040,7 +1140,7 @@ static int setup_one(cbmf_ctx* c, cbmf_template t)
     SetupArgs sa;
     sa.bank = c->d_bank; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = 1;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr; sa.pn_half_order = c->pn_half_order;
+    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr; sa.tcount = nullptr; sa.pn_half_order = c->pn_half_order;
     template_setup_kernel<<<1, 32, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     c->launches += 1;
@@ -1158,7 +1258,7 @@ extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_de
     SetupArgs sa;
     sa.bank = (const double*)bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
-    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr; sa.pn_half_order = c->pn_half_order;
+    sa.threshold = 0.f; sa.err_flag = c->d_err; sa.bad_idx = nullptr; sa.tcount = nullptr; sa.pn_half_order = c->pn_half_order;
     template_setup_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, c->stream>>>(sa);
     CU(cudaGetLastError());
     const int nh = (int)(c->n / 2);
@@ -1200,6 +1300,15 @@ extern "C" int cbmf_last_pass_time(const cbmf_ctx* c, int which, double* ms_out,
     if (!c || which < 0 || which > 1) return CBMF_EINVAL;
     if (ms_out) *ms_out = c->last_ms[which];
     if (launches_out) *launches_out = c->last_launches[which];
+    return CBMF_OK;
+}
+
+extern "C" int cbmf_debug_timeline(const cbmf_ctx* c, int which, float* start_end_ms, int64_t max_launches, int64_t* n_launches)
+{
+    if (!c || which < 0 || which > 1 || max_launches < 0 || (max_launches && !start_end_ms)) return CBMF_EINVAL;
+    const int64_t n = (int64_t)c->timeline[which].size() / 2, k = n < max_launches ? n : max_launches;
+    for (int64_t i = 0; i < 2 * k; ++i) start_end_ms[i] = c->timeline[which][(size_t)i];
+    if (n_launches) *n_launches = n;
     return CBMF_OK;
 }
 

@@ -94,7 +94,7 @@ __device__ __forceinline__ constexpr float cos32_table(int a)
 
 // Butterfly lo = e + o w, hi = e - o w with w = e^{+2 pi i q / R}, 0 <= q < R/2 (compile-time
 // after unrolling).  w = 1 or i: two FADD2; w = (+-1 + i)/sqrt 2: FADD2 + two FFMA2; general:
-// lo = e + o.x (c, s) + o.y (-s, c) is two FFMA2 and hi = 2 e - lo a third.
+// lo = e + c (o.x, o.y) + s (-o.y, o.x) is two FFMA2 and hi = 2 e - lo a third.
 template <int R>
 __device__ __forceinline__ void bfly(const c2 e, const c2 o, const int q, c2& lo, c2& hi)
 {
@@ -116,7 +116,9 @@ __device__ __forceinline__ void bfly(const c2 e, const c2 o, const int q, c2& lo
     } else {
         const float c = (a <= 8) ? cos32_table(a) : -cos32_table(16 - a);
         const float s = (a <= 8) ? cos32_table(8 - a) : cos32_table(a - 8);
-        lo = fma2(bc(oy), pk(-s, c), fma2(bc(ox), pk(c, s), e));
+        // o w = c (ox, oy) + s (-oy, ox): the constants enter as BROADCAST scalars (immediates), the swap / sign flip
+        // of o is an operand modifier -- no (c, s) register pairs to assemble
+        lo = fma2(pk(-oy, ox), bc(s), fma2(o, bc(c), e));
         hi = fma2(e, bc(2.0f), neg2(lo));
     }
 }

@@ -33,6 +33,11 @@ struct __align__(16) TemplCoef {
 };
 static_assert(sizeof(TemplCoef) == 64, "TemplCoef layout");
 
+// Status word of a bank call: index of its first invalid template (template_setup_kernel, atomicMin) or this value.
+// The pass kernels of the call read it first and return at once when a template is invalid, so the host need not
+// wait for the check before it enqueues them.
+constexpr long long NO_BAD_TEMPLATE = 0x7FFFFFFFFFFFFFFFLL;
+
 struct PeakOut { float snr_max; int32_t idx_peak; float phase; float sigma; };
 struct TrigOut { int32_t template_idx; int32_t sample_idx; float snr; float phase; };
 
@@ -62,6 +67,14 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+}
+// The same with compile-time byte offsets on both addresses: one base register pair serves a whole unrolled
+// sequence of copies ([reg + imm] addressing instead of a 64-bit add per copy).
+template <int SMEM_OFF, long long GMEM_OFF>
+__device__ __forceinline__ void cp_async16_off(const unsigned smem_base, const void* gmem_base)
+{
+    asm volatile("cp.async.cg.shared.global [%0+%2], [%1+%3], 16;\n" ::"r"(smem_base), "l"(gmem_base), "n"(SMEM_OFF), "n"(GMEM_OFF)
+                 : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
@@ -505,6 +518,7 @@ struct P1Args {
     const float* __restrict__ in_r;        // [batch][N] (LOAD_REAL)
     c2* __restrict__ Y;                    // [batch][N], Y[j1*N2 + k2]
     int* err_flag;                         // set to 1 on a non-finite real input sample
+    const long long* bad;                  // LOAD_GEN: *bad != NO_BAD_TEMPLATE (an invalid template in the bank): do nothing
     int batch;                             // templates (or vectors) in this launch
     int use_series;                        // LOAD_GEN: k^{-1/3} by the series of spa_correlate (host checks its range)
 };
@@ -558,6 +572,9 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<
     constexpr bool BYROWS = (MODE == LOAD_GEN) && p1_by_rows<L1>();
     constexpr int RS = p1_rc_split<L1>();                  // row records k1 < RS: own array; the rest: exchange-buffer tail
 
+    if constexpr (MODE == LOAD_GEN) {
+        if (a.bad != nullptr && __ldg(a.bad) != NO_BAD_TEMPLATE) return;               // uniform over the grid
+    }
     const int tile = blockIdx.x;
     const int c = threadIdx.x % NC, t = threadIdx.x / NC;
     const int k2 = tile * NC + c;
@@ -766,6 +783,7 @@ struct P2Args {
     unsigned int* trig_count;              // [batch] triggers found per template (for a deterministic truncated list)
     int tmpl_base;                         // bank index of template 0 of this sub-batch
     int j_min;                             // MASK: samples j < j_min take no part in the peak or the trigger list
+    const long long* bad;                  // EPI_MAX: *bad != NO_BAD_TEMPLATE: do nothing
     // EPI_STORE
     c2* __restrict__ z_out;                // [batch][N], natural order
     // EPI_WSTORE (load_segment): w[k] = conj(Z[k]) * wfac[k] for k < N/2
@@ -794,15 +812,33 @@ template <int L2> __host__ __device__ constexpr int p2_row_stride()
 
 // Start the asynchronous copy of row j1 of one template's Y (tile-major: segments of NC columns)
 // into the row group's shared-memory buffer (unpadded, element k2 at sm[k2]); T threads take part.
+template <int L1, int L2, int I>
+struct P2Prefetch {
+    // chunk I of a thread: columns k2 = 2 (t + T I), k2 + 1; consecutive chunks lie 2 T / NC tiles = 2 T L1 elements apart
+    static __device__ __forceinline__ void run(const unsigned sm_t, const c2* __restrict__ src_t)
+    {
+        constexpr int T = Cfg<L2>::T, E = Cfg<L2>::E;
+        if constexpr (I < E / 2) {
+            cp_async16_off<(int)(sizeof(c2) * 2 * T * I), (long long)(sizeof(c2) * 2 * T * L1) * I>(sm_t, src_t);
+            P2Prefetch<L1, L2, I + 1>::run(sm_t, src_t);
+        }
+    }
+};
 template <int L1, int L2>
 __device__ __forceinline__ void p2_prefetch_row(c2* __restrict__ sm, const c2* __restrict__ yb, const int j1, const int t)
 {
     constexpr int T = Cfg<L2>::T, E = Cfg<L2>::E, NC = Cfg<L1>::C;
     static_assert(NC % 2 == 0, "16-byte chunks must not straddle tiles");
+    // the chunks of one thread are whole tiles apart and the largest offset fits the immediate field of the copy
+    constexpr bool IMM = ((2 * T) % NC == 0) && ((long long)sizeof(c2) * 2 * T * L1 * (E / 2) < (1LL << 23));
+    if constexpr (IMM) {
+        P2Prefetch<L1, L2, 0>::run((unsigned)__cvta_generic_to_shared(sm + 2 * t), yb + y_index<L1, NC>(j1, 2 * t));
+    } else {
 #pragma unroll
-    for (int i = 0; i < E / 2; ++i) {
-        const int k2 = 2 * (t + T * i);
-        cp_async16(sm + k2, yb + y_index<L1, NC>(j1, k2));
+        for (int i = 0; i < E / 2; ++i) {
+            const int k2 = 2 * (t + T * i);
+            cp_async16(sm + k2, yb + y_index<L1, NC>(j1, k2));
+        }
     }
     cp_async_commit();
 }
@@ -1087,6 +1123,9 @@ template <int L1, int L2, int MODE, bool MASK = false>
 __global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
 {
     extern __shared__ __align__(16) c2 smem[];
+    if constexpr (MODE == EPI_MAX) {
+        if (a.bad != nullptr && __ldg(a.bad) != NO_BAD_TEMPLATE) return;               // uniform over the grid
+    }
     p2_item<L1, L2, MODE, MASK>(a, blockIdx.x, blockIdx.y, smem);
 }
 
@@ -1200,6 +1239,7 @@ struct SetupArgs {
     int pn_half_order;                   // 4: 2PN phase (default), 5: + the 2.5PN term
     int* err_flag;
     long long* bad_idx;                  // smallest index of an invalid template (atomicMin), may be null
+    unsigned int* tcount;                // [n] per-template trigger counters, zeroed here (may be null)
 };
 
 __global__ void template_setup_kernel(const SetupArgs a)
@@ -1207,6 +1247,7 @@ __global__ void template_setup_kernel(const SetupArgs a)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= a.n_templates) return;
     const double m1 = a.bank[2 * i], m2 = a.bank[2 * i + 1];
+    if (a.tcount) a.tcount[i] = 0u;
     TemplCoef c;
     c.A1 = c.A2 = c.A3 = c.A5 = 0.0;
     c.k_lo = a.k_lo; c.k_hi = -1;
@@ -1333,6 +1374,45 @@ __global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, in
     unsigned short* pos = reinterpret_cast<unsigned short*>(rec + n_pow2);                    // [n_pow2]
     for (int i = threadIdx.x; i < n_pow2; i += blockDim.x) {
         unsigned long long k = ~0ULL;                                  // padding sorts last
+        if (i < n) { const TrigOut o = trig[i]; rec[i] = o; k = trig_key(o); }
+        key[i] = k;
+        pos[i] = (unsigned short)i;
+    }
+    __syncthreads();
+    const int n_pairs = n_pow2 >> 1;
+    for (int kk = 2; kk <= n_pow2; kk <<= 1)
+        for (int jj = kk >> 1; jj > 0; jj >>= 1) {
+            for (int p = threadIdx.x; p < n_pairs; p += blockDim.x) {
+                const int i = ((p & ~(jj - 1)) << 1) | (p & (jj - 1)), x = i | jj;
+                const unsigned long long a = key[i], b = key[x];
+                if ((a > b) == ((i & kk) == 0)) {
+                    key[i] = b; key[x] = a;
+                    const unsigned short t = pos[i]; pos[i] = pos[x]; pos[x] = t;
+                }
+            }
+            __syncthreads();
+        }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = rec[pos[i]];
+}
+
+// The same with the count read on the device (the total of the bank's trigger cursor): lets the host enqueue the sort
+// behind the bank without waiting for the count.  Does nothing when there are more triggers than `limit` (the list
+// capacity or TRIG_SMALL): the host then takes the general path.
+__global__ void __launch_bounds__(1024) trig_sort_small_dev_kernel(TrigOut* trig, const unsigned long long* __restrict__ cursor,
+                                                                   const long long* __restrict__ bad, int limit)
+{
+    extern __shared__ __align__(16) unsigned char trig_smem_raw[];
+    if (__ldg(bad) != NO_BAD_TEMPLATE) return;
+    const unsigned long long found = __ldg(cursor);
+    if (found > (unsigned long long)limit || found < 2ULL) return;
+    const int n = (int)found;
+    int n_pow2 = 2;
+    while (n_pow2 < n) n_pow2 <<= 1;
+    unsigned long long* key = reinterpret_cast<unsigned long long*>(trig_smem_raw);          // [n_pow2]
+    TrigOut* rec = reinterpret_cast<TrigOut*>(key + n_pow2);                                  // [n_pow2]
+    unsigned short* pos = reinterpret_cast<unsigned short*>(rec + n_pow2);                    // [n_pow2]
+    for (int i = threadIdx.x; i < n_pow2; i += blockDim.x) {
+        unsigned long long k = ~0ULL;
         if (i < n) { const TrigOut o = trig[i]; rec[i] = o; k = trig_key(o); }
         key[i] = k;
         pos[i] = (unsigned short)i;
