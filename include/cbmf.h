@@ -26,9 +26,16 @@
  * Return codes: 0 success, < 0 error, > 0 warning.  All pointers are HOST pointers
  * unless the function name ends in _dev, in which case every array pointer is a
  * DEVICE pointer on the context's device (scalars stay host values).  The caller
- * owns every array; the context owns all of its device memory.  Every call is
- * synchronous with respect to the context's stream: results are complete on return.
- * A context is not thread-safe; contexts are independent.
+ * owns every array; the context owns all of its device memory.  Every call that
+ * returns results is synchronous with respect to the context's stream: they are
+ * complete on return.  cbmf_set_psd_dev and cbmf_load_segment_dev, which return no
+ * results, are STREAM-ORDERED: they enqueue their work on the context's stream and
+ * return without waiting; the check of their input (a PSD entry <= 0 or NaN, a NaN /
+ * Inf sample) comes back with the next call that waits (any cbmf_filter_* / chisq /
+ * debug call, or a host-pointer set / load), which then returns CBMF_EINVAL and leaves the
+ * context without that PSD or segment (ESTATE afterwards).  The input arrays of a _dev call
+ * must stay valid until such a call has returned.  A context is not thread-safe; contexts
+ * are independent.
  */
 #ifndef CBMF_H
 #define CBMF_H

@@ -61,6 +61,9 @@ struct cbmf_ctx {
     // device, so the cache belongs to the context, not to the process)
     std::unordered_set<const void*> attr_set;
     unsigned int* d_tcount = nullptr;  int64_t tcount_cap = 0;    // [n_templates] triggers per template
+    int* d_perr = nullptr;                 // status block + 16: set_psd found an entry <= 0 or NaN inside the band
+    int* d_serr = nullptr;                 // status block + 20: load_segment found a NaN / Inf sample
+    bool pend_psd = false, pend_seg = false;   // a *_dev call enqueued the check; the next waiting call resolves it
     long long* d_bad = nullptr;            // = d_cursor + 1: index of the first invalid template of the last bank, or NO_BAD_TEMPLATE
     unsigned char* h_stage = nullptr;  size_t stage_bytes = 0;    // pinned staging of a bank call's results
     int64_t last_bad = -1;
@@ -390,8 +393,11 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     CUF(cudaMalloc(&c->d_u, sizeof(double) * nh));
     CUF(cudaMalloc(&c->d_err, sizeof(int)));
     // status block of a bank call: {trigger cursor, first invalid template}: one reset copy, one read-back
-    CUF(cudaMalloc(&c->d_cursor, 2 * sizeof(unsigned long long)));
+    CUF(cudaMalloc(&c->d_cursor, 4 * sizeof(unsigned long long)));
+    CUF(cudaMemset(c->d_cursor, 0, 4 * sizeof(unsigned long long)));
     c->d_bad = reinterpret_cast<long long*>(c->d_cursor + 1);
+    c->d_perr = reinterpret_cast<int*>(c->d_cursor + 2);
+    c->d_serr = c->d_perr + 1;
     CUF(cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, device));
     CUF(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
     rcbrt_table_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(c->d_u, (int)nh);
@@ -456,26 +462,39 @@ extern "C" int cbmf_get_split(const cbmf_ctx* c, int* log2_n1, int* log2_n2)
 extern "C" int64_t cbmf_last_bad_template(const cbmf_ctx* c) { return c ? c->last_bad : -1; }
 
 // ======================================================================= S0: set_psd
-static int set_psd_impl(cbmf_ctx* c, const double* psd_dev)
+// Resolve the input checks that the *_dev calls enqueue without waiting (cbmf.h): one 8-byte read-back.
+static int check_pending(cbmf_ctx* c)
+{
+    if (!c->pend_psd && !c->pend_seg) return CBMF_OK;
+    int err[2] = {0, 0};
+    CU(cudaMemcpyAsync(err, c->d_perr, sizeof(err), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    const bool bad_psd = c->pend_psd && err[0], bad_seg = c->pend_seg && err[1];
+    c->pend_psd = c->pend_seg = false;
+    if (bad_psd) { c->have_psd = false; c->have_seg = false; return CBMF_EINVAL; }
+    if (bad_seg) { c->have_seg = false; return CBMF_EINVAL; }
+    return CBMF_OK;
+}
+
+// defer: enqueue only and report an invalid entry at the next call that waits (the *_dev entry point).
+static int set_psd_impl(cbmf_ctx* c, const double* psd_dev, bool defer)
 {
     const int nh = (int)(c->n / 2);
     c->have_psd = false; c->have_seg = false;
-    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    c->pend_psd = c->pend_seg = false;
+    CU(cudaMemsetAsync(c->d_perr, 0, 2 * sizeof(int), c->stream));
     const int nblk = (nh + SCAN_TILE - 1) / SCAN_TILE;
     psd_terms_kernel<<<nblk, SCAN_THREADS, 0, c->stream>>>(psd_dev, c->d_wfac, c->d_term, c->d_bsum, nh, c->k_lo,
-                                                           c->df, c->dt, c->d_err);
+                                                           c->df, c->dt, c->d_perr);
     CU(cudaGetLastError());
     scan_block_sums_kernel<<<1, SCAN_THREADS, 0, c->stream>>>(c->d_bsum, nblk);
     CU(cudaGetLastError());
     prefix_tile_kernel<<<nblk, SCAN_THREADS, 0, c->stream>>>(c->d_term, c->d_bsum, c->d_prefix, nh);
     CU(cudaGetLastError());
     c->launches += 3;
-    int err = 0;
-    CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    if (err) return CBMF_EINVAL;
     c->have_psd = true;
-    return CBMF_OK;
+    c->pend_psd = true;
+    return defer ? CBMF_OK : check_pending(c);
 }
 
 extern "C" int cbmf_set_psd_dev(cbmf_ctx* c, const double* psd_dev, int64_t n_bins)
@@ -483,7 +502,7 @@ extern "C" int cbmf_set_psd_dev(cbmf_ctx* c, const double* psd_dev, int64_t n_bi
     if (!c || !psd_dev) return CBMF_EINVAL;
     if (n_bins != c->n / 2 + 1) return CBMF_EINVAL;
     DeviceGuard g(c->device);
-    return set_psd_impl(c, psd_dev);
+    return set_psd_impl(c, psd_dev, true);
 }
 
 extern "C" int cbmf_set_psd(cbmf_ctx* c, const double* psd, int64_t n_bins)
@@ -494,7 +513,7 @@ extern "C" int cbmf_set_psd(cbmf_ctx* c, const double* psd, int64_t n_bins)
     int rc = grow_scratch(c, sizeof(double) * (size_t)n_bins);
     if (rc) return rc;
     CU(cudaMemcpyAsync(c->d_scratch, psd, sizeof(double) * (size_t)n_bins, cudaMemcpyHostToDevice, c->stream));
-    return set_psd_impl(c, (const double*)c->d_scratch);
+    return set_psd_impl(c, (const double*)c->d_scratch, false);
 }
 
 // ======================================================================= S1: load_segment
@@ -520,17 +539,14 @@ static int enqueue_load_segment(cbmf_ctx* c, const float* samples_dev, c2* w_out
     return CBMF_OK;
 }
 
-static int load_segment_impl(cbmf_ctx* c, const float* samples_dev)
+static int load_segment_impl(cbmf_ctx* c, const float* samples_dev, bool defer)
 {
     c->have_seg = false;
-    int rc = enqueue_load_segment(c, samples_dev, c->d_w, c->d_Y, c->stream, c->d_err);
+    int rc = enqueue_load_segment(c, samples_dev, c->d_w, c->d_Y, c->stream, c->d_serr);
     if (rc) return rc;
-    int err = 0;
-    CU(cudaMemcpyAsync(&err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    if (err) return CBMF_EINVAL;
     c->have_seg = true;
-    return CBMF_OK;
+    c->pend_seg = true;
+    return defer ? CBMF_OK : check_pending(c);
 }
 
 extern "C" int cbmf_load_segment_dev(cbmf_ctx* c, const float* samples_dev, int64_t n_samples)
@@ -539,7 +555,7 @@ extern "C" int cbmf_load_segment_dev(cbmf_ctx* c, const float* samples_dev, int6
     if (n_samples != c->n) return CBMF_EINVAL;
     if (!c->have_psd) return CBMF_ESTATE;
     DeviceGuard g(c->device);
-    return load_segment_impl(c, samples_dev);
+    return load_segment_impl(c, samples_dev, true);
 }
 
 extern "C" int cbmf_load_segment(cbmf_ctx* c, const float* samples, int64_t n_samples)
@@ -548,10 +564,11 @@ extern "C" int cbmf_load_segment(cbmf_ctx* c, const float* samples, int64_t n_sa
     if (n_samples != c->n) return CBMF_EINVAL;
     if (!c->have_psd) return CBMF_ESTATE;
     DeviceGuard g(c->device);
-    int rc = grow_scratch(c, sizeof(float) * (size_t)c->n);
+    int rc = check_pending(c);
     if (rc) return rc;
+    if ((rc = grow_scratch(c, sizeof(float) * (size_t)c->n))) return rc;
     CU(cudaMemcpyAsync(c->d_scratch, samples, sizeof(float) * (size_t)c->n, cudaMemcpyHostToDevice, c->stream));
-    return load_segment_impl(c, (const float*)c->d_scratch);
+    return load_segment_impl(c, (const float*)c->d_scratch, false);
 }
 
 // ======================================================================= S2-S8: filter_bank
@@ -750,7 +767,7 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
     const bool to_host = (out_kind == cudaMemcpyDeviceToHost);
     const int64_t n_fast = trig_capacity < TRIG_SMALL ? trig_capacity : TRIG_SMALL;      // triggers the fast path delivers
-    const size_t b_status = 16, b_peaks = sizeof(PeakOut) * (size_t)nt, b_trig = sizeof(TrigOut) * (size_t)n_fast;
+    const size_t b_status = 32, b_peaks = sizeof(PeakOut) * (size_t)nt, b_trig = sizeof(TrigOut) * (size_t)n_fast;
     if (b_status + b_peaks + b_trig > c->stage_bytes) {
         if (c->h_stage) { CU(cudaFreeHost(c->h_stage)); c->h_stage = nullptr; c->stage_bytes = 0; }
         CU(cudaMallocHost(&c->h_stage, b_status + b_peaks + b_trig));
@@ -761,7 +778,7 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     unsigned char* h_trig = h_peaks + b_peaks;
 
     h_status[0] = 0ULL; h_status[1] = (unsigned long long)NO_BAD_TEMPLATE;
-    CU(cudaMemcpyAsync(c->d_cursor, h_status, b_status, cudaMemcpyHostToDevice, c->stream));      // cursor = 0, bad = none
+    CU(cudaMemcpyAsync(c->d_cursor, h_status, 16, cudaMemcpyHostToDevice, c->stream));            // cursor = 0, bad = none
     SetupArgs sa;
     sa.bank = bank_dev; sa.prefix = c->d_prefix; sa.coef = c->d_coef; sa.n_templates = (int)nt;
     sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.n_over_fs = (double)c->n / c->fs; sa.df = c->df;
@@ -785,6 +802,13 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     }
     CU(cudaStreamSynchronize(c->stream));
     if ((rc = ev_collect(c))) return rc;
+    {   // input checks that cbmf_set_psd_dev / cbmf_load_segment_dev left pending come back with the same copy
+        const int* errs = reinterpret_cast<const int*>(h_status + 2);
+        const bool bad_psd = c->pend_psd && errs[0], bad_seg = c->pend_seg && errs[1];
+        c->pend_psd = c->pend_seg = false;
+        if (bad_psd) { c->have_psd = false; c->have_seg = false; return CBMF_EINVAL; }
+        if (bad_seg) { c->have_seg = false; return CBMF_EINVAL; }
+    }
     if ((long long)h_status[1] != NO_BAD_TEMPLATE) { c->last_bad = (int64_t)h_status[1]; return CBMF_EINVAL; }
     const int64_t found = (int64_t)h_status[0];
     if (n_trig_found) *n_trig_found = found;
@@ -920,6 +944,7 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
     c->last_bad = -1;
     if (nt == 0) return CBMF_OK;
     DeviceGuard g(c->device);
+    if ((rc = check_pending(c))) return rc;
     if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
     if ((rc = pipe_alloc(c))) return rc;
     CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
@@ -1027,9 +1052,10 @@ extern "C" int cbmf_filter_stream(cbmf_ctx* c, const float* samples, int64_t n_t
     if (n_trig_found) *n_trig_found = 0;
     if (seg_offsets_out) seg_offsets_out[0] = 0;
     c->last_bad = -1;
-    c->have_seg = false;                       // the context's own segment slot is used as buffer 0 of the stream
     DeviceGuard g(c->device);
     int rc;
+    if ((rc = check_pending(c))) return rc;
+    c->have_seg = false;                       // the context's own segment slot is used as buffer 0 of the stream
     if (!c->d_w2) {
         CU(cudaMalloc(&c->d_w2, sizeof(c2) * (size_t)(n / 2)));
         CU(cudaMalloc(&c->d_segY, sizeof(c2) * (size_t)n));
@@ -1101,6 +1127,7 @@ extern "C" int cbmf_chisq(cbmf_ctx* c, const cbmf_template* bank, int64_t nt, co
     if (nt == 0) return CBMF_OK;
     DeviceGuard g(c->device);
     int rc;
+    if ((rc = check_pending(c))) return rc;
     if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
     CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
     if ((rc = bank_setup(c, c->d_bank, nt, 0.f))) return rc;
@@ -1156,6 +1183,7 @@ extern "C" int cbmf_debug_snr_series(cbmf_ctx* c, cbmf_template t, float* snr_ou
     if (!c->have_psd || !c->have_seg) return CBMF_ESTATE;
     DeviceGuard g(c->device);
     int rc;
+    if ((rc = check_pending(c))) return rc;
     if ((rc = setup_one(c, t))) return rc;
     const size_t n = (size_t)c->n;
     if ((rc = grow_scratch(c, sizeof(float2) * n + sizeof(float) * n))) return rc;
@@ -1185,6 +1213,7 @@ extern "C" int cbmf_debug_template(cbmf_ctx* c, cbmf_template t, float* h_out)
     if (!c->have_psd) return CBMF_ESTATE;                 // sigma comes from the PSD prefix table
     DeviceGuard g(c->device);
     int rc;
+    if ((rc = check_pending(c))) return rc;
     if ((rc = setup_one(c, t))) return rc;
     // the PRODUCT generator (pass 1 of filter_bank) with unit weights, its inputs dumped instead of transformed
     const size_t n = (size_t)c->n, nh = n / 2;
@@ -1253,6 +1282,7 @@ extern "C" int cbmf_debug_generate_dev(cbmf_ctx* c, const cbmf_template* bank_de
     if (nt == 0) return CBMF_OK;
     DeviceGuard g(c->device);
     int rc;
+    if ((rc = check_pending(c))) return rc;
     if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
     CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
     SetupArgs sa;
@@ -1277,6 +1307,7 @@ extern "C" int cbmf_debug_get_prefix(cbmf_ctx* c, double* p_out)
     if (!c || !p_out) return CBMF_EINVAL;
     if (!c->have_psd) return CBMF_ESTATE;
     DeviceGuard g(c->device);
+    if (int r = check_pending(c)) return r;
     CU(cudaMemcpyAsync(p_out, c->d_prefix, sizeof(double) * (size_t)(c->n / 2), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return CBMF_OK;
@@ -1287,6 +1318,7 @@ extern "C" int cbmf_debug_get_weights(cbmf_ctx* c, float* w_out)
     if (!c || !w_out) return CBMF_EINVAL;
     if (!c->have_seg) return CBMF_ESTATE;
     DeviceGuard g(c->device);
+    if (int r = check_pending(c)) return r;
     CU(cudaMemcpyAsync(w_out, c->d_w, sizeof(float2) * (size_t)(c->n / 2), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return CBMF_OK;

@@ -545,3 +545,35 @@ def test_device_pointer_entry_points(cbmf):
     tr = trig.cpu().numpy().view(cbmf.TRIG_DTYPE)[:nf]
     assert np.array_equal(pk, ref_pk) and np.array_equal(tr, ref_tr)
     g.close()
+
+
+def test_device_entry_points_defer_their_input_checks(cbmf):
+    """cbmf.h: cbmf_set_psd_dev / cbmf_load_segment_dev are stream-ordered -- they enqueue and return; an invalid PSD
+    entry or sample is reported (EINVAL) by the next call that waits, which leaves the context without it."""
+    import torch
+    wl = W.small_case(log2n=13, n_templates=3, seed=5)
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    psd_bad = wl.psd.copy(); psd_bad[wl.n // 4] = -3.0
+    g.set_psd(torch.from_numpy(psd_bad).cuda())                    # returns: the check is enqueued
+    g.load_segment(torch.from_numpy(wl.samples).cuda())
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.filter_bank(wl.bank, 6.0)
+    assert e.value.rc == cbmf.EINVAL
+    with pytest.raises(cbmf.CbmfError) as e:                       # the context has no PSD now
+        g.filter_bank(wl.bank, 6.0)
+    assert e.value.rc == cbmf.ESTATE
+    g.set_psd(torch.from_numpy(wl.psd).cuda())
+    s_bad = wl.samples.copy(); s_bad[100] = np.nan
+    g.load_segment(torch.from_numpy(s_bad).cuda())
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.debug_snr_series(1.4, 1.4)                               # any waiting call reports it
+    assert e.value.rc == cbmf.EINVAL
+    with pytest.raises(cbmf.CbmfError) as e:
+        g.filter_bank(wl.bank, 6.0)
+    assert e.value.rc == cbmf.ESTATE                               # PSD kept, segment gone
+    g.load_segment(torch.from_numpy(wl.samples).cuda())
+    a = g.filter_bank(wl.bank, 6.0)
+    g.set_psd(wl.psd); g.load_segment(wl.samples)                  # host-pointer calls: checked at once, same results
+    b = g.filter_bank(wl.bank, 6.0)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    g.close()
