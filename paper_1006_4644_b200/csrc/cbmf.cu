@@ -789,10 +789,9 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
     c->ev_used[0] = c->ev_used[1] = 0;
     if ((rc = run_bank_passes(c, nt, c->trig_cap))) return rc;
     const int sort_limit = (int)(c->trig_cap < TRIG_SMALL ? c->trig_cap : TRIG_SMALL);
-    CU(ensure_smem_attr(c, trig_sort_small_dev_kernel,
-                        (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL));
-    trig_sort_small_dev_kernel<<<1, 1024, (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL,
-                                 c->stream>>>(c->d_trig, c->d_cursor, c->d_bad, sort_limit);
+    CU(ensure_smem_attr(c, trig_sort_small_dev_kernel, trig_sort_dev_smem()));
+    trig_sort_small_dev_kernel<<<1, 1024, trig_sort_dev_smem(), c->stream>>>(c->d_trig, c->d_cursor, c->d_bad, sort_limit,
+                                                                              c->d_tcount, (int)nt);
     CU(cudaGetLastError());
     c->launches += 1;
     CU(cudaMemcpyAsync(h_status, c->d_cursor, b_status, cudaMemcpyDeviceToHost, c->stream));

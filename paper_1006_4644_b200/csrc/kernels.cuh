@@ -46,7 +46,7 @@ template <int L> struct Cfg;
 #define CBMF_CFG(L_, E_, R1_, R2_, R3_, NT1_)                                            \
     template <> struct Cfg<L_> {                                                         \
         static constexpr int E = E_, R1 = R1_, R2 = R2_, R3 = R3_, T = L_ / E_;          \
-        static constexpr int NT1 = NT1_, NT2 = 256;                                      \
+        static constexpr int NT1 = NT1_, NT2 = (L_ == 1024 ? 128 : 256);                                      \
         static constexpr int C = NT1 / T, ROWS = NT2 / T;                                \
         static constexpr int PADDED = L_ + L_ / R1_;                                     \
         static_assert(R1_ * R2_ * R3_ == L_, "radices");                                 \
@@ -1120,7 +1120,7 @@ __device__ __forceinline__ void p2_item(const P2Args& a, const int item, const i
 }
 
 template <int L1, int L2, int MODE, bool MASK = false>
-__global__ void __launch_bounds__(256, 2) p2_kernel(const P2Args a)
+__global__ void __launch_bounds__(Cfg<L2>::NT2, 512 / Cfg<L2>::NT2) p2_kernel(const P2Args a)
 {
     extern __shared__ __align__(16) c2 smem[];
     if constexpr (MODE == EPI_MAX) {
@@ -1395,17 +1395,78 @@ __global__ void __launch_bounds__(1024) trig_sort_small_kernel(TrigOut* trig, in
     for (int i = threadIdx.x; i < n; i += blockDim.x) trig[i] = rec[pos[i]];
 }
 
-// The same with the count read on the device (the total of the bank's trigger cursor): lets the host enqueue the sort
+// The small sort with the count read on the device (the total of the bank's trigger cursor): lets the host enqueue it
 // behind the bank without waiting for the count.  Does nothing when there are more triggers than `limit` (the list
 // capacity or TRIG_SMALL): the host then takes the general path.
+// Fast path (banks of up to TRIG_GROUP_MAX_T templates, no template with more than TRIG_GROUP_MAX_PER triggers -- the
+// usual case: a few above-threshold samples per ringing template): the per-template counts the epilogue keeps give
+// every template its range by one scan; the records are scattered to their ranges in shared memory and every record
+// finds its place by counting the smaller samples of its own range (the threads of a warp mostly share the range, so
+// its records are read as broadcasts).  Otherwise the bitonic network of trig_sort_small_kernel.
+constexpr int TRIG_GROUP_MAX_T = 8192, TRIG_GROUP_MAX_PER = 1024;
+__host__ __device__ constexpr size_t trig_sort_dev_smem()
+{
+    const size_t bitonic = (sizeof(unsigned long long) + sizeof(TrigOut) + sizeof(unsigned short)) * TRIG_SMALL;
+    const size_t group = sizeof(TrigOut) * TRIG_SMALL + 2 * sizeof(int) * (TRIG_GROUP_MAX_T + 1);
+    return bitonic > group ? bitonic : group;
+}
 __global__ void __launch_bounds__(1024) trig_sort_small_dev_kernel(TrigOut* trig, const unsigned long long* __restrict__ cursor,
-                                                                   const long long* __restrict__ bad, int limit)
+                                                                   const long long* __restrict__ bad, int limit,
+                                                                   const unsigned int* __restrict__ tcount, int n_templates)
 {
     extern __shared__ __align__(16) unsigned char trig_smem_raw[];
+    __shared__ int s_part[32];
+    __shared__ int s_max;
     if (__ldg(bad) != NO_BAD_TEMPLATE) return;
     const unsigned long long found = __ldg(cursor);
     if (found > (unsigned long long)limit || found < 2ULL) return;
     const int n = (int)found;
+    if (n_templates <= TRIG_GROUP_MAX_T) {
+        TrigOut* rec = reinterpret_cast<TrigOut*>(trig_smem_raw);                             // [TRIG_SMALL]
+        int* off = reinterpret_cast<int*>(rec + TRIG_SMALL);                                  // [n_templates + 1] range starts
+        int* fill = off + (TRIG_GROUP_MAX_T + 1);                                             // [n_templates] running fill
+        // per-thread chunk of the counts: local sum and maximum, block scan of the sums, then the starts
+        const int per = (n_templates + (int)blockDim.x - 1) / (int)blockDim.x;
+        const int t0 = threadIdx.x * per, t1 = min(n_templates, t0 + per);
+        int sum = 0, mx = 0;
+        for (int t = t0; t < t1; ++t) { const int cnt = (int)tcount[t]; sum += cnt; mx = max(mx, cnt); }
+        int inc = sum;
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xFFFFFFFFu, inc, o); if (lane >= o) inc += v; }
+        mx = __reduce_max_sync(0xFFFFFFFFu, mx);
+        if (threadIdx.x == 0) s_max = 0;
+        if (lane == 31) s_part[warp] = inc;
+        __syncthreads();
+        if (lane == 0) atomicMax(&s_max, mx);
+        if (warp == 0) {
+            int v = s_part[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int w = __shfl_up_sync(0xFFFFFFFFu, v, o); if (lane >= o) v += w; }
+            s_part[lane] = v;
+        }
+        __syncthreads();
+        if (s_max <= TRIG_GROUP_MAX_PER) {
+            int run = inc - sum + (warp > 0 ? s_part[warp - 1] : 0);
+            for (int t = t0; t < t1; ++t) { off[t] = run; fill[t] = 0; run += (int)tcount[t]; }
+            if (threadIdx.x == 0) off[n_templates] = n;
+            __syncthreads();
+            for (int i = threadIdx.x; i < n; i += blockDim.x) {
+                const TrigOut o = trig[i];
+                rec[off[o.template_idx] + atomicAdd(&fill[o.template_idx], 1)] = o;
+            }
+            __syncthreads();
+            for (int i = threadIdx.x; i < n; i += blockDim.x) {                               // rank inside the template's range
+                const TrigOut o = rec[i];
+                const int a0 = off[o.template_idx], a1 = off[o.template_idx + 1];
+                int r = 0;
+                for (int j = a0; j < a1; ++j) r += (rec[j].sample_idx < o.sample_idx) ? 1 : 0;
+                trig[a0 + r] = o;
+            }
+            return;
+        }
+        __syncthreads();
+    }
     int n_pow2 = 2;
     while (n_pow2 < n) n_pow2 <<= 1;
     unsigned long long* key = reinterpret_cast<unsigned long long*>(trig_smem_raw);          // [n_pow2]
