@@ -830,7 +830,7 @@ __device__ __forceinline__ void p2_prefetch_row(c2* __restrict__ sm, const c2* _
     constexpr int T = Cfg<L2>::T, E = Cfg<L2>::E, NC = Cfg<L1>::C;
     static_assert(NC % 2 == 0, "16-byte chunks must not straddle tiles");
     // the chunks of one thread are whole tiles apart and the largest offset fits the immediate field of the copy
-    constexpr bool IMM = ((2 * T) % NC == 0) && ((long long)sizeof(c2) * 2 * T * L1 * (E / 2) < (1LL << 23));
+    constexpr bool IMM = ((2 * T) % NC == 0) && ((long long)sizeof(c2) * 2 * T * L1 * (E / 2 - 1) < (1LL << 23));
     if constexpr (IMM) {
         P2Prefetch<L1, L2, 0>::run((unsigned)__cvta_generic_to_shared(sm + 2 * t), yb + y_index<L1, NC>(j1, 2 * t));
     } else {
