@@ -145,10 +145,11 @@ int ilog2(int64_t n) { int l = 0; while ((int64_t(1) << l) < n) ++l; return l; }
 
 // ---------------------------------------------------------------- launch dispatch over (N1, N2)
 // Blocks per column tile of a pass-1 launch (LOAD_GEN).  Each block stages its tile of w once and walks
-// through its share of the templates, so FEW, LONG-LIVED blocks are wanted: about one per SM in total.  They
-// then occupy one of the two block slots of an SM for the whole launch and the pass-2 blocks of the other
-// streams take the second slot, which pairs the generator / exchange phases of pass 1 with the FMA-bound
-// row FFTs of pass 2 on every SM (+12 % over short-lived blocks at 4 streams).
+// through its share of the templates, so FEW, LONG-LIVED blocks are wanted (+12 % over
+// short-lived blocks at 4 streams): as many as the SMs hold at once, two per SM.  With four launch pairs in
+// flight the block scheduler then mixes them with the pass-2 blocks of the other pairs on every SM, which
+// pairs the generator / exchange phases of pass 1 with the FMA-bound row FFTs of pass 2; a launch timed alone
+// fills the GPU by itself (one block per SM left half of every SM idle in that measurement, same bank throughput).
 // Series for k^{-1/3} in the generator (spa_correlate): valid where (columns of a tile - 1) / (first bin
 // of the first in-band row) <= 2e-3.
 bool p1_series_ok(int k_lo, int l2, int tile_cols)
@@ -159,7 +160,7 @@ bool p1_series_ok(int k_lo, int l2, int tile_cols)
 
 int p1_groups(int n_sm, int n_tiles, int batch)
 {
-    int g = n_sm / n_tiles;
+    int g = 2 * n_sm / n_tiles;            // two blocks fit an SM (registers, shared memory)
     if (g < 1) g = 1;
     if (g > batch) g = batch;
     return g;

@@ -603,8 +603,10 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<
     double* __restrict__ ub = reinterpret_cast<double*>(wt + (size_t)(L1 / 2) * NC);                    // (!BYROWS)
     float* __restrict__ inv = reinterpret_cast<float*>(ub + L1 / 2);
     // Row records are WARP-LOCAL: a warp holds T_W = 32 / NC values of t and needs the rows k1 = t + T r, r < R1/2, of
-    // exactly those; its 32 lanes fill them (RPT = T_W (R1/2) / 32 rows each: lane (t, c) takes r = RPT c + i), so a
-    // __syncwarp orders fill and use and no block barrier is involved.  kb^{-1/3} of a lane's rows stays in registers.
+    // exactly those; its 32 lanes fill them (RPT = T_W (R1/2) / 32 rows each: lane (t, c) takes r = c + NC i, so that
+    // the rows of one i are the NC lowest ones still open and a band that ends below them skips that i for the whole
+    // warp), so a __syncwarp orders fill and use and no block barrier is involved.  kb^{-1/3} of a lane's rows stays
+    // in registers.
     static_assert(!BYROWS || (NC <= 32 && ((R1 / 2) % NC == 0 || NC % (R1 / 2) == 0)), "rows of a warp divide among its lanes");
     constexpr int RPT_W = ((R1 / 2) / NC > 1) ? (R1 / 2) / NC : 1;      // lanes c >= R1/2 of a wide tile stay idle
     double u_mine[RPT_W];
@@ -612,8 +614,8 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<
         if constexpr (BYROWS) {
 #pragma unroll
             for (int i = 0; i < RPT_W; ++i) {
-                const int k1 = t + T * (RPT_W * c + i);
-                u_mine[i] = (RPT_W * c + i < R1 / 2) ? __ldg(a.u + (k1 * L2 + tile * NC)) : 0.0;
+                const int k1 = t + T * (c + NC * i);
+                u_mine[i] = (c + NC * i < R1 / 2) ? __ldg(a.u + (k1 * L2 + tile * NC)) : 0.0;
             }
         } else {
             for (int k1 = threadIdx.x; k1 < L1 / 2; k1 += NT) {
@@ -629,9 +631,9 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<
         const SpaCoef sc = spa_coef(tn);
 #pragma unroll
         for (int i = 0; i < RPT_W; ++i) {
-            const int k1 = t + T * (RPT_W * c + i);
+            const int k1 = t + T * (c + NC * i);
             const int kb = k1 * L2 + tile * NC;
-            if (RPT_W * c + i < R1 / 2 && kb + NC - 1 >= k_lo && kb <= k_hi) {
+            if (c + NC * i < R1 / 2 && kb + NC - 1 >= k_lo && kb <= k_hi) {
                 const RowCoef r = spa_row_coef(u_mine[i], kb, sc, a.lnk);
                 if (k1 < RS) rc_lo[k1] = r; else rc_hi[k1 - RS] = r;
             }
