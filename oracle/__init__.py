@@ -75,6 +75,12 @@ def lib():
         L.orc_chisq.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int64, C.c_int, dp, dp, C.POINTER(C.c_int64)]
         L.orc_cluster_triggers.argtypes = [C.POINTER(Trigger), C.c_int64, C.c_int64, C.c_int64,
                                            C.POINTER(Trigger), C.c_int64, C.POINTER(C.c_int64)]
+        L.orc_td_phase.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, dp, dp]
+        L.orc_td_extent.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, dp, dp, dp]
+        L.orc_td_template.argtypes = [C.c_void_p, C.c_double, C.c_double, dp, dp]
+        L.orc_td_snr_series.argtypes = [C.c_void_p, C.c_double, C.c_double, dp, dp, dp, dp, dp]
+        L.orc_td_filter_bank.argtypes = [C.c_void_p, dp, C.c_int64, C.c_double, C.POINTER(Peak),
+                                         C.POINTER(Trigger), C.c_int64, C.POINTER(C.c_int64)]
         L.orc_num_threads.restype = C.c_int
         L.orc_set_num_threads.argtypes = [C.c_int]
         _lib = L
@@ -119,6 +125,24 @@ def band(n: int, fs: float, f_low: float, m1: float, m2: float):
     if rc:
         raise OracleError(rc, "orc_band")
     return klo.value, khi.value
+
+
+def td_phase(m1: float, m2: float, tau: float, half_order: int):
+    """NEXT-3 (time domain): -> (phi_gw [rad], F [Hz]) at tau = t_c - t seconds before coalescence."""
+    phi, f = C.c_double(), C.c_double()
+    rc = lib().orc_td_phase(float(m1), float(m2), float(tau), int(half_order), C.byref(phi), C.byref(f))
+    if rc:
+        raise OracleError(rc, "orc_td_phase")
+    return phi.value, f.value
+
+
+def td_extent(m1: float, m2: float, f_low: float, half_order: int):
+    """-> (tau_start, tau_end, f_end): the time-domain template lives on tau_end <= t_c - t <= tau_start."""
+    a, b, f = C.c_double(), C.c_double(), C.c_double()
+    rc = lib().orc_td_extent(float(m1), float(m2), float(f_low), int(half_order), C.byref(a), C.byref(b), C.byref(f))
+    if rc:
+        raise OracleError(rc, "orc_td_extent")
+    return a.value, b.value, f.value
 
 
 def cluster_triggers(trig: np.ndarray, n_samples: int, window: int, capacity: int | None = None):
@@ -254,6 +278,37 @@ class Oracle:
         if rc:
             raise OracleError(rc, "orc_chisq")
         return chi.value, zl, edges
+
+    def td_template(self, m1: float, m2: float):
+        """NEXT-3 (time domain): -> (h_plus[n], h_cross[n]), coalescence at sample 0 (= n)."""
+        hp, hc = np.empty(self.n), np.empty(self.n)
+        rc = lib().orc_td_template(self._h, m1, m2, _dp(hp), _dp(hc))
+        if rc:
+            raise OracleError(rc, "orc_td_template")
+        return hp, hc
+
+    def td_snr_series(self, m1: float, m2: float):
+        """-> (rho[n], c_plus/sigma_plus [n], c_cross/sigma_cross [n], sigma_plus, sigma_cross)"""
+        rho, cp, cc = np.empty(self.n), np.empty(self.n), np.empty(self.n)
+        sp, sc = C.c_double(), C.c_double()
+        rc = lib().orc_td_snr_series(self._h, m1, m2, _dp(rho), _dp(cp), _dp(cc), C.byref(sp), C.byref(sc))
+        if rc:
+            raise OracleError(rc, "orc_td_snr_series")
+        return rho, cp, cc, sp.value, sc.value
+
+    def td_filter_bank(self, bank: np.ndarray, snr_threshold: float, trig_capacity: int = 1 << 20):
+        """-> (peaks[PEAK_DTYPE], triggers[TRIG_DTYPE], n_found, rc) with the time-domain templates"""
+        b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+        nt = b.shape[0]
+        peaks = np.zeros(max(nt, 1), dtype=PEAK_DTYPE)
+        trig = np.zeros(max(trig_capacity, 1), dtype=TRIG_DTYPE)
+        nf = C.c_int64()
+        rc = lib().orc_td_filter_bank(self._h, _dp(b), nt, float(snr_threshold),
+                                      peaks.ctypes.data_as(C.POINTER(Peak)),
+                                      trig.ctypes.data_as(C.POINTER(Trigger)), trig_capacity, C.byref(nf))
+        if rc < 0:
+            raise OracleError(rc, "orc_td_filter_bank")
+        return peaks[:nt], trig[:min(nf.value, trig_capacity)], nf.value, rc
 
     def filter_bank(self, bank: np.ndarray, snr_threshold: float, trig_capacity: int = 1 << 20):
         """-> (peaks[PEAK_DTYPE], triggers[TRIG_DTYPE], n_found, rc)"""

@@ -25,7 +25,10 @@
  * twin added in round 2, is pinned by hand-built trigger lists whose clusters
  * follow from the definition by inspection: test_cluster_*; orc_chisq, the
  * NEXT-4 twin, by sum_l z_l = z, chi^2 = 0 for data proportional to the
- * template, <chi^2> = 2p - 2 in noise and equal band powers: test_chisq_*.)
+ * template, <chi^2> = 2p - 2 in noise and equal band powers: test_chisq_*;
+ * orc_td_*, the time-domain generator and two-polarisation filter of NEXT-3,
+ * by the energy-balance equation, d phi/dt = 2 pi F, the closed forms of a
+ * noise-free injection and the agreement with the SPA filter: test_td_*.)
  *
  * Threads: OpenMP across templates only (orc_filter_bank).
  */
@@ -581,6 +584,225 @@ int orc_cluster_triggers(const orc_trigger *trig, int64_t n_trig, int64_t n_samp
     *n_out = n_ev;
     free(label); free(ev);
     return (out && n_ev > w) ? ORC_WTRUNC : ORC_OK;
+}
+
+/* ------------------------------------------------- NEXT-3, second part: the paper's own generator */
+
+/* "the two polarization of the template signal are generated, FFT transformed and normalized" (steps
+ * device_template_proc / complex_mf / two cufft_C2R / madd2 of PAPER.md:127-131; "order 2.5 in phase and 0 in
+ * amplitude").  The paper prints no formula.  Reading A28: the time-domain
+ * approximant is the one with an EXPLICIT phase as a function of time, so that every sample is an independent
+ * evaluation (what a one-thread-per-sample generator needs) -- "TaylorT3", Blanchet, Living Rev. Relativity 9, 4
+ * (2006), eq. (234), and Buonanno, Iyer, Ochsner, Pan & Sathyaprakash, Phys. Rev. D 80, 084043 (2009), eq. (3.8):
+ * with tau = t_c - t, Theta = eta tau / (5 M), y = Theta^{-1/8},
+ *   phi_orb(t) = -(1/eta) [ y^-5 + a2 y^-3 - (3 pi/4) y^-2 + a4 y^-1 + a5 ln(Theta) ],   phi_gw = 2 phi_orb,
+ *   a2 = 3715/8064 + 55 eta/96,
+ *   a4 = 9275495/14450688 + 284875 eta/258048 + 1855 eta^2/2048,
+ *   a5 = (-38645/172032 + 65 eta/2048) pi        (the 2.5PN term; 0 at half_order 4),
+ * and the gravitational-wave frequency is the exact derivative of that phase, F = (1/2 pi) d phi_gw/dt:
+ *   F(y) = Phi(y) / (5 pi M),  Phi(y) = (5/8) y^3 + (3/8) a2 y^5 - (3 pi/16) y^6 + (1/8) a4 y^7 + a5 y^8.
+ * Polarisations (amplitude at Newtonian order, i.e. proportional to F^{2/3}; overall scale irrelevant, the
+ * template is normalised):  h_+ = (F/f_low)^{2/3} cos(phi_gw),  h_x = (F/f_low)^{2/3} sin(phi_gw).
+ * Extent: from F = f_low up to F = f_ISCO (reading A1's cut-off), or up to the maximum of F where the series stops
+ * sweeping upward before f_ISCO (it does at 2.5PN): y_t = smallest positive root of dPhi/dy (scan in steps of
+ * 1/256 up to y = 4, then bisection); y_end = root of F = f_ISCO on (0, y_t] if F(y_t) >= f_ISCO, else y_t;
+ * y_start = root of F = f_low on (0, y_end]; empty if F(y_end) <= f_low.  tau = (5 M/eta) y^-8.
+ * Pins (tests/test_oracle_pins.py, test_td_*): the frequency against the energy-balance equation
+ * dv/dt = -Flux(v)/(M e'(v)) with the 2.5PN energy and flux (residual of relative order v^6), d phi/dt = 2 pi F,
+ * the end points, and the filter pins below. */
+typedef struct { double M, eta, a2, a4, a5; } td_coef;
+
+static td_coef td_coefs(double m1, double m2, int half_order)
+{
+    td_coef q;
+    q.M = (m1 + m2) * ORC_TSUN;
+    q.eta = m1 * m2 / ((m1 + m2) * (m1 + m2));
+    q.a2 = 3715.0 / 8064.0 + 55.0 * q.eta / 96.0;
+    q.a4 = 9275495.0 / 14450688.0 + 284875.0 * q.eta / 258048.0 + 1855.0 * q.eta * q.eta / 2048.0;
+    q.a5 = half_order >= 5 ? (-38645.0 / 172032.0 + 65.0 * q.eta / 2048.0) * ORC_PI : 0.0;
+    return q;
+}
+static double td_Phi(const td_coef *q, double y)
+{
+    double y2 = y * y, y3 = y2 * y;
+    return y3 * (5.0 / 8.0 + y2 * (3.0 / 8.0 * q->a2 + y * (-3.0 * ORC_PI / 16.0 + y * (q->a4 / 8.0 + y * q->a5))));
+}
+static double td_dPhi_over_y2(const td_coef *q, double y)       /* (dPhi/dy) / y^2 */
+{
+    double y2 = y * y;
+    return 15.0 / 8.0 + y2 * (15.0 / 8.0 * q->a2 + y * (-9.0 * ORC_PI / 8.0 + y * (7.0 / 8.0 * q->a4 + y * 8.0 * q->a5)));
+}
+/* root of g(y) = target on [lo, hi], g increasing there, g(lo) <= target <= g(hi): 200 bisections */
+static double td_bisect(const td_coef *q, double lo, double hi, double target)
+{
+    for (int i = 0; i < 200; ++i) {
+        double mid = 0.5 * (lo + hi);
+        if (td_Phi(q, mid) < target) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+/* phi_gw and F at tau = t_c - t > 0 (seconds). */
+int orc_td_phase(double m1, double m2, double tau, int half_order, double *phi_gw, double *f_gw)
+{
+    if (!(m1 > 0) || !(m2 > 0) || !(tau > 0) || (half_order != 4 && half_order != 5)) return ORC_EINVAL;
+    td_coef q = td_coefs(m1, m2, half_order);
+    double theta = q.eta * tau / (5.0 * q.M);
+    double y = pow(theta, -0.125);
+    if (phi_gw)
+        *phi_gw = -(2.0 / q.eta) * (pow(y, -5.0) + q.a2 * pow(y, -3.0) - 0.75 * ORC_PI / (y * y) + q.a4 / y + q.a5 * log(theta));
+    if (f_gw) *f_gw = td_Phi(&q, y) / (5.0 * ORC_PI * q.M);
+    return ORC_OK;
+}
+
+/* Extent of the time-domain template: tau_start >= tau >= tau_end (both 0 when empty), f_end = F(tau_end). */
+int orc_td_extent(double m1, double m2, double f_low, int half_order, double *tau_start, double *tau_end, double *f_end)
+{
+    if (!(m1 > 0) || !(m2 > 0) || !(f_low > 0) || (half_order != 4 && half_order != 5)) return ORC_EINVAL;
+    td_coef q = td_coefs(m1, m2, half_order);
+    const double scale = 5.0 * ORC_PI * q.M;                  /* Phi = scale * F */
+    double y_t = 4.0;
+    for (int i = 1; i <= 1024; ++i) {
+        double y = (double)i / 256.0;
+        if (td_dPhi_over_y2(&q, y) <= 0.0) {
+            double lo = (double)(i - 1) / 256.0, hi = y;
+            for (int it = 0; it < 200; ++it) {
+                double mid = 0.5 * (lo + hi);
+                if (td_dPhi_over_y2(&q, mid) > 0.0) lo = mid; else hi = mid;
+            }
+            y_t = 0.5 * (lo + hi);
+            break;
+        }
+    }
+    double f_isco = orc_f_isco(m1, m2);
+    double y_end = (td_Phi(&q, y_t) >= scale * f_isco) ? td_bisect(&q, 0.0, y_t, scale * f_isco) : y_t;
+    double fe = td_Phi(&q, y_end) / scale;
+    if (tau_start) *tau_start = 0.0;
+    if (tau_end) *tau_end = 0.0;
+    if (f_end) *f_end = fe;
+    if (!(fe > f_low)) return ORC_OK;                          /* empty */
+    double y_start = td_bisect(&q, 0.0, y_end, scale * f_low);
+    if (tau_start) *tau_start = 5.0 * q.M / q.eta * pow(y_start, -8.0);
+    if (tau_end) *tau_end = 5.0 * q.M / q.eta * pow(y_end, -8.0);
+    return ORC_OK;
+}
+
+/* The two polarisations on the sample grid of the context, coalescence at sample 0 (= n, the segment is a circle):
+ * sample j has tau_j = (n - j) dt (j = 0: tau = n dt); h = 0 outside [tau_end, tau_start].  hp, hc: n doubles each.
+ * EINVAL if the template does not fit the segment (tau_start >= n dt). */
+int orc_td_template(const orc_ctx *c, double m1, double m2, double *hp, double *hc)
+{
+    if (!c || !hp || !hc) return ORC_EINVAL;
+    double ts, te, fe;
+    int rc = orc_td_extent(m1, m2, c->f_low, c->pn_half_order, &ts, &te, &fe);
+    if (rc) return rc;
+    int64_t n = c->n;
+    if (!(ts < (double)n * c->dt)) return ORC_EINVAL;
+    for (int64_t j = 0; j < n; ++j) {
+        double tau = (double)(n - j) * c->dt;
+        hp[j] = hc[j] = 0.0;
+        if (ts > 0.0 && tau <= ts && tau >= te) {
+            double phi, f;
+            orc_td_phase(m1, m2, tau, c->pn_half_order, &phi, &f);
+            double a = pow(f / c->f_low, 2.0 / 3.0);
+            hp[j] = a * cos(phi);
+            hc[j] = a * sin(phi);
+        }
+    }
+    return ORC_OK;
+}
+
+/* The filter of PAPER.md:96-101 with that template, as the definition: for each polarisation p in {+, x}
+ *   H_p[k] = dt sum_j h_p[j] e^{-2 pi i jk/n}                                   (forward FFT)
+ *   sigma_p^2 = 4 df sum_{k=k_lo}^{n/2-1} |H_p[k]|^2 / S_n[k]                    (normalisation)
+ *   c_p[j] = 4 df Re sum_{k=k_lo}^{n/2-1} d~[k] H_p*[k] / S_n[k] e^{+2 pi i jk/n} (correlator, eq. 2.1)
+ *   rho[j] = sqrt( (c_+[j]/sigma_+)^2 + (c_x[j]/sigma_x)^2 )                     (reading A4:
+ *            each polarisation of unit norm, so that noise alone gives <rho^2> = 2)
+ * over every bin from k_lo to Nyquist where S_n is finite (the time-domain template has no band of its own).
+ * cp_out / cc_out (n doubles each, may be NULL) receive c_+/sigma_+ and c_x/sigma_x. */
+int orc_td_snr_series(const orc_ctx *c, double m1, double m2, double *rho_out, double *cp_out, double *cc_out,
+                      double *sigma_p_out, double *sigma_c_out)
+{
+    if (!c || !rho_out) return ORC_EINVAL;
+    if (!c->psd || !c->dtil) return ORC_ESTATE;
+    int64_t n = c->n;
+    int64_t klo = (int64_t)ceil(c->f_low * ((double)n / c->fs));
+    double *hp = (double *)malloc(sizeof(double) * (size_t)n), *hc = (double *)malloc(sizeof(double) * (size_t)n);
+    double *x = (double *)malloc(sizeof(double) * 2 * (size_t)n), *q = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    if (!hp || !hc || !x || !q) { free(hp); free(hc); free(x); free(q); return ORC_ENOMEM; }
+    int rc = orc_td_template(c, m1, m2, hp, hc);
+    double sig[2] = {0.0, 0.0};
+    for (int64_t j = 0; j < n; ++j) rho_out[j] = 0.0;
+    for (int pol = 0; pol < 2 && !rc; ++pol) {
+        const double *h = pol ? hc : hp;
+        for (int64_t j = 0; j < n; ++j) { x[2 * j] = h[j]; x[2 * j + 1] = 0.0; }
+        rc = fft_radix2(x, n, -1, c->tw_re, c->tw_im);
+        if (rc) break;
+        memset(q, 0, sizeof(double) * 2 * (size_t)n);
+        double s2 = 0.0;
+        for (int64_t k = klo; k < n / 2; ++k) {
+            if (isinf(c->psd[k])) continue;
+            double hr = c->dt * x[2 * k], hi = c->dt * x[2 * k + 1];
+            double wgt = 4.0 * c->df / c->psd[k];
+            s2 += wgt * (hr * hr + hi * hi);
+            double dr = c->dtil[2 * k], di = c->dtil[2 * k + 1];
+            q[2 * k]     = wgt * (dr * hr + di * hi);           /* d~ conj(H) */
+            q[2 * k + 1] = wgt * (di * hr - dr * hi);
+        }
+        sig[pol] = sqrt(s2);
+        rc = fft_radix2(q, n, +1, c->tw_re, c->tw_im);
+        if (rc) break;
+        double *cout = pol ? cc_out : cp_out;
+        for (int64_t j = 0; j < n; ++j) {
+            double v = sig[pol] > 0 ? q[2 * j] / sig[pol] : 0.0;
+            if (cout) cout[j] = v;
+            rho_out[j] += v * v;
+        }
+    }
+    if (!rc) for (int64_t j = 0; j < n; ++j) rho_out[j] = sqrt(rho_out[j]);
+    if (sigma_p_out) *sigma_p_out = sig[0];
+    if (sigma_c_out) *sigma_c_out = sig[1];
+    free(hp); free(hc); free(x); free(q);
+    return rc;
+}
+
+/* The bank loop with the time-domain templates: peak = smallest j attaining max rho, phase = atan2(c_x/sigma_x,
+ * c_+/sigma_+) there, sigma = sigma_+; triggers rho[j] > threshold (strict), sorted by (template, sample),
+ * truncated at the capacity (ORC_WTRUNC).  An empty template returns {0, -1, 0, 0}. */
+int orc_td_filter_bank(const orc_ctx *c, const double *bank_m1m2, int64_t n_templates, double snr_threshold,
+                       orc_peak *peaks_out, orc_trigger *trig_out, int64_t trig_capacity, int64_t *n_trig_found)
+{
+    if (!c || (!bank_m1m2 && n_templates) || n_templates < 0 || (!peaks_out && n_templates)) return ORC_EINVAL;
+    if (!(snr_threshold >= 0)) return ORC_EINVAL;
+    if (!c->psd || !c->dtil) return ORC_ESTATE;
+    int64_t n = c->n, total = 0, written = 0;
+    double *rho = (double *)malloc(sizeof(double) * (size_t)n), *cp = (double *)malloc(sizeof(double) * (size_t)n);
+    double *cc = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!rho || !cp || !cc) { free(rho); free(cp); free(cc); return ORC_ENOMEM; }
+    int rc = ORC_OK;
+    for (int64_t t = 0; t < n_templates && !rc; ++t) {
+        double sp = 0.0, sc = 0.0;
+        rc = orc_td_snr_series(c, bank_m1m2[2 * t], bank_m1m2[2 * t + 1], rho, cp, cc, &sp, &sc);
+        if (rc) break;
+        orc_peak *pk = &peaks_out[t];
+        if (!(sp > 0) || !(sc > 0)) { pk->snr_max = 0.0; pk->idx_peak = -1; pk->phase = 0.0; pk->sigma = 0.0; continue; }
+        int64_t jb = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (rho[j] > rho[jb]) jb = j;
+            if (rho[j] > snr_threshold) {
+                if (trig_out && written < trig_capacity) {
+                    orc_trigger *o = &trig_out[written++];
+                    o->template_idx = t; o->sample_idx = j; o->snr = rho[j]; o->phase = atan2(cc[j], cp[j]);
+                }
+                ++total;
+            }
+        }
+        pk->snr_max = rho[jb]; pk->idx_peak = jb; pk->phase = atan2(cc[jb], cp[jb]); pk->sigma = sp;
+    }
+    free(rho); free(cp); free(cc);
+    if (n_trig_found) *n_trig_found = total;
+    if (rc) return rc;
+    return (total > written && trig_out) ? ORC_WTRUNC : ORC_OK;
 }
 
 /* Threads orc_filter_bank will use (for bench.py's cpu_baseline "cores"). */

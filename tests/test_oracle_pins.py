@@ -820,3 +820,194 @@ def test_p3b_chirp_time_with_the_25pn_term():
     c5 = np.pi * (38645 / 756 - 65 * eta / 9)
     assert abs((tau(5) - tau(4)) + 3 / (128 * eta) * c5 / (2 * np.pi * f)) < 1e-6
     assert -0.25 < tau(5) - tau(4) < -0.05
+
+
+# ------------------------------------------------------------------ NEXT-3, second part: the time-domain generator
+# (PAPER.md:173-179).  Pins of orc_td_phase / orc_td_extent / orc_td_template / orc_td_snr_series / orc_td_filter_bank.
+
+def _energy_balance_dvdt(M, eta, v, half_order):
+    """dv/dt = -Flux(v) / (M e'(v)) with the energy function and flux quoted in _taylorf2_from_energy_balance
+    (Blanchet, Living Rev. Relativity 9, 4 (2006), eqs. (194), (231)), the flux cut at the same order as the phase."""
+    pi = np.pi
+    a2, a4 = -(9 + eta) / 12.0, -(81 - 57 * eta + eta ** 2) / 24.0
+    eprime = -eta * v * (1 + 2 * a2 * v ** 2 + 3 * a4 * v ** 4)
+    series = (1 - (1247 / 336 + 35 * eta / 12) * v ** 2 + 4 * pi * v ** 3
+              + (-44711 / 9072 + 9271 * eta / 504 + 65 * eta ** 2 / 18) * v ** 4)
+    if half_order >= 5:
+        series -= (8191 / 672 + 583 * eta / 24) * pi * v ** 5
+    flux = 32 / 5 * eta ** 2 * v ** 10 * series
+    return -flux / (M * eprime)
+
+
+def _tau_at_v(m1, m2, v, order):
+    M = (m1 + m2) * 4.925490947641267e-6
+    target = v ** 3 / (np.pi * M)
+    lo, hi = 1e-6, 1e9                                   # F decreases with tau on the branch that sweeps upward
+    for _ in range(200):
+        mid = np.sqrt(lo * hi)
+        if oracle.td_phase(m1, m2, mid, order)[1] > target:
+            lo = mid
+        else:
+            hi = mid
+    return np.sqrt(lo * hi)
+
+
+@pytest.mark.parametrize("m1,m2", [(1.4, 1.4), (1.0, 3.0), (10.0, 1.2)])
+@pytest.mark.parametrize("order", [4, 5])
+def test_td_frequency_obeys_energy_balance(m1, m2, order):
+    """The explicit-in-time series is the inversion of t(v) from dE/dt = -Flux, so v(t) = (pi M F)^(1/3) of
+    orc_td_phase satisfies dv/dt = -Flux/(M e'(v)) up to the first neglected order: a relative residual c v^(n+1)
+    with c nearly constant (n = 4: 2PN, n = 5: 2.5PN).  A wrong coefficient at order m <= n leaves a residual
+    ~ v^m instead: the ratio residual / v^(n+1) would then change by (0.15/0.05)^(n+1-m) >= 3 over the range."""
+    M = (m1 + m2) * 4.925490947641267e-6
+    eta = m1 * m2 / (m1 + m2) ** 2
+    ratios = []
+    for v in (0.05, 0.07, 0.10, 0.15):
+        tau = _tau_at_v(m1, m2, v, order)
+        h = tau * 1e-5
+        v_hi = (np.pi * M * oracle.td_phase(m1, m2, tau - h, order)[1]) ** (1 / 3)
+        v_lo = (np.pi * M * oracle.td_phase(m1, m2, tau + h, order)[1]) ** (1 / 3)
+        dvdt = (v_hi - v_lo) / (2 * h)
+        want = _energy_balance_dvdt(M, eta, v, order)
+        ratios.append((dvdt - want) / want / v ** (order + 1))
+    ratios = np.array(ratios)
+    assert np.all(np.abs(ratios) < 250) and np.all(np.abs(ratios) > 20)
+    assert np.max(np.abs(ratios)) / np.min(np.abs(ratios)) < 1.35, ratios
+    assert np.all(np.sign(ratios) == np.sign(ratios[0]))
+
+
+@pytest.mark.parametrize("order", [4, 5])
+def test_td_frequency_is_the_phase_derivative(order):
+    """F = (1/2 pi) d phi_gw / dt = -(1/2 pi) d phi_gw / d tau; the phase grows with time; to leading order F is the
+    textbook Newtonian chirp F = (1/pi) (5/(256 tau))^(3/8) Mc^(-5/8), the corrections being of relative order v^2."""
+    m1, m2 = 1.4, 1.4
+    Mc = (m1 * m2) ** 0.6 / (m1 + m2) ** 0.2 * 4.925490947641267e-6
+    for tau in (30.0, 3.0, 0.3, 0.03):
+        h = tau * 1e-6
+        p_late, f = oracle.td_phase(m1, m2, tau - h, order)[0], oracle.td_phase(m1, m2, tau, order)[1]
+        p_early = oracle.td_phase(m1, m2, tau + h, order)[0]
+        assert p_late > p_early
+        assert (p_late - p_early) / (2 * h) / (2 * np.pi) == pytest.approx(f, rel=2e-6)
+        newton = (5.0 / (256.0 * tau)) ** 0.375 * Mc ** -0.625 / np.pi
+        assert f == pytest.approx(newton, rel=0.02 + 2.0 * (np.pi * (m1 + m2) * 4.925490947641267e-6 * f) ** (2 / 3))
+
+
+def test_td_extent_end_points():
+    """The template starts where F = f_low and ends at f_ISCO (2PN, comparable masses) or at the maximum of F where
+    the series stops sweeping upward first (2.5PN); 1.4 + 1.4 Msun from 40 Hz lasts 25 s (Newtonian chirp time 24.9 s
+    plus post-Newtonian corrections of a few per cent)."""
+    m1 = m2 = 1.4
+    ts, te, fe = oracle.td_extent(m1, m2, 40.0, 4)
+    assert oracle.td_phase(m1, m2, ts, 4)[1] == pytest.approx(40.0, rel=1e-12)
+    assert fe == pytest.approx(oracle.f_isco(m1, m2), rel=1e-12)
+    assert oracle.td_phase(m1, m2, te, 4)[1] == pytest.approx(fe, rel=1e-12)
+    Mc = (m1 * m2) ** 0.6 / (m1 + m2) ** 0.2 * 4.925490947641267e-6
+    t_newton = 5.0 / 256.0 * (np.pi * 40.0) ** (-8.0 / 3.0) * Mc ** (-5.0 / 3.0)
+    assert 24.5 < t_newton < 25.5 and ts == pytest.approx(t_newton, rel=0.06)
+    ts5, te5, fe5 = oracle.td_extent(m1, m2, 40.0, 5)
+    assert 300.0 < fe5 < oracle.f_isco(m1, m2)                    # stops early: F has a maximum there
+    for sgn in (-1, 1):
+        assert oracle.td_phase(m1, m2, te5 * (1 + sgn * 1e-3), 5)[1] < fe5 * (1 + 1e-12)
+    assert ts5 == pytest.approx(ts, rel=0.02) and ts5 != ts
+    # a system whose f_ISCO lies below the cut-off has no template
+    assert oracle.td_extent(60.0, 60.0, 40.0, 4)[:2] == (0.0, 0.0)
+
+
+def _td_case(n=1 << 15, fs=2048.0, f_low=40.0, order=4):
+    psd = W.onesided_psd("A", n, fs, f_low)
+    o = oracle.Oracle(n, fs, f_low)
+    o.set_pn_order(order)
+    o.set_psd(psd)
+    return o, psd
+
+
+def test_td_template_layout():
+    n, fs = 1 << 15, 2048.0
+    o, _ = _td_case(n, fs)
+    m1, m2 = 3.0, 2.5
+    ts, te, fe = oracle.td_extent(m1, m2, 40.0, 4)
+    hp, hc = o.td_template(m1, m2)
+    nz = np.nonzero(hp ** 2 + hc ** 2)[0]
+    assert nz[0] == n - int(np.floor(ts * fs)) and nz[-1] == n - int(np.ceil(te * fs))
+    amp = np.sqrt(hp ** 2 + hc ** 2)[nz]
+    assert amp[0] == pytest.approx(1.0, rel=1e-3)                  # (F / f_low)^(2/3) at F = f_low
+    assert np.all(np.diff(amp) > 0)                                # Newtonian amplitude grows with F
+    assert amp[-1] == pytest.approx((oracle.td_phase(m1, m2, (n - nz[-1]) / fs, 4)[1] / 40.0) ** (2 / 3), rel=1e-9)
+    assert 0.9 * (fe / 40.0) ** (2 / 3) < amp[-1] <= (fe / 40.0) ** (2 / 3)
+    # the instantaneous frequency read off the samples equals F
+    j = nz[len(nz) // 2]
+    dphi = np.angle((hp[j + 1] + 1j * hc[j + 1]) / (hp[j - 1] + 1j * hc[j - 1]))
+    assert dphi * fs / (4 * np.pi) == pytest.approx(oracle.td_phase(m1, m2, (n - j) / fs, 4)[1], rel=1e-4)
+    # too long for the segment
+    with pytest.raises(oracle.OracleError):
+        oracle.Oracle(1 << 12, fs, 40.0).td_template(1.0, 1.0)
+
+
+@pytest.mark.parametrize("order", [4, 5])
+def test_td_noise_free_injection_closed_forms(order):
+    """Data = A h_+ of the same template, shifted circularly by t0: c_+(t0) = A sigma_+, c_x(t0) = A (h_+|h_x)/sigma_x
+    with the two polarisations in quadrature, so rho_max = A sigma_+ at sample t0 with phase 0; injecting h_x gives
+    phase pi/2; sigma_+ = sigma_x to the accuracy of the quadrature."""
+    n, fs = 1 << 15, 2048.0
+    o, psd = _td_case(n, fs, order=order)
+    m1, m2 = 3.0, 2.5
+    hp, hc = o.td_template(m1, m2)
+    t0, A = 9000, 0.37
+    for h, want_phase in ((hp, 0.0), (hc, np.pi / 2)):
+        o.load_segment(np.roll(A * h, t0).astype(np.float32))
+        rho, cp, cc, sp, sc = o.td_snr_series(m1, m2)
+        assert int(np.argmax(rho)) == t0
+        assert sp == pytest.approx(sc, rel=2e-3)
+        assert rho[t0] == pytest.approx(A * (sp if h is hp else sc), rel=2e-4)
+        assert np.arctan2(cc[t0], cp[t0]) == pytest.approx(want_phase, abs=2e-2)
+    # the definition of sigma_+ by hand: 4 df sum |H_+|^2 / S_n with numpy's FFT
+    H = np.fft.rfft(hp) / fs
+    klo = int(np.ceil(40.0 * n / fs))
+    k = np.arange(klo, n // 2)
+    assert sp == pytest.approx(np.sqrt(4 * fs / n * np.sum(np.abs(H[k]) ** 2 / psd[k])), rel=1e-10)
+    # and the correlator at one lag by a direct time-frequency sum
+    D = np.fft.rfft(np.roll(A * hc, t0).astype(np.float32).astype(np.float64)) / fs
+    j = t0 - 3
+    cdir = 4 * fs / n * np.real(np.sum(D[k] * np.conj(H[k]) / psd[k] * np.exp(2j * np.pi * j * k / n))) / sp
+    assert cp[j] == pytest.approx(cdir, rel=1e-8, abs=1e-10)
+
+
+def test_td_filter_agrees_with_the_spa_filter():
+    """The same binary in the two domains: a noise-free time-domain injection filtered with the stationary-phase
+    template of the same masses (orc_snr_series) peaks at the injected coalescence sample (within the few samples by
+    which the two approximants' end points differ) and recovers most of its SNR -- pins the placement of t_c, the sign
+    of the phase and the sweep direction of the time-domain generator against the independently pinned SPA one."""
+    n, fs = 1 << 16, 2048.0
+    o, psd = _td_case(n, fs, order=4)
+    m1 = m2 = 1.4
+    hp, hc = o.td_template(m1, m2)
+    t0 = 40960
+    o.load_segment(np.roll(hp, t0).astype(np.float32))
+    rho_td, *_ , sp, sc = o.td_snr_series(m1, m2)
+    rho, z, sigma = o.snr_series(m1, m2)
+    assert abs(int(np.argmax(rho)) - t0) <= 3
+    assert rho.max() > 0.95 * rho_td.max()
+    # a time-REVERSED chirp (sweeping down) is not found
+    o.load_segment(np.roll(hp[::-1], t0).astype(np.float32))
+    assert o.snr_series(m1, m2)[0].max() < 0.2 * rho_td.max()
+
+
+def test_td_noise_statistics_and_bank():
+    w = W.small_case(log2n=15, fs=2048.0, f_low=40.0, n_templates=3, seed=11)
+    o = _oracle_for(w)
+    bank = np.array([[2.4, 2.2], [3.0, 2.9], [80.0, 70.0]])
+    rhos = [o.td_snr_series(m1, m2) for m1, m2 in bank[:2]]
+    for rho, cp, cc, sp, sc in rhos:
+        assert np.mean(cp ** 2) == pytest.approx(1.0, rel=0.15) and np.mean(cc ** 2) == pytest.approx(1.0, rel=0.15)
+    pk, tr, nf, rc = o.td_filter_bank(bank, 2.5)
+    assert rc == 0 and pk[2]["idx_peak"] == -1 and pk[2]["snr_max"] == 0.0          # f_ISCO < f_low
+    want = []
+    for t, (rho, cp, cc, sp, sc) in enumerate(rhos):
+        j = int(np.argmax(rho))
+        assert pk[t]["idx_peak"] == j and pk[t]["snr_max"] == rho[j] and pk[t]["sigma"] == sp
+        assert pk[t]["phase"] == pytest.approx(np.arctan2(cc[j], cp[j]), abs=1e-12)
+        want += [(t, int(jj)) for jj in np.nonzero(rho > 2.5)[0]]
+    assert nf == len(want) > 0
+    assert [(int(a), int(b)) for a, b in zip(tr["template_idx"], tr["sample_idx"])] == want
+    pk2, tr2, nf2, rc2 = o.td_filter_bank(bank, 2.5, trig_capacity=5)
+    assert rc2 == oracle.WTRUNC and nf2 == nf and len(tr2) == 5 and np.array_equal(tr2, tr[:5])
