@@ -221,10 +221,35 @@ int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
  * Buonanno et al., Phys. Rev. D 80, 084043 (2009), eq. 3.18):
  *     Psi += 3/(128 eta v^5) * pi (38645/756 - 65 eta/9) (1 + 3 ln(v / v_lso)) v^5,   v_lso = 6^{-1/2}.
  * Applies to every later call (filter, stream, chisq, debug); amplitude, band and sigma do not change, so PSD and
- * segment stay loaded.  EINVAL for any other value.  (The paper's own variant -- time-domain generation, forward
- * FFT and normalisation by a reduction -- is not built: DESIGN.md §10.) */
+ * segment stay loaded.  EINVAL for any other value. */
 int cbmf_set_pn_order(cbmf_ctx *ctx, int half_order);
 int cbmf_get_pn_order(const cbmf_ctx *ctx);
+
+/* ---- the paper's own template path (second part) ----
+ * "the two polarization of the template signal are generated, FFT transformed and normalized ... with a complex
+ * product and reduction algorithms", then the two correlators and the quadrature sum
+ * (PAPER.md:99-101, :127-131).  The paper prints no waveform; reading A28: the time-domain chirp with
+ * an explicit phase, every sample an independent evaluation ("TaylorT3": Blanchet, Living Rev. Relativity 9, 4 (2006),
+ * eq. (234)), phase order as cbmf_set_pn_order says, amplitude at Newtonian order:  with tau = t_c - t,
+ * Theta = eta tau / (5 M), x = Theta^{1/8},
+ *     phi_gw = -(2/eta) [x^5 + a2 x^3 - (3 pi/4) x^2 + a4 x + a5 ln Theta],   F = (1/2 pi) d phi_gw / dt,
+ *     a2 = 3715/8064 + 55 eta/96,  a4 = 9275495/14450688 + 284875 eta/258048 + 1855 eta^2/2048,
+ *     a5 = (-38645/172032 + 65 eta/2048) pi  (2.5PN only),
+ *     h_+ = (F/f_low)^{2/3} cos phi_gw,  h_x = (F/f_low)^{2/3} sin phi_gw,
+ * from F = f_low up to F = f_ISCO, or to the maximum of F where the series stops sweeping upward first; the
+ * coalescence sits at sample 0 (= n: the segment is a circle).  Per polarisation p: H_p = forward transform,
+ * sigma_p^2 = 4 df sum_k |H_p[k]|^2 / S_n[k], c_p[j] = 4 df Re sum_k d~[k] H_p*[k] / S_n[k] e^{+2 pi i jk/n}, both over
+ * k_lo <= k < n/2, and rho[j] = sqrt((c_+/sigma_+)^2 + (c_x/sigma_x)^2).
+ * Arguments, results, truncation and errors as cbmf_filter_bank (host pointers); phase = atan2(c_x/sigma_x,
+ * c_+/sigma_+) at the peak, sigma = sigma_+.  Additional EINVAL: a template longer than the segment
+ * (cbmf_last_bad_template names it).  A template whose f_ISCO lies below f_low is empty: {0, -1, 0, 0}.
+ * This is the comparison path (generation + two transforms + a reduction per template, every intermediate in device
+ * memory, as in the paper); the tuned path is cbmf_filter_bank. */
+int cbmf_filter_bank_td(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_templates,
+                        float snr_threshold, cbmf_peak *peaks_out,
+                        cbmf_trigger *trig_out, int64_t trig_capacity, int64_t *n_trig_found);
+/* Diagnostic: the two polarisations of one template on the sample grid, (h_+[j], h_x[j]) interleaved, 2n floats. */
+int cbmf_debug_td_template(cbmf_ctx *ctx, cbmf_template t, float *h_out);
 
 /* ---- tuning ---- */
 /* Templates per launch pair (pass 1 + pass 2).  Default: 512 MiB of inter-pass buffer

@@ -51,6 +51,8 @@ def lib() -> C.CDLL:
         "cbmf_filter_bank_clustered": (C.c_int, [vp, vp, i64, flt, i64, vp, vp, i64, C.POINTER(i64), C.POINTER(i64)]),
         "cbmf_filter_stream": (C.c_int, [vp, vp, i64, vp, i64, flt, i64, vp, vp, i64, vp, C.POINTER(i64), C.POINTER(i64)]),
         "cbmf_chisq": (C.c_int, [vp, vp, i64, vp, C.c_int, vp, vp]),
+        "cbmf_filter_bank_td": (C.c_int, [vp, vp, i64, flt, vp, vp, i64, C.POINTER(i64)]),
+        "cbmf_debug_td_template": (C.c_int, [vp, Template, vp]),
         "cbmf_debug_snr_series": (C.c_int, [vp, Template, vp, vp]),
         "cbmf_debug_template": (C.c_int, [vp, Template, vp]),
         "cbmf_debug_ifft": (C.c_int, [vp, vp, vp, i64, i64]),
@@ -83,7 +85,7 @@ def lib() -> C.CDLL:
 
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_cluster_triggers "
-           "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_chisq cbmf_debug_snr_series "
+           "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_chisq cbmf_filter_bank_td cbmf_debug_td_template cbmf_debug_snr_series "
            "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
            "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_pn_order cbmf_get_pn_order cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
@@ -210,6 +212,20 @@ class Context:
         self._check(rc, "cbmf_filter_bank")
         return peaks, trig[:min(nf.value, int(trig_capacity))], nf.value, rc
 
+    def filter_bank_td(self, bank, snr_threshold: float, trig_capacity: int = 1 << 16):
+        """cbmf_filter_bank_td (the paper's own path: time-domain templates, two polarisations): same results layout
+        as filter_bank.  -> (peaks[PEAK_DTYPE], triggers[TRIG_DTYPE], n_found, rc)."""
+        b = np.ascontiguousarray(bank, dtype=np.float64).reshape(-1, 2)
+        nt = b.shape[0]
+        peaks = np.zeros(nt, dtype=PEAK_DTYPE)
+        trig = np.zeros(max(int(trig_capacity), 1), dtype=TRIG_DTYPE)
+        nf = C.c_int64(0)
+        rc = lib().cbmf_filter_bank_td(self._h, b.ctypes.data if nt else None, nt, float(snr_threshold),
+                                       peaks.ctypes.data if nt else None,
+                                       trig.ctypes.data if trig_capacity else None, int(trig_capacity), C.byref(nf))
+        self._check(rc, "cbmf_filter_bank_td")
+        return peaks, trig[:min(nf.value, int(trig_capacity))], nf.value, rc
+
     def filter_bank_into(self, bank, snr_threshold: float, peaks_out, trig_out, trig_capacity: int):
         """Caller-owned buffers (all host -- numpy / pinned tensors -- or all CUDA tensors):
         bank float64 [B,2], peaks_out 16 B/template, trig_out 16 B/entry.  -> (n_found, rc)."""
@@ -306,6 +322,12 @@ class Context:
                                          z.ctypes.data if want_z else None)
         self._check(rc, "cbmf_debug_snr_series")
         return snr, z
+
+    def debug_td_template(self, m1: float, m2: float):
+        """-> (h_plus[n], h_cross[n]) float32: the time-domain polarisations of cbmf_filter_bank_td."""
+        h = np.empty((self.n, 2), dtype=np.float32)
+        self._check(lib().cbmf_debug_td_template(self._h, Template(m1, m2), h.ctypes.data), "cbmf_debug_td_template")
+        return h[:, 0].copy(), h[:, 1].copy()
 
     def debug_template(self, m1: float, m2: float) -> np.ndarray:
         h = np.empty(self.n // 2 + 1, dtype=np.complex64)

@@ -6,6 +6,7 @@
 // of kernels.cuh.  There is no CPU fallback and nothing here touches oracle/.
 #include "../../include/cbmf.h"
 #include "kernels.cuh"
+#include "td.cuh"
 #include "cluster.h"
 
 #include <cmath>
@@ -87,6 +88,14 @@ struct cbmf_ctx {
     TrigOut* h_ptrig = nullptr;            // pinned [PIPE_RING][PAIR_TRIG_CAP]
     unsigned long long* h_pcursor = nullptr;   // pinned [PIPE_RING]
     cudaEvent_t ev_pipe[32] = {};
+
+    // time-domain template path (cbmf_filter_bank_td)
+    TdCoef* d_td = nullptr;        int64_t td_cap = 0;
+    double* d_tdnorm = nullptr;    int64_t tdnorm_cap = 0;      // [n][2]
+    float2* d_tdinv = nullptr;     int64_t tdinv_cap = 0;       // [n] 1/sigma_+, 1/sigma_x
+    float* d_winv = nullptr;       // [N/2] 4 df / S_n
+    c2* d_wd = nullptr;            // [N/2] 4 df d~ / S_n
+    c2* d_tdU = nullptr;           int64_t tdU_cap = 0;         // [templates per step][N]
 
     int64_t launches = 0;
     int profiling = 0;                     // 0 off, 1 every launch alone on the context's stream, 2 in the real schedule
@@ -331,6 +340,7 @@ extern "C" int cbmf_destroy(cbmf_ctx* c)
     if (c->seg_stream) { cudaStreamSynchronize(c->seg_stream); cudaStreamDestroy(c->seg_stream); }
     for (cudaEvent_t e : c->ev_seg_ready) if (e) cudaEventDestroy(e);
     cudaFree(c->d_ptrig); cudaFree(c->d_pcursor); cudaFreeHost(c->h_ptrig); cudaFreeHost(c->h_pcursor);
+    cudaFree(c->d_td); cudaFree(c->d_tdnorm); cudaFree(c->d_tdinv); cudaFree(c->d_winv); cudaFree(c->d_wd); cudaFree(c->d_tdU);
     for (cudaEvent_t e : c->ev_pipe) if (e) cudaEventDestroy(e);
     for (int w = 0; w < 2; ++w) for (cudaEvent_t e : c->ev[w]) cudaEventDestroy(e);
     for (int i = 0; i < CBMF_MAX_STREAMS; ++i) {
@@ -1153,6 +1163,158 @@ extern "C" int cbmf_chisq(cbmf_ctx* c, const cbmf_template* bank, int64_t nt, co
     if (zl_out) CU(cudaMemcpyAsync(zl_out, d_zl, b_zl, cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return CBMF_OK;
+}
+
+// ======================================================================= NEXT-3, second part: time-domain templates
+// The paper's own template path (td.cuh): per step of up to TD_STEP templates
+//   generate -> forward FFT (one complex transform for both polarisations) -> normalisation sums -> two-sided product
+//   -> inverse FFT -> the arg-max / threshold epilogue of the SPA path on rho^2 = |c_+/sigma_+ + i c_x/sigma_x|^2,
+// everything on the context's stream.  It is the comparison path, not the tuned one: ~100 bytes of HBM traffic per
+// sample and template against 16 for the SPA path.
+namespace {
+constexpr int TD_STEP = 16;
+
+int td_alloc(cbmf_ctx* c, int64_t nt, int step)
+{
+    int rc;
+    if ((rc = grow(c, c->d_td, c->td_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_tdnorm, c->tdnorm_cap, 2 * nt))) return rc;
+    if ((rc = grow(c, c->d_tdinv, c->tdinv_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_tdU, c->tdU_cap, (int64_t)step * c->n))) return rc;
+    const size_t nh = (size_t)c->n / 2;
+    if (!c->d_winv) CU(cudaMalloc(&c->d_winv, sizeof(float) * nh));
+    if (!c->d_wd) CU(cudaMalloc(&c->d_wd, sizeof(c2) * nh));
+    return CBMF_OK;
+}
+
+int td_setup(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr)
+{
+    TdSetupArgs sa;
+    sa.bank = bank_dev; sa.td = c->d_td; sa.coef = c->d_coef; sa.norm = c->d_tdnorm; sa.tcount = c->d_tcount;
+    sa.n_templates = (int)nt; sa.n_half = (int)(c->n / 2); sa.k_lo = c->k_lo; sa.pn_half_order = c->pn_half_order;
+    sa.f_low = c->f_low; sa.seg_seconds = (double)c->n * c->dt; sa.threshold = thr;
+    sa.err_flag = c->d_err; sa.bad_idx = c->d_bad;
+    td_setup_kernel<<<(unsigned)((nt + 63) / 64), 64, 0, c->stream>>>(sa);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    return CBMF_OK;
+}
+
+// One pass over the bank into c->d_peaks / c->d_trig (dev_cap entries); the total count stays in c->d_cursor.
+int td_run(cbmf_ctx* c, int64_t nt, int step, int64_t dev_cap)
+{
+    const int n = (int)c->n, nh = n / 2;
+    const size_t ncand = cand_per_template(c);
+    int gx = (nh + 255) / 256; if (gx > 1184) gx = 1184;
+    for (int64_t t0 = 0; t0 < nt; t0 += step) {
+        const int nb = (int)((nt - t0 < step) ? (nt - t0) : step);
+        td_generate_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)nb), 256, 0, c->stream>>>(c->d_td + t0, c->d_tdU, n, c->dt, -1.0f);
+        CU(cudaGetLastError());
+        P1Args a1; memset(&a1, 0, sizeof(a1));
+        a1.in_c = c->d_tdU; a1.Y = c->d_Y; a1.err_flag = c->d_err;
+        CU(launch_p1<LOAD_CPLX>(c, c->stream, a1, nb));
+        P2Args a2; memset(&a2, 0, sizeof(a2));
+        a2.Y = c->d_Y; a2.z_out = c->d_tdU;
+        CU(launch_p2<EPI_STORE>(c, c->stream, a2, nb));
+        td_norm_kernel<<<dim3(64, (unsigned)nb), 256, 0, c->stream>>>(c->d_tdU, c->d_winv, c->d_tdnorm + 2 * t0, n, c->k_lo, (float)c->dt);
+        CU(cudaGetLastError());
+        td_norm_finish_kernel<<<1, 64, 0, c->stream>>>(c->d_tdnorm + 2 * t0, c->d_coef + t0, c->d_tdinv + t0, nb);
+        CU(cudaGetLastError());
+        td_product_kernel<<<dim3((unsigned)gx, (unsigned)nb), 256, 0, c->stream>>>(c->d_tdU, c->d_wd, c->d_tdinv + t0, n, c->k_lo, (float)c->dt);
+        CU(cudaGetLastError());
+        CU(launch_p1<LOAD_CPLX>(c, c->stream, a1, nb));
+        P2Args a3; memset(&a3, 0, sizeof(a3));
+        a3.Y = c->d_Y; a3.coef = c->d_coef + t0; a3.cand = c->d_cand; a3.best_key = c->d_key; a3.done_ctr = c->d_done;
+        a3.peaks = c->d_peaks + t0; a3.trig = c->d_trig; a3.trig_cursor = c->d_cursor; a3.trig_cap = (unsigned long long)dev_cap;
+        a3.trig_count = c->d_tcount + t0; a3.tmpl_base = (int)t0; a3.j_min = 0; a3.bad = c->d_bad;
+        (void)ncand;
+        CU(launch_p2<EPI_MAX>(c, c->stream, a3, nb));
+        c->launches += 8;
+    }
+    return CBMF_OK;
+}
+}  // namespace
+
+extern "C" int cbmf_filter_bank_td(cbmf_ctx* c, const cbmf_template* bank, int64_t nt, float thr,
+                                   cbmf_peak* peaks_out, cbmf_trigger* trig_out, int64_t trig_capacity,
+                                   int64_t* n_trig_found)
+{
+    int rc = filter_args_ok(c, bank, nt, thr, peaks_out, trig_out, trig_capacity);
+    if (rc) return rc;
+    if (n_trig_found) *n_trig_found = 0;
+    c->last_bad = -1;
+    if (nt == 0) return CBMF_OK;
+    DeviceGuard g(c->device);
+    if ((rc = check_pending(c))) return rc;
+    const int step = c->sub_batch < TD_STEP ? c->sub_batch : TD_STEP;
+    if ((rc = grow(c, c->d_bank, c->bank_cap, 2 * nt))) return rc;
+    if ((rc = grow(c, c->d_coef, c->coef_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_peaks, c->peaks_cap, nt))) return rc;
+    if ((rc = grow(c, c->d_tcount, c->tcount_cap, nt))) return rc;
+    if ((rc = td_alloc(c, nt, step))) return rc;
+    int64_t tcap = 1;
+    while (tcap < trig_capacity) tcap <<= 1;
+    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
+    CU(cudaMemcpyAsync(c->d_bank, bank, sizeof(cbmf_template) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
+    const int nh = (int)(c->n / 2);
+    td_tables_kernel<<<(unsigned)((nh + 255) / 256), 256, 0, c->stream>>>(c->d_wfac, c->d_w, c->d_winv, c->d_wd, nh, c->k_lo, c->df, c->dt);
+    CU(cudaGetLastError());
+    c->launches += 1;
+    int64_t found = 0;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        unsigned long long status[2] = {0ULL, (unsigned long long)NO_BAD_TEMPLATE};
+        CU(cudaMemcpyAsync(c->d_cursor, status, sizeof(status), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+        if ((rc = td_setup(c, c->d_bank, nt, thr))) return rc;
+        CU(cudaMemcpyAsync(status, c->d_cursor, sizeof(status), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        if ((long long)status[1] != NO_BAD_TEMPLATE) { c->last_bad = (int64_t)status[1]; return CBMF_EINVAL; }
+        if ((rc = td_run(c, nt, step, c->trig_cap))) return rc;
+        CU(cudaMemcpyAsync(status, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        found = (int64_t)status[0];
+        if (found <= c->trig_cap || !trig_out || trig_capacity == 0) break;
+        // the device list is incomplete: once more with room for all of them (the kept ones are the FIRST in order)
+        int64_t need = 1;
+        while (need < found) need <<= 1;
+        if ((rc = grow(c, c->d_trig, c->trig_cap, need))) return rc;
+    }
+    if (n_trig_found) *n_trig_found = found;
+    const int64_t kept = found < trig_capacity ? found : trig_capacity;
+    if (kept > 0 && trig_out) {
+        if ((rc = sort_triggers(c, found))) return rc;
+        CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
+}
+
+extern "C" int cbmf_debug_td_template(cbmf_ctx* c, cbmf_template t, float* h_out)
+{
+    if (!c || !h_out) return CBMF_EINVAL;
+    DeviceGuard g(c->device);
+    int rc;
+    if ((rc = grow(c, c->d_bank, c->bank_cap, 2))) return rc;
+    if ((rc = grow(c, c->d_coef, c->coef_cap, 1))) return rc;
+    if ((rc = grow(c, c->d_tcount, c->tcount_cap, 1))) return rc;
+    if ((rc = td_alloc(c, 1, 1))) return rc;
+    const size_t n = (size_t)c->n;
+    if ((rc = grow_scratch(c, sizeof(float2) * n))) return rc;
+    unsigned long long status[2] = {0ULL, (unsigned long long)NO_BAD_TEMPLATE};
+    CU(cudaMemcpyAsync(c->d_cursor, status, sizeof(status), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream));
+    CU(cudaMemcpyAsync(c->d_bank, &t, sizeof(t), cudaMemcpyHostToDevice, c->stream));
+    if ((rc = td_setup(c, c->d_bank, 1, 0.f))) return rc;
+    td_generate_kernel<<<dim3((unsigned)((n + 255) / 256), 1), 256, 0, c->stream>>>(c->d_td, c->d_tdU, (int)n, c->dt, 1.0f);
+    CU(cudaGetLastError());
+    td_copy_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->d_tdU, (float2*)c->d_scratch, (int)n);
+    CU(cudaGetLastError());
+    c->launches += 2;
+    CU(cudaMemcpyAsync(status, c->d_cursor, sizeof(status), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(h_out, c->d_scratch, sizeof(float2) * n, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return ((long long)status[1] != NO_BAD_TEMPLATE) ? CBMF_EINVAL : CBMF_OK;
 }
 
 // ======================================================================= diagnostics
