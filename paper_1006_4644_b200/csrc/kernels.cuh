@@ -56,8 +56,8 @@ CBMF_CFG(128, 16, 16, 8, 1, 256)
 CBMF_CFG(256, 16, 16, 16, 1, 256)
 CBMF_CFG(512, 32, 32, 16, 1, 256)
 CBMF_CFG(1024, 32, 32, 32, 1, 256)
-CBMF_CFG(2048, 16, 16, 16, 8, 512)
-CBMF_CFG(4096, 16, 16, 16, 16, 1024)
+CBMF_CFG(2048, 32, 32, 32, 2, 512)
+CBMF_CFG(4096, 32, 32, 32, 4, 512)
 #undef CBMF_CFG
 
 __host__ __device__ constexpr int ilog2c(int x) { return x <= 1 ? 0 : 1 + ilog2c(x >> 1); }
