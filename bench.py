@@ -365,6 +365,21 @@ def measure(torch, dist, cbmf, wl, dev, local, world, K, Wm, cap, args, with_e2e
             barrier()
             out["c_ms_max"] = max_over_ranks(c_ms)
             out["n_events"] = int(n_ev)
+            # the paper's own template path (NEXT-3: time-domain generation, forward FFT, normalisation by a
+            # reduction, product, inverse FFT -- every intermediate in device memory) on a bounded sample
+            if args.workload == "cfg1" and world == 1:
+                n_td = min(B, 128)
+                bank_td = np.ascontiguousarray(wl.bank[:n_td])
+                ctx.load_segment(smp_h)
+                ctx.filter_bank_td(bank_td, wl.threshold)                      # warm-up (allocations)
+                a_ev, b_ev = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a_ev.record(stream)
+                for _ in range(3):
+                    ctx.filter_bank_td(bank_td, wl.threshold)
+                b_ev.record(stream)
+                stream.synchronize()
+                out["td_us_per_template"] = 1e3 * a_ev.elapsed_time(b_ev) / (3 * n_td)
+                out["td_templates"] = n_td
             out["h2d"] = psd_h.numel() * 8 + smp_h.numel() * 4 + bank_h.numel() * 8
             # peaks, kept triggers, the early template-status word (8 B) and the trigger count (8 B)
             out["d2h"] = B * 16 + min(nf_h, cap) * 16 + 4 + 4 + 8 + 8
@@ -508,10 +523,10 @@ def run_ours(args):
         "flops_per_launch": flops_launch, "avg_launch_ms": avg_launch_ms, "templates_per_launch": tmpl_per_launch,
         "pass_ms_per_step": [p_ms[0] / K, p_ms[1] / K],
         "pass_launch_ms_overlapped": [o_ms[0] / max(o_n[0], 1), o_ms[1] / max(o_n[1], 1)],
-        "note": ("`achieved` and pass_ms_per_step are taken with every launch ALONE on the GPU (one stream); pass 1 is launched "
-                 "with few long-lived blocks so that pass-2 blocks of the other launch pairs share its SMs in the timed "
-                 "schedule, where the passes overlap (pass_launch_ms_overlapped: mean duration of a launch in that schedule, "
-                 "events on its own stream); whole_path gives the fraction of the FP32 peak reached by the whole step"),
+        "note": ("`achieved` and pass_ms_per_step are taken with every launch ALONE on the GPU (one stream); in the timed "
+                 "schedule four launch pairs are in flight and the long-lived pass-1 blocks share the SMs with pass-2 blocks "
+                 "of the other pairs, so the passes overlap (pass_launch_ms_overlapped: mean duration of a launch in that "
+                 "schedule, events on its own stream); whole_path gives the fraction of the FP32 peak reached by the whole step"),
         "whole_path": {
             "flops_per_template": f1 + f2, "us_per_template": 1e3 * ms_max / (B * K),
             "achieved_tflops": (f1 + f2) * B * K / (ms_max * 1e-3) / 1e12,
@@ -549,6 +564,13 @@ def run_ours(args):
                           "window_samples": args.cluster_window,
                           "what": "cbmf_filter_bank_clustered: raw triggers reduced to events on the host while the GPU "
                                   "filters the next sub-batches (NEXT-1, PAPER.md:103, :131)"},
+        "paper_path": None if "td_us_per_template" not in m else {
+            "us_per_template": m["td_us_per_template"], "value": 1e6 / m["td_us_per_template"], "unit": UNIT,
+            "templates": m["td_templates"],
+            "what": "cbmf_filter_bank_td: the paper's own per-template pipeline on the same GPU (time-domain generation of two "
+                    "polarisations, forward FFT, normalisation by a reduction, product, inverse FFT, every intermediate in "
+                    "device memory: PAPER.md:127-131, :177-179; 28 ms per template on the paper's GTX 275, PAPER.md:231) -- "
+                    "the comparison path, not the product's"},
         "gpu_launches": int(m["launches"]),
         "clocks": m["clocks"],
         "roofline": roofline,

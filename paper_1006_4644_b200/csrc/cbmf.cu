@@ -27,6 +27,7 @@ struct cbmf_ctx {
     cudaStream_t stream = nullptr;
     int64_t n = 0;
     int log2n = 0, lg1 = 0, lg2 = 0;      // N = N1 * N2, N1 = 2^lg1 (pass 1), N2 = 2^lg2 (pass 2)
+    int ifft_lg1 = 0, ifft_lg2 = 0;       // the split of the stand-alone transform (cbmf_debug_ifft)
     double fs = 0, f_low = 0, df = 0, dt = 0;
     int k_lo = 0;
     bool have_psd = false, have_seg = false;
@@ -249,6 +250,20 @@ cudaError_t launch_p2(cbmf_ctx* c, cudaStream_t s, const P2Args& a, int batch)
     CBMF_DISPATCH(c->lg1, c->lg2, (launch_p2_L<L1, L2, MODE, MASK>(c, s, a, batch)))
 }
 
+// The stand-alone transform (plain load and store epilogues only) with its own split.
+cudaError_t launch_p1_ifft(cbmf_ctx* c, cudaStream_t s, const P1Args& a, int batch)
+{
+    if (c->ifft_lg1 == 10 && c->ifft_lg2 == 11) return launch_p1_L<1024, 2048, LOAD_CPLX>(c, s, a, batch);
+    if (c->ifft_lg1 == 11 && c->ifft_lg2 == 11) return launch_p1_L<2048, 2048, LOAD_CPLX>(c, s, a, batch);
+    return launch_p1<LOAD_CPLX>(c, s, a, batch);
+}
+cudaError_t launch_p2_ifft(cbmf_ctx* c, cudaStream_t s, const P2Args& a, int batch)
+{
+    if (c->ifft_lg1 == 10 && c->ifft_lg2 == 11) return launch_p2_L<1024, 2048, EPI_STORE>(c, s, a, batch);
+    if (c->ifft_lg1 == 11 && c->ifft_lg2 == 11) return launch_p2_L<2048, 2048, EPI_STORE>(c, s, a, batch);
+    return launch_p2<EPI_STORE>(c, s, a, batch);
+}
+
 // candidate slots per template of the arg-max pass: one per (row j1, thread of the row group) = N / E2
 template <int L1, int L2> constexpr int cand_count() { return L1 * Cfg<L2>::T; }
 size_t cand_per_template(const cbmf_ctx* c)
@@ -377,6 +392,11 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     // ... except at N = 2^21 and 2^22, where pass 2 keeps its best shape (rows of 1024 points, one warp per row,
     // one exchange) and pass 1 takes the 2048- / 4096-point columns: 22 % / 34 % faster than 1024 x 2048 / 2048 x 2048
     if (c->log2n == 21 || c->log2n == 22) { c->lg2 = 10; c->lg1 = c->log2n - 10; }
+    // the stand-alone transform (cbmf_debug_ifft: all N inputs non-zero, plain store epilogue) prefers the shorter
+    // column FFT at these sizes: 1024 x 2048 and 2048 x 2048 run at 0.97-0.99 of the library transform, against 0.75
+    c->ifft_lg1 = c->lg1; c->ifft_lg2 = c->lg2;
+    if (c->log2n == 21) { c->ifft_lg1 = 10; c->ifft_lg2 = 11; }
+    if (c->log2n == 22) { c->ifft_lg1 = 11; c->ifft_lg2 = 11; }
     c->fs = fs_hz; c->f_low = f_low_hz;
     c->df = fs_hz / (double)n; c->dt = 1.0 / fs_hz;
     c->k_lo = (int)std::ceil(f_low_hz * ((double)n / fs_hz));       // reading A7: inclusive, in double
@@ -1405,10 +1425,10 @@ extern "C" int cbmf_debug_ifft_dev(cbmf_ctx* c, const float* in_dev, float* out_
         const int nb = (int)((batch - b0 < sb) ? (batch - b0) : sb);
         P1Args a1; memset(&a1, 0, sizeof(a1));
         a1.in_c = (const c2*)in_dev + (size_t)b0 * n; a1.Y = c->d_Y; a1.err_flag = c->d_err;
-        CU(launch_p1<LOAD_CPLX>(c, c->stream, a1, nb));
+        CU(launch_p1_ifft(c, c->stream, a1, nb));
         P2Args a2; memset(&a2, 0, sizeof(a2));
         a2.Y = c->d_Y; a2.z_out = (c2*)out_dev + (size_t)b0 * n;
-        CU(launch_p2<EPI_STORE>(c, c->stream, a2, nb));
+        CU(launch_p2_ifft(c, c->stream, a2, nb));
         c->launches += 2;
     }
     CU(cudaStreamSynchronize(c->stream));

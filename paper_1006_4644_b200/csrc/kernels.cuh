@@ -1128,7 +1128,9 @@ __global__ void __launch_bounds__(Cfg<L2>::NT2, 512 / Cfg<L2>::NT2) p2_kernel(co
     if constexpr (MODE == EPI_MAX) {
         if (a.bad != nullptr && __ldg(a.bad) != NO_BAD_TEMPLATE) return;               // uniform over the grid
     }
-    p2_item<L1, L2, MODE, MASK>(a, blockIdx.x, blockIdx.y, smem);
+    // templates in reverse order: pass 1 wrote the last ones most recently, so part of their Y is still in the L2
+    // when this launch starts (4 % fewer DRAM reads of a launch timed alone)
+    p2_item<L1, L2, MODE, MASK>(a, blockIdx.x, gridDim.y - 1 - blockIdx.y, smem);
 }
 
 // ------------------------------------------------------------------ S0: PSD tables (fp64)
