@@ -252,8 +252,9 @@ int cbmf_filter_bank_td(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_temp
 int cbmf_debug_td_template(cbmf_ctx *ctx, cbmf_template t, float *h_out);
 
 /* ---- tuning ---- */
-/* Templates per launch pair (pass 1 + pass 2).  Default: 512 MiB of inter-pass buffer
- * (8 n bytes per template) per pair, i.e. 64 templates at n = 2^20; results do not depend on it.
+/* Templates per launch pair (pass 1 + pass 2), an upper limit: a call over a small bank uses fewer, so that every
+ * launch pair in flight has work.  Default: 2 GiB of inter-pass buffer (8 n bytes per template) per pair, at most
+ * 256 templates (256 at n <= 2^20, 64 at 2^22, 16 at 2^24); results do not depend on it.
  * 1 <= templates_per_launch <= 4096; ENOMEM if the larger buffer cannot be allocated. */
 int cbmf_set_sub_batch(cbmf_ctx *ctx, int templates_per_launch);
 int cbmf_get_sub_batch(const cbmf_ctx *ctx);

@@ -402,9 +402,11 @@ extern "C" int cbmf_create(cbmf_ctx** out, int device, int64_t n, double fs_hz, 
     c->k_lo = (int)std::ceil(f_low_hz * ((double)n / fs_hz));       // reading A7: inclusive, in double
     if (c->k_lo < 1) c->k_lo = 1;
 
-    // templates per launch pair: 512 MiB of inter-pass buffer per pair (64 templates at N = 2^20).  Measured
-    // (DESIGN.md §7): larger grids matter more than keeping Y inside the L2 at the present kernel speed.
-    int64_t sb = (int64_t(512) << 20) / (8 * n);
+    // templates per launch pair: up to 2 GiB of inter-pass buffer per pair (256 templates at N = 2^20).  Measured
+    // (DESIGN.md §7): long launches matter more than keeping Y inside the L2 at the present kernel speed
+    // (cfg2: 282 k templates/s at 64 per pair, 286 k at 128, 288 k at 256).  A call uses fewer per pair when the
+    // bank is too small to give every stream a pair (eff_sub_batch).
+    int64_t sb = (int64_t(2048) << 20) / (8 * n);
     if (sb < 1) sb = 1;
     if (sb > 256) sb = 256;
     const int ns = 4;                      // launch pairs in flight (cbmf_set_streams)
@@ -639,13 +641,24 @@ static int sort_triggers(cbmf_ctx* c, int64_t count)
     return CBMF_OK;
 }
 
+// Templates per launch pair of a call over nt templates: the context's sub-batch, or fewer so that every stream gets
+// a pair (at least 16 where the bank has them).
+static int eff_sub_batch(const cbmf_ctx* c, int64_t nt)
+{
+    int64_t per = (nt + c->n_streams - 1) / c->n_streams;
+    const int64_t floor16 = nt < 16 ? nt : 16;
+    if (per < floor16) per = floor16;
+    int64_t sb = c->sub_batch < per ? c->sub_batch : per;
+    return (int)(sb < 1 ? 1 : sb);
+}
+
 // Pass-1 / pass-2 launch pairs for templates [0, nt) whose constants are in c->d_coef; peaks to c->d_peaks,
 // triggers to c->d_trig (dev_cap entries; the total is counted in c->d_cursor whatever the capacity).
 static int run_bank_passes(cbmf_ctx* c, int64_t nt, int64_t dev_cap, const c2* w = nullptr, int j_min = 0)
 {
     if (!w) w = c->d_w;
     int rc;
-    const int sb = c->sub_batch;
+    const int sb = eff_sub_batch(c, nt);
     // Launch pairs go round-robin over ns streams, each with its own slice of Y / cand / done, so
     // that the tail of one kernel overlaps the head of the next pair.  With per-pass event timing on
     // (cbmf_set_profiling mode 1) everything stays on the context's stream: each launch is timed alone;
@@ -981,7 +994,7 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
     if ((rc = bank_setup(c, c->d_bank, nt, thr))) return rc;
     CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
 
-    const int sb = c->sub_batch, ns = c->n_streams;
+    const int sb = eff_sub_batch(c, nt), ns = c->n_streams;
     const size_t ncand = cand_per_template(c);
     const int64_t n_pairs = (nt + sb - 1) / sb;
     CU(cudaEventRecord(c->ev_fork, c->stream));

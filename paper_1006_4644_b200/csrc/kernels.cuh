@@ -685,14 +685,23 @@ __global__ void __launch_bounds__(Cfg<L1>::NT1, (Cfg<L1>::NT1 <= 128 ? 4 : (Cfg<
                         }
                     };
                     if constexpr (R1 >= 32) {
-                        if (nz <= 2) run(std::integral_constant<int, 2>());
-                        else if (nz <= 4) run(std::integral_constant<int, 4>());
-                        else if (nz <= 6) run(std::integral_constant<int, 6>());
-                        else if (nz <= 8) run(std::integral_constant<int, 8>());
-                        else if (nz <= 10) run(std::integral_constant<int, 10>());
-                        else if (nz <= 12) run(std::integral_constant<int, 12>());
-                        else if (nz <= 14) run(std::integral_constant<int, 14>());
-                        else run(std::integral_constant<int, 16>());
+                        switch (nz) {
+                            case 0: case 1: case 2: run(std::integral_constant<int, 2>()); break;
+                            case 3: run(std::integral_constant<int, 3>()); break;
+                            case 4: run(std::integral_constant<int, 4>()); break;
+                            case 5: run(std::integral_constant<int, 5>()); break;
+                            case 6: run(std::integral_constant<int, 6>()); break;
+                            case 7: run(std::integral_constant<int, 7>()); break;
+                            case 8: run(std::integral_constant<int, 8>()); break;
+                            case 9: run(std::integral_constant<int, 9>()); break;
+                            case 10: run(std::integral_constant<int, 10>()); break;
+                            case 11: run(std::integral_constant<int, 11>()); break;
+                            case 12: run(std::integral_constant<int, 12>()); break;
+                            case 13: run(std::integral_constant<int, 13>()); break;
+                            case 14: run(std::integral_constant<int, 14>()); break;
+                            case 15: run(std::integral_constant<int, 15>()); break;
+                            default: run(std::integral_constant<int, 16>()); break;
+                        }
                     } else if constexpr (R1 >= 16) {
                         if (nz <= 2) run(std::integral_constant<int, 2>());
                         else if (nz <= 4) run(std::integral_constant<int, 4>());
