@@ -1,7 +1,8 @@
 /* asan_driver.c -- exercises oracle/mf_oracle.c under -fsanitize=address,undefined.
  * Built and run by tests/test_oracle_pins.py::test_oracle_under_sanitizers; exit code 0 = clean.
  * Two pins are repeated here in C: P1 (FFT = direct DFT) and the truncation / empty-band paths of
- * orc_filter_bank, which allocate and free the most. */
+ * orc_filter_bank, which allocate and free the most; the SURVEY.md section-8(f) twins (clustering, chi-squared,
+ * time-domain bank) run once each. */
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -18,6 +19,11 @@ int orc_load_segment(orc_ctx *c, const float *samples, int64_t n);
 int orc_snr_series(const orc_ctx *c, double m1, double m2, double *rho, double *z, double *sigma);
 int orc_filter_bank(const orc_ctx *c, const double *bank, int64_t nt, double thr, orc_peak *peaks,
                     orc_trigger *trig, int64_t cap, int64_t *n_found);
+int orc_td_filter_bank(const orc_ctx *c, const double *bank, int64_t nt, double thr, orc_peak *peaks,
+                       orc_trigger *trig, int64_t cap, int64_t *n_found);
+int orc_chisq(const orc_ctx *c, double m1, double m2, int64_t j, int p, double *chisq, double *zl, int64_t *edges);
+int orc_cluster_triggers(const orc_trigger *trig, int64_t n_trig, int64_t n_samples, int64_t window,
+                         orc_trigger *out, int64_t out_capacity, int64_t *n_out);
 
 static uint64_t lcg(uint64_t *s) { *s = *s * 6364136223846793005ULL + 1442695040888963407ULL; return *s >> 11; }
 
@@ -59,6 +65,19 @@ int main(void)
     double sig = 0;
     if (orc_snr_series(c, 1.4, 1.4, rho, NULL, &sig) || !(sig > 0)) return 8;
     if (fabs(rho[pk[0].idx_peak] - pk[0].snr_max) > 1e-12) return 9;
+    /* the section-8(f) twins: clustering of that list, chi-squared bands, the time-domain bank (heavy masses: the
+     * chirp must fit 0.5 s; one template too long for the segment -> EINVAL, one below the cut-off -> empty) */
+    orc_trigger ev[100];
+    int64_t n_ev = 0;
+    if (orc_cluster_triggers(tr, 100, M, 3, ev, 100, &n_ev) || n_ev != 1) return 10;
+    double chi = -1.0, zl[2 * 7];
+    int64_t edges[8];
+    if (orc_chisq(c, 3.0, 2.0, pk[2].idx_peak, 7, &chi, zl, edges) || !(chi >= 0.0)) return 11;
+    const double tbank[4] = {30.0, 28.0, 90.0, 80.0};
+    orc_peak tpk[2];
+    if (orc_td_filter_bank(c, tbank, 2, 0.5, tpk, tr, 100, &nf) < 0 || tpk[1].idx_peak != -1 || !(tpk[0].sigma > 0)) return 12;
+    const double too_long[2] = {1.4, 1.4};
+    if (orc_td_filter_bank(c, too_long, 1, 0.5, tpk, tr, 100, &nf) != -1) return 13;
     free(rho); free(psd); free(d);
     orc_destroy(c);
     puts("asan driver ok");
