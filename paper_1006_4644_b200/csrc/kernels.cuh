@@ -964,30 +964,52 @@ __device__ __forceinline__ void p2_row(const P2Args& a, const int j1, const int 
     if constexpr (ROT) rtw.advance();
 
     // v[u*RL + q] = z[j1 + L1 * j2],  j2 = t + T u + (L2/RL) q
-    if constexpr (MODE == EPI_STORE) {
-        c2* __restrict__ zb = a.z_out + (size_t)b * n_total + j1;
-#pragma unroll
-        for (int u = 0; u < E / RL; ++u)
-#pragma unroll
-            for (int q = 0; q < RL; ++q)
-                zb[(size_t)(t + T * u + (L2 / RL) * q) << LG1] = v[u * RL + q];
-    } else if constexpr (MODE == EPI_WSTORE) {
-        const int k_lo = a.coef->k_lo;
+    if constexpr (MODE == EPI_STORE || MODE == EPI_WSTORE) {
+        // z[j1 + L1 j2]: a thread's outputs lie L1 samples apart, so direct stores would touch one 32-byte sector per
+        // 8-byte value (four times the sector writes: 2.0 ms instead of 1.1 ms per 256 transforms at N = 2^20).  The
+        // ROWS adjacent rows of the block are transposed through its shared memory instead (T[j2][row], one pad element
+        // every PAD values of j2 against bank conflicts) and leave as runs of ROWS consecutive samples.
+        constexpr int ROWS = C::ROWS, NT = C::NT2;
+        constexpr int CAP = ROWS * p2_row_stride<L2>();
+        constexpr int SPARE = CAP - L2 * ROWS;
+        static_assert(SPARE > 0, "transposed store needs spare shared memory");
+        constexpr int PAD_MIN = (L2 + SPARE - 1) / SPARE;
+        constexpr int PAD = PAD_MIN <= 4 ? 4 : (PAD_MIN <= 8 ? 8 : (PAD_MIN <= 16 ? 16 : 32));
+        static_assert(L2 * ROWS + L2 / PAD <= CAP, "transposed store fits the block's buffers");
+        const int row = threadIdx.x / T;
+        c2* __restrict__ tt = sm - row * p2_row_stride<L2>();
+        __syncthreads();                                    // every row group has read its exchange buffer
 #pragma unroll
         for (int u = 0; u < E / RL; ++u)
 #pragma unroll
             for (int q = 0; q < RL; ++q) {
                 const int j2 = t + T * u + (L2 / RL) * q;
-                const size_t k = ((size_t)j2 << LG1) + j1;
-                if (k < n_total / 2) {
-                    c2 o = czero();
-                    if ((long long)k >= k_lo) {
-                        const double f = a.wfac[k];
-                        o = pk((float)(f * (double)re(v[u * RL + q])), (float)(-f * (double)im(v[u * RL + q])));
-                    }
-                    a.w_out[k] = o;
-                }
+                tt[j2 * ROWS + j2 / PAD + row] = v[u * RL + q];
             }
+        __syncthreads();
+        if constexpr (MODE == EPI_STORE) {
+            c2* __restrict__ zb = a.z_out + (size_t)b * n_total + (j1 - row);
+#pragma unroll 8
+            for (int m = threadIdx.x; m < L2 * ROWS; m += NT) {
+                const int j2 = m / ROWS, r = m % ROWS;
+                zb[((size_t)j2 << LG1) + r] = tt[m + j2 / PAD];
+            }
+        } else {
+            // load_segment: w[k] = conj(Z[k]) wfac[k] for k_lo <= k < N/2, zero below
+            const int k_lo = a.coef->k_lo;
+#pragma unroll 4
+            for (int m = threadIdx.x; m < L2 * ROWS / 2; m += NT) {     // j2 < L2 / 2: k < N / 2
+                const int j2 = m / ROWS, r = m % ROWS;
+                const size_t k = ((size_t)j2 << LG1) + (size_t)(j1 - row + r);
+                c2 o = czero();
+                if ((long long)k >= k_lo) {
+                    const c2 zv = tt[m + j2 / PAD];
+                    const double f = a.wfac[k];
+                    o = pk((float)(f * (double)re(zv)), (float)(-f * (double)im(zv)));
+                }
+                a.w_out[k] = o;
+            }
+        }
     } else {
         // ---- S6/S7: |z|^2, arg-max (lowest index on ties), threshold.
         // Fast path: the thread's maximum of |z|^2 against the template's running maximum (read at

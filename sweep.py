@@ -65,7 +65,10 @@ def run_point(log2n: int, batch: int, repeats: int, max_gib: float):
         x = torch.view_as_complex(torch.randn(b_run, n, 2, generator=g, device=dev, dtype=torch.float32))
         y = torch.empty_like(x)
         ms_h = _time(lambda: ctx.debug_ifft(x, y), stream, repeats)
-        ms_c = _time(lambda: torch.fft.ifft(x, dim=1, norm="forward", out=y), stream, repeats)
+        # torch adds an element-wise pass of its own behind the library transform when it is given `out=` (ncu shows
+        # it); the comparison figure is the faster of the two ways of calling it
+        ms_c = min(_time(lambda: torch.fft.ifft(x, dim=1, norm="forward", out=y), stream, repeats),
+                   _time(lambda: torch.fft.ifft(x, dim=1, norm="forward"), stream, repeats))
         ref = torch.fft.ifft(x[:1], dim=1, norm="forward")
         got = ctx.debug_ifft(x[:1].contiguous())
         err = float((got - ref).abs().max() / ref.abs().max())
