@@ -326,6 +326,12 @@ def test_filter_bank_cfg2_sampled(cbmf):
     tr_o = tr_o.copy()
     tr_o["template_idx"] = sel[tr_o["template_idx"]]
     check_triggers(tr_g[np.isin(tr_g["template_idx"], sel)], tr_o, wl.threshold)
+    # soak (the analogue of the paper's long-run check): the same 65 536-template bank again, and once
+    # more through the clustered call -- bit-identical peaks and triggers, whatever the block scheduler did
+    pk_2, tr_2, nf_2, rc_2 = g.filter_bank(wl.bank, wl.threshold, trig_capacity=1 << 20)
+    assert rc_2 == 0 and nf_2 == nf_g and np.array_equal(pk_2, pk_g) and np.array_equal(tr_2, tr_g)
+    pk_3, ev_3, n_ev, nf_3, rc_3 = g.filter_bank_clustered(wl.bank, wl.threshold, 64, event_capacity=1 << 20)
+    assert rc_3 == 0 and nf_3 == nf_g and np.array_equal(pk_3, pk_g) and 0 < n_ev <= nf_g
     g.close(); o.close()
     p = pk_g[inj.template_idx]
     assert abs(int(p["idx_peak"]) - inj.sample(wl.fs)) <= 2 and abs(p["snr_max"] - inj.snr) < 3.5
