@@ -51,6 +51,7 @@ extern "C" {
 #define CBMF_ESTATE   -2   /* call order: PSD, then segment, then filter */
 #define CBMF_ECUDA    -3   /* a CUDA runtime call failed; cbmf_last_cuda_error() names it */
 #define CBMF_ENOMEM   -4   /* host or device allocation failed */
+#define CBMF_ELIMIT   -5   /* size beyond the fixed limit of a no-allocation entry point (cbmf_ifft_noalloc_dev) */
 #define CBMF_WTRUNC    1   /* more triggers found than trig_capacity: list truncated */
 
 typedef struct cbmf_ctx cbmf_ctx;                 /* opaque */
@@ -212,6 +213,47 @@ int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_
  * (n/2 complex floats, interleaved). */
 int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);
 int cbmf_debug_get_weights(cbmf_ctx *ctx, float *w_out);
+
+/* ---- inverse FFT for callers that must not allocate device memory ----
+ * Who this is for.  Every other device-side call of this library goes through a cbmf_ctx, and creating or growing
+ * a context calls cudaMalloc (the inter-pass buffer Y of the two-pass FFT alone is 8 n bytes per transform).  Some
+ * users of the transform cannot do that at the point where they need it:
+ *   - code that runs inside someone else's memory budget -- a plug-in of a framework whose caching allocator has
+ *     already taken (nearly) all of the GPU, so that a raw cudaMalloc fails or fragments the pool;
+ *   - a real-time analysis loop (the online search of PAPER.md:247-255) that may not stall: cudaMalloc / cudaFree
+ *     synchronise the whole device and take an unbounded time;
+ *   - code that is between cudaStreamBeginCapture and cudaStreamEndCapture on some stream of the process, where an
+ *     allocation is an error.
+ * cbmf_ifft_noalloc_dev is the stand-alone transform of cbmf_debug_ifft_dev (same kernels, same split of n, same
+ * results: S5 of SURVEY.md §8(a), "inverse FFT") WITHOUT a context and without any allocation: its
+ * inter-pass buffer is a fixed array of CBMF_NOALLOC_MAX_N complex floats (8 MiB) that is part of the library image.
+ * Every GPU that loads this library's device code holds that array from then until the process exits, whether or
+ * not this function is ever called there: that is the price, and the reason for the modest limit.
+ *   out_dev[b][j] = sum_k in_dev[b][k] e^{+2 pi i jk/n}     (unnormalised, b < batch, interleaved re,im float32)
+ *   in_dev, out_dev  DEVICE pointers on `device`, batch * n complex floats each, 16-byte aligned, caller-owned,
+ *                    not overlapping; in_dev is only read.
+ *   n                a power of two, 2^12 <= n <= CBMF_NOALLOC_MAX_N.  batch >= 0: the transforms run
+ *                    CBMF_NOALLOC_MAX_N / n at a time, one launch pair after the other.
+ *   cuda_stream      a cudaStream_t of `device`, or NULL for the default stream.
+ * STREAM-ORDERED: the launches are enqueued on cuda_stream and the call returns without waiting; out_dev is
+ * complete once the stream has reached that point.  in_dev must stay valid until then.
+ * First call on a device: with that device current it looks the array's device address up (cudaGetSymbolAddress)
+ * and reads the SM count; the first call for each n on a device also opts that size's two kernels in to their
+ * shared-memory size (cudaFuncSetAttribute).  That is a one-off set-up of a few runtime calls: make a first call
+ * for every (device, n) you will use at start-up, before any stream capture begins and outside the part of the
+ * program that must not stall.  Later calls only launch kernels.  No call, first or later, uses cudaMalloc, cudaFree, or a library routine that
+ * allocates device memory.
+ * ONE array per GPU serves every call of the process.  Calls on the same stream follow each other and are safe.
+ * Calls whose kernels may run at the same time on one GPU (different streams, different threads) would write the
+ * same buffer: the results of both are then undefined -- order them yourself (one stream, or events).  The array
+ * keeps what the last call left in it; nothing in it has to start at zero, because pass 1 writes every element that
+ * pass 2 reads before pass 2 starts, so no clearing is done or needed.
+ * Errors: CBMF_ELIMIT if n > CBMF_NOALLOC_MAX_N (nothing is enqueued; use a context and cbmf_debug_ifft_dev);
+ * CBMF_EINVAL for a NULL pointer with batch > 0, a misaligned pointer, n not a power of two or below 2^12,
+ * batch < 0, a device index that does not exist or is >= 64; CBMF_ECUDA if a runtime call fails. */
+#define CBMF_NOALLOC_MAX_N (1 << 20)
+int cbmf_ifft_noalloc_dev(int device, void *cuda_stream, const float *in_dev, float *out_dev,
+                          int64_t n, int64_t batch);
 
 /* ---- waveform order ----
  * Phase order of the SPA templates, in half post-Newtonian orders: 4 = 2PN (default: BASELINE.json configs[0], the

@@ -17,7 +17,8 @@ i64_t = C.c_int64
 
 from . import build as _build
 
-OK, EINVAL, ESTATE, ECUDA, ENOMEM, WTRUNC = 0, -1, -2, -3, -4, 1
+OK, EINVAL, ESTATE, ECUDA, ENOMEM, ELIMIT, WTRUNC = 0, -1, -2, -3, -4, -5, 1
+NOALLOC_MAX_N = 1 << 20                  # CBMF_NOALLOC_MAX_N of cbmf.h
 
 PEAK_DTYPE = np.dtype([("snr_max", "<f4"), ("idx_peak", "<i4"), ("phase", "<f4"), ("sigma", "<f4")])
 TRIG_DTYPE = np.dtype([("template_idx", "<i4"), ("sample_idx", "<i4"), ("snr", "<f4"), ("phase", "<f4")])
@@ -58,6 +59,7 @@ def lib() -> C.CDLL:
         "cbmf_debug_ifft": (C.c_int, [vp, vp, vp, i64, i64]),
         "cbmf_debug_ifft_dev": (C.c_int, [vp, vp, vp, i64, i64]),
         "cbmf_debug_generate_dev": (C.c_int, [vp, vp, i64, vp]),
+        "cbmf_ifft_noalloc_dev": (C.c_int, [C.c_int, vp, vp, vp, i64, i64]),
         "cbmf_debug_get_prefix": (C.c_int, [vp, vp]),
         "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
         "cbmf_set_pn_order": (C.c_int, [vp, C.c_int]),
@@ -86,7 +88,7 @@ def lib() -> C.CDLL:
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_cluster_triggers "
            "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_chisq cbmf_filter_bank_td cbmf_debug_td_template cbmf_debug_snr_series "
-           "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev "
+           "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev cbmf_ifft_noalloc_dev "
            "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_pn_order cbmf_get_pn_order cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
            "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_debug_timeline cbmf_strerror "
@@ -427,6 +429,24 @@ def cluster_triggers(trig, n_samples: int, window_samples: int, event_capacity: 
     if rc < 0:
         raise CbmfError(rc, "cbmf_cluster_triggers")
     return ev[:min(n.value, cap)], n.value, rc
+
+
+def ifft_noalloc_dev(x, out, n: int, stream: int | None = None) -> int:
+    """cbmf_ifft_noalloc_dev: unnormalised inverse DFT of the vectors of `x` ([batch, n] complex64 CUDA tensor) into
+    `out` (same shape, same device, preallocated by the caller), for callers that must not allocate device memory
+    (a guest of a framework that owns the GPU's memory, a loop that may not stall in cudaMalloc, code running while
+    a stream is being captured): no context, the scratch buffer is a fixed 8 MiB array inside the library, hence
+    n <= NOALLOC_MAX_N.  This wrapper allocates nothing either and only marshals; the work is enqueued on `stream`
+    (a cudaStream_t handle, default stream if None) and NOT waited for.  Calls that may overlap on one GPU share
+    the scratch array and race: keep them on one stream.  Returns the raw code (OK, or ELIMIT / EINVAL / ECUDA:
+    no exception, so that a caller can probe the limit)."""
+    xp, xdev = _ptr(x, "complex64")
+    op, odev = _ptr(out, "complex64")
+    if not (xdev and odev) or x.device != out.device:
+        raise ValueError("x and out must be CUDA tensors on the same device")
+    if x.numel() % int(n) or out.numel() != x.numel():
+        raise ValueError("x must hold whole vectors of n values and out must match it")
+    return int(lib().cbmf_ifft_noalloc_dev(x.device.index, C.c_void_p(stream or 0), xp, op, int(n), x.numel() // int(n)))
 
 
 def version() -> str:

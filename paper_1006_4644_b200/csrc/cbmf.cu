@@ -14,6 +14,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <unordered_set>
 #include <vector>
@@ -1519,6 +1520,97 @@ extern "C" int cbmf_debug_get_weights(cbmf_ctx* c, float* w_out)
     return CBMF_OK;
 }
 
+// ======================================================================= transform without allocation
+// cbmf_ifft_noalloc_dev (include/cbmf.h): the stand-alone inverse FFT for callers that cannot allocate device memory
+// where they need the transform -- guests of a framework whose allocator owns the GPU, real-time loops that must not
+// hit the device-wide synchronisation of cudaMalloc / cudaFree, code running while a stream of the process is being
+// captured.  Same kernels and the same split of n as cbmf_debug_ifft_dev, so the same numbers; the one difference is
+// where the inter-pass buffer Y lives: in the array below, which is part of the library image, instead of in a
+// context's cudaMalloc'ed d_Y.
+namespace {
+
+// Inter-pass buffer of the two-pass FFT: CBMF_NOALLOC_MAX_N packed complex floats = 8 MiB, held by every GPU that
+// loads this library's device code until the process exits.  One array per GPU, shared by every call.
+//
+// In HOST code the name g_noalloc_Y is only a host-side handle of the symbol: its host "address" is not where the
+// array lives on any GPU, and a kernel handed &g_noalloc_Y[0] from the host would fault (or, on a system whose GPUs
+// can reach host memory, quietly scribble over host memory).  Host code therefore never passes the name to a
+// kernel: noalloc_device() asks the runtime for the array's address ON THE CURRENT DEVICE (it differs from GPU to
+// GPU) and the launches get that pointer.
+static __device__ __align__(256) c2 g_noalloc_Y[CBMF_NOALLOC_MAX_N];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+struct NoAllocDevice {
+    c2* y = nullptr;                // device address of g_noalloc_Y on this GPU
+    cbmf_ctx* shell = nullptr;      // host-only record the launch helpers want (SM count, shared-memory opt-ins): no device memory
+};
+NoAllocDevice g_noalloc_dev[NOALLOC_MAX_DEVICES];
+std::mutex g_noalloc_mutex;         // guards the table above and the shell's fields
+
+// Once per device, with that device current: the array's device address and the host-side record.  Runtime calls
+// made: cudaGetSymbolAddress, cudaDeviceGetAttribute.  Nothing here allocates device memory.
+int noalloc_device(int device, NoAllocDevice** out)
+{
+    NoAllocDevice& d = g_noalloc_dev[device];
+    if (!d.y) {
+        cbmf_ctx* c = nullptr;      // for CU()
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_noalloc_Y));
+        if (!p) return CBMF_ECUDA;
+        if (!d.shell) {
+            d.shell = new (std::nothrow) cbmf_ctx();       // host heap only; lives as long as the process
+            if (!d.shell) return CBMF_ENOMEM;
+            d.shell->device = device;
+        }
+        CU(cudaDeviceGetAttribute(&d.shell->n_sm, cudaDevAttrMultiProcessorCount, device));
+        d.y = (c2*)p;
+    }
+    *out = &d;
+    return CBMF_OK;
+}
+
+}  // namespace
+
+extern "C" int cbmf_ifft_noalloc_dev(int device, void* cuda_stream, const float* in_dev, float* out_dev,
+                                     int64_t n, int64_t batch)
+{
+    if (batch < 0 || n < (int64_t(1) << 12) || (n & (n - 1)) != 0) return CBMF_EINVAL;
+    if (n > (int64_t)CBMF_NOALLOC_MAX_N) return CBMF_ELIMIT;         // the fixed array holds one transform of at most this size
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) return CBMF_EINVAL;
+    if (batch > 0 && (!in_dev || !out_dev)) return CBMF_EINVAL;
+    if (((uintptr_t)in_dev | (uintptr_t)out_dev) & 15) return CBMF_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return CBMF_ECUDA; }
+    if (device >= ndev) return CBMF_EINVAL;
+
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    DeviceGuard g(device);
+    if (!g.ok) { cudaGetLastError(); return CBMF_ECUDA; }
+    NoAllocDevice* d = nullptr;
+    if (int rc = noalloc_device(device, &d)) return rc;
+    if (batch == 0) return CBMF_OK;
+
+    cbmf_ctx* c = d->shell;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int lg = ilog2(n);
+    c->n = n; c->log2n = lg;
+    c->lg1 = lg / 2; c->lg2 = lg - c->lg1;                 // the split cbmf_create chooses for n <= 2^20
+    // as many transforms per launch pair as the array holds; pairs follow each other on the stream, so pass 1 of
+    // the next pair overwrites Y only after pass 2 of this one has read it
+    const int64_t per_pair = (int64_t)CBMF_NOALLOC_MAX_N / n;
+    for (int64_t b0 = 0; b0 < batch; b0 += per_pair) {
+        const int nb = (int)std::min(per_pair, batch - b0);
+        P1Args a1; memset(&a1, 0, sizeof(a1));
+        a1.in_c = (const c2*)in_dev + (size_t)b0 * (size_t)n; a1.Y = d->y;
+        CU(launch_p1<LOAD_CPLX>(c, st, a1, nb));
+        P2Args a2; memset(&a2, 0, sizeof(a2));
+        a2.Y = d->y; a2.z_out = (c2*)out_dev + (size_t)b0 * (size_t)n;
+        CU(launch_p2<EPI_STORE>(c, st, a2, nb));
+        c->launches += 2;
+    }
+    return CBMF_OK;
+}
+
 // ======================================================================= introspection
 extern "C" int64_t cbmf_launch_count(const cbmf_ctx* c) { return c ? c->launches : -1; }
 
@@ -1554,6 +1646,7 @@ extern "C" const char* cbmf_strerror(int rc)
         case CBMF_ESTATE: return "call order: set_psd, then load_segment, then filter_bank";
         case CBMF_ECUDA: return "CUDA runtime error";
         case CBMF_ENOMEM: return "out of memory";
+        case CBMF_ELIMIT: return "size exceeds the fixed scratch array of the no-allocation entry point";
         case CBMF_WTRUNC: return "trigger list truncated at trig_capacity";
         default: return "unknown code";
     }
