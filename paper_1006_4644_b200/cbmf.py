@@ -143,12 +143,25 @@ def _nbytes(a) -> int:
     return int(a.numel() * a.element_size()) if _is_tensor(a) else int(a.nbytes)
 
 
+# Calls that return only after the context's stream has drained (cbmf.h: "every call that returns results is
+# synchronous"; the host-pointer set / load wait too).  Matched as prefixes of the name handed to Context._check;
+# the two stream-ordered calls are named cbmf_set_psd_dev / cbmf_load_segment_dev there and are excluded below.
+_WAITING = ("cbmf_filter_", "cbmf_chisq", "cbmf_debug_snr_series", "cbmf_debug_template", "cbmf_debug_td_template",
+            "cbmf_debug_ifft", "cbmf_debug_generate_dev", "cbmf_debug_get_")
+
+
 class Context:
     """cbmf_ctx: one segment length / sample rate / lower cutoff on one device and stream."""
 
     def __init__(self, n: int, fs: float, f_low: float, device: int = 0, stream: int | None = None):
         self.n, self.fs, self.f_low, self.device = int(n), float(fs), float(f_low), int(device)
         self._h = C.c_void_p()
+        # CUDA tensors handed to the stream-ordered calls (cbmf_set_psd_dev, cbmf_load_segment_dev): those return
+        # before the device has read their input, so the binding keeps the tensors alive until a call that waits
+        # for the context's stream has returned.  Otherwise a temporary (g.load_segment(x.cuda())) would go back to
+        # torch's caching allocator at once and, with the context on another stream than the one the tensor was
+        # allocated on, could be handed out again and overwritten before the kernel reads it.
+        self._held = []
         rc = lib().cbmf_create(C.byref(self._h), self.device, self.n, self.fs, self.f_low,
                                C.c_void_p(stream or 0))
         if rc:
@@ -158,8 +171,10 @@ class Context:
     # -- lifetime
     def close(self):
         if getattr(self, "_h", None):
-            lib().cbmf_destroy(self._h)
+            lib().cbmf_destroy(self._h)          # waits for the context's stream
             self._h = C.c_void_p()
+        if getattr(self, "_held", None):
+            self._held.clear()
 
     def __del__(self):
         try:
@@ -174,6 +189,8 @@ class Context:
         self.close()
 
     def _check(self, rc: int, what: str) -> int:
+        if rc >= 0 and (what in ("cbmf_set_psd", "cbmf_load_segment") or what.startswith(_WAITING)):
+            self._held.clear()                   # the context's stream has been waited for: the device is done with them
         if rc < 0:
             detail = lib().cbmf_last_cuda_error(self._h).decode() if rc == ECUDA else ""
             if rc == EINVAL and what == "cbmf_filter_bank":
@@ -189,16 +206,22 @@ class Context:
             psd = np.ascontiguousarray(psd, dtype=np.float64)
         p, dev = _ptr(psd, "float64", self.device)
         n_bins = int(psd.numel() if _is_tensor(psd) else psd.size)
-        f = lib().cbmf_set_psd_dev if dev else lib().cbmf_set_psd
-        self._check(f(self._h, p, n_bins), "cbmf_set_psd")
+        if dev:
+            self._held.append(psd)
+            self._check(lib().cbmf_set_psd_dev(self._h, p, n_bins), "cbmf_set_psd_dev")
+        else:
+            self._check(lib().cbmf_set_psd(self._h, p, n_bins), "cbmf_set_psd")
 
     def load_segment(self, samples):
         if isinstance(samples, np.ndarray):
             samples = np.ascontiguousarray(samples, dtype=np.float32)
         p, dev = _ptr(samples, "float32", self.device)
         n = int(samples.numel() if _is_tensor(samples) else samples.size)
-        f = lib().cbmf_load_segment_dev if dev else lib().cbmf_load_segment
-        self._check(f(self._h, p, n), "cbmf_load_segment")
+        if dev:
+            self._held.append(samples)
+            self._check(lib().cbmf_load_segment_dev(self._h, p, n), "cbmf_load_segment_dev")
+        else:
+            self._check(lib().cbmf_load_segment(self._h, p, n), "cbmf_load_segment")
 
     def filter_bank(self, bank, snr_threshold: float, trig_capacity: int = 1 << 16):
         """Host arrays in, host arrays out: -> (peaks[PEAK_DTYPE], triggers[TRIG_DTYPE], n_found, rc)."""

@@ -89,3 +89,49 @@ def test_binding_rejects_wrong_dtypes():
     assert cbmf._ptr(torch.zeros(32, dtype=torch.uint8), "peak records", itemsize=16)[1] is False
     assert cbmf._ptr(np.zeros(2, dtype=cbmf.PEAK_DTYPE), "peak records", itemsize=16)[1] is False
     assert cbmf._ptr(torch.zeros(8, dtype=torch.float64), "float64")[1] is False
+
+
+def test_binding_keeps_stream_ordered_inputs_alive(monkeypatch):
+    """cbmf_set_psd_dev / cbmf_load_segment_dev return before the device has read their input: the binding holds
+    the tensors until a call that waits for the context's stream has returned (no GPU: stubbed library, fake tensors)."""
+    from paper_1006_4644_b200 import cbmf
+
+    class Stub:
+        def __getattr__(self, name):
+            if name == "cbmf_strerror":
+                return lambda rc: b"stub"
+            return lambda *a: 0
+
+    class FakeTensor:
+        is_cuda = True
+        dtype = "torch.float64"
+
+        class device:
+            index = 0
+
+        def __init__(self, n, dtype):
+            self._n, self.dtype = n, dtype
+
+        def data_ptr(self):
+            return 4096
+
+        def is_contiguous(self):
+            return True
+
+        def numel(self):
+            return self._n
+
+    monkeypatch.setattr(cbmf, "lib", lambda: Stub())
+    g = cbmf.Context(1 << 12, 4096.0, 40.0)
+    psd, seg = FakeTensor((1 << 11) + 1, "torch.float64"), FakeTensor(1 << 12, "torch.float32")
+    g.set_psd(psd)
+    g.load_segment(seg)
+    assert g._held == [psd, seg]
+    g.set_profiling(0); g.get_split()                  # calls that do not wait keep them
+    assert g._held == [psd, seg]
+    g.filter_bank([[1.4, 1.4]], 6.0)                   # a call that waits releases them
+    assert g._held == []
+    g.load_segment(seg)
+    assert g._held == [seg]
+    g.close()
+    assert g._held == []

@@ -553,6 +553,45 @@ def test_device_pointer_entry_points(cbmf):
     g.close()
 
 
+def test_device_inputs_may_be_temporaries_on_a_side_stream(cbmf):
+    """The stream-ordered *_dev calls return before the device has read their input.  With the context on a side
+    stream, a temporary input tensor (g.set_psd(x.cuda())) would go back to torch's caching allocator when the call
+    returns and be handed out again to the next allocation of that size on the tensor's own stream: the binding must
+    keep it alive until a call that waits.  The context's stream is stalled before each call, so that its kernels run
+    long after the call has returned and after the same-sized junk tensors have been written."""
+    import torch
+    wl = W.config0()
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low)
+    g.set_psd(wl.psd); g.load_segment(wl.samples)
+    ref_pk, ref_tr, ref_nf, _ = g.filter_bank(wl.bank, wl.threshold, trig_capacity=4096)
+    g.close()
+    main = torch.cuda.current_stream()
+    s = torch.cuda.Stream()
+    g = cbmf.Context(wl.n, wl.fs, wl.f_low, stream=s.cuda_stream)
+    psd_h, seg_h = torch.from_numpy(wl.psd), torch.from_numpy(wl.samples)
+
+    def stall():
+        with torch.cuda.stream(s):
+            torch.cuda._sleep(200_000_000)              # ~0.1 s of the context's stream
+
+    def send(host):
+        t = host.cuda()                                 # allocated and filled on torch's current stream
+        s.wait_stream(main)                             # what a correct caller does: the copy precedes the use
+        return t
+
+    stall(); g.set_psd(send(psd_h))
+    junk_a = torch.full((psd_h.numel(),), -1.0, dtype=torch.float64, device="cuda")       # an invalid PSD
+    stall(); g.load_segment(send(seg_h))
+    junk_b = torch.full((seg_h.numel(),), float("nan"), dtype=torch.float32, device="cuda")
+    assert len(g._held) == 2
+    pk, tr, nf, rc = g.filter_bank(wl.bank, wl.threshold, trig_capacity=4096)
+    assert g._held == []                                # released by the call that waited
+    assert rc == 0 and nf == ref_nf
+    assert np.array_equal(pk, ref_pk) and np.array_equal(tr, ref_tr)
+    assert float(junk_a[0]) == -1.0 and bool(torch.isnan(junk_b[0]))
+    g.close()
+
+
 def test_device_entry_points_defer_their_input_checks(cbmf):
     """cbmf.h: cbmf_set_psd_dev / cbmf_load_segment_dev are stream-ordered -- they enqueue and return; an invalid PSD
     entry or sample is reported (EINVAL) by the next call that waits, which leaves the context without it."""

@@ -48,10 +48,12 @@ def test_template_25pn_vs_oracle(log2n, fs, f_low, kind):
     g.close(); o.close()
 
 
-@pytest.mark.parametrize("name", ["cfg0", "small15", "small19"])
+@pytest.mark.parametrize("name", ["cfg0", "small15", "small19", "cfg1x64"])
 def test_filter_bank_25pn_vs_oracle(name):
+    # cfg1x64: the first 64 templates of configs[1] at its full size, N = 2^20 (the by-rows ln k path of the bench split)
     wl = {"cfg0": W.config0, "small15": lambda: W.small_case(log2n=15, n_templates=6, seed=88),
-          "small19": lambda: W.small_case(log2n=19, fs=4096.0, n_templates=4, seed=89)}[name]()
+          "small19": lambda: W.small_case(log2n=19, fs=4096.0, n_templates=4, seed=89),
+          "cfg1x64": lambda: W.config1(64)}[name]()
     g, o = _pair(wl)
     for (m1, m2) in wl.bank[:3]:
         rho_g, z_g = g.debug_snr_series(m1, m2)
