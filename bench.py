@@ -148,6 +148,19 @@ def mean_band_bins(wl) -> float:
     return float(np.mean(np.maximum(k_hi - k_lo + 1, 0)))
 
 
+def cpu_model() -> str:
+    """The host CPU as /proc/cpuinfo names it (read at run time)."""
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for ln in fh:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    import platform
+    return platform.processor() or platform.machine()
+
+
 def oracle_rate(wl, n_sample: int, repeats: int = 1):
     """Time the CPU oracle, as it stands, on the first n_sample templates of the workload."""
     import oracle
@@ -195,7 +208,8 @@ def run_reference(args):
         "data": "synthetic",
         "config": {"workload": wl.name, "n": wl.n, "fs_hz": wl.fs, "f_low_hz": wl.f_low,
                    "templates_per_step": n_sample, "threshold": wl.threshold},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -219,7 +233,7 @@ def kernel_source_hash() -> str:
 
 def load_traffic(n: int):
     """DRAM bytes per template of the two pass kernels from the tracked ncu summary profiles/traffic.json
-    (written by bench_traffic.py from one `ncu --set full` capture).  None unless the capture was taken on
+    (written by `bench.py --traffic-report` from one `ncu --set full` capture).  None unless the capture was taken on
     exactly the kernel sources of this tree (hash) and at this N."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
@@ -234,18 +248,10 @@ def load_traffic(n: int):
 
 
 def fp32_probe(device: int):
-    """Measured FFMA / FFMA2 TFLOP/s from the stand-alone probe bench_fp32_probe.cu (not the product library)."""
-    import ctypes
-    import subprocess
-    src, lib = os.path.join(ROOT, "bench_fp32_probe.cu"), os.path.join(ROOT, "bench_fp32_probe.so")
+    """Measured FFMA / FFMA2 TFLOP/s on dependent FMA chains: the library's diagnostic cbmf_debug_fp32_peak."""
     try:
-        if not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
-            subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-Xcompiler", "-fPIC",
-                            "-shared", "-o", lib, src], check=True, capture_output=True)
-        L = ctypes.CDLL(lib)
-        a, b = ctypes.c_double(0), ctypes.c_double(0)
-        rc = L.fp32_probe(int(device), ctypes.byref(a), ctypes.byref(b))
-        return (a.value, b.value) if rc == 0 else (None, None)
+        from paper_1006_4644_b200 import cbmf
+        return cbmf.debug_fp32_peak(device)
     except Exception:
         return None, None
 
@@ -381,8 +387,14 @@ def measure(torch, dist, cbmf, wl, dev, local, world, K, Wm, cap, args, with_e2e
                 out["td_us_per_template"] = 1e3 * a_ev.elapsed_time(b_ev) / (3 * n_td)
                 out["td_templates"] = n_td
             out["h2d"] = psd_h.numel() * 8 + smp_h.numel() * 4 + bank_h.numel() * 8
-            # peaks, kept triggers, the early template-status word (8 B) and the trigger count (8 B)
-            out["d2h"] = B * 16 + min(nf_h, cap) * 16 + 4 + 4 + 8 + 8
+            # what the three host-pointer calls copy back (csrc/cbmf.cu): the 8-byte input-check word of set_psd and of
+            # load_segment; filter_bank's 32-byte status block, the peaks and its trigger staging block, which is
+            # min(capacity, 4096) records whatever the count; a bank with more triggers than that block holds goes
+            # through the general collection: the kept triggers and the peaks once more
+            n_fast = min(cap, 4096)
+            out["d2h"] = 8 + 8 + 32 + B * 16 + n_fast * 16
+            if nf_h > n_fast:
+                out["d2h"] += min(nf_h, cap) * 16 + B * 16
         ctx.close()
     return out
 
@@ -515,8 +527,9 @@ def run_ours(args):
                                    "p2_kernel (twiddle + row FFT + |z|^2 + arg-max/threshold)")[which],
         "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "peak_source": "148 SM x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md §6)",
-        "peak_measured_tflops": {"ffma": fp32_meas[0], "ffma2_packed": fp32_meas[1],
-                                 "how": "bench_fp32_probe.cu: dependent FMA chains on every SM, CUDA events (cross-check, not the denominator)"},
+        "peak_measured_tflops": fp32_meas[1],          # packed-FFMA2 chains on every SM (the cross-check)
+        "peak_measured_ffma_tflops": fp32_meas[0],
+        "frac_of_measured_peak": (achieved / fp32_meas[1]) if fp32_meas[1] else None,
         "traffic": None if tr_per_tmpl is None else tr_per_tmpl * tmpl_per_launch,
         "traffic_source": traffic_src,
         "algorithmic_bytes_per_launch": 8.0 * n * tmpl_per_launch,
@@ -544,8 +557,18 @@ def run_ours(args):
         cores = oracle.num_threads()
         n_sample = min(B, max(64, 16 * cores))         # ~0.1 core-second per template at N = 2^20
         v, secs, cores = oracle_rate(wl, n_sample)
+        # one thread, mean over >= 8 templates (the paper compares with ONE core)
+        n_one = min(B, 8)
+        oracle.set_num_threads(1)
+        try:
+            v1, secs1, _ = oracle_rate(wl, n_one)
+        finally:
+            oracle.set_num_threads(cores)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {n_sample} templates of {wl.name}, filter_bank only, {secs:.2f} s wall"}
+               "sample": f"first {n_sample} templates of {wl.name}, filter_bank only, {secs:.2f} s wall",
+               "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "ms_per_template": 1e3 * secs1 / n_one,
+                                 "sample": f"first {n_one} templates of {wl.name}, filter_bank only, {secs1:.2f} s wall"},
+               "cpu_model": cpu_model()}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
@@ -578,9 +601,162 @@ def run_ours(args):
         "online_capacity": online,
         "cpu_baseline": cpu,
     }
+    # the second bound of the whole step: the inter-pass buffer Y goes through HBM once each way (16 N bytes per
+    # template: ncu reads 16.6 MB at N = 2^20, profiles/); the regime is the bound the step sits closer to
+    hbm_peak = peaks_file.get("hbm_gbs")
+    hbm_gbs = 16.0 * n * value / world / 1e9
+    alu_frac = roofline["whole_path"]["frac_of_fp32_peak"]
+    roofline["hbm"] = {"bytes_per_template": 16 * n, "achieved_gbs": hbm_gbs, "peak": hbm_peak, "unit": "GB/s",
+                       "frac": (hbm_gbs / hbm_peak) if hbm_peak else None,
+                       "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm_peak else "MEASURED_PEAKS.json missing"}
+    roofline["regime"] = ("hbm" if (hbm_peak and hbm_gbs / hbm_peak > alu_frac) else "alu")
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+# --------------------------------------------------------------------------- configs[4]: the kernel sweep
+# Segment lengths N = 2^16 .. 2^24 x template batch sizes 1 / 8 / 64 / 512, fs = 4096 Hz, f_low = 40 Hz, PSD of
+# config 0, m1, m2 uniform in [1, 3] Msun (BASELINE.json configs[4]).  For every point, on one GPU,
+# device-resident data:
+#   ifft      the hand-written batched inverse FFT alone (cbmf_debug_ifft_dev: pass 1 + pass 2 with plain load /
+#             store epilogues) on random complex input, out of place
+#   cufft     the same transform by cuFFT (torch.fft.ifft, norm="forward" = unnormalised) -- the comparison
+#             baseline only; cuFFT is never on the product path
+#   generate  the SPA generator alone writing q~ = w e^{i Psi} to HBM (cbmf_debug_generate_dev)
+#   filter    the whole hot path (cbmf_filter_bank_dev: S2-S8) in templates/s
+#     python bench.py --workload cfg4 [--log2n 16 ... 24] [--batches 1 8 64 512] [--repeats 5] [--markdown]
+# One JSON line per point on stdout (not the driver's bench line: that is cfg1); --markdown prints a table instead.
+# Points whose buffers would exceed --max-gib (input + output of the FFT comparison) run with the largest batch
+# that fits and say so in "batch_run".
+def _sweep_time(fn, stream, repeats):
+    import torch
+    fn()
+    stream.synchronize()
+    best = None
+    for _ in range(repeats):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        fn()
+        b.record(stream)
+        stream.synchronize()
+        ms = a.elapsed_time(b)
+        best = ms if best is None else min(best, ms)
+    return best
+
+
+def sweep_point(log2n: int, batch: int, repeats: int, max_gib: float):
+    import torch
+    from paper_1006_4644_b200 import cbmf
+    from testsupport import workloads as W
+    n = 1 << log2n
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.Stream(device=dev)
+    b_run = batch
+    while b_run > 1 and 2 * 8 * n * b_run > max_gib * (1 << 30):
+        b_run //= 2
+    wl = W.sweep_point(log2n, batch)
+    out = {"log2n": log2n, "batch": batch, "batch_run": b_run}
+    with torch.cuda.stream(stream):
+        ctx = cbmf.Context(n, wl.fs, wl.f_low, device=0, stream=stream.cuda_stream)
+        ctx.set_psd(wl.psd)
+        ctx.load_segment(wl.samples)
+        g = torch.Generator(device=dev).manual_seed(1000 + log2n)
+        x = torch.view_as_complex(torch.randn(b_run, n, 2, generator=g, device=dev, dtype=torch.float32))
+        y = torch.empty_like(x)
+        ms_h = _sweep_time(lambda: ctx.debug_ifft(x, y), stream, repeats)
+        # torch adds an element-wise pass of its own behind the library transform when it is given `out=` (ncu shows
+        # it); the comparison figure is the faster of the two ways of calling it
+        ms_c = min(_sweep_time(lambda: torch.fft.ifft(x, dim=1, norm="forward", out=y), stream, repeats),
+                   _sweep_time(lambda: torch.fft.ifft(x, dim=1, norm="forward"), stream, repeats))
+        ref = torch.fft.ifft(x[:1], dim=1, norm="forward")
+        got = ctx.debug_ifft(x[:1].contiguous())
+        err = float((got - ref).abs().max() / ref.abs().max())
+        flops = 5.0 * n * log2n * b_run
+        out.update(ifft_ms=ms_h, cufft_ms=ms_c, ifft_vs_cufft=ms_c / ms_h, ifft_gflops=flops / ms_h / 1e6,
+                   cufft_gflops=flops / ms_c / 1e6, ifft_max_rel_diff_vs_cufft=err)
+        del x, y
+        bank = torch.from_numpy(np.ascontiguousarray(wl.bank[:b_run])).to(dev)
+        q = torch.empty(b_run * (n // 2), dtype=torch.complex64, device=dev)
+        ms_g = _sweep_time(lambda: ctx.debug_generate_dev(bank, q), stream, repeats)
+        out.update(generate_ms=ms_g, generate_gbins_per_s=b_run * (n // 2) / ms_g / 1e6)
+        del q
+        bank_full = torch.from_numpy(np.ascontiguousarray(wl.bank)).to(dev)
+        peaks = torch.empty(batch * 16, dtype=torch.uint8, device=dev)
+        trig = torch.empty((1 << 16) * 16, dtype=torch.uint8, device=dev)
+        ms_f = _sweep_time(lambda: ctx.filter_bank_into(bank_full, wl.threshold, peaks, trig, 1 << 16), stream, repeats)
+        out.update(filter_ms=ms_f, filter_templates_per_s=batch / ms_f * 1e3,
+                   filter_us_per_template=ms_f * 1e3 / batch)
+        ctx.close()
+    return out
+
+
+def run_cfg4(a):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --workload cfg4: no CUDA device -- the product path has no CPU fallback")
+    rows = []
+    for l in a.log2n:
+        for b in a.batches:
+            r = sweep_point(l, b, a.repeats, a.max_gib)
+            rows.append(r)
+            if not a.markdown:
+                print(json.dumps(r), flush=True)
+    if a.markdown:
+        print("| log2 N | batch (run) | hand IFFT ms | cuFFT ms | cuFFT / hand | hand GFLOP/s | generator Gbin/s | "
+              "filter templates/s | filter us/template |")
+        print("|---:|---:|---:|---:|---:|---:|---:|---:|---:|")
+        for r in rows:
+            print(f"| {r['log2n']} | {r['batch']} ({r['batch_run']}) | {r['ifft_ms']:.4f} | {r['cufft_ms']:.4f} | "
+                  f"{r['ifft_vs_cufft']:.2f} | {r['ifft_gflops']:.0f} | {r['generate_gbins_per_s']:.1f} | "
+                  f"{r['filter_templates_per_s']:.0f} | {r['filter_us_per_template']:.2f} |")
+    return 0
+
+
+# --------------------------------------------------------------------------- profiles/traffic.json
+# One `ncu --set full` capture of the two FFT-pass kernels -> the tracked summary profiles/traffic.json that
+# `roofline.traffic` is read from.  On the GPU box, in the same gpurun command as the capture (stamps the kernel
+# sources the capture ran on):      python bench.py --traffic-stamp > gpurun_out/src_hash.txt
+# Here (ncu reads reports without a GPU):
+#     python bench.py --traffic-report gpurun_out/prof.ncu-rep --traffic-stamp-file gpurun_out/src_hash.txt \
+#         --traffic-templates-per-launch 256 --traffic-command "<the ncu command line>"
+# dram bytes per template = (dram__bytes_read.sum + dram__bytes_write.sum) of a launch / templates per launch,
+# averaged over the captured launches of each kernel.
+def write_traffic(a):
+    import csv
+    import io
+    import subprocess
+    stamp = open(a.stamp_file).read().strip() if a.stamp_file else kernel_source_hash()
+    raw = subprocess.run(["ncu", "-i", a.report, "--page", "raw", "--csv"], check=True, capture_output=True, text=True).stdout
+    rows = list(csv.reader(io.StringIO(raw)))
+    hdr = rows[0]
+    col = {name: i for i, name in enumerate(hdr)}
+    per = {"p1_kernel": [], "p2_kernel": []}
+    dur = {"p1_kernel": [], "p2_kernel": []}
+    for r in rows[2:]:                       # row 1 holds the units
+        name = r[col["Kernel Name"]]
+        for k in per:
+            if k in name:
+                rd = float(r[col["dram__bytes_read.sum"]].replace(",", ""))
+                wr = float(r[col["dram__bytes_write.sum"]].replace(",", ""))
+                unit_r = rows[1][col["dram__bytes_read.sum"]]
+                unit_w = rows[1][col["dram__bytes_write.sum"]]
+                scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+                per[k].append(rd * scale.get(unit_r, 1.0) + wr * scale.get(unit_w, 1.0))
+                d = float(r[col["gpu__time_duration.sum"]].replace(",", ""))
+                dur[k].append(d * {"ns": 1e-3, "us": 1.0, "ms": 1e3}.get(rows[1][col["gpu__time_duration.sum"]], 1.0))
+    out = {
+        "kernel_source_hash": stamp, "n": a.n, "templates_per_launch": a.templates_per_launch,
+        "launches_captured": [len(per["p1_kernel"]), len(per["p2_kernel"])],
+        "dram_bytes_per_template": [sum(v) / len(v) / a.templates_per_launch if v else None for v in (per["p1_kernel"], per["p2_kernel"])],
+        "gpu_time_us_per_launch_under_ncu": [sum(v) / len(v) if v else None for v in (dur["p1_kernel"], dur["p2_kernel"])],
+        "source": f"ncu --set full, {os.path.basename(a.report)} (profiles/traffic.json)", "command": a.command,
+    }
+    with open(a.out, "w") as fh:
+        json.dump(out, fh, indent=1)
+        fh.write("\n")
+    print(json.dumps(out))
     return 0
 
 
@@ -590,7 +766,20 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3"], default="cfg1")
+    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3", "cfg4"], default="cfg1",
+                    help="cfg4 = the configs[4] kernel sweep (one JSON line per point; not the driver's bench line)")
+    ap.add_argument("--log2n", type=int, nargs="*", default=list(range(16, 25)), help="cfg4: segment lengths")
+    ap.add_argument("--batches", type=int, nargs="*", default=[1, 8, 64, 512], help="cfg4: templates per point")
+    ap.add_argument("--repeats", type=int, default=5, help="cfg4: timed repeats per measurement (best of)")
+    ap.add_argument("--max-gib", type=float, default=16.0, help="cfg4: cap on the FFT comparison buffers")
+    ap.add_argument("--markdown", action="store_true", help="cfg4: print a table instead of JSON lines")
+    ap.add_argument("--traffic-stamp", action="store_true", help="print the hash of the kernel sources and exit")
+    ap.add_argument("--traffic-report", dest="report", help="ncu report to turn into profiles/traffic.json")
+    ap.add_argument("--traffic-stamp-file", dest="stamp_file")
+    ap.add_argument("--traffic-n", dest="n", type=int, default=1 << 20)
+    ap.add_argument("--traffic-templates-per-launch", dest="templates_per_launch", type=int, default=256)
+    ap.add_argument("--traffic-command", dest="command", default="")
+    ap.add_argument("--traffic-out", dest="out", default=os.path.join(ROOT, "profiles", "traffic.json"))
     ap.add_argument("--sub-batch", type=int, default=0, help="templates per launch pair (0 = library default)")
     ap.add_argument("--streams", type=int, default=0, help="launch pairs in flight (0 = library default)")
     ap.add_argument("--trig-capacity", type=int, default=1 << 16)
@@ -600,6 +789,13 @@ def main():
     ap.add_argument("--no-sustained", action="store_true", help="skip the cfg2 `sustained` record of the default run")
     ap.add_argument("--sustained-steps", type=int, default=3)
     args = ap.parse_args()
+    if args.traffic_stamp:
+        print(kernel_source_hash())
+        return 0
+    if args.report:
+        return write_traffic(args)
+    if args.workload == "cfg4":
+        return run_cfg4(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)

@@ -209,6 +209,11 @@ int cbmf_debug_ifft_dev(cbmf_ctx *ctx, const float *in_dev, float *out_dev, int6
  * template, device array) -- SURVEY.md config 4 "template-generator-only throughput". */
 int cbmf_debug_generate_dev(cbmf_ctx *ctx, const cbmf_template *bank_dev, int64_t n_templates,
                             float *q_out_dev);
+/* The FP32 throughput this GPU reaches on dependent FMA chains (one 1024-thread block per SM, eight chains per
+ * thread), in TFLOP/s: scalar FFMA and packed FFMA2 (fma.rn.f32x2).  bench.py reports it beside the unit-count peak
+ * that is the roofline denominator.  Allocates a small buffer, runs on the legacy default stream of
+ * `device` and waits.  EINVAL for a NULL pointer or a device that does not exist; ECUDA. */
+int cbmf_debug_fp32_peak(int device, double *tflops_ffma, double *tflops_ffma2);
 /* Copies of device state for tests: sigma^2 prefix table P[k] (n/2 doubles) and w[k]
  * (n/2 complex floats, interleaved). */
 int cbmf_debug_get_prefix(cbmf_ctx *ctx, double *p_out);

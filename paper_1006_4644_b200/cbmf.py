@@ -60,6 +60,7 @@ def lib() -> C.CDLL:
         "cbmf_debug_ifft_dev": (C.c_int, [vp, vp, vp, i64, i64]),
         "cbmf_debug_generate_dev": (C.c_int, [vp, vp, i64, vp]),
         "cbmf_ifft_noalloc_dev": (C.c_int, [C.c_int, vp, vp, vp, i64, i64]),
+        "cbmf_debug_fp32_peak": (C.c_int, [C.c_int, C.POINTER(dbl), C.POINTER(dbl)]),
         "cbmf_debug_get_prefix": (C.c_int, [vp, vp]),
         "cbmf_debug_get_weights": (C.c_int, [vp, vp]),
         "cbmf_set_pn_order": (C.c_int, [vp, C.c_int]),
@@ -88,7 +89,7 @@ def lib() -> C.CDLL:
 EXPORTS = ("cbmf_create cbmf_destroy cbmf_set_psd cbmf_set_psd_dev cbmf_load_segment "
            "cbmf_load_segment_dev cbmf_filter_bank cbmf_filter_bank_dev cbmf_cluster_triggers "
            "cbmf_filter_bank_clustered cbmf_filter_stream cbmf_chisq cbmf_filter_bank_td cbmf_debug_td_template cbmf_debug_snr_series "
-           "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev cbmf_ifft_noalloc_dev "
+           "cbmf_debug_template cbmf_debug_ifft cbmf_debug_ifft_dev cbmf_debug_generate_dev cbmf_ifft_noalloc_dev cbmf_debug_fp32_peak "
            "cbmf_debug_get_prefix cbmf_debug_get_weights cbmf_set_pn_order cbmf_get_pn_order cbmf_set_sub_batch cbmf_get_sub_batch "
            "cbmf_set_streams cbmf_get_streams cbmf_get_split cbmf_last_bad_template "
            "cbmf_launch_count cbmf_last_pass_time cbmf_set_profiling cbmf_debug_timeline cbmf_strerror "
@@ -470,6 +471,15 @@ def ifft_noalloc_dev(x, out, n: int, stream: int | None = None) -> int:
     if x.numel() % int(n) or out.numel() != x.numel():
         raise ValueError("x must hold whole vectors of n values and out must match it")
     return int(lib().cbmf_ifft_noalloc_dev(x.device.index, C.c_void_p(stream or 0), xp, op, int(n), x.numel() // int(n)))
+
+
+def debug_fp32_peak(device: int = 0):
+    """cbmf_debug_fp32_peak -> (FFMA TFLOP/s, packed FFMA2 TFLOP/s) measured on dependent FMA chains."""
+    a, b = C.c_double(0), C.c_double(0)
+    rc = lib().cbmf_debug_fp32_peak(int(device), C.byref(a), C.byref(b))
+    if rc < 0:
+        raise CbmfError(rc, "cbmf_debug_fp32_peak")
+    return a.value, b.value
 
 
 def version() -> str:

@@ -8,6 +8,7 @@
 #include "kernels.cuh"
 #include "td.cuh"
 #include "cluster.h"
+#include "probe.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -1608,6 +1609,18 @@ extern "C" int cbmf_ifft_noalloc_dev(int device, void* cuda_stream, const float*
         CU(launch_p2<EPI_STORE>(c, st, a2, nb));
         c->launches += 2;
     }
+    return CBMF_OK;
+}
+
+// ======================================================================= FP32 pipe probe (diagnostic)
+extern "C" int cbmf_debug_fp32_peak(int device, double* tflops_ffma, double* tflops_ffma2)
+{
+    if (!tflops_ffma || !tflops_ffma2) return CBMF_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return CBMF_ECUDA; }
+    if (device < 0 || device >= ndev) return CBMF_EINVAL;
+    const cudaError_t e = cbmf_probe::fp32_peak(device, tflops_ffma, tflops_ffma2);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cbmf_debug_fp32_peak");
     return CBMF_OK;
 }
 

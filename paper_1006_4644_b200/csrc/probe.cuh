@@ -1,15 +1,14 @@
-// bench_fp32_probe.cu -- stand-alone FP32 pipe probe used by bench.py as a cross-check of the roofline
-// denominator.  NOT part of the product library: it shares no code with
-// paper_1006_4644_b200/csrc and nothing on the filter path calls it.
+// probe.cuh -- FP32 pipe probe behind cbmf_debug_fp32_peak (include/cbmf.h): the measured cross-check of the
+// roofline denominator that bench.py reports.  A diagnostic of the library: nothing on the filter
+// path calls it and it shares no code with the filter kernels.
 //
 // Eight independent FMA chains per thread, 1024 threads per block, one block per SM.  Scalar FFMA
 // (2 flop per lane and instruction) and packed FFMA2 (fma.rn.f32x2, 4 flop).  Both should read close to
 // SMs x 128 lanes x 2 flop x SM clock.
-//
-// Build (bench.py does it on demand; __graft_entry__.build() too):
-//   nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -Xcompiler -fPIC -shared \
-//        -o bench_fp32_probe.so bench_fp32_probe.cu
+#pragma once
 #include <cuda_runtime.h>
+
+namespace cbmf_probe {
 
 typedef unsigned long long pk2;
 
@@ -53,19 +52,20 @@ __global__ void __launch_bounds__(1024, 1) fp32_probe_kernel(float* __restrict__
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 
-// Returns 0 on success, the cudaError_t otherwise.  Times on the legacy default stream of `device`.
-extern "C" int fp32_probe(int device, double* tflops_ffma, double* tflops_ffma2)
+// Times on the legacy default stream of `device`; restores the caller's current device.
+inline cudaError_t fp32_peak(int device, double* tflops_ffma, double* tflops_ffma2)
 {
-    if (!tflops_ffma || !tflops_ffma2) return (int)cudaErrorInvalidValue;
+    int prev = -1;
+    cudaGetDevice(&prev);
     cudaError_t e = cudaSetDevice(device);
-    if (e != cudaSuccess) return (int)e;
+    if (e != cudaSuccess) return e;
     int n_sm = 0;
-    if ((e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return (int)e;
     float* buf = nullptr;
-    if ((e = cudaMalloc(&buf, sizeof(float) * 1024 * (size_t)n_sm)) != cudaSuccess) return (int)e;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if ((e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device)) == cudaSuccess)
+        e = cudaMalloc(&buf, sizeof(float) * 1024 * (size_t)n_sm);
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
     const int iters = 4000;
     double res[2] = {0, 0};
     for (int packed = 0; packed < 2 && e == cudaSuccess; ++packed) {
@@ -80,12 +80,15 @@ extern "C" int fp32_probe(int device, double* tflops_ffma, double* tflops_ffma2)
         float ms = 0.f;
         if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
         const double flops = 2.0 * (packed ? 2.0 : 1.0) * 8.0 * 4.0 * (double)iters * 1024.0 * (double)n_sm;
-        res[packed] = flops / ((double)ms * 1e-3) / 1e12;
+        if (e == cudaSuccess && ms > 0.f) res[packed] = flops / ((double)ms * 1e-3) / 1e12;
     }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
     cudaFree(buf);
+    if (prev >= 0) cudaSetDevice(prev);
     *tflops_ffma = res[0];
     *tflops_ffma2 = res[1];
-    return (int)e;
+    return e;
 }
+
+}  // namespace cbmf_probe

@@ -66,7 +66,7 @@ def test_product_does_not_import_oracle():
                     # the 2PN phase coefficients (3715/756, 15293365/508032) belong to csrc/ only
                     assert "3715" not in txt and "15293365" not in txt and "4.925490947641267e-6" not in txt, f
     assert sorted(py_files) == ["__init__.py", "build.py", "cbmf.py", "sharding.py"], py_files
-    assert sorted(os.listdir(os.path.join(pkg, "csrc"))) == ["cbmf.cu", "cluster.h", "fft_regs.cuh", "kernels.cuh", "td.cuh"]
+    assert sorted(os.listdir(os.path.join(pkg, "csrc"))) == ["cbmf.cu", "cluster.h", "fft_regs.cuh", "kernels.cuh", "probe.cuh", "td.cuh"]
 
 
 def test_binding_rejects_wrong_dtypes():

@@ -1,7 +1,7 @@
 """Seeded synthetic workloads (SURVEY.md §8(d) "Synthetic inputs"; BASELINE.json configs[0..4]).
 
 TEST SUPPORT, NOT PRODUCT: this module lives outside the product package and is the ONE piece
-that serves both the CPU oracle (tests) and the CUDA path (tests, bench.py, sweep.py, smoke()).  It holds none of the filter's arithmetic: no matched
+that serves both the CPU oracle (tests) and the CUDA path (tests, bench.py, smoke()).  It holds none of the filter's arithmetic: no matched
 filter, no FFT of the product, no template generator of the product, no sigma
 table.  What it does hold is the *source model* used to simulate the detector
 data -- coloured Gaussian noise plus injected chirps -- written in numpy
