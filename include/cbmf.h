@@ -148,7 +148,8 @@ int cbmf_cluster_triggers(const cbmf_trigger *trig, int64_t n_trig, int64_t n_sa
  * host sorts and clusters them while the GPU filters the following pairs.  All pointers are HOST pointers.
  * peaks_out[n_templates] as in cbmf_filter_bank; events_out[event_capacity] the events of the whole bank in
  * (template_idx, sample_idx) order, truncated like the trigger list (CBMF_WTRUNC); *n_events the full event count;
- * *n_trig_found (may be NULL) the number of raw above-threshold samples.  Same errors as cbmf_filter_bank. */
+ * *n_trig_found (may be NULL) the number of raw above-threshold samples.  Same errors as cbmf_filter_bank.
+ * The call is not profiled: cbmf_last_pass_time and cbmf_debug_timeline read empty after it. */
 int cbmf_filter_bank_clustered(cbmf_ctx *ctx, const cbmf_template *bank, int64_t n_templates, float snr_threshold,
                                int64_t window_samples, cbmf_peak *peaks_out, cbmf_trigger *events_out,
                                int64_t event_capacity, int64_t *n_events, int64_t *n_trig_found);

@@ -738,28 +738,15 @@ static int bank_setup(cbmf_ctx* c, const double* bank_dev, int64_t nt, float thr
     return CBMF_OK;
 }
 
-// One bank pass over the segment whose weights are w (default: the context's), samples j < j_min excluded: filter,
-// count, sort and deliver.  Outputs go to host or device pointers (out_kind); *found_out = all triggers found.
-static int bank_filter(cbmf_ctx* c, int64_t nt, const c2* w, int j_min, void* peaks_out, void* trig_out,
-                       int64_t trig_capacity, int64_t* found_out, cudaMemcpyKind out_kind)
+// The general trigger collection behind a bank pass over templates [0, nt) that has completed with `found` triggers
+// counted (c->d_cursor) and at most c->trig_cap of them on the device: a list of any size is sorted and its first
+// trig_capacity entries delivered with the peaks (host or device pointers, out_kind); a list the device buffer could
+// not hold is rebuilt first.  Shared by the plain bank call, the streamed segments and the single-pair re-runs of
+// the clustered call.  -> CBMF_WTRUNC if found > trig_capacity.
+static int collect_triggers(cbmf_ctx* c, int64_t nt, const c2* w, int j_min, int64_t found, void* peaks_out,
+                            void* trig_out, int64_t trig_capacity, cudaMemcpyKind out_kind)
 {
     int rc;
-    // device trigger buffer: capacity rounded up to a power of two (bitonic padding), >= 1
-    int64_t tcap = 1;
-    while (tcap < trig_capacity) tcap <<= 1;
-    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
-    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
-    CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
-    c->ev_used[0] = c->ev_used[1] = 0;
-    if ((rc = run_bank_passes(c, nt, c->trig_cap, w, j_min))) return rc;
-
-    // trigger count back to the host, then sort what was kept
-    unsigned long long found_u = 0;
-    CU(cudaMemcpyAsync(&found_u, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    if ((rc = ev_collect(c))) return rc;
-    const int64_t found = (int64_t)found_u;
-    if (found_out) *found_out = found;
     const int64_t kept = found < trig_capacity ? found : trig_capacity;
     if (kept > 0 && trig_out) {
         int64_t on_device = found;
@@ -791,6 +778,31 @@ static int bank_filter(cbmf_ctx* c, int64_t nt, const c2* w, int j_min, void* pe
     CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, out_kind, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
+}
+
+// One bank pass over the segment whose weights are w (default: the context's), samples j < j_min excluded: filter,
+// count, sort and deliver.  Outputs go to host or device pointers (out_kind); *found_out = all triggers found.
+static int bank_filter(cbmf_ctx* c, int64_t nt, const c2* w, int j_min, void* peaks_out, void* trig_out,
+                       int64_t trig_capacity, int64_t* found_out, cudaMemcpyKind out_kind)
+{
+    int rc;
+    // device trigger buffer: capacity rounded up to a power of two (bitonic padding), >= 1
+    int64_t tcap = 1;
+    while (tcap < trig_capacity) tcap <<= 1;
+    if ((rc = grow(c, c->d_trig, c->trig_cap, tcap))) return rc;
+    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
+    CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
+    c->ev_used[0] = c->ev_used[1] = 0;
+    if ((rc = run_bank_passes(c, nt, c->trig_cap, w, j_min))) return rc;
+
+    // trigger count back to the host, then sort what was kept
+    unsigned long long found_u = 0;
+    CU(cudaMemcpyAsync(&found_u, c->d_cursor, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if ((rc = ev_collect(c))) return rc;
+    const int64_t found = (int64_t)found_u;
+    if (found_out) *found_out = found;
+    return collect_triggers(c, nt, w, j_min, found, peaks_out, trig_out, trig_capacity, out_kind);
 }
 
 // The plain bank call.  Everything is enqueued behind one another -- status reset, template setup, the launch pairs
@@ -871,36 +883,7 @@ static int filter_bank_impl(cbmf_ctx* c, const double* bank_dev, int64_t nt, flo
         return CBMF_OK;
     }
     // many triggers: the general collection (sort of any size, truncated lists)
-    if (kept > 0 && trig_out) {
-        int64_t on_device = found;
-        if (found > c->trig_cap) {
-            // Truncated and the device list is incomplete.  The contract (cbmf.h) keeps the FIRST trig_capacity
-            // triggers in (template, sample) order, so the whole lists of the leading templates are needed:
-            // find the shortest bank prefix [0, t_cut] holding at least trig_capacity triggers from the
-            // per-template counts and filter that prefix again into a buffer that takes all of its triggers.
-            std::vector<unsigned int> cnt((size_t)nt);
-            CU(cudaMemcpyAsync(cnt.data(), c->d_tcount, sizeof(unsigned int) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
-            CU(cudaStreamSynchronize(c->stream));
-            int64_t cum = 0, t_cut = 0;
-            for (; t_cut < nt; ++t_cut) { cum += cnt[(size_t)t_cut]; if (cum >= trig_capacity) break; }
-            int64_t need = 1;
-            while (need < cum) need <<= 1;
-            if ((rc = grow(c, c->d_trig, c->trig_cap, need))) return rc;
-            CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(unsigned long long), c->stream));
-            CU(cudaMemsetAsync(c->d_tcount, 0, sizeof(unsigned int) * (size_t)nt, c->stream));
-            const int prof = c->profiling;
-            c->profiling = 0;                           // the repeat is not part of the per-pass timing
-            rc = run_bank_passes(c, t_cut + 1, c->trig_cap);
-            c->profiling = prof;
-            if (rc) return rc;
-            on_device = cum;
-        }
-        if ((rc = sort_triggers(c, on_device))) return rc;
-        CU(cudaMemcpyAsync(trig_out, c->d_trig, sizeof(TrigOut) * (size_t)kept, out_kind, c->stream));
-    }
-    CU(cudaMemcpyAsync(peaks_out, c->d_peaks, b_peaks, out_kind, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    return (found > trig_capacity) ? CBMF_WTRUNC : CBMF_OK;
+    return collect_triggers(c, nt, nullptr, 0, found, peaks_out, trig_out, trig_capacity, out_kind);
 }
 
 static int filter_args_ok(cbmf_ctx* c, const void* bank, int64_t nt, float thr, void* peaks,
@@ -999,6 +982,11 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
     const int sb = eff_sub_batch(c, nt), ns = c->n_streams;
     const size_t ncand = cand_per_template(c);
     const int64_t n_pairs = (nt + sb - 1) / sb;
+    // this call records no per-pass events: cbmf_last_pass_time / cbmf_debug_timeline read empty after it
+    auto reset_profile = [&]() {
+        for (int w = 0; w < 2; ++w) { c->ev_used[w] = 0; c->last_ms[w] = 0; c->last_launches[w] = 0; c->timeline[w].clear(); }
+    };
+    reset_profile();
     CU(cudaEventRecord(c->ev_fork, c->stream));
     for (int s = 0; s < ns; ++s) CU(cudaStreamWaitEvent(c->aux[s], c->ev_fork, 0));
 
@@ -1035,20 +1023,31 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
     auto key_less = [](const HostTrig& a, const HostTrig& b) {
         return a.template_idx != b.template_idx ? a.template_idx < b.template_idx : a.sample_idx < b.sample_idx;
     };
-    int64_t next_enq = 0;
-    for (int64_t done = 0; done < n_pairs; ++done) {
-        // ns pairs share the ring slot's stream order; keep the ring one short of full so a slot is never re-armed
-        // before the host has consumed it
-        while (next_enq < n_pairs && next_enq - done < PIPE_RING - 1)
-            if ((rc = enqueue(next_enq++))) return rc;
-        const int ring = (int)(done % PIPE_RING);
-        CU(cudaEventSynchronize(c->ev_pipe[ring]));
-        const int64_t found = (int64_t)c->h_pcursor[ring];
-        found_total += found;
-        if (found > PAIR_TRIG_CAP) { overflow.push_back(done); continue; }
-        HostTrig* t = reinterpret_cast<HostTrig*>(c->h_ptrig + (size_t)ring * PAIR_TRIG_CAP);
-        std::sort(t, t + found, key_less);
-        if (!cluster_sorted(t, found, c->n, window_samples, events)) return CBMF_ECUDA;      // cannot happen: device indices are in range
+    auto pipeline = [&]() -> int {
+        int64_t next_enq = 0;
+        for (int64_t done = 0; done < n_pairs; ++done) {
+            // ns pairs share the ring slot's stream order; keep the ring one short of full so a slot is never re-armed
+            // before the host has consumed it
+            while (next_enq < n_pairs && next_enq - done < PIPE_RING - 1)
+                if (int e = enqueue(next_enq++)) return e;
+            const int ring = (int)(done % PIPE_RING);
+            CU(cudaEventSynchronize(c->ev_pipe[ring]));
+            const int64_t found = (int64_t)c->h_pcursor[ring];
+            found_total += found;
+            if (found > PAIR_TRIG_CAP) { overflow.push_back(done); continue; }
+            HostTrig* t = reinterpret_cast<HostTrig*>(c->h_ptrig + (size_t)ring * PAIR_TRIG_CAP);
+            std::sort(t, t + found, key_less);
+            if (!cluster_sorted(t, found, c->n, window_samples, events)) return CBMF_ECUDA;  // cannot happen: device indices are in range
+        }
+        return CBMF_OK;
+    };
+    rc = pipeline();
+    if (rc) {
+        // leave nothing running on the internal streams: a later call reuses d_Y, d_w and the pair regions
+        for (int s = 0; s < ns; ++s) cudaStreamSynchronize(c->aux[s]);
+        cudaStreamSynchronize(c->stream);
+        cudaGetLastError();
+        return rc;
     }
     for (int s = 0; s < ns; ++s) {
         CU(cudaEventRecord(c->ev_join[s], c->aux[s]));
@@ -1057,21 +1056,35 @@ extern "C" int cbmf_filter_bank_clustered(cbmf_ctx* c, const cbmf_template* bank
     CU(cudaMemcpyAsync(peaks_out, c->d_peaks, sizeof(PeakOut) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (!overflow.empty()) {
-        // a pair with more raw triggers than its region holds (a loud transient): filter its templates again through
-        // the plain call with a list that takes all of them, then cluster
-        PeakOut pk;
-        std::vector<HostTrig> raw((size_t)c->n);
+        // A pair with more raw triggers than its region holds (a loud transient): its templates are filtered again
+        // through the plain call, in runs of consecutive templates whose trigger counts (known from the first pass)
+        // add up to at most RERUN_TRIG, each run with a list that takes all of its triggers, and clustered.
+        constexpr int64_t RERUN_TRIG = int64_t(1) << 22;          // 64 MiB of trigger list per re-run
+        std::vector<unsigned int> cnt((size_t)nt);
+        CU(cudaMemcpyAsync(cnt.data(), c->d_tcount, sizeof(unsigned int) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));                      // the re-runs below reuse d_tcount
+        std::vector<PeakOut> pk;
+        std::vector<HostTrig> raw;
         for (int64_t pair : overflow) {
-            const int64_t t0 = pair * sb, nb = (nt - t0 < sb) ? (nt - t0) : sb;
-            for (int64_t i = 0; i < nb; ++i) {                     // template by template: at most n triggers each
-                int64_t nf = 0;
-                rc = filter_bank_impl(c, c->d_bank + 2 * (t0 + i), 1, thr, &pk, raw.data(), c->n, &nf, cudaMemcpyDeviceToHost);
-                if (rc < 0) return rc;
-                for (int64_t j = 0; j < nf; ++j) raw[(size_t)j].template_idx = (int32_t)(t0 + i);
-                if (!cluster_sorted(raw.data(), nf, c->n, window_samples, events)) return CBMF_ECUDA;
+            const int64_t t0 = pair * sb, t_end = (nt - t0 < sb) ? nt : t0 + sb;
+            for (int64_t a = t0; a < t_end;) {
+                int64_t b = a, sum = 0;
+                do { sum += cnt[(size_t)b]; ++b; } while (b < t_end && sum + (int64_t)cnt[(size_t)b] <= RERUN_TRIG);
+                if (sum > 0) {
+                    pk.resize((size_t)(b - a));
+                    raw.resize((size_t)sum);
+                    int64_t nf = 0;
+                    rc = filter_bank_impl(c, c->d_bank + 2 * a, b - a, thr, pk.data(), raw.data(), sum, &nf, cudaMemcpyDeviceToHost);
+                    if (rc < 0) return rc;
+                    const int64_t got = nf < sum ? nf : sum;       // the same kernels on the same input: nf == sum
+                    for (int64_t j = 0; j < got; ++j) raw[(size_t)j].template_idx += (int32_t)a;
+                    if (!cluster_sorted(raw.data(), got, c->n, window_samples, events)) return CBMF_ECUDA;
+                }
+                a = b;
             }
         }
         std::stable_sort(events.begin(), events.end(), key_less);
+        reset_profile();                                           // the re-runs are not the call's passes
     }
     const int64_t n_ev = (int64_t)events.size(), kept = n_ev < event_capacity ? n_ev : event_capacity;
     if (kept) memcpy(events_out, events.data(), sizeof(HostTrig) * (size_t)kept);

@@ -138,17 +138,27 @@ def test_filter_bank_clustered_vs_oracle(name, window, sub_batch):
 
 
 @pytest.mark.gpu
-def test_filter_bank_clustered_overflow_path():
+@pytest.mark.parametrize("log2n,n_templates,sub_batch", [(13, 5, 2), (20, 6, 6)])
+def test_filter_bank_clustered_overflow_path(log2n, n_templates, sub_batch):
     """threshold 0: every sample of every template is a trigger, far more than a launch pair's region holds; the call
-    falls back to the plain path template by template.  With a window of one sample every template is one closed ring
-    of triggers: one event, its global maximum."""
+    filters the overflowed pairs again through the plain path, in runs of templates whose triggers fit one list
+    (at 2^20 the single pair of 6 templates holds 6 M triggers: a run of 4 and a run of 2).  With a window of one
+    sample every template is one closed ring of triggers: one event, its global maximum.  The call is not profiled:
+    the per-pass record of an earlier profiled call does not survive it."""
     from paper_1006_4644_b200 import cbmf
-    wl = W.small_case(log2n=13, n_templates=5, seed=77)
+    wl = W.small_case(log2n=log2n, n_templates=n_templates, seed=77)
     g = cbmf.Context(wl.n, wl.fs, wl.f_low)
     g.set_psd(wl.psd); g.load_segment(wl.samples)
-    g.set_sub_batch(2)
+    g.set_sub_batch(sub_batch)
+    g.set_profiling(2)
+    g.filter_bank(wl.bank, wl.threshold)
+    assert g.last_pass_time(0)[1] > 0
     pk, ev, n_ev, nf, rc = g.filter_bank_clustered(wl.bank, 0.0, 1)
+    assert g.last_pass_time(0) == (0.0, 0) and g.last_pass_time(1) == (0.0, 0) and len(g.debug_timeline(0)) == 0
+    g.set_profiling(0)
+    pk_plain = g.filter_bank(wl.bank, 0.0, trig_capacity=0)[0]
     g.close()
-    assert rc == 0 and nf == 5 * wl.n and n_ev == 5
-    assert np.array_equal(ev["template_idx"], np.arange(5)) and np.array_equal(ev["sample_idx"], pk["idx_peak"])
+    assert rc == 0 and nf == n_templates * wl.n and n_ev == n_templates
+    assert np.array_equal(pk, pk_plain)
+    assert np.array_equal(ev["template_idx"], np.arange(n_templates)) and np.array_equal(ev["sample_idx"], pk["idx_peak"])
     assert np.array_equal(ev["snr"], pk["snr_max"])
