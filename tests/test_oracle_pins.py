@@ -943,6 +943,45 @@ def test_td_template_layout():
         oracle.Oracle(1 << 12, fs, 40.0).td_template(1.0, 1.0)
 
 
+def test_td_template_amplitude_law_by_stationary_phase():
+    """The amplitude law (F / f_low)^(2/3) of orc_td_template, pinned by something other than its own formula:
+    for a chirp A(t) cos phi(t) the stationary-phase spectrum is |H(f)| = A(t_f) / (2 sqrt(dF/dt)) at F(t_f) = f, so
+    with dF/dt ~ F^(11/3) the spectrum must fall as f^(-7/6) (an exponent 1/3 would give f^(-3/2), an exponent 1
+    f^(-5/6)), and its absolute level must equal the prediction built from A and from dF/dt read off orc_td_phase by
+    a finite difference.  The spectrum is numpy's FFT of the samples, averaged over 6 % bands to smooth the ripple of
+    the sharp start at f_low."""
+    n, fs, f_low = 1 << 16, 2048.0, 40.0
+    o, _ = _td_case(n, fs)
+    m1 = m2 = 1.4
+    hp, _hc = o.td_template(m1, m2)
+    H = np.abs(np.fft.rfft(hp))
+    f = np.fft.rfftfreq(n, 1.0 / fs)
+    ts, te, _fe = oracle.td_extent(m1, m2, f_low, 4)
+
+    def band_rms(F):
+        m = (f >= 0.97 * F) & (f < 1.03 * F)
+        return np.sqrt(np.mean(H[m] ** 2))
+
+    def tau_of(F):                                       # F(tau) falls with tau = t_c - t: bisection
+        lo, hi = te, ts
+        for _ in range(100):
+            mid = 0.5 * (lo + hi)
+            lo, hi = (mid, hi) if oracle.td_phase(m1, m2, mid, 4)[1] > F else (lo, mid)
+        return 0.5 * (lo + hi)
+
+    freqs = np.array([60.0, 100.0, 200.0, 400.0])        # a decade, away from both ends of the chirp
+    meas = np.array([band_rms(F) for F in freqs])
+    slope = np.polyfit(np.log(freqs), np.log(meas), 1)[0]
+    # -3/2 or -5/6 for a wrong exponent; the post-Newtonian terms of dF/dt steepen the Newtonian -7/6 by a few per cent
+    assert abs(slope + 7.0 / 6.0) < 0.06, slope
+    for F, got in zip(freqs, meas):
+        tau = tau_of(F)
+        d = 1e-4 * tau
+        f_dot = (oracle.td_phase(m1, m2, tau - d, 4)[1] - oracle.td_phase(m1, m2, tau + d, 4)[1]) / (2 * d)
+        want = fs * (F / f_low) ** (2.0 / 3.0) / (2.0 * np.sqrt(f_dot))       # numpy's FFT carries no dt: times fs
+        assert got == pytest.approx(want, rel=1e-2), (F, got, want)
+
+
 @pytest.mark.parametrize("order", [4, 5])
 def test_td_noise_free_injection_closed_forms(order):
     """Data = A h_+ of the same template, shifted circularly by t0: c_+(t0) = A sigma_+, c_x(t0) = A (h_+|h_x)/sigma_x
