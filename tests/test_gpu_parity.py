@@ -512,6 +512,55 @@ def test_two_contexts_interleaved(cbmf):
         assert np.array_equal(got[0], want[0]) and np.array_equal(got[1], want[1]) and got[2] == want[2]
 
 
+def _n_gpus():
+    try:
+        import torch
+        return torch.cuda.device_count()
+    except Exception:
+        return 0
+
+
+@pytest.mark.skipif(_n_gpus() < 2, reason="needs two CUDA devices (the round's boxes have one: skipped there)")
+def test_two_devices_interleaved(cbmf):
+    """Contexts on cuda:0 and cuda:1 of ONE process, calls interleaved (PAPER.md:281 multi-GPU; cbmf.h: per-device
+    state lives in the context): each gives the bytes the same workload gives on cuda:0 alone, whatever device is
+    current in the caller, and the caller's current device is left as it was.  The no-allocation transform keeps one
+    scratch array per device: its result on cuda:1 equals the one on cuda:0."""
+    import torch
+    wa, wb = W.config0(), W.small_case(log2n=17, n_templates=5, seed=91)
+    ref = []
+    for wl in (wa, wb):
+        g = cbmf.Context(wl.n, wl.fs, wl.f_low, device=0)
+        g.set_psd(wl.psd); g.load_segment(wl.samples)
+        ref.append(g.filter_bank(wl.bank, wl.threshold))
+        g.close()
+    torch.cuda.set_device(0)
+    ga, gb = cbmf.Context(wa.n, wa.fs, wa.f_low, device=1), cbmf.Context(wb.n, wb.fs, wb.f_low, device=0)
+    ga.set_psd(wa.psd); gb.set_psd(wb.psd)
+    gb.load_segment(wb.samples); ga.load_segment(wa.samples)
+    ra = ga.filter_bank(wa.bank, wa.threshold)
+    assert torch.cuda.current_device() == 0
+    rb = gb.filter_bank(wb.bank, wb.threshold)
+    torch.cuda.set_device(1)
+    ra2 = ga.filter_bank(wa.bank, wa.threshold)
+    rb2 = gb.filter_bank(wb.bank, wb.threshold)
+    assert torch.cuda.current_device() == 1
+    torch.cuda.set_device(0)
+    ga.close(); gb.close()
+    for got, want in ((ra, ref[0]), (rb, ref[1]), (ra2, ref[0]), (rb2, ref[1])):
+        assert np.array_equal(got[0], want[0]) and np.array_equal(got[1], want[1]) and got[2] == want[2]
+    n = 1 << 16
+    x0 = torch.view_as_complex(torch.randn(2, n, 2, generator=torch.Generator().manual_seed(5)))
+    outs = []
+    for d in (0, 1):
+        x = x0.to(f"cuda:{d}")
+        out = torch.empty_like(x)
+        assert cbmf.ifft_noalloc_dev(x, out, n) == cbmf.OK
+        torch.cuda.synchronize(d)
+        outs.append(out.cpu())
+    assert torch.equal(outs[0], outs[1])
+
+
 def test_trigger_sort_paths(cbmf):
     """threshold 0 with one and two templates of 4096 samples: exactly 4096 triggers (the single-block sort,
     full) and 8192 (tile sort + global merges); both must come back in (template, sample) order."""
